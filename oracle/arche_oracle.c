@@ -1,0 +1,658 @@
+/* CPU ORACLE -- TEST INFRASTRUCTURE ONLY (see arche_oracle.h).
+ *
+ * Written from PAPER.md (arXiv 2606.13283).  Deliberately plain: textbook recursive mixed-radix
+ * FFT, adaptive Gauss-Kronrod quadrature for the Fermi-Dirac integrals, full-phase sincos sums
+ * for the structure factor and forces, bracketing (Illinois) solve for mu, long-double serial sums.
+ * Nothing here is shared with the CUDA path.
+ */
+#include "arche_oracle.h"
+
+#include <complex.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef double complex cplx;
+static const double PI = 3.14159265358979323846264338327950288;
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+/* ======================================================================================== */
+/* Fermi-Dirac integrals: I_j(x) = int_0^inf t^j / (exp(t-x)+1) dt.           */
+/* Substitution t = s^2 removes the sqrt endpoint singularity:                              */
+/*   I_j = int_0^inf 2 s^(2j+1) / (exp(s^2 - x) + 1) ds.                                    */
+/* ======================================================================================== */
+static double fd_integrand(int twice_j, double s, double eta) {
+  double a = s * s - eta;
+  if (a > 700.0) return 0.0;
+  double f = 2.0 / (exp(a) + 1.0);
+  if (twice_j == -1) return f;
+  if (twice_j == 1) return f * s * s;
+  return f * s * s * s * s; /* twice_j == 3 */
+}
+
+/* 7-point Gauss / 15-point Kronrod nodes and weights on [-1,1] (standard QUADPACK values). */
+static const double XGK[8] = {0.991455371120812639206854697526329, 0.949107912342758524526189684047851,
+                              0.864864423359769072789712788640926, 0.741531185599394439863864773280788,
+                              0.586087235467691130294144838258730, 0.405845151377397166906606412076961,
+                              0.207784955007898467600689403773245, 0.000000000000000000000000000000000};
+static const double WGK[8] = {0.022935322010529224963732008058970, 0.063092092629978553290700663189204,
+                              0.104790010322250183839876322541518, 0.140653259715525918745189590510238,
+                              0.169004726639267902826583426598550, 0.190350578064785409913256402421014,
+                              0.204432940075298892414161999234649, 0.209482141084727828012999174891714};
+static const double WG[4] = {0.129484966168869693270611432679082, 0.279705391489276667901467771423780,
+                             0.381830050505118944950369775488975, 0.417959183673469387755102040816327};
+
+static void gk15(int twice_j, double eta, double a, double b, double *rk, double *rg) {
+  double c = 0.5 * (a + b), h = 0.5 * (b - a);
+  double fc = fd_integrand(twice_j, c, eta);
+  double k = WGK[7] * fc, g = WG[3] * fc;
+  for (int i = 0; i < 7; ++i) {
+    double dx = h * XGK[i];
+    double f = fd_integrand(twice_j, c - dx, eta) + fd_integrand(twice_j, c + dx, eta);
+    k += WGK[i] * f;
+    if (i & 1) g += WG[i / 2] * f;
+  }
+  *rk = k * h;
+  *rg = g * h;
+}
+
+static double fd_adapt(int twice_j, double eta, double a, double b, double tol_abs, int depth) {
+  double k, g;
+  gk15(twice_j, eta, a, b, &k, &g);
+  if (depth >= 3 && (fabs(k - g) <= tol_abs || depth > 40)) return k;
+  double c = 0.5 * (a + b);
+  return fd_adapt(twice_j, eta, a, c, 0.5 * tol_abs, depth + 1) +
+         fd_adapt(twice_j, eta, c, b, 0.5 * tol_abs, depth + 1);
+}
+
+double oracle_fd(int twice_j, double eta) {
+  double e0 = eta > 0.0 ? eta : 0.0;
+  double s0 = sqrt(e0), s1 = sqrt(e0 + 80.0);
+  /* scale for the tolerance: crude estimate with one GK15 panel per piece */
+  double k, g, est = 0.0;
+  if (s0 > 0.0) { gk15(twice_j, eta, 0.0, s0, &k, &g); est += fabs(k); }
+  gk15(twice_j, eta, s0, s1, &k, &g); est += fabs(k);
+  double tol = 1e-14 * est;
+  double r = 0.0;
+  if (s0 > 0.0) r += fd_adapt(twice_j, eta, 0.0, s0, tol, 0);
+  r += fd_adapt(twice_j, eta, s0, s1, tol, 0);
+  return r;
+}
+
+double oracle_fd_half_inverse(double y) {
+  /* bounds: I_{1/2}(eta) <= Gamma(3/2) e^eta  and  I_{1/2}(eta) >= (2/3) eta^{3/2} (eta>0) */
+  double g32 = 0.5 * sqrt(PI);
+  double lo = log(y / g32), hi = pow(1.5 * y, 2.0 / 3.0) + 2.0;
+  if (hi < lo + 2.0) hi = lo + 2.0;
+  for (int it = 0; it < 200; ++it) {
+    double mid = 0.5 * (lo + hi);
+    if (mid == lo || mid == hi) break;
+    if (oracle_fd(1, mid) < y) lo = mid; else hi = mid;
+  }
+  return 0.5 * (lo + hi);
+}
+
+/* ======================================================================================== */
+/* FFT: textbook recursive decimation-in-time for any length (smallest-prime-factor split).  */
+/* ======================================================================================== */
+static int smallest_factor(int n) {
+  for (int p = 2; p * p <= n; ++p)
+    if (n % p == 0) return p;
+  return n;
+}
+
+/* tw[a] = exp(sign 2 pi i a / N) for the top-level N; a sub-transform of length n uses tw[a*(N/n)] */
+static void fft_rec(int n, const cplx *in, int stride, cplx *out, const cplx *tw, int N) {
+  if (n == 1) { out[0] = in[0]; return; }
+  int p = smallest_factor(n), m = n / p;
+  for (int q = 0; q < p; ++q) fft_rec(m, in + (size_t)q * stride, stride * p, out + (size_t)q * m, tw, N);
+  cplx tmp[64];
+  cplx *t = tmp, *heap = NULL;
+  if (p > 64) t = heap = (cplx *)malloc(sizeof(cplx) * p);
+  int d = N / n;
+  for (int k = 0; k < m; ++k) {
+    for (int q = 0; q < p; ++q) t[q] = out[(size_t)q * m + k] * tw[(size_t)((long)q * k % n) * d];
+    for (int s = 0; s < p; ++s) {
+      cplx acc = 0.0;
+      for (int q = 0; q < p; ++q) acc += t[q] * tw[(size_t)((long)q * s % p) * (N / p)];
+      out[(size_t)s * m + k] = acc;
+    }
+  }
+  free(heap);
+}
+
+static cplx *make_twiddles(int N, int sign) {
+  cplx *tw = (cplx *)malloc(sizeof(cplx) * N);
+  for (int a = 0; a < N; ++a) {
+    long double ang = 2.0L * 3.14159265358979323846264338327950288L * (long double)a / (long double)N;
+    tw[a] = (double)cosl(ang) + I * (double)(sign * sinl(ang));
+  }
+  return tw;
+}
+
+static void transform_axis(int nx, int ny, int nz, cplx *a, int axis, int sign, int naive) {
+  int dims[3] = {nx, ny, nz};
+  size_t strides[3] = {1, (size_t)nx, (size_t)nx * ny};
+  int n = dims[axis];
+  size_t st = strides[axis];
+  int o1 = (axis + 1) % 3, o2 = (axis + 2) % 3;
+  cplx *tw = make_twiddles(n, sign);
+  long nlines = (long)dims[o1] * dims[o2];
+#pragma omp parallel
+  {
+    cplx *line = (cplx *)malloc(sizeof(cplx) * n), *res = (cplx *)malloc(sizeof(cplx) * n);
+#pragma omp for schedule(static)
+    for (long l = 0; l < nlines; ++l) {
+      int i1 = (int)(l % dims[o1]), i2 = (int)(l / dims[o1]);
+      cplx *base = a + i1 * strides[o1] + i2 * strides[o2];
+      for (int i = 0; i < n; ++i) line[i] = base[i * st];
+      if (naive) {
+        for (int k = 0; k < n; ++k) { /* the O(N^2) definition */
+          cplx acc = 0.0;
+          for (int j = 0; j < n; ++j) acc += line[j] * tw[(long)j * k % n];
+          res[k] = acc;
+        }
+      } else {
+        fft_rec(n, line, 1, res, tw, n);
+      }
+      for (int i = 0; i < n; ++i) base[i * st] = res[i];
+    }
+    free(line); free(res);
+  }
+  free(tw);
+}
+
+void oracle_fft3d(int nx, int ny, int nz, double *a, int sign) {
+  for (int ax = 0; ax < 3; ++ax) transform_axis(nx, ny, nz, (cplx *)a, ax, sign, 0);
+}
+void oracle_dft3d_naive(int nx, int ny, int nz, double *a, int sign) {
+  for (int ax = 0; ax < 3; ++ax) transform_axis(nx, ny, nz, (cplx *)a, ax, sign, 1);
+}
+
+/* ======================================================================================== */
+/* XC: Perdew-Zunger 1981 parametrisation of the Ceperley-Alder unpolarised gas (Hartree).   */
+/* DESIGN.md reading D5 (BASELINE.json fixes PZ81; PAPER.md:491 only says "LibXC").          */
+/* ======================================================================================== */
+void oracle_xc(int xc, double n, double *eps, double *v) {
+  if (xc == 0 || !(n > 0.0)) { *eps = 0.0; *v = 0.0; return; }
+  double ex = -0.75 * cbrt(3.0 / PI) * cbrt(n);
+  double vx = (4.0 / 3.0) * ex;
+  double rs = cbrt(3.0 / (4.0 * PI * n));
+  double ec, vc;
+  if (rs >= 1.0) {
+    const double gam = -0.1423, b1 = 1.0529, b2 = 0.3334;
+    double sq = sqrt(rs), den = 1.0 + b1 * sq + b2 * rs;
+    ec = gam / den;
+    vc = ec * (1.0 + (7.0 / 6.0) * b1 * sq + (4.0 / 3.0) * b2 * rs) / den;
+  } else {
+    const double A = 0.0311, B = -0.048, C = 0.0020, D = -0.0116;
+    double l = log(rs);
+    ec = A * l + B + C * rs * l + D * rs;
+    vc = A * l + (B - A / 3.0) + (2.0 / 3.0) * C * rs * l + (2.0 * D - C) / 3.0 * rs;
+  }
+  *eps = ex + ec;
+  *v = vx + vc;
+}
+
+/* ======================================================================================== */
+/* Grid helpers                                                                              */
+/* ======================================================================================== */
+static inline int kindex(int i, int N) { return i <= N / 2 ? i : i - N; }
+
+double oracle_vps_unit(double k, double rc) {
+  if (k == 0.0) return 0.0;
+  return -cos(2.0 * PI * k * rc) / (PI * k * k);
+}
+
+void oracle_structure_factor(const double cell[3], const int grid[3], int n_ions, const double *pos,
+                             const double *Z, double *S_out) {
+  cplx *S = (cplx *)S_out;
+  int nx = grid[0], ny = grid[1], nz = grid[2];
+#pragma omp parallel for schedule(static) collapse(2)
+  for (int iz = 0; iz < nz; ++iz)
+    for (int iy = 0; iy < ny; ++iy)
+      for (int ix = 0; ix < nx; ++ix) {
+        double kx = kindex(ix, nx) / cell[0], ky = kindex(iy, ny) / cell[1], kz = kindex(iz, nz) / cell[2];
+        long double sr = 0.0L, si = 0.0L;
+        for (int j = 0; j < n_ions; ++j) {
+          double ph = -2.0 * PI * (kx * pos[3 * j] + ky * pos[3 * j + 1] + kz * pos[3 * j + 2]);
+          sr += Z[j] * cos(ph);
+          si += Z[j] * sin(ph);
+        }
+        S[((size_t)iz * ny + iy) * nx + ix] = (double)sr + I * (double)si;
+      }
+}
+
+/* ======================================================================================== */
+/* Ewald, PAPER.md:377-421 (Eq. 40-47), readings A18 in DESIGN.md                            */
+/* ======================================================================================== */
+double oracle_ewald_alpha(const double cell[3], const int grid[3]) {
+  double rc = 0.5 * fmin(cell[0], fmin(cell[1], cell[2]));
+  double kc = fmin(grid[0] / (2.0 * cell[0]), fmin(grid[1] / (2.0 * cell[1]), grid[2] / (2.0 * cell[2])));
+  return sqrt(PI * kc / rc);
+}
+
+void oracle_ewald(const double cell[3], const int grid[3], int n, const double *pos, const double *Z,
+                  double alpha, double U[3], double *F) {
+  double vol = cell[0] * cell[1] * cell[2];
+  int nx = grid[0], ny = grid[1], nz = grid[2];
+  for (int i = 0; i < 3 * n; ++i) F[i] = 0.0;
+  /* short range, minimum image (Eq. 41, 46) */
+  long double upp = 0.0L;
+  for (int j = 0; j < n; ++j)
+    for (int k = 0; k < n; ++k) {
+      if (k == j) continue;
+      double d[3], r2 = 0.0;
+      for (int c = 0; c < 3; ++c) {
+        d[c] = pos[3 * j + c] - pos[3 * k + c];
+        d[c] -= cell[c] * rint(d[c] / cell[c]);
+        r2 += d[c] * d[c];
+      }
+      double r = sqrt(r2);
+      double e = erfc(alpha * r) / r;
+      if (k > j) upp += Z[j] * Z[k] * e;
+      double fr = Z[j] * Z[k] * (e + 2.0 * alpha / sqrt(PI) * exp(-alpha * alpha * r2)) / r2;
+      for (int c = 0; c < 3; ++c) F[3 * j + c] += fr * d[c]; /* repulsive along r_j - r_k */
+    }
+  /* long range over the FFT grid's k points (Eq. 42, 43, 47) */
+  size_t ng = (size_t)nx * ny * nz;
+  cplx *S = (cplx *)malloc(sizeof(cplx) * ng);
+  oracle_structure_factor(cell, grid, n, pos, Z, (double *)S);
+  long double upm = 0.0L;
+  for (size_t g = 0; g < ng; ++g) {
+    int ix = (int)(g % nx), iy = (int)((g / nx) % ny), iz = (int)(g / ((size_t)nx * ny));
+    double kx = kindex(ix, nx) / cell[0], ky = kindex(iy, ny) / cell[1], kz = kindex(iz, nz) / cell[2];
+    double k2 = kx * kx + ky * ky + kz * kz;
+    if (k2 == 0.0) continue;
+    double va = exp(-PI * PI * k2 / (alpha * alpha)) / (PI * k2);
+    upm += va * (creal(S[g]) * creal(S[g]) + cimag(S[g]) * cimag(S[g]));
+  }
+  upm *= 0.5L / vol;
+  double q = 0.0, q2 = 0.0;
+  for (int j = 0; j < n; ++j) { q += Z[j]; q2 += Z[j] * Z[j]; }
+  upm -= alpha / sqrt(PI) * q2;
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < n; ++j) {
+    long double f[3] = {0.0L, 0.0L, 0.0L};
+    for (size_t g = 0; g < ng; ++g) {
+      int ix = (int)(g % nx), iy = (int)((g / nx) % ny), iz = (int)(g / ((size_t)nx * ny));
+      double kx = kindex(ix, nx) / cell[0], ky = kindex(iy, ny) / cell[1], kz = kindex(iz, nz) / cell[2];
+      double k2 = kx * kx + ky * ky + kz * kz;
+      if (k2 == 0.0) continue;
+      double va = exp(-PI * PI * k2 / (alpha * alpha)) / (PI * k2);
+      double ph = 2.0 * PI * (kx * pos[3 * j] + ky * pos[3 * j + 1] + kz * pos[3 * j + 2]);
+      double im = cimag((cos(ph) + I * sin(ph)) * S[g]); /* Im(e^{+2 pi i k.r_j} S_Z(k)), Eq. 47 */
+      f[0] += va * im * kx; f[1] += va * im * ky; f[2] += va * im * kz;
+    }
+    for (int c = 0; c < 3; ++c) F[3 * j + c] += Z[j] * 2.0 * PI / vol * (double)f[c];
+  }
+  free(S);
+  U[0] = (double)upp;
+  U[1] = (double)upm;
+  U[2] = -PI * q * q / (2.0 * alpha * alpha * vol); /* Eq. 44 */
+}
+
+/* F^ie, Eq. 56 with the normalisation/sign of DESIGN.md reading A17:                         */
+/* F_j = -(2 pi/|Omega|) Z_j sum_k k v(k) Im( conj(nhat(k)) exp(-2 pi i k.r_j) )               */
+void oracle_force_ie(const double cell[3], const int grid[3], int n, const double *pos, const double *Z,
+                     double rc, const double *nhat_in, double *F) {
+  const cplx *nh = (const cplx *)nhat_in;
+  double vol = cell[0] * cell[1] * cell[2];
+  int nx = grid[0], ny = grid[1], nz = grid[2];
+  size_t ng = (size_t)nx * ny * nz;
+#pragma omp parallel for schedule(static)
+  for (int j = 0; j < n; ++j) {
+    long double f[3] = {0.0L, 0.0L, 0.0L};
+    for (size_t g = 0; g < ng; ++g) {
+      int ix = (int)(g % nx), iy = (int)((g / nx) % ny), iz = (int)(g / ((size_t)nx * ny));
+      double kx = kindex(ix, nx) / cell[0], ky = kindex(iy, ny) / cell[1], kz = kindex(iz, nz) / cell[2];
+      double k = sqrt(kx * kx + ky * ky + kz * kz);
+      if (k == 0.0) continue;
+      double v = oracle_vps_unit(k, rc);
+      double ph = -2.0 * PI * (kx * pos[3 * j] + ky * pos[3 * j + 1] + kz * pos[3 * j + 2]);
+      double im = cimag(conj(nh[g]) * (cos(ph) + I * sin(ph)));
+      f[0] += v * im * kx; f[1] += v * im * ky; f[2] += v * im * kz;
+    }
+    for (int c = 0; c < 3; ++c) F[3 * j + c] = -2.0 * PI / vol * Z[j] * (double)f[c];
+  }
+}
+
+/* ======================================================================================== */
+/* SCF context                                                                                */
+/* ======================================================================================== */
+struct oracle_ctx {
+  oracle_params p;
+  double *Z, *mass, *pos, *F;
+  size_t ng;
+  double vol, dV, cTF, Ne, Q, alpha, E_ie0, U_ii;
+  double *n_i, *n_a, *V_i, *tmp1, *tmp2, *tmp3;
+  cplx *nh_i, *nh_a, *Vh_ie, *S, *gh, *work;
+  double *F_ii;
+  double mu;
+  int have_g, have_solution, have_forces;
+  oracle_result last;
+};
+
+static double serial_sum(const double *a, size_t n) {
+  long double s = 0.0L;
+  for (size_t i = 0; i < n; ++i) s += a[i];
+  return (double)s;
+}
+
+int oracle_init(const oracle_params *p, oracle_ctx **out) {
+  if (!p || !out || p->n_ions < 0 || p->kT <= 0.0) return -1;
+  for (int c = 0; c < 3; ++c)
+    if (p->grid[c] < 2 || !(p->cell[c] > 0.0)) return -1;
+  oracle_ctx *c = (oracle_ctx *)calloc(1, sizeof(oracle_ctx));
+  c->p = *p;
+  int n = p->n_ions;
+  c->Z = (double *)malloc(sizeof(double) * (n + 1));
+  c->mass = (double *)malloc(sizeof(double) * (n + 1));
+  c->pos = (double *)calloc(3 * n + 1, sizeof(double));
+  c->F = (double *)calloc(3 * n + 1, sizeof(double));
+  c->F_ii = (double *)calloc(3 * n + 1, sizeof(double));
+  if (n > 0) { memcpy(c->Z, p->Z, sizeof(double) * n); memcpy(c->mass, p->mass, sizeof(double) * n); }
+  c->p.Z = c->Z; c->p.mass = c->mass;
+  c->ng = (size_t)p->grid[0] * p->grid[1] * p->grid[2];
+  c->vol = p->cell[0] * p->cell[1] * p->cell[2];
+  c->dV = c->vol / (double)c->ng;
+  c->cTF = sqrt(2.0) / (PI * PI) * pow(p->kT, 1.5);
+  c->Q = 0.0;
+  for (int j = 0; j < n; ++j) c->Q += c->Z[j];
+  c->Ne = p->n_electrons > 0.0 ? p->n_electrons : c->Q; /* neutral cell unless overridden */
+  c->alpha = p->ewald_alpha > 0.0 ? p->ewald_alpha : oracle_ewald_alpha(p->cell, p->grid);
+  /* non-Coulomb k=0 term (reading A16): alpha_s = 2 pi Z rc^2 per ion */
+  double asum = 0.0;
+  for (int j = 0; j < n; ++j) asum += 2.0 * PI * c->Z[j] * p->psp_rc * p->psp_rc;
+  c->E_ie0 = c->Ne / c->vol * asum;
+  size_t ng = c->ng;
+  c->n_i = (double *)calloc(ng, sizeof(double));
+  c->n_a = (double *)calloc(ng, sizeof(double));
+  c->V_i = (double *)calloc(ng, sizeof(double));
+  c->tmp1 = (double *)calloc(ng, sizeof(double));
+  c->tmp2 = (double *)calloc(ng, sizeof(double));
+  c->tmp3 = (double *)calloc(ng, sizeof(double));
+  c->nh_i = (cplx *)calloc(ng, sizeof(cplx));
+  c->nh_a = (cplx *)calloc(ng, sizeof(cplx));
+  c->Vh_ie = (cplx *)calloc(ng, sizeof(cplx));
+  c->S = (cplx *)calloc(ng, sizeof(cplx));
+  c->gh = (cplx *)calloc(ng, sizeof(cplx));
+  c->work = (cplx *)calloc(ng, sizeof(cplx));
+  *out = c;
+  return 0;
+}
+
+void oracle_destroy(oracle_ctx *c) {
+  if (!c) return;
+  free(c->Z); free(c->mass); free(c->pos); free(c->F); free(c->F_ii);
+  free(c->n_i); free(c->n_a); free(c->V_i); free(c->tmp1); free(c->tmp2); free(c->tmp3);
+  free(c->nh_i); free(c->nh_a); free(c->Vh_ie); free(c->S); free(c->gh); free(c->work);
+  free(c);
+}
+
+static void kvec(const oracle_ctx *c, size_t g, double k[3]) {
+  int nx = c->p.grid[0], ny = c->p.grid[1], nz = c->p.grid[2];
+  int ix = (int)(g % nx), iy = (int)((g / nx) % ny), iz = (int)(g / ((size_t)nx * ny));
+  k[0] = kindex(ix, nx) / c->p.cell[0];
+  k[1] = kindex(iy, ny) / c->p.cell[1];
+  k[2] = kindex(iz, nz) / c->p.cell[2];
+}
+
+/* fhat = dV * DFT(f) */
+static void forward_real(const oracle_ctx *c, const double *f, cplx *fh) {
+  for (size_t g = 0; g < c->ng; ++g) fh[g] = f[g];
+  oracle_fft3d(c->p.grid[0], c->p.grid[1], c->p.grid[2], (double *)fh, -1);
+  for (size_t g = 0; g < c->ng; ++g) fh[g] *= c->dV;
+}
+/* f = Re[(1/|Omega|) * inverse-DFT(fh)]  (reading A6: real part) */
+static void inverse_to_real(const oracle_ctx *c, const cplx *fh, double *f, cplx *work) {
+  memcpy(work, fh, sizeof(cplx) * c->ng);
+  oracle_fft3d(c->p.grid[0], c->p.grid[1], c->p.grid[2], (double *)work, +1);
+  for (size_t g = 0; g < c->ng; ++g) f[g] = creal(work[g]) / c->vol;
+}
+
+int oracle_set_input_density(oracle_ctx *c, const double *n_i) {
+  memcpy(c->n_i, n_i, sizeof(double) * c->ng);
+  forward_real(c, c->n_i, c->nh_i);
+  return 0;
+}
+
+int oracle_scf_begin(oracle_ctx *c, const double *pos) {
+  int n = c->p.n_ions;
+  memcpy(c->pos, pos, sizeof(double) * 3 * n);
+  /* P1/P2: structure factor and ionic potential */
+  oracle_structure_factor(c->p.cell, c->p.grid, n, c->pos, c->Z, (double *)c->S);
+  for (size_t g = 0; g < c->ng; ++g) {
+    double k[3];
+    kvec(c, g, k);
+    double ka = sqrt(k[0] * k[0] + k[1] * k[1] + k[2] * k[2]);
+    c->Vh_ie[g] = oracle_vps_unit(ka, c->p.psp_rc) * c->S[g];
+  }
+  /* P3: Ewald */
+  double U[3];
+  oracle_ewald(c->p.cell, c->p.grid, n, c->pos, c->Z, c->alpha, U, c->F_ii);
+  c->U_ii = U[0] + U[1] + U[2];
+  /* P4: input density */
+  if (c->p.init_mode == 1 && c->have_g) {
+    /* nhat_i = S_Z^{new} ghat^{old} (Eq. 20); IFFT, real part, clip, renormalise (reading A10) */
+    for (size_t g = 0; g < c->ng; ++g) c->nh_i[g] = c->S[g] * c->gh[g];
+    inverse_to_real(c, c->nh_i, c->n_i, c->work);
+    double floor_n = 1e-3 * c->Ne / c->vol;
+    for (size_t g = 0; g < c->ng; ++g)
+      if (c->n_i[g] < floor_n) c->n_i[g] = floor_n;
+    double tot = serial_sum(c->n_i, c->ng) * c->dV;
+    double sc = c->Ne / tot;
+    for (size_t g = 0; g < c->ng; ++g) c->n_i[g] *= sc;
+    forward_real(c, c->n_i, c->nh_i);
+  } else {
+    double n0 = c->Ne / c->vol;
+    for (size_t g = 0; g < c->ng; ++g) { c->n_i[g] = n0; c->nh_i[g] = 0.0; }
+    c->nh_i[0] = c->Ne;
+  }
+  c->have_solution = 0;
+  c->have_forces = 0;
+  c->last.scf_iters = 0;
+  c->last.mu_evals = 0;
+  c->last.converged = 0;
+  c->last.F_total = 0.0;
+  return 0;
+}
+
+static double electron_count(const oracle_ctx *c, double mu, double *scratch) {
+  size_t ng = c->ng;
+  double kT = c->p.kT;
+#pragma omp parallel for schedule(dynamic, 256)
+  for (size_t g = 0; g < ng; ++g) scratch[g] = oracle_fd(1, (mu - c->V_i[g]) / kT);
+  return c->cTF * c->dV * serial_sum(scratch, ng);
+}
+
+int oracle_scf_iter(oracle_ctx *c, oracle_result *out) {
+  size_t ng = c->ng;
+  double kT = c->p.kT, vol = c->vol, dV = c->dV, cTF = c->cTF;
+  /* S1: Vhat = nhat_i/(pi k^2) + Vhat_ie (Eq. 12, 14), inverse transform, real part */
+  for (size_t g = 0; g < ng; ++g) {
+    double k[3];
+    kvec(c, g, k);
+    double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+    c->work[g] = (k2 == 0.0) ? 0.0 : c->nh_i[g] / (PI * k2) + c->Vh_ie[g];
+  }
+  oracle_fft3d(c->p.grid[0], c->p.grid[1], c->p.grid[2], (double *)c->work, +1);
+  /* S2: V_i = V_H + V_ie + V_xc(n_i) */
+  double vmin = INFINITY, vmax = -INFINITY;
+  for (size_t g = 0; g < ng; ++g) {
+    double e, v;
+    oracle_xc(c->p.xc, c->n_i[g], &e, &v);
+    c->V_i[g] = creal(c->work[g]) / vol + v;
+    if (c->V_i[g] < vmin) vmin = c->V_i[g];
+    if (c->V_i[g] > vmax) vmax = c->V_i[g];
+  }
+  /* S3: mu from charge neutrality (Eq. 19) by a bracketing, derivative-free solve (Illinois).   */
+  /* bracket: eta0 = I_{1/2}^{-1}(Ne/(|Omega| cTF)); N(mu) is strictly increasing (reading D1).  */
+  double eta0 = oracle_fd_half_inverse(c->Ne / (vol * cTF));
+  double lo = vmin + kT * eta0, hi = vmax + kT * eta0;
+  int evals = 0;
+  double mu;
+  if (hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi))) {
+    mu = 0.5 * (lo + hi);
+  } else {
+    /* widen by one ulp-ish so that rounding cannot leave the root outside */
+    double pad = 1e-12 * (fabs(lo) + fabs(hi) + kT);
+    lo -= pad; hi += pad;
+    double flo = electron_count(c, lo, c->tmp1) - c->Ne;
+    double fhi = electron_count(c, hi, c->tmp1) - c->Ne;
+    evals += 2;
+    mu = lo; double fmu = flo;
+    int side = 0;
+    for (int it = 0; it < 200; ++it) {
+      if (fabs(fmu) <= 1e-14 * c->Ne) break;
+      if (hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi))) break;
+      double x = (lo * fhi - hi * flo) / (fhi - flo);
+      if (!(x > lo && x < hi)) x = 0.5 * (lo + hi);
+      double fx = electron_count(c, x, c->tmp1) - c->Ne;
+      ++evals;
+      mu = x; fmu = fx;
+      if (fx == 0.0) break;
+      if ((fx > 0.0) == (fhi > 0.0)) { hi = x; fhi = fx; if (side == -1) flo *= 0.5; side = -1; }
+      else { lo = x; flo = fx; if (side == +1) fhi *= 0.5; side = +1; }
+    }
+  }
+  c->mu = mu;
+  /* S4: n_a, chi = dn_a/dmu, local reductions */
+  double *t_chi = c->tmp1, *t_f0 = c->tmp2, *t_ke = c->tmp3;
+#pragma omp parallel for schedule(dynamic, 256)
+  for (size_t g = 0; g < ng; ++g) {
+    double eta = (mu - c->V_i[g]) / kT;
+    double i12 = oracle_fd(1, eta), im12 = oracle_fd(-1, eta), i32 = oracle_fd(3, eta);
+    c->n_a[g] = cTF * i12;                       /* Eq. 9 */
+    t_chi[g] = cTF * 0.5 * im12 / kT;            /* d/dmu of Eq. 9, I_j' = j I_{j-1} */
+    t_f0[g] = kT * cTF * (eta * i12 - (2.0 / 3.0) * i32); /* f_0 from Eq. 38-39 (reading O7) */
+    t_ke[g] = kT * cTF * i32;                    /* Eq. 38 */
+  }
+  long double sK = 0, sdn2 = 0, sna2 = 0, sF0 = 0, sKe = 0, sExc = 0;
+  for (size_t g = 0; g < ng; ++g) {
+    double dn = c->n_i[g] - c->n_a[g];
+    sK += dn * dn / t_chi[g];                    /* Eq. 31 */
+    sdn2 += dn * dn;
+    sna2 += c->n_a[g] * c->n_a[g];
+    sF0 += t_f0[g];
+    sKe += t_ke[g];
+    double e, v;
+    oracle_xc(c->p.xc, c->n_a[g], &e, &v);
+    sExc += c->n_a[g] * e;
+  }
+  double K = (double)sK * dV, F0 = (double)sF0 * dV, Ke = (double)sKe * dV, Exc = (double)sExc * dV;
+  /* S5: forward transform of n_a, G-space reductions */
+  forward_real(c, c->n_a, c->nh_a);
+  long double sU = 0, sEH = 0, sEie = 0;
+  for (size_t g = 0; g < ng; ++g) {
+    double k[3];
+    kvec(c, g, k);
+    double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+    sEie += creal(conj(c->nh_a[g]) * c->Vh_ie[g]);
+    if (k2 == 0.0) continue;
+    cplx d = c->nh_i[g] - c->nh_a[g];
+    sU += (creal(d) * creal(d) + cimag(d) * cimag(d)) / (PI * k2);            /* Eq. 30 */
+    sEH += (creal(c->nh_a[g]) * creal(c->nh_a[g]) + cimag(c->nh_a[g]) * cimag(c->nh_a[g])) / (PI * k2);
+  }
+  double U = (double)sU / vol, EH = 0.5 * (double)sEH / vol /* Eq. 53 */, Eie = (double)sEie / vol;
+  double Ftot = F0 + Exc + EH + Eie + c->E_ie0 + c->U_ii;
+  /* S6: mixing n_o = n_a + w (n_i - n_a), w = U/(K+U) */
+  int it = c->last.scf_iters + 1;
+  double w;
+  if (c->p.mix_mode == 1 && it > c->p.mix_warmup) w = (K + U > 0.0) ? U / (K + U) : 0.0;
+  else w = c->p.mix_w_fixed;
+  for (size_t g = 0; g < ng; ++g) {
+    c->n_i[g] = c->n_a[g] + w * (c->n_i[g] - c->n_a[g]);
+    c->nh_i[g] = c->nh_a[g] + w * (c->nh_i[g] - c->nh_a[g]);
+  }
+  /* S7: convergence (reading D4) */
+  double dn_rel = sqrt((double)sdn2 / (double)sna2);
+  double dF = fabs(Ftot - c->last.F_total);
+  oracle_result r = c->last;
+  r.converged = (it >= 2 && dF < c->p.scf_tol_F && dn_rel < c->p.scf_tol_dn);
+  r.mu = mu; r.F_total = Ftot; r.F0 = F0; r.E_H = EH; r.E_xc = Exc; r.E_ie = Eie; r.E_ie0 = c->E_ie0;
+  r.U_ii = c->U_ii; r.K_e = Ke; r.dn_l2 = dn_rel; r.w_last = w; r.U_mix = U; r.K_mix = K;
+  r.scf_iters = it; r.mu_evals += evals;
+  c->last = r;
+  c->have_solution = 1;
+  c->have_forces = 0;
+  if (out) *out = r;
+  return 0;
+}
+
+int oracle_scf_solve(oracle_ctx *c, const double *pos, oracle_result *out) {
+  oracle_scf_begin(c, pos);
+  int maxit = c->p.scf_fixed_iter > 0 ? c->p.scf_fixed_iter : c->p.scf_max_iter;
+  for (int it = 0; it < maxit; ++it) {
+    oracle_scf_iter(c, NULL);
+    if (c->p.scf_fixed_iter <= 0 && c->last.converged) break;
+  }
+  /* P6: store the one-center profile ghat = nhat/S_Z, regularised (reading A10) */
+  double epsS = 1e-8 * c->Q * c->Q;
+  for (size_t g = 0; g < c->ng; ++g) {
+    double s2 = creal(c->S[g]) * creal(c->S[g]) + cimag(c->S[g]) * cimag(c->S[g]);
+    c->gh[g] = c->nh_a[g] * conj(c->S[g]) / fmax(s2, epsS);
+  }
+  c->have_g = 1;
+  if (out) *out = c->last;
+  return (c->last.converged || c->p.scf_fixed_iter > 0) ? 0 : -3;
+}
+
+int oracle_forces(oracle_ctx *c, double *F) {
+  if (!c->have_solution) return -1;
+  int n = c->p.n_ions;
+  oracle_force_ie(c->p.cell, c->p.grid, n, c->pos, c->Z, c->p.psp_rc, (const double *)c->nh_a, c->F);
+  for (int i = 0; i < 3 * n; ++i) c->F[i] += c->F_ii[i];
+  c->have_forces = 1;
+  if (F) memcpy(F, c->F, sizeof(double) * 3 * n);
+  return 0;
+}
+
+int oracle_md_step(oracle_ctx *c, double dt, double *pos, double *vel, oracle_result *out) {
+  int n = c->p.n_ions, rc = 0;
+  if (!c->have_forces) { /* forces at the starting positions */
+    rc = oracle_scf_solve(c, pos, NULL);
+    oracle_forces(c, NULL);
+  }
+  for (int j = 0; j < n; ++j)
+    for (int d = 0; d < 3; ++d) {
+      vel[3 * j + d] += 0.5 * dt * c->F[3 * j + d] / c->mass[j];
+      pos[3 * j + d] += dt * vel[3 * j + d];
+    }
+  rc = oracle_scf_solve(c, pos, NULL);
+  oracle_forces(c, NULL);
+  long double ki = 0.0L;
+  for (int j = 0; j < n; ++j)
+    for (int d = 0; d < 3; ++d) {
+      vel[3 * j + d] += 0.5 * dt * c->F[3 * j + d] / c->mass[j];
+      ki += 0.5 * c->mass[j] * vel[3 * j + d] * vel[3 * j + d]; /* Eq. 36 */
+    }
+  c->last.K_i = (double)ki;
+  if (out) *out = c->last;
+  return rc;
+}
+
+int oracle_get_real(oracle_ctx *c, int which, double *dst) {
+  const double *src = which == 0 ? c->n_a : which == 1 ? c->n_i : which == 2 ? c->V_i : NULL;
+  if (!src) return -1;
+  memcpy(dst, src, sizeof(double) * c->ng);
+  return 0;
+}
+int oracle_get_complex(oracle_ctx *c, int which, double *dst) {
+  const cplx *src = which == 0 ? c->nh_a : which == 1 ? c->Vh_ie : which == 2 ? c->S : which == 3 ? c->gh
+                    : which == 4 ? c->nh_i : NULL;
+  if (!src) return -1;
+  memcpy(dst, src, sizeof(cplx) * c->ng);
+  return 0;
+}

@@ -1,0 +1,98 @@
+/* CPU ORACLE -- TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, obviously-correct fp64 implementation of the finite-temperature Thomas-Fermi SCF
+ * hot path of PAPER.md (arXiv 2606.13283, "Arche"), written from the paper.  It shares no code,
+ * tables or headers with the CUDA path in paper_2606_13283_b200/.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use it.
+ *
+ * Every host pointer is owned by the caller.  All arrays are row-major; grid fields are
+ * [z][y][x] with x fastest; complex = interleaved (re, im) doubles (C99 double complex).
+ *
+ * Conventions: k = (mx/Lx, my/Ly, mz/Lz) with m in [-N/2+1, N/2]
+ * (PAPER.md:142), storage index i -> m = i (i <= N/2) else i-N;
+ * fhat(k) = dV * sum_r f(r) exp(-2 pi i k.r),  f(r) = (1/|Omega|) sum_k fhat(k) exp(+2 pi i k.r)
+ * (PAPER.md:144-149 discretised so that both lines of Eq. 53, agree).
+ *
+ * Parity pins: tests/test_oracle_pins.py (every function below is pinned there except the SCF
+ * iteration count / w history, which are "parity unpinned": they depend on DESIGN.md readings).
+ */
+#ifndef ARCHE_ORACLE_H
+#define ARCHE_ORACLE_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct oracle_ctx oracle_ctx;
+
+typedef struct {
+  double cell[3];      /* Lx, Ly, Lz (bohr) */
+  int grid[3];         /* Nx, Ny, Nz */
+  int n_ions;
+  const double *Z;     /* [n_ions] valence charges */
+  const double *mass;  /* [n_ions] electron masses */
+  double kT;           /* Hartree */
+  int xc;              /* 0 none (paper's TF-only derivations), 1 PZ81 LDA */
+  double psp_rc;       /* Ashcroft empty-core radius (bohr) */
+  int init_mode;       /* 0 uniform density every step, 1 one-center profile */
+  int mix_mode;        /* 0 fixed w, 1 More et al. w = U/(K+U) */
+  double mix_w_fixed;  /* n_o = n_a + w (n_i - n_a) */
+  int mix_warmup;      /* iterations with the fixed w before More's w */
+  double scf_tol_F;    /* Ha */
+  double scf_tol_dn;   /* relative L2 */
+  int scf_max_iter;
+  int scf_fixed_iter;  /* >0: run exactly this many iterations */
+  double ewald_alpha;  /* <=0: auto */
+  double n_electrons;  /* <=0: sum_j Z_j (neutral cell); >0: that many electrons on a
+                          uniform neutralising background (uniform-gas and linear-response pins) */
+} oracle_params;
+
+typedef struct {
+  double mu, F_total, F0, E_H, E_xc, E_ie, E_ie0, U_ii, K_e, K_i, dn_l2, w_last, U_mix, K_mix;
+  int scf_iters, mu_evals, converged;
+} oracle_result;
+
+/* --- primitives ------------------------------------------------------------------------ */
+/* I_j(eta) = int_0^inf t^j/(exp(t-eta)+1) dt, j = twice_j/2 in {-1/2,1/2,3/2} */
+double oracle_fd(int twice_j, double eta);
+double oracle_fd_half_inverse(double y);             /* eta with I_{1/2}(eta) = y */
+/* unnormalised DFT along all three axes, in place; sign=-1: exp(-2 pi i mn/N), +1: exp(+...) */
+void oracle_fft3d(int nx, int ny, int nz, double *a_complex, int sign);
+void oracle_dft3d_naive(int nx, int ny, int nz, double *a_complex, int sign);
+/* xc=1: Perdew-Zunger 1981 LDA, unpolarised: energy per electron and potential */
+void oracle_xc(int xc, double n, double *eps_xc, double *v_xc);
+/* S_Z(k) = sum_j Z_j exp(-2 pi i k.r_j) on the grid */
+void oracle_structure_factor(const double cell[3], const int grid[3], int n_ions,
+                             const double *pos, const double *Z, double *S_complex);
+/* Ashcroft empty-core form factor per unit charge: -cos(2 pi k rc)/(pi k^2), 0 at k=0 */
+double oracle_vps_unit(double kabs, double rc);
+double oracle_ewald_alpha(const double cell[3], const int grid[3]);
+/* Ewald: U[0]=U_pp, U[1]=U_pm (incl. self term), U[2]=U_je; F[n_ions*3] = F_pp + F_pm */
+void oracle_ewald(const double cell[3], const int grid[3], int n_ions, const double *pos,
+                  const double *Z, double alpha, double U[3], double *F);
+
+/* --- SCF / MD context -------------------------------------------------------------------- */
+int oracle_init(const oracle_params *p, oracle_ctx **out);
+void oracle_destroy(oracle_ctx *c);
+/* per-MD-step ion-grid work + input-density initialisation for positions pos[n_ions*3] */
+int oracle_scf_begin(oracle_ctx *c, const double *pos);
+/* supply the input density explicitly (real field); n_hat_i is recomputed by FFT */
+int oracle_set_input_density(oracle_ctx *c, const double *n_i);
+/* one SCF iteration (PAPER.md:217-231 + 257-311) from the current input density */
+int oracle_scf_iter(oracle_ctx *c, oracle_result *out);
+int oracle_scf_solve(oracle_ctx *c, const double *pos, oracle_result *out);
+/* total force F^ie + F^ii on every ion from the last active density */
+int oracle_forces(oracle_ctx *c, double *F);
+/* one velocity-Verlet step (reading D2) */
+int oracle_md_step(oracle_ctx *c, double dt, double *pos, double *vel, oracle_result *out);
+/* field access: which = 0 n_a, 1 n_i (next input), 2 V_i ; complex: 0 nhat_a, 1 Vhat_ie, 2 S_Z, 3 ghat, 4 nhat_i */
+int oracle_get_real(oracle_ctx *c, int which, double *dst);
+int oracle_get_complex(oracle_ctx *c, int which, double *dst);
+/* F^ie only, for an arbitrary density given in G-space (used by the fixed-density FD pin) */
+void oracle_force_ie(const double cell[3], const int grid[3], int n_ions, const double *pos,
+                     const double *Z, double rc, const double *nhat_complex, double *F);
+int oracle_num_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
