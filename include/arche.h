@@ -1,0 +1,119 @@
+/* arche.h -- C ABI of the B200-native hot path of Arche's orbital-free MD (arXiv 2606.13283):
+ * finite-temperature Thomas-Fermi SCF on a periodic 3D grid + the per-MD-step ion-grid work.
+ *
+ * Citations: P:NNN = PAPER.md line NNN.  All computation behind these calls runs in hand-written
+ * CUDA kernels for sm_100a in fp64 (own 3D FFT included); there is no CPU fallback.
+ *
+ * Conventions
+ *   grid fields      real or complex (interleaved re,im) fp64, layout [z][y][x], x fastest
+ *   reciprocal grid  k = (mx/Lx, my/Ly, mz/Lz), m in [-N/2+1, N/2], storage index i -> m = i (i<=N/2) else i-N
+ *   transform        fhat(k) = dV sum_r f(r) exp(-2 pi i k.r);  f(r) = (1/|Omega|) sum_k fhat(k) exp(+2 pi i k.r)
+ *   units            Hartree atomic units; positions in bohr, any value (periodic)
+ *   pointers         "d_" = DEVICE pointer, "h_" = HOST pointer; the caller owns every array and the workspace
+ *   errors           every call returns ARCHE_OK (0) or a negative code; nothing throws or aborts
+ *   stream           all work is ordered on params.stream; calls that fill a host result synchronise that stream
+ */
+#ifndef ARCHE_H
+#define ARCHE_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ARCHE_OK 0
+#define ARCHE_EINVAL (-1)   /* bad argument / call order */
+#define ARCHE_ENOMEM (-2)   /* workspace too small */
+#define ARCHE_ENOCONV (-3)  /* SCF hit scf_max_iter; the last iterate stays readable */
+#define ARCHE_ENAN (-4)     /* non-finite value met */
+#define ARCHE_ECUDA (-5)    /* CUDA runtime error (see arche_last_error) */
+
+typedef struct arche_ctx arche_ctx; /* opaque, owned by the library */
+
+typedef struct {
+  double cell[3];        /* Lx, Ly, Lz in bohr, orthorhombic */
+  int grid[3];           /* Nx, Ny, Nz; each 2^a 3^b, >= 4 and <= 1024 */
+  int n_ions;            /* >= 0 */
+  const double *h_Z;     /* [n_ions] valence charges, host, copied at init */
+  const double *h_mass;  /* [n_ions] ion masses in electron masses, host, copied at init */
+  double kT;             /* electron (= ion) temperature in Hartree */
+  int xc;                /* 0: none (the paper's own TF derivations); 1: Perdew-Zunger 1981 LDA */
+  double psp_rc;         /* Ashcroft empty-core radius in bohr (BASELINE.json: 1.12) */
+  int init_mode;         /* 0: uniform input density each step; 1: one-center profile */
+  int mix_mode;          /* 0: fixed w; 1: More et al. w = U/(K+U) */
+  double mix_w_fixed;    /* n_o = n_a + w (n_i - n_a) */
+  int mix_warmup;        /* SCF iterations run with mix_w_fixed before More's w is used */
+  double scf_tol_F;      /* stop when |F_k - F_{k-1}| < scf_tol_F (Ha) ... */
+  double scf_tol_dn;     /* ... and ||n_i - n_a||_L2 / ||n_a||_L2 < scf_tol_dn */
+  int scf_max_iter;
+  int scf_fixed_iter;    /* > 0: run exactly this many iterations (parity replay) */
+  double ewald_alpha;    /* <= 0: automatic (reading A18) */
+  double n_electrons;    /* <= 0: sum_j Z_j (neutral cell); > 0: that many electrons on a uniform background */
+  void *d_workspace;     /* device memory, >= arche_workspace_bytes(), 256-byte aligned */
+  size_t workspace_bytes;
+  void *stream;          /* cudaStream_t (0 = default stream) */
+} arche_params;
+
+typedef struct {
+  double mu;                                   /* chemical potential mu_a of Eq. 19 */
+  double F_total;                              /* F0 + E_xc + E_H + E_ie + E_ie0 + U_ii (P:327-332 without K_i) */
+  double F0, E_H, E_xc, E_ie, E_ie0, U_ii;
+  double K_e, K_i;                             /* Eq. 38 and Eq. 36 */
+  double dn_l2;                                /* ||n_i - n_a|| / ||n_a|| of the last iteration */
+  double w_last, U_mix, K_mix;                 /* Eq. 30-31 */
+  int scf_iters, mu_evals, converged;
+} arche_result;
+
+/* Bytes of device workspace arche_scf_init will carve up for these parameters (0 on bad parameters). */
+size_t arche_workspace_bytes(const arche_params *p);
+
+/* Validate, copy Z/mass, build twiddle tables and reciprocal-space factors on the device (they depend only on
+ * cell/grid/T).  *out is set on success; destroy with arche_destroy.  No device allocation happens after init. */
+int arche_scf_init(const arche_params *p, arche_ctx **out);
+void arche_destroy(arche_ctx *c);
+const char *arche_last_error(const arche_ctx *c);
+
+/* One SCF solve for ion positions d_pos[n_ions*3] (row-major [ion][xyz]):
+ * structure factor S_Z(k), ionic potential Vhat_ie, Ewald, input density
+ * (uniform or Eq. 20), then SCF iterations with mixing until the stop rule;
+ * finally stores ghat = nhat/S_Z.  *h_out filled after a stream synchronise. */
+int arche_scf_solve(arche_ctx *c, const double *d_pos, arche_result *h_out);
+
+/* Split form of the solve (used for step-by-step parity and for timing single iterations):
+ * begin = per-step ion-grid work + input density; iter = exactly one SCF iteration. */
+int arche_scf_begin(arche_ctx *c, const double *d_pos);
+int arche_scf_iter(arche_ctx *c, arche_result *h_out);
+/* Replace the input density n_i (d_n: [Nz][Ny][Nx] real, device); nhat_i is recomputed by the FFT. */
+int arche_set_input_density(arche_ctx *c, const double *d_n);
+
+/* Total force F^ie (Eq. 56) + F^ii (Eq. 45-47) on every ion from the last active density,
+ * written to d_F[n_ions*3].  ARCHE_EINVAL before any solve. */
+int arche_forces(arche_ctx *c, double *d_F);
+
+/* One velocity-Verlet step of length dt (a.u.) (reading D2): half kick, drift, SCF solve at the
+ * new positions, forces, half kick.  d_pos/d_vel [n_ions*3] are updated in place.  The first call also solves
+ * at the starting positions to obtain the initial forces. */
+int arche_md_step(arche_ctx *c, double dt, double *d_pos, double *d_vel, arche_result *h_out);
+/* Same step through HOST buffers: positions/velocities are copied in, the step runs, positions, velocities and
+ * forces (h_F may be NULL) are copied back -- the paper's per-step host<->device traffic. */
+int arche_md_step_host(arche_ctx *c, double dt, double *h_pos, double *h_vel, double *h_F, arche_result *h_out);
+
+/* Field read-back for parity tests (device destination buffers).
+ * real   which: 0 n_a (active density of the last iteration), 1 n_i (next input density), 2 V_i
+ * complex which: 0 nhat_a, 1 Vhat_ie, 2 S_Z, 3 ghat, 4 nhat_i */
+int arche_get_real(arche_ctx *c, int which, double *d_dst);
+int arche_get_complex(arche_ctx *c, int which, double *d_dst);
+int arche_get_density(arche_ctx *c, double *d_n); /* = arche_get_real(c, 0, d_n) */
+
+/* Stand-alone entry points of individual kernels (unit parity + roofline benches). */
+/* 3D complex FFT, unnormalised, out-of-place or in-place (d_in == d_out allowed); sign = -1 forward, +1 inverse.
+ * d_scratch: 16*Nx*Ny*Nz bytes. */
+int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, double *d_scratch, int sign);
+/* I_j(eta) for twice_j in {-1,1,3} on n device values */
+int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta, double *d_out, size_t n);
+/* number of kernels this context has launched so far (for bench.py's gpu_launches) */
+long long arche_launch_count(const arche_ctx *c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,233 @@
+"""paper_2606_13283_b200 -- B200-native (sm_100a, fp64 CUDA) hot path of Arche's orbital-free MD:
+finite-temperature Thomas-Fermi SCF on a periodic grid + per-MD-step ion-grid work (arXiv 2606.13283).
+
+This package is a thin ctypes binding over the C ABI in include/arche.h: it marshals arguments and lets
+PyTorch own device memory and streams.  Every step of the path runs in the CUDA kernels of csrc/.
+There is no CPU fallback: if the library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from .build import LIB, build
+
+__all__ = ["Arche", "ArcheError", "load", "SYMBOLS", "Params", "Result"]
+
+SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_last_error", "arche_scf_solve",
+           "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_md_step",
+           "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
+           "arche_fermi_dirac", "arche_launch_count"]
+
+ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
+
+
+class ArcheError(RuntimeError):
+    pass
+
+
+class Params(C.Structure):
+    _fields_ = [("cell", C.c_double * 3), ("grid", C.c_int * 3), ("n_ions", C.c_int),
+                ("h_Z", C.c_void_p), ("h_mass", C.c_void_p), ("kT", C.c_double), ("xc", C.c_int),
+                ("psp_rc", C.c_double), ("init_mode", C.c_int), ("mix_mode", C.c_int),
+                ("mix_w_fixed", C.c_double), ("mix_warmup", C.c_int), ("scf_tol_F", C.c_double),
+                ("scf_tol_dn", C.c_double), ("scf_max_iter", C.c_int), ("scf_fixed_iter", C.c_int),
+                ("ewald_alpha", C.c_double), ("n_electrons", C.c_double), ("d_workspace", C.c_void_p),
+                ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p)]
+
+
+class Result(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "E_ie0", "U_ii", "K_e",
+                                          "K_i", "dn_l2", "w_last", "U_mix", "K_mix")] + \
+               [(k, C.c_int) for k in ("scf_iters", "mu_evals", "converged")]
+
+    def asdict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def load(rebuild_if_stale: bool = True):
+    """dlopen the C-ABI library (building it in-tree first if the sources are newer). Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = build() if rebuild_if_stale else LIB
+    if not os.path.exists(path):
+        raise ArcheError(f"CUDA library missing: {path} (run python -m paper_2606_13283_b200.build)")
+    L = C.CDLL(path)
+    vp, dp = C.c_void_p, C.c_void_p
+    L.arche_workspace_bytes.restype = C.c_size_t
+    L.arche_workspace_bytes.argtypes = [C.POINTER(Params)]
+    L.arche_scf_init.argtypes = [C.POINTER(Params), C.POINTER(vp)]
+    L.arche_destroy.argtypes = [vp]; L.arche_destroy.restype = None
+    L.arche_last_error.argtypes = [vp]; L.arche_last_error.restype = C.c_char_p
+    L.arche_scf_solve.argtypes = [vp, dp, C.POINTER(Result)]
+    L.arche_scf_begin.argtypes = [vp, dp]
+    L.arche_scf_iter.argtypes = [vp, C.POINTER(Result)]
+    L.arche_set_input_density.argtypes = [vp, dp]
+    L.arche_forces.argtypes = [vp, dp]
+    L.arche_md_step.argtypes = [vp, C.c_double, dp, dp, C.POINTER(Result)]
+    L.arche_md_step_host.argtypes = [vp, C.c_double, dp, dp, dp, C.POINTER(Result)]
+    L.arche_get_real.argtypes = [vp, C.c_int, dp]
+    L.arche_get_complex.argtypes = [vp, C.c_int, dp]
+    L.arche_get_density.argtypes = [vp, dp]
+    L.arche_fft3d.argtypes = [vp, dp, dp, dp, C.c_int]
+    L.arche_fermi_dirac.argtypes = [vp, C.c_int, dp, dp, C.c_size_t]
+    L.arche_launch_count.argtypes = [vp]; L.arche_launch_count.restype = C.c_longlong
+    _lib = L
+    return L
+
+
+_DEFAULTS = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=0, scf_tol_F=1e-10,
+                 scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0, ewald_alpha=0.0, n_electrons=0.0)
+
+
+class Arche:
+    """One SCF/MD context on the current CUDA device; torch owns the workspace and the stream."""
+
+    def __init__(self, cfg: dict, device="cuda:0", stream=None, **over):
+        import torch
+        if not torch.cuda.is_available():
+            raise ArcheError("no CUDA device: the Arche hot path has no CPU fallback")
+        self.torch = torch
+        self.lib = load()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        p = dict(_DEFAULTS)
+        for k in p:
+            if k in cfg:
+                p[k] = cfg[k]
+        p.update(over)
+        self._Z = np.ascontiguousarray(cfg["Z"], dtype=np.float64)
+        self._m = np.ascontiguousarray(cfg["mass"], dtype=np.float64)
+        self.n_ions = len(self._Z)
+        self.grid = [int(g) for g in cfg["grid"]]
+        self.shape = (self.grid[2], self.grid[1], self.grid[0])
+        self.ng = self.grid[0] * self.grid[1] * self.grid[2]
+        P = Params()
+        P.cell[:] = [float(x) for x in cfg["cell"]]
+        P.grid[:] = self.grid
+        P.n_ions = self.n_ions
+        P.h_Z = self._Z.ctypes.data if self.n_ions else None
+        P.h_mass = self._m.ctypes.data if self.n_ions else None
+        P.kT = float(cfg["kT"])
+        for k, v in p.items():
+            setattr(P, k, v)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        P.stream = self.stream.cuda_stream
+        nbytes = self.lib.arche_workspace_bytes(C.byref(P))
+        if nbytes == 0:
+            raise ArcheError("arche_workspace_bytes: invalid parameters")
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self.workspace.data_ptr() + 255) & ~255
+        P.d_workspace = ptr
+        P.workspace_bytes = nbytes
+        self.params = P
+        self._h = C.c_void_p()
+        rc = self.lib.arche_scf_init(C.byref(P), C.byref(self._h))
+        if rc != 0:
+            raise ArcheError(f"arche_scf_init failed: {ERRORS.get(rc, rc)}")
+
+    # -- helpers
+    def _check(self, rc, allow_noconv=True):
+        if rc == 0 or (allow_noconv and rc == -3):
+            return rc
+        msg = self.lib.arche_last_error(self._h)
+        raise ArcheError(f"{ERRORS.get(rc, rc)}: {msg.decode() if msg else ''}")
+
+    def _dev(self, a):
+        t = self.torch
+        if isinstance(a, t.Tensor):
+            assert a.is_cuda and a.dtype in (t.float64, t.complex128) and a.is_contiguous()
+            return a
+        return t.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device=self.device)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.arche_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the C-ABI calls
+    def scf_solve(self, pos) -> dict:
+        d = self._dev(pos); r = Result()
+        with self.torch.cuda.stream(self.stream):
+            rc = self._check(self.lib.arche_scf_solve(self._h, d.data_ptr(), C.byref(r)))
+        out = r.asdict(); out["rc"] = rc
+        return out
+
+    def scf_begin(self, pos):
+        d = self._dev(pos)
+        self._check(self.lib.arche_scf_begin(self._h, d.data_ptr() if self.n_ions else None))
+
+    def scf_iter(self) -> dict:
+        r = Result()
+        self._check(self.lib.arche_scf_iter(self._h, C.byref(r)))
+        return r.asdict()
+
+    def set_input_density(self, n):
+        d = self._dev(n)
+        self._check(self.lib.arche_set_input_density(self._h, d.data_ptr()))
+
+    def forces(self, out=None):
+        t = self.torch
+        F = out if out is not None else t.empty((self.n_ions, 3), dtype=t.float64, device=self.device)
+        self._check(self.lib.arche_forces(self._h, F.data_ptr()))
+        return F
+
+    def md_step(self, dt, pos, vel) -> dict:
+        """pos, vel: CUDA float64 tensors [n_ions,3], updated in place."""
+        r = Result()
+        rc = self._check(self.lib.arche_md_step(self._h, float(dt), pos.data_ptr(), vel.data_ptr(), C.byref(r)))
+        out = r.asdict(); out["rc"] = rc
+        return out
+
+    def md_step_host(self, dt, pos, vel, F=None) -> dict:
+        """pos, vel (and F): host float64 arrays (numpy or pinned torch CPU tensors), updated in place."""
+        r = Result()
+        ptr = lambda a: a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
+        rc = self._check(self.lib.arche_md_step_host(self._h, float(dt), ptr(pos), ptr(vel),
+                                                     ptr(F) if F is not None else None, C.byref(r)))
+        out = r.asdict(); out["rc"] = rc
+        return out
+
+    def get_real(self, which: str):
+        t = self.torch
+        a = t.empty(self.shape, dtype=t.float64, device=self.device)
+        self._check(self.lib.arche_get_real(self._h, {"n_a": 0, "n_i": 1, "V_i": 2}[which], a.data_ptr()))
+        return a
+
+    def get_complex(self, which: str):
+        t = self.torch
+        a = t.empty(self.shape, dtype=t.complex128, device=self.device)
+        idx = {"nhat_a": 0, "Vhat_ie": 1, "S_Z": 2, "ghat": 3, "nhat_i": 4}[which]
+        self._check(self.lib.arche_get_complex(self._h, idx, a.data_ptr()))
+        return a
+
+    def fft3d(self, a, sign: int):
+        t = self.torch
+        a = a.to(device=self.device, dtype=t.complex128).contiguous()
+        out = t.empty_like(a); scratch = t.empty_like(a)
+        self._check(self.lib.arche_fft3d(self._h, a.data_ptr(), out.data_ptr(), scratch.data_ptr(), int(sign)))
+        return out
+
+    def fermi_dirac(self, twice_j: int, eta):
+        t = self.torch
+        e = self._dev(eta); out = t.empty_like(e)
+        self._check(self.lib.arche_fermi_dirac(self._h, int(twice_j), e.data_ptr(), out.data_ptr(), e.numel()))
+        return out
+
+    def launch_count(self) -> int:
+        return int(self.lib.arche_launch_count(self._h))
+
+    def sync(self):
+        self.stream.synchronize()

@@ -1,0 +1,550 @@
+// arche.cu -- host control + C ABI (include/arche.h) of the B200 Thomas-Fermi SCF / OFMD hot path.
+// Every step of the path runs in the CUDA kernels of fft.cuh, scf_kernels.cuh and ion_kernels.cuh; the host only
+// sequences launches on the caller's stream and reads one small scalar block per SCF iteration.
+#include "../../include/arche.h"
+
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+#include "fd.cuh"
+#include "fft.cuh"
+#include "ion_kernels.cuh"
+#include "scf_kernels.cuh"
+
+using namespace arche;
+
+namespace {
+
+constexpr int kMuMaxPasses = 12;
+constexpr int kEwBlocks = 148 * 8;
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Carver {  // carves 256-byte aligned arrays out of the caller's workspace (or just measures)
+  char *base;
+  size_t off;
+  template <class T> T *take(size_t count) {
+    T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+    off += align256(count * sizeof(T));
+    return p;
+  }
+};
+
+// host evaluation of the same fits (only for eta0 = I_{1/2}^{-1}(Ne/(|Omega| cTF)), once per init)
+double fd_half_host(double eta) {
+  int seg; double v, pre;
+  if (eta <= 0.0) { double x = exp(eta); seg = 0; for (int a = 1; a < FD_NA; ++a) seg += (x > FD_XA_BREAK[a]); v = x; pre = x; }
+  else if (eta < (double)FD_ETA_C) { seg = FD_ETA_SEG[(int)eta]; v = eta; pre = 1.0; }
+  else { seg = FD_NSEG - 1; v = 1.0 / (eta * eta); pre = sqrt(eta) * eta; }
+  double t = (v - FD_CENTER[seg]) * FD_INVHALF[seg], a = FD_COEF[seg][1][FD_NC - 1];
+  for (int i = FD_NC - 2; i >= 0; --i) a = fma(a, t, FD_COEF[seg][1][i]);
+  return a * pre;
+}
+double fd_half_inverse_host(double y) {
+  double lo = log(y / 0.88622692545275801365), hi = pow(1.5 * y, 2.0 / 3.0) + 2.0;
+  if (hi < lo + 2.0) hi = lo + 2.0;
+  for (int it = 0; it < 200; ++it) {
+    double mid = 0.5 * (lo + hi);
+    if (mid == lo || mid == hi) break;
+    if (fd_half_host(mid) < y) lo = mid; else hi = mid;
+  }
+  return 0.5 * (lo + hi);
+}
+
+bool grid_ok(int n) {
+  if (n < 4 || n > 1024) return false;
+  while (n % 2 == 0) n /= 2;
+  while (n % 3 == 0) n /= 3;
+  return n == 1;
+}
+
+}  // namespace
+
+struct arche_ctx {
+  arche_params p;
+  cudaStream_t stream;
+  GridGeom G;
+  ScfConst C;
+  long long ng;
+  int nions;
+  double alpha, Q;
+  FftAxisPlan plan[3];
+  int red_blocks;  // capacity of the partials buffer (blocks)
+  int ew_grid;     // blocks of grid-stride elementwise kernels
+  int force_slabs, force_rows_per_slab;
+  // device arrays (all inside the caller's workspace)
+  double *n_i, *n_a, *V_i, *vps, *va;
+  double2 *nh_i, *nh_a, *vh_ie, *S, *gh, *work;
+  double *kx, *ky, *kz, *kx2, *ky2, *kz2;
+  double2 *tw[3];
+  double2 *ax_ij, *ax_ji, *by_ij, *cz_ij;
+  double *Z, *mass, *pos, *F, *F_pp, *e_pp, *F_part, *vel_tmp;
+  double *fdtab, *partials;
+  unsigned int *counter;
+  DevScalars *sc;
+  DevScalars *h_sc;  // pinned
+  bool have_g, have_solution, have_forces;
+  long long launches;
+  char err[256];
+};
+
+namespace {
+
+int fail(arche_ctx *c, int code, const char *what, cudaError_t e = cudaSuccess) {
+  if (c) snprintf(c->err, sizeof(c->err), "%s%s%s", what, e != cudaSuccess ? ": " : "", e != cudaSuccess ? cudaGetErrorString(e) : "");
+  return code;
+}
+#define CK(call)                                                             \
+  do {                                                                       \
+    cudaError_t e__ = (call);                                                \
+    if (e__ != cudaSuccess) return fail(c, ARCHE_ECUDA, #call, e__);         \
+  } while (0)
+#define LAUNCHED(c) do { ++(c)->launches; CK(cudaGetLastError()); } while (0)
+
+int fft_tile_blocks(int axis, int n, int nx, int ny, int nz) {
+  int L = fft_pick_L(axis, n, nx, ny, nz);
+  return axis == 0 ? (int)((long long)ny * nz / L) : (axis == 1 ? nz * (nx / L) : ny * (nx / L));
+}
+
+// lays out the workspace; with base == nullptr only sizes it
+size_t layout(arche_ctx *c, char *base) {
+  Carver w{base, 0};
+  const size_t ng = (size_t)c->ng, ni = (size_t)(c->nions > 0 ? c->nions : 1);
+  const int nx = c->p.grid[0], ny = c->p.grid[1], nz = c->p.grid[2];
+  c->n_i = w.take<double>(ng); c->n_a = w.take<double>(ng); c->V_i = w.take<double>(ng);
+  c->vps = w.take<double>(ng); c->va = w.take<double>(ng);
+  c->nh_i = w.take<double2>(ng); c->nh_a = w.take<double2>(ng); c->vh_ie = w.take<double2>(ng);
+  c->S = w.take<double2>(ng); c->gh = w.take<double2>(ng); c->work = w.take<double2>(ng);
+  c->kx = w.take<double>(nx); c->ky = w.take<double>(ny); c->kz = w.take<double>(nz);
+  c->kx2 = w.take<double>(nx); c->ky2 = w.take<double>(ny); c->kz2 = w.take<double>(nz);
+  c->tw[0] = w.take<double2>(nx); c->tw[1] = w.take<double2>(ny); c->tw[2] = w.take<double2>(nz);
+  c->ax_ij = w.take<double2>(ni * nx); c->ax_ji = w.take<double2>(ni * nx);
+  c->by_ij = w.take<double2>(ni * ny); c->cz_ij = w.take<double2>(ni * nz);
+  c->Z = w.take<double>(ni); c->mass = w.take<double>(ni); c->pos = w.take<double>(3 * ni);
+  c->F = w.take<double>(3 * ni); c->F_pp = w.take<double>(3 * ni); c->e_pp = w.take<double>(ni);
+  c->vel_tmp = w.take<double>(3 * ni);
+  c->F_part = w.take<double>((size_t)c->force_slabs * ni * 3);
+  c->fdtab = w.take<double>(kFdTabDoubles);
+  c->partials = w.take<double>((size_t)c->red_blocks * kMaxRed);
+  c->counter = w.take<unsigned int>(64);
+  c->sc = w.take<DevScalars>(1);
+  return w.off;
+}
+
+void derive_sizes(arche_ctx *c) {
+  const int nx = c->p.grid[0], ny = c->p.grid[1], nz = c->p.grid[2];
+  c->ng = (long long)nx * ny * nz;
+  c->nions = c->p.n_ions;
+  c->ew_grid = (int)((c->ng + 255) / 256 < kEwBlocks ? (c->ng + 255) / 256 : kEwBlocks);
+  int rb = c->ew_grid;
+  for (int a = 0; a < 3; ++a) { int b = fft_tile_blocks(a, c->p.grid[a], nx, ny, nz); if (b > rb) rb = b; }
+  long long sfb = ((long long)ny * nz + SF_ROWS - 1) / SF_ROWS * ((nx + SF_THREADS - 1) / SF_THREADS);
+  if (sfb > rb) rb = (int)sfb;
+  c->red_blocks = rb + 8;
+  const long long rows = (long long)ny * nz;
+  const int tiles = (c->nions + FC_THREADS - 1) / FC_THREADS;
+  int slabs = tiles > 0 ? (148 * 4 + tiles - 1) / tiles : 1;
+  if (slabs > rows) slabs = (int)rows;
+  if (slabs < 1) slabs = 1;
+  c->force_rows_per_slab = (int)((rows + slabs - 1) / slabs);
+  c->force_slabs = (int)((rows + c->force_rows_per_slab - 1) / c->force_rows_per_slab);
+}
+
+bool params_ok(const arche_params *p) {
+  if (!p || p->n_ions < 0 || !(p->kT > 0.0)) return false;
+  for (int a = 0; a < 3; ++a)
+    if (!grid_ok(p->grid[a]) || !(p->cell[a] > 0.0)) return false;
+  if (p->n_ions > 0 && (!p->h_Z || !p->h_mass)) return false;
+  if (p->xc != 0 && p->xc != 1) return false;
+  return true;
+}
+
+}  // namespace
+
+extern "C" size_t arche_workspace_bytes(const arche_params *p) {
+  if (!params_ok(p)) return 0;
+  arche_ctx tmp;
+  memset(&tmp, 0, sizeof(tmp));
+  tmp.p = *p;
+  derive_sizes(&tmp);
+  return layout(&tmp, nullptr);
+}
+
+extern "C" const char *arche_last_error(const arche_ctx *c) { return c ? c->err : "null context"; }
+extern "C" long long arche_launch_count(const arche_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" void arche_destroy(arche_ctx *c) {
+  if (!c) return;
+  if (c->h_sc) cudaFreeHost(c->h_sc);
+  delete c;
+}
+
+extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
+  if (!out) return ARCHE_EINVAL;
+  *out = nullptr;
+  if (!params_ok(p)) return ARCHE_EINVAL;
+  arche_ctx *c = new (std::nothrow) arche_ctx;
+  if (!c) return ARCHE_ENOMEM;
+  memset(c, 0, sizeof(*c));
+  c->p = *p;
+  c->stream = (cudaStream_t)p->stream;
+  derive_sizes(c);
+  size_t need = layout(c, nullptr);
+  if (!p->d_workspace || p->workspace_bytes < need || ((uintptr_t)p->d_workspace & 255)) { delete c; return ARCHE_ENOMEM; }
+  layout(c, (char *)p->d_workspace);
+  const int nx = p->grid[0], ny = p->grid[1], nz = p->grid[2];
+  cudaError_t e = cudaMallocHost((void **)&c->h_sc, sizeof(DevScalars));
+  if (e != cudaSuccess) { delete c; return ARCHE_ECUDA; }
+  // ---- geometry and constants
+  GridGeom &G = c->G;
+  G.nx = nx; G.ny = ny; G.nz = nz; G.ng = c->ng;
+  G.Lx = p->cell[0]; G.Ly = p->cell[1]; G.Lz = p->cell[2];
+  G.vol = G.Lx * G.Ly * G.Lz; G.dV = G.vol / (double)c->ng;
+  G.kx = c->kx; G.ky = c->ky; G.kz = c->kz; G.kx2 = c->kx2; G.ky2 = c->ky2; G.kz2 = c->kz2;
+  std::vector<double> hZ(c->nions + 1, 0.0);
+  c->Q = 0.0;
+  for (int j = 0; j < c->nions; ++j) { hZ[j] = p->h_Z[j]; c->Q += hZ[j]; }
+  ScfConst &C = c->C;
+  C.kT = p->kT; C.cTF = sqrt(2.0) / (ARCHE_PI * ARCHE_PI) * pow(p->kT, 1.5);
+  C.Ne = p->n_electrons > 0.0 ? p->n_electrons : c->Q;
+  C.vol = G.vol; C.dV = G.dV;
+  if (!(C.Ne > 0.0)) { arche_destroy(c); return ARCHE_EINVAL; }
+  C.eta0 = fd_half_inverse_host(C.Ne / (G.vol * C.cTF));
+  double asum = 0.0;
+  for (int j = 0; j < c->nions; ++j) asum += 2.0 * ARCHE_PI * hZ[j] * p->psp_rc * p->psp_rc;  // alpha_s = 2 pi Z rc^2
+  C.E_ie0 = C.Ne / G.vol * asum;
+  C.xc = p->xc; C.mix_mode = p->mix_mode; C.mix_warmup = p->mix_warmup; C.mix_w_fixed = p->mix_w_fixed;
+  C.tol_F = p->scf_tol_F; C.tol_dn = p->scf_tol_dn;
+  {  // Ewald alpha (reading A18)
+    double rc = 0.5 * fmin(G.Lx, fmin(G.Ly, G.Lz));
+    double kc = fmin(nx / (2.0 * G.Lx), fmin(ny / (2.0 * G.Ly), nz / (2.0 * G.Lz)));
+    c->alpha = p->ewald_alpha > 0.0 ? p->ewald_alpha : sqrt(ARCHE_PI * kc / rc);
+  }
+  // ---- per-axis tables: k, k^2, twiddles (long double on the host)
+  const int dims[3] = {nx, ny, nz};
+  const double Ls[3] = {G.Lx, G.Ly, G.Lz};
+  double *dk[3] = {c->kx, c->ky, c->kz}, *dk2[3] = {c->kx2, c->ky2, c->kz2};
+  for (int a = 0; a < 3; ++a) {
+    const int n = dims[a];
+    std::vector<double> k(n), k2(n);
+    std::vector<double2> tw(n);
+    for (int i = 0; i < n; ++i) {
+      int m = i <= n / 2 ? i : i - n;
+      k[i] = m / Ls[a]; k2[i] = k[i] * k[i];
+      long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)i / (long double)n;
+      tw[i] = make_double2((double)cosl(ang), (double)sinl(ang));
+    }
+    CK(cudaMemcpyAsync(dk[a], k.data(), n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(dk2[a], k2.data(), n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->tw[a], tw.data(), n * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (!fft_make_plan(n, c->tw[a], &c->plan[a])) { arche_destroy(c); return ARCHE_EINVAL; }
+  }
+  if (c->nions > 0) {
+    CK(cudaMemcpyAsync(c->Z, p->h_Z, c->nions * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->mass, p->h_mass, c->nions * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  }
+  std::vector<double> tab(kFdTabDoubles);
+  fd_pack_tables(tab.data());
+  CK(cudaMemcpyAsync(c->fdtab, tab.data(), kFdTabDoubles * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemsetAsync(c->counter, 0, 64 * sizeof(unsigned int), c->stream));
+  CK(cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream));
+  CK(cudaMemsetAsync(c->F, 0, 3 * (c->nions > 0 ? c->nions : 1) * sizeof(double), c->stream));
+  form_factor_kernel<<<c->ew_grid, 256, 0, c->stream>>>(G, p->psp_rc, c->alpha, c->vps, c->va);
+  LAUNCHED(c);
+  CK(cudaStreamSynchronize(c->stream));
+  c->p.h_Z = nullptr; c->p.h_mass = nullptr;  // copied; do not keep the caller's pointers
+  *out = c;
+  return ARCHE_OK;
+}
+
+// =============================================================================================
+// 3D transforms with fused prologue / epilogue
+// =============================================================================================
+namespace {
+
+// inverse: axis order z, y, x (the x pass writes the real field contiguously)
+template <class LoadOp, class StoreOp>
+int fft3d_inverse(arche_ctx *c, LoadOp ld, StoreOp st) {
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  CK((fft_launch_pass<2, true>(c->plan[2], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches;
+  CK((fft_launch_pass<1, true>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches;
+  CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches;
+  return ARCHE_OK;
+}
+// forward: axis order x, y, z
+template <class LoadOp, class StoreOp>
+int fft3d_forward(arche_ctx *c, LoadOp ld, StoreOp st) {
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  CK((fft_launch_pass<0, false>(c->plan[0], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches;
+  CK((fft_launch_pass<1, false>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches;
+  CK((fft_launch_pass<2, false>(c->plan[2], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches;
+  return ARCHE_OK;
+}
+
+int read_scalars(arche_ctx *c) {
+  CK(cudaMemcpyAsync(c->h_sc, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return ARCHE_OK;
+}
+
+void fill_result(const arche_ctx *c, arche_result *r) {
+  if (!r) return;
+  const DevScalars &s = *c->h_sc;
+  r->mu = s.mu; r->F_total = s.F_total; r->F0 = s.F0; r->E_H = s.EH; r->E_xc = s.Exc; r->E_ie = s.Eie;
+  r->E_ie0 = c->C.E_ie0; r->U_ii = s.U_ii; r->K_e = s.Ke; r->K_i = s.K_i; r->dn_l2 = s.dn_rel;
+  r->w_last = s.w; r->U_mix = s.U; r->K_mix = s.K;
+  r->scf_iters = s.iter; r->mu_evals = s.mu_evals_total; r->converged = s.converged;
+}
+
+// forward transform of the real input density into nhat_i (scaled by dV)
+int input_density_to_g(arche_ctx *c) {
+  return fft3d_forward(c, LoadReal{c->n_i}, StoreScaled{c->nh_i, c->G.dV});
+}
+
+int scf_iteration(arche_ctx *c) {
+  const GridGeom &G = c->G;
+  const ScfConst &C = c->C;
+  // S1 + S2
+  StoreVi sv;
+  sv.V_i = c->V_i; sv.n_i = c->n_i; sv.sc = c->sc; sv.partials = c->partials; sv.counter = c->counter;
+  sv.inv_vol = 1.0 / G.vol; sv.kT_eta0 = C.kT * C.eta0; sv.xc = C.xc;
+  sv.acc_min = 1.0e308; sv.acc_max = -1.0e308; sv.acc_sum = 0.0;
+  int rc = fft3d_inverse(c, LoadPotentialG{c->nh_i, c->vh_ie, c->kx2, c->ky2, c->kz2}, sv);
+  if (rc) return rc;
+  // S3
+  mu_guess_kernel<<<1, 1, 0, c->stream>>>(c->sc, (double)c->ng, C.kT * C.eta0);
+  LAUNCHED(c);
+  for (int pass = 0; pass < kMuMaxPasses; ++pass) {
+    mu_pass_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->V_i, c->ng, C, c->sc, c->fdtab, c->partials, c->counter,
+                                                     pass == kMuMaxPasses - 1);
+    LAUNCHED(c);
+  }
+  // S4
+  density_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->V_i, c->n_i, c->n_a, c->ng, C, c->sc, c->fdtab, c->partials, c->counter);
+  LAUNCHED(c);
+  // S5 (+ w, F, stop flags in the epilogue's last block)
+  StoreNhatA sn;
+  sn.nh_a = c->nh_a; sn.nh_i = c->nh_i; sn.vh_ie = c->vh_ie; sn.kx2 = c->kx2; sn.ky2 = c->ky2; sn.kz2 = c->kz2;
+  sn.sc = c->sc; sn.partials = c->partials; sn.counter = c->counter; sn.C = C; sn.aU = sn.aEH = sn.aEie = 0.0;
+  rc = fft3d_forward(c, LoadReal{c->n_a}, sn);
+  if (rc) return rc;
+  // S6
+  mix_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->n_a, c->nh_i, c->nh_a, c->ng, c->sc);
+  LAUNCHED(c);
+  c->have_solution = true;
+  c->have_forces = false;
+  return ARCHE_OK;
+}
+
+int scf_begin(arche_ctx *c, const double *d_pos) {
+  const GridGeom &G = c->G;
+  const int ni = c->nions;
+  if (ni > 0) {
+    if (!d_pos) return fail(c, ARCHE_EINVAL, "d_pos is null");
+    if (d_pos != c->pos) CK(cudaMemcpyAsync(c->pos, d_pos, 3 * ni * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+    // P1: separable phase tables, then S_Z with the V_ie / Ewald-reciprocal epilogue (P2, P3)
+    const int pb = 148 * 2;
+    phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 0, G.Lx, G.nx, ni, c->ax_ij, c->ax_ji); LAUNCHED(c);
+    phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 1, G.Ly, G.ny, ni, c->by_ij, nullptr); LAUNCHED(c);
+    phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 2, G.Lz, G.nz, ni, c->cz_ij, nullptr); LAUNCHED(c);
+    dim3 sg((unsigned)(((long long)G.ny * G.nz + SF_ROWS - 1) / SF_ROWS), (unsigned)((G.nx + SF_THREADS - 1) / SF_THREADS));
+    structure_factor_kernel<<<sg, SF_THREADS, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S,
+                                                              c->vh_ie, c->partials, c->counter, c->sc);
+    LAUNCHED(c);
+    ewald_pp_kernel<<<ni, 128, 0, c->stream>>>(c->pos, c->Z, ni, G.Lx, G.Ly, G.Lz, c->alpha, c->F_pp, c->e_pp); LAUNCHED(c);
+    ewald_finish_kernel<<<1, 256, 0, c->stream>>>(c->e_pp, c->Z, ni, c->alpha, G.vol, c->sc); LAUNCHED(c);
+  } else {
+    CK(cudaMemsetAsync(c->S, 0, c->ng * sizeof(double2), c->stream));
+    CK(cudaMemsetAsync(c->vh_ie, 0, c->ng * sizeof(double2), c->stream));
+  }
+  // P4: input density
+  if (c->p.init_mode == 1 && c->have_g && ni > 0) {
+    StoreClip sk;
+    sk.n_i = c->n_i; sk.sc = c->sc; sk.partials = c->partials; sk.counter = c->counter;
+    sk.inv_vol = 1.0 / G.vol; sk.floor_n = 1e-3 * c->C.Ne / G.vol; sk.Ne = c->C.Ne; sk.dV = G.dV; sk.acc = 0.0;
+    int rc = fft3d_inverse(c, LoadSG{c->S, c->gh}, sk);
+    if (rc) return rc;
+    rc = fft3d_forward(c, LoadRealScaled{c->n_i, c->sc}, StoreScaled{c->nh_i, G.dV});
+    if (rc) return rc;
+  } else {
+    set_uniform_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->nh_i, c->ng, c->C.Ne / G.vol, c->C.Ne);
+    LAUNCHED(c);
+  }
+  // reset per-solve scalars (iter, F_total, converged); mu and U_ii persist
+  CK(cudaMemsetAsync(&c->sc->iter, 0, sizeof(int) * 2, c->stream));
+  CK(cudaMemsetAsync(&c->sc->F_total, 0, sizeof(double), c->stream));
+  CK(cudaMemsetAsync(&c->sc->mu_evals_total, 0, sizeof(int), c->stream));
+  c->have_solution = false;
+  c->have_forces = false;
+  return ARCHE_OK;
+}
+
+int scf_solve(arche_ctx *c, const double *d_pos) {
+  int rc = scf_begin(c, d_pos);
+  if (rc) return rc;
+  const int fixed = c->p.scf_fixed_iter;
+  const int maxit = fixed > 0 ? fixed : (c->p.scf_max_iter > 0 ? c->p.scf_max_iter : 200);
+  bool conv = false;
+  for (int it = 0; it < maxit; ++it) {
+    rc = scf_iteration(c);
+    if (rc) return rc;
+    rc = read_scalars(c);
+    if (rc) return rc;
+    if (!isfinite(c->h_sc->F_total) || !isfinite(c->h_sc->mu)) return fail(c, ARCHE_ENAN, "non-finite free energy or mu");
+    if (fixed <= 0 && c->h_sc->converged) { conv = true; break; }
+  }
+  // P6: one-center profile of this step's converged density (reading A10)
+  if (c->nions > 0) {
+    g_store_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->gh, c->nh_a, c->S, c->ng, 1e-8 * c->Q * c->Q);
+    LAUNCHED(c);
+    c->have_g = true;
+  }
+  return (conv || fixed > 0) ? ARCHE_OK : fail(c, ARCHE_ENOCONV, "SCF did not converge within scf_max_iter");
+}
+
+int compute_forces(arche_ctx *c) {
+  if (!c->have_solution) return fail(c, ARCHE_EINVAL, "arche_forces before a solve");
+  const int ni = c->nions;
+  if (ni == 0) { c->have_forces = true; return ARCHE_OK; }
+  const GridGeom &G = c->G;
+  dim3 fg((unsigned)((ni + FC_THREADS - 1) / FC_THREADS), (unsigned)c->force_slabs);
+  force_kernel<<<fg, FC_THREADS, 2 * G.nx * sizeof(double2), c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij,
+                                                                        c->cz_ij, c->vps, c->va, c->nh_a, c->S, c->F_part);
+  LAUNCHED(c);
+  force_finish_kernel<<<(3 * ni + 127) / 128, 128, 0, c->stream>>>(ni, c->force_slabs, c->F_part, c->F_pp, c->Z,
+                                                                   -2.0 * ARCHE_PI / G.vol, c->F);
+  LAUNCHED(c);
+  c->have_forces = true;
+  return ARCHE_OK;
+}
+
+}  // namespace
+
+// =============================================================================================
+// C ABI
+// =============================================================================================
+extern "C" int arche_scf_begin(arche_ctx *c, const double *d_pos) {
+  if (!c) return ARCHE_EINVAL;
+  return scf_begin(c, d_pos);
+}
+
+extern "C" int arche_scf_iter(arche_ctx *c, arche_result *h_out) {
+  if (!c) return ARCHE_EINVAL;
+  int rc = scf_iteration(c);
+  if (rc) return rc;
+  rc = read_scalars(c);
+  if (rc) return rc;
+  fill_result(c, h_out);
+  return ARCHE_OK;
+}
+
+extern "C" int arche_set_input_density(arche_ctx *c, const double *d_n) {
+  if (!c || !d_n) return ARCHE_EINVAL;
+  CK(cudaMemcpyAsync(c->n_i, d_n, c->ng * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  return input_density_to_g(c);
+}
+
+extern "C" int arche_scf_solve(arche_ctx *c, const double *d_pos, arche_result *h_out) {
+  if (!c) return ARCHE_EINVAL;
+  int rc = scf_solve(c, d_pos);
+  if (rc != ARCHE_OK && rc != ARCHE_ENOCONV) return rc;
+  int r2 = read_scalars(c);
+  if (r2) return r2;
+  fill_result(c, h_out);
+  return rc;
+}
+
+extern "C" int arche_forces(arche_ctx *c, double *d_F) {
+  if (!c) return ARCHE_EINVAL;
+  int rc = compute_forces(c);
+  if (rc) return rc;
+  if (d_F && c->nions > 0) CK(cudaMemcpyAsync(d_F, c->F, 3 * c->nions * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  return ARCHE_OK;
+}
+
+extern "C" int arche_md_step(arche_ctx *c, double dt, double *d_pos, double *d_vel, arche_result *h_out) {
+  if (!c || !d_pos || !d_vel || c->nions <= 0) return ARCHE_EINVAL;
+  const int ni = c->nions, nb = (3 * ni + 127) / 128;
+  int rc;
+  if (!c->have_forces) {  // forces at the starting positions
+    rc = scf_solve(c, d_pos);
+    if (rc != ARCHE_OK && rc != ARCHE_ENOCONV) return rc;
+    rc = compute_forces(c);
+    if (rc) return rc;
+  }
+  kick_drift_kernel<<<nb, 128, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, dt, ni, 1); LAUNCHED(c);
+  int rc_solve = scf_solve(c, d_pos);
+  if (rc_solve != ARCHE_OK && rc_solve != ARCHE_ENOCONV) return rc_solve;
+  rc = compute_forces(c);
+  if (rc) return rc;
+  kick_drift_kernel<<<nb, 128, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, dt, ni, 0); LAUNCHED(c);
+  kinetic_kernel<<<1, 256, 0, c->stream>>>(d_vel, c->mass, ni, c->sc); LAUNCHED(c);
+  rc = read_scalars(c);
+  if (rc) return rc;
+  fill_result(c, h_out);
+  return rc_solve;
+}
+
+extern "C" int arche_md_step_host(arche_ctx *c, double dt, double *h_pos, double *h_vel, double *h_F, arche_result *h_out) {
+  if (!c || !h_pos || !h_vel || c->nions <= 0) return ARCHE_EINVAL;
+  const size_t nb = 3 * (size_t)c->nions * sizeof(double);
+  // c->pos doubles as the device position buffer; velocities go through vel_tmp
+  CK(cudaMemcpyAsync(c->pos, h_pos, nb, cudaMemcpyHostToDevice, c->stream));
+  CK(cudaMemcpyAsync(c->vel_tmp, h_vel, nb, cudaMemcpyHostToDevice, c->stream));
+  int rc = arche_md_step(c, dt, c->pos, c->vel_tmp, h_out);
+  if (rc != ARCHE_OK && rc != ARCHE_ENOCONV) return rc;
+  CK(cudaMemcpyAsync(h_pos, c->pos, nb, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaMemcpyAsync(h_vel, c->vel_tmp, nb, cudaMemcpyDeviceToHost, c->stream));
+  if (h_F) CK(cudaMemcpyAsync(h_F, c->F, nb, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  return rc;
+}
+
+extern "C" int arche_get_real(arche_ctx *c, int which, double *d_dst) {
+  if (!c || !d_dst) return ARCHE_EINVAL;
+  const double *src = which == 0 ? c->n_a : which == 1 ? c->n_i : which == 2 ? c->V_i : nullptr;
+  if (!src) return ARCHE_EINVAL;
+  CK(cudaMemcpyAsync(d_dst, src, c->ng * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  return ARCHE_OK;
+}
+extern "C" int arche_get_complex(arche_ctx *c, int which, double *d_dst) {
+  if (!c || !d_dst) return ARCHE_EINVAL;
+  const double2 *src = which == 0 ? c->nh_a : which == 1 ? c->vh_ie : which == 2 ? c->S : which == 3 ? c->gh
+                       : which == 4 ? c->nh_i : nullptr;
+  if (!src) return ARCHE_EINVAL;
+  CK(cudaMemcpyAsync(d_dst, src, c->ng * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
+  return ARCHE_OK;
+}
+extern "C" int arche_get_density(arche_ctx *c, double *d_n) { return arche_get_real(c, 0, d_n); }
+
+extern "C" int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, double *d_scratch, int sign) {
+  if (!c || !d_in || !d_out || !d_scratch || (sign != 1 && sign != -1)) return ARCHE_EINVAL;
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  double2 *w = (double2 *)d_scratch, *o = (double2 *)d_out;
+  const double2 *in = (const double2 *)d_in;
+  if (sign < 0) {
+    CK((fft_launch_pass<0, false>(c->plan[0], nx, ny, nz, LoadComplex{in}, StoreComplex{w}, c->stream))); ++c->launches;
+    CK((fft_launch_pass<1, false>(c->plan[1], nx, ny, nz, LoadComplex{w}, StoreComplex{w}, c->stream))); ++c->launches;
+    CK((fft_launch_pass<2, false>(c->plan[2], nx, ny, nz, LoadComplex{w}, StoreComplex{o}, c->stream))); ++c->launches;
+  } else {
+    CK((fft_launch_pass<2, true>(c->plan[2], nx, ny, nz, LoadComplex{in}, StoreComplex{w}, c->stream))); ++c->launches;
+    CK((fft_launch_pass<1, true>(c->plan[1], nx, ny, nz, LoadComplex{w}, StoreComplex{w}, c->stream))); ++c->launches;
+    CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz, LoadComplex{w}, StoreComplex{o}, c->stream))); ++c->launches;
+  }
+  return ARCHE_OK;
+}
+
+extern "C" int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta, double *d_out, size_t n) {
+  if (!c || !d_eta || !d_out || (twice_j != -1 && twice_j != 1 && twice_j != 3)) return ARCHE_EINVAL;
+  if (n == 0) return ARCHE_OK;
+  int blocks = (int)((n + 255) / 256 < (size_t)kEwBlocks ? (n + 255) / 256 : kEwBlocks);
+  fermi_dirac_kernel<<<blocks, 256, 0, c->stream>>>(twice_j, d_eta, d_out, n, c->fdtab);
+  LAUNCHED(c);
+  return ARCHE_OK;
+}

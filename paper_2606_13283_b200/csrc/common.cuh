@@ -1,0 +1,104 @@
+// common.cuh -- shared device helpers of the B200 path (sm_100a, fp64).
+// Deterministic reductions: warp shuffles -> block partials -> the last-arriving block sums all block
+// partials in index order (fixed order => bit-reproducible; no fp64 atomics in any value path).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define ARCHE_PI 3.14159265358979323846264338327950288
+
+namespace arche {
+
+constexpr int kMaxRed = 8;        // max simultaneous sums per reduction
+constexpr int kRedBlocksMax = 2048;
+
+struct GridGeom {
+  int nx, ny, nz;
+  long long ng;
+  double Lx, Ly, Lz, vol, dV;
+  const double *kx, *ky, *kz;     // k components per storage index, device
+  const double *kx2, *ky2, *kz2;  // squares
+};
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_min(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+// op: 0 sum, 1 min, 2 max
+__device__ __forceinline__ double red_combine(double a, double b, int op) {
+  return op == 0 ? a + b : (op == 1 ? fmin(a, b) : fmax(a, b));
+}
+__device__ __forceinline__ double warp_red(double v, int op) {
+  return op == 0 ? warp_sum(v) : (op == 1 ? warp_min(v) : warp_max(v));
+}
+
+// Block-level reduction of NQ quantities; result valid in thread 0.  Block size <= 1024.
+template <int NQ>
+__device__ __forceinline__ void block_reduce(double (&v)[NQ], const int (&op)[NQ], double *smem /*[NQ*32]*/) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) {
+    double x = warp_red(v[q], op[q]);
+    if (lane == 0) smem[q * 32 + wid] = x;
+  }
+  __syncthreads();
+  if (wid == 0) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+      double ident = op[q] == 0 ? 0.0 : (op[q] == 1 ? 1.0e308 : -1.0e308);
+      double x = lane < nw ? smem[q * 32 + lane] : ident;
+      v[q] = warp_red(x, op[q]);
+    }
+  }
+  __syncthreads();
+}
+
+// Grid-level deterministic reduction.  Every block calls this once with its per-thread values.
+// partials: [gridDim.x * NQ]; counter: zero before the launch (reset by the last block);
+// returns true in ALL threads of the last block, with the totals in `out` (shared memory, [NQ]).
+template <int NQ>
+__device__ __forceinline__ bool grid_reduce(double (&v)[NQ], const int (&op)[NQ], double *partials,
+                                            unsigned int *counter, double *smem /*[NQ*32 + NQ]*/) {
+  block_reduce<NQ>(v, op, smem);
+  __shared__ bool s_last;
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) partials[(size_t)blockIdx.x * NQ + q] = v[q];
+    __threadfence();
+    unsigned int t = atomicAdd(counter, 1u);
+    s_last = (t == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!s_last) return false;
+  __threadfence();
+  // fixed-order sum over blocks: thread t takes blocks t, t+B, ... (order independent of which block is last)
+  double acc[NQ];
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) acc[q] = op[q] == 0 ? 0.0 : (op[q] == 1 ? 1.0e308 : -1.0e308);
+  for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = red_combine(acc[q], __ldcg(&partials[(size_t)b * NQ + q]), op[q]);
+  }
+  block_reduce<NQ>(acc, op, smem);
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) smem[NQ * 32 + q] = acc[q];
+    *counter = 0u;
+  }
+  __syncthreads();
+  return true;
+}
+
+}  // namespace arche

@@ -1,0 +1,250 @@
+// fft.cuh -- hand-written fp64 complex 3D FFT for sm_100a (no cuFFT anywhere on the product path).
+//
+// One kernel launch per axis.  A block owns a tile of L lines of length N of that axis:
+//   axis x: L consecutive x-lines (each line contiguous in memory);
+//   axis y/z: L consecutive x positions for a fixed z (or y): every global row of the tile is L*16 contiguous
+//             bytes, the "transpose" happens in shared memory ([i][l] layout, l fastest => conflict-free).
+// Inside the block: Stockham autosort radix-8/4/3/2 stages ping-ponging between two shared-memory buffers
+// (split re/im arrays so that every access is an 8-byte word).  Twiddles come from a per-axis table
+// exp(-2 pi i a/N) built on the host in long double.
+// The inverse transform uses the swap identity IDFT(x) = swap(DFT(swap(x))) (swap = exchange re and im), so only
+// forward butterflies exist.  Pointwise work is fused through LoadOp / StoreOp functors applied when a tile
+// is first read / last written (G-space Poisson + V_ie assembly, real-part + V_xc epilogue, reductions).
+#pragma once
+#include "common.cuh"
+
+namespace arche {
+
+constexpr int kFftThreads = 256;
+constexpr int kFftMaxStages = 12;
+
+struct FftAxisPlan {
+  int n;
+  int nstages;
+  int radix[kFftMaxStages];
+  const double2 *tw;  // device, [n], exp(-2 pi i a / n)
+};
+
+struct FftPass {
+  FftAxisPlan plan;
+  int nx, ny, nz;
+  int L;  // lines per block
+};
+
+struct Cplx { double re, im; };
+
+__device__ __forceinline__ void bfly2(Cplx &a, Cplx &b) {
+  Cplx t = {a.re - b.re, a.im - b.im};
+  a.re += b.re; a.im += b.im;
+  b = t;
+}
+// forward DFT-4 in place, natural order output
+__device__ __forceinline__ void dft4(Cplx &v0, Cplx &v1, Cplx &v2, Cplx &v3) {
+  Cplx a = {v0.re + v2.re, v0.im + v2.im}, b = {v0.re - v2.re, v0.im - v2.im};
+  Cplx c = {v1.re + v3.re, v1.im + v3.im}, d = {v1.re - v3.re, v1.im - v3.im};
+  v0 = {a.re + c.re, a.im + c.im};
+  v2 = {a.re - c.re, a.im - c.im};
+  v1 = {b.re + d.im, b.im - d.re};  // b - i d
+  v3 = {b.re - d.im, b.im + d.re};  // b + i d
+}
+__device__ __forceinline__ void dft3(Cplx &v0, Cplx &v1, Cplx &v2) {
+  const double h = 0.86602540378443864676372317075294;  // sqrt(3)/2
+  Cplx s = {v1.re + v2.re, v1.im + v2.im}, d = {v1.re - v2.re, v1.im - v2.im};
+  Cplx m = {v0.re - 0.5 * s.re, v0.im - 0.5 * s.im};
+  v0 = {v0.re + s.re, v0.im + s.im};
+  v1 = {m.re + h * d.im, m.im - h * d.re};
+  v2 = {m.re - h * d.im, m.im + h * d.re};
+}
+__device__ __forceinline__ void dft8(Cplx (&v)[8]) {
+  const double c = 0.70710678118654752440084436210485;
+  dft4(v[0], v[2], v[4], v[6]);
+  dft4(v[1], v[3], v[5], v[7]);
+  // odd part times W8^t
+  Cplx o1 = {c * (v[3].re + v[3].im), c * (v[3].im - v[3].re)};    // * (c, -c)
+  Cplx o2 = {v[5].im, -v[5].re};                                   // * (-i)
+  Cplx o3 = {c * (v[7].im - v[7].re), -c * (v[7].re + v[7].im)};   // * (-c, -c)
+  Cplx e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
+  v[0] = {e0.re + o0.re, e0.im + o0.im}; v[4] = {e0.re - o0.re, e0.im - o0.im};
+  v[1] = {e1.re + o1.re, e1.im + o1.im}; v[5] = {e1.re - o1.re, e1.im - o1.im};
+  v[2] = {e2.re + o2.re, e2.im + o2.im}; v[6] = {e2.re - o2.re, e2.im - o2.im};
+  v[3] = {e3.re + o3.re, e3.im + o3.im}; v[7] = {e3.re - o3.re, e3.im - o3.im};
+}
+
+template <int R, int AXIS>
+__device__ __forceinline__ void fft_stage(const double *__restrict__ sre, const double *__restrict__ sim,
+                                          double *__restrict__ dre, double *__restrict__ dim, int N, int Ns, int L,
+                                          const double2 *__restrict__ tw) {
+  const int nb = N / R;
+  const int twmul = N / (Ns * R);
+  for (int w = threadIdx.x; w < L * nb; w += blockDim.x) {
+    int l, j;
+    if (AXIS == 0) { j = w % nb; l = w / nb; } else { l = w % L; j = w / L; }
+    const int k = j % Ns;
+    Cplx v[R];
+#pragma unroll
+    for (int t = 0; t < R; ++t) {
+      const int i = j + t * nb;
+      const int a = (AXIS == 0) ? l * N + i : i * L + l;
+      v[t].re = sre[a]; v[t].im = sim[a];
+    }
+    if (Ns > 1) {
+#pragma unroll
+      for (int t = 1; t < R; ++t) {
+        const double2 wv = __ldg(&tw[t * k * twmul]);
+        const double re = v[t].re * wv.x - v[t].im * wv.y;
+        v[t].im = v[t].re * wv.y + v[t].im * wv.x;
+        v[t].re = re;
+      }
+    }
+    if (R == 2) bfly2(v[0], v[1]);
+    if (R == 3) dft3(v[0], v[1], v[2]);
+    if (R == 4) dft4(v[0], v[1], v[2], v[3]);
+    if (R == 8) dft8(reinterpret_cast<Cplx(&)[8]>(v));
+    const int j0 = (j - k) * R + k;
+#pragma unroll
+    for (int t = 0; t < R; ++t) {
+      const int i = j0 + t * Ns;
+      const int a = (AXIS == 0) ? l * N + i : i * L + l;
+      dre[a] = v[t].re; dim[a] = v[t].im;
+    }
+  }
+}
+
+// Plain complex array load / store functors.
+struct LoadComplex {
+  const double2 *src;
+  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
+    double2 v = src[idx]; re = v.x; im = v.y;
+  }
+};
+struct StoreComplex {
+  double2 *dst;
+  __device__ __forceinline__ void store(long long idx, int, int, int, double re, double im) { dst[idx] = make_double2(re, im); }
+  __device__ __forceinline__ void finish(double *) {}
+};
+
+template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, LoadOp ld, StoreOp st_in) {
+  extern __shared__ double smem[];
+  const int N = P.plan.n, L = P.L;
+  double *b0re = smem, *b0im = smem + (size_t)L * N, *b1re = smem + 2 * (size_t)L * N, *b1im = smem + 3 * (size_t)L * N;
+  StoreOp st = st_in;
+  // tile geometry
+  const long long nxny = (long long)P.nx * P.ny;
+  long long tile_base;
+  int fx = 0, fy = 0, fz = 0;  // fixed coordinates of the tile origin
+  if (AXIS == 0) {
+    long long line0 = (long long)blockIdx.x * L;  // line = iy + ny*iz
+    tile_base = line0 * P.nx;
+    fy = (int)(line0 % P.ny); fz = (int)(line0 / P.ny);
+  } else if (AXIS == 1) {
+    const int xt = P.nx / L;
+    fz = blockIdx.x / xt; fx = (blockIdx.x % xt) * L;
+    tile_base = fz * nxny + fx;
+  } else {
+    const int xt = P.nx / L;
+    fy = blockIdx.x / xt; fx = (blockIdx.x % xt) * L;
+    tile_base = (long long)fy * P.nx + fx;
+  }
+  const long long estride = AXIS == 0 ? 1 : (AXIS == 1 ? P.nx : nxny);
+  // ---- load tile
+  for (int e = threadIdx.x; e < L * N; e += blockDim.x) {
+    int l, i;
+    if (AXIS == 0) { i = e % N; l = e / N; } else { l = e % L; i = e / L; }
+    long long idx; int ix, iy, iz;
+    if (AXIS == 0) {
+      idx = tile_base + (long long)l * N + i;
+      ix = i; int ln = fy + l; iy = ln % P.ny; iz = fz + ln / P.ny;
+    } else if (AXIS == 1) {
+      idx = tile_base + i * estride + l; ix = fx + l; iy = i; iz = fz;
+    } else {
+      idx = tile_base + i * estride + l; ix = fx + l; iy = fy; iz = i;
+    }
+    double re, im;
+    ld(idx, ix, iy, iz, re, im);
+    const int a = (AXIS == 0) ? l * N + i : i * L + l;
+    if (INVERSE) { b0re[a] = im; b0im[a] = re; } else { b0re[a] = re; b0im[a] = im; }
+  }
+  __syncthreads();
+  // ---- Stockham stages
+  double *sre = b0re, *sim = b0im, *dre = b1re, *dim = b1im;
+  int Ns = 1;
+  for (int s = 0; s < P.plan.nstages; ++s) {
+    const int R = P.plan.radix[s];
+    if (R == 8) fft_stage<8, AXIS>(sre, sim, dre, dim, N, Ns, L, P.plan.tw);
+    else if (R == 4) fft_stage<4, AXIS>(sre, sim, dre, dim, N, Ns, L, P.plan.tw);
+    else if (R == 3) fft_stage<3, AXIS>(sre, sim, dre, dim, N, Ns, L, P.plan.tw);
+    else fft_stage<2, AXIS>(sre, sim, dre, dim, N, Ns, L, P.plan.tw);
+    __syncthreads();
+    double *t;
+    t = sre; sre = dre; dre = t;
+    t = sim; sim = dim; dim = t;
+    Ns *= R;
+  }
+  // ---- store tile
+  for (int e = threadIdx.x; e < L * N; e += blockDim.x) {
+    int l, i;
+    if (AXIS == 0) { i = e % N; l = e / N; } else { l = e % L; i = e / L; }
+    long long idx; int ix, iy, iz;
+    if (AXIS == 0) {
+      idx = tile_base + (long long)l * N + i;
+      ix = i; int ln = fy + l; iy = ln % P.ny; iz = fz + ln / P.ny;
+    } else if (AXIS == 1) {
+      idx = tile_base + i * estride + l; ix = fx + l; iy = i; iz = fz;
+    } else {
+      idx = tile_base + i * estride + l; ix = fx + l; iy = fy; iz = i;
+    }
+    const int a = (AXIS == 0) ? l * N + i : i * L + l;
+    if (INVERSE) st.store(idx, ix, iy, iz, sim[a], sre[a]); else st.store(idx, ix, iy, iz, sre[a], sim[a]);
+  }
+  __syncthreads();
+  st.finish(smem);
+}
+
+// ---- host side ------------------------------------------------------------------------------
+static inline bool fft_make_plan(int n, const double2 *d_tw, FftAxisPlan *p) {
+  p->n = n; p->tw = d_tw; p->nstages = 0;
+  int m = n;
+  // radix-3 factors first (small Ns => no twiddles on the odd radix), then 8s, then the 4/2 remainder
+  while (m % 3 == 0) { p->radix[p->nstages++] = 3; m /= 3; }
+  while (m % 8 == 0) { p->radix[p->nstages++] = 8; m /= 8; }
+  if (m % 4 == 0) { p->radix[p->nstages++] = 4; m /= 4; }
+  if (m % 2 == 0) { p->radix[p->nstages++] = 2; m /= 2; }
+  return m == 1 && p->nstages <= kFftMaxStages;
+}
+
+static inline int fft_pick_L(int axis, int n, int nx, int ny, int nz) {
+  const int max_elems = 3072;  // 4 arrays * 8 B * L*N <= 96 KB
+  if (axis == 0) {
+    long long lines = (long long)ny * nz;
+    int L = 1;
+    while (L * 2 * n <= max_elems && lines % (L * 2) == 0 && L < 64) L *= 2;
+    return L;
+  }
+  int L = 1;
+  while (L * 2 * n <= max_elems && nx % (L * 2) == 0 && L < 16) L *= 2;
+  return L;
+}
+
+template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
+static inline cudaError_t fft_launch_pass(const FftAxisPlan &plan, int nx, int ny, int nz, LoadOp ld, StoreOp st,
+                                          cudaStream_t stream, int *blocks_out = nullptr) {
+  FftPass P;
+  P.plan = plan; P.nx = nx; P.ny = ny; P.nz = nz;
+  P.L = fft_pick_L(AXIS, plan.n, nx, ny, nz);
+  long long blocks = AXIS == 0 ? (long long)ny * nz / P.L : (AXIS == 1 ? (long long)nz * (nx / P.L) : (long long)ny * (nx / P.L));
+  size_t smem = 4 * sizeof(double) * (size_t)P.L * plan.n;
+  if (smem < 1024) smem = 1024;  // room for the reduction scratch used by StoreOp::finish
+  auto kern = fft_pass_kernel<AXIS, INVERSE, LoadOp, StoreOp>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  if (blocks_out) *blocks_out = (int)blocks;
+  kern<<<(unsigned)blocks, kFftThreads, smem, stream>>>(P, ld, st);
+  return cudaGetLastError();
+}
+
+}  // namespace arche

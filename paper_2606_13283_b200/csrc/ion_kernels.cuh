@@ -1,0 +1,249 @@
+// ion_kernels.cuh -- per-MD-step ion-grid work: separable phase tables, structure factor S_Z(k),
+// ionic potential, Ewald, G-space forces, velocity Verlet.
+// The O(N_i N_g) sums are tiled through shared memory and run on the fp64 FMA pipe (not tensor-core work).
+#pragma once
+#include "common.cuh"
+#include "scf_kernels.cuh"
+
+namespace arche {
+
+// exp(-2 pi i m(i) x_j / L) for every storage index i of one axis and every ion j.
+// tab_ij: [i][j] (j fastest); tab_ji: [j][i] (i fastest, optional).
+__global__ void phase_table_kernel(const double *__restrict__ pos, int comp, double L, int N, int nions,
+                                   double2 *__restrict__ tab_ij, double2 *__restrict__ tab_ji) {
+  const long long tot = (long long)N * nions;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < tot; e += (long long)gridDim.x * blockDim.x) {
+    const int j = (int)(e % nions), i = (int)(e / nions);
+    const int m = i <= N / 2 ? i : i - N;
+    double f = pos[3 * j + comp] / L;
+    f -= floor(f);
+    double t = (double)m * f;
+    t -= rint(t);
+    double s, c;
+    sincospi(-2.0 * t, &s, &c);
+    tab_ij[e] = make_double2(c, s);
+    if (tab_ji) tab_ji[(long long)j * N + i] = make_double2(c, s);
+  }
+}
+
+// reciprocal-space form factors that depend only on the cell: Ashcroft v(k) = -cos(2 pi k rc)/(pi k^2) (per unit
+// charge, 0 at k=0) and the Ewald kernel V_alpha(k) = exp(-(pi k/alpha)^2)/(pi k^2) (Eq. 43).
+__global__ void form_factor_kernel(GridGeom G, double rc, double alpha, double *__restrict__ vps, double *__restrict__ va) {
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < G.ng; g += (long long)gridDim.x * blockDim.x) {
+    const int ix = (int)(g % G.nx), iy = (int)((g / G.nx) % G.ny), iz = (int)(g / ((long long)G.nx * G.ny));
+    const double k2 = G.kx2[ix] + G.ky2[iy] + G.kz2[iz];
+    if (k2 == 0.0) { vps[g] = 0.0; va[g] = 0.0; continue; }
+    const double k = sqrt(k2);
+    vps[g] = -cospi(2.0 * k * rc) / (ARCHE_PI * k2);
+    va[g] = exp(-ARCHE_PI * ARCHE_PI * k2 / (alpha * alpha)) / (ARCHE_PI * k2);
+  }
+}
+
+// S_Z(k) = sum_j Z_j a_j(kx) b_j(ky) c_j(kz).  A block owns SF_ROWS (ky,kz) rows and a chunk of kx; the ion sum is
+// tiled: d_j = Z_j b_j c_j for SF_JT ions of every row is staged in shared memory, a_j(kx) streams coalesced.
+// Epilogue: Vhat_ie = v(k) S (Eq. 14) and the Ewald reciprocal energy sum of Eq. 42.
+constexpr int SF_ROWS = 4;
+constexpr int SF_JT = 128;
+constexpr int SF_THREADS = 128;
+__global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
+    GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ji /*[j][ix]*/,
+    const double2 *__restrict__ by_ij /*[iy][j]*/, const double2 *__restrict__ cz_ij /*[iz][j]*/,
+    const double *__restrict__ vps, const double *__restrict__ va, double2 *__restrict__ S, double2 *__restrict__ vh_ie,
+    double *partials, unsigned int *counter, DevScalars *sc) {
+  __shared__ double2 s_d[SF_ROWS][SF_JT];
+  __shared__ double s_red[32 + 1];
+  const long long nrows = (long long)G.ny * G.nz;
+  const long long row0 = (long long)blockIdx.x * SF_ROWS;
+  const int ix = blockIdx.y * SF_THREADS + threadIdx.x;
+  double2 acc[SF_ROWS];
+#pragma unroll
+  for (int r = 0; r < SF_ROWS; ++r) acc[r] = make_double2(0.0, 0.0);
+  for (int j0 = 0; j0 < nions; j0 += SF_JT) {
+    __syncthreads();
+    for (int e = threadIdx.x; e < SF_ROWS * SF_JT; e += SF_THREADS) {
+      const int r = e / SF_JT, jj = e % SF_JT, j = j0 + jj;
+      const long long row = row0 + r;
+      double2 d = make_double2(0.0, 0.0);
+      if (j < nions && row < nrows) {
+        const int iy = (int)(row % G.ny), iz = (int)(row / G.ny);
+        const double2 b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
+        const double z = Z[j];
+        d = make_double2(z * (b.x * c.x - b.y * c.y), z * (b.x * c.y + b.y * c.x));
+      }
+      s_d[r][jj] = d;
+    }
+    __syncthreads();
+    if (ix < G.nx) {
+      const int jn = min(SF_JT, nions - j0);
+      for (int jj = 0; jj < jn; ++jj) {
+        const double2 a = ax_ji[(long long)(j0 + jj) * G.nx + ix];
+#pragma unroll
+        for (int r = 0; r < SF_ROWS; ++r) {
+          const double2 d = s_d[r][jj];
+          acc[r].x = fma(a.x, d.x, fma(-a.y, d.y, acc[r].x));
+          acc[r].y = fma(a.x, d.y, fma(a.y, d.x, acc[r].y));
+        }
+      }
+    }
+  }
+  double epm = 0.0;
+  if (ix < G.nx) {
+#pragma unroll
+    for (int r = 0; r < SF_ROWS; ++r) {
+      const long long row = row0 + r;
+      if (row < nrows) {
+        const long long g = row * G.nx + ix;
+        S[g] = acc[r];
+        const double v = vps[g];
+        vh_ie[g] = make_double2(v * acc[r].x, v * acc[r].y);
+        epm += va[g] * (acc[r].x * acc[r].x + acc[r].y * acc[r].y);
+      }
+    }
+  }
+  // deterministic grid sum of the Ewald reciprocal term (2D grid flattened)
+  double v[1] = {epm};
+  const int op[1] = {0};
+  // grid_reduce uses blockIdx.x/gridDim.x: emulate a flat grid
+  block_reduce<1>(v, op, s_red);
+  __shared__ bool s_last;
+  const unsigned int nblk = gridDim.x * gridDim.y, bid = blockIdx.y * gridDim.x + blockIdx.x;
+  if (threadIdx.x == 0) {
+    partials[bid] = v[0];
+    __threadfence();
+    s_last = (atomicAdd(counter, 1u) == nblk - 1);
+  }
+  __syncthreads();
+  if (s_last) {
+    __threadfence();
+    double a = 0.0;
+    for (unsigned int b = threadIdx.x; b < nblk; b += blockDim.x) a += __ldcg(&partials[b]);
+    double w[1] = {a};
+    block_reduce<1>(w, op, s_red);
+    if (threadIdx.x == 0) { sc->U_pm_sum = w[0]; *counter = 0u; }
+  }
+}
+
+// Ewald short-range part (Eq. 41, 46) with the minimum-image convention: one block per ion j.
+__global__ void __launch_bounds__(128) ewald_pp_kernel(const double *__restrict__ pos, const double *__restrict__ Z,
+                                                       int nions, double Lx, double Ly, double Lz, double alpha,
+                                                       double *__restrict__ F_pp, double *__restrict__ e_pp) {
+  __shared__ double s_red[4 * 32];
+  const int j = blockIdx.x;
+  const double xj = pos[3 * j], yj = pos[3 * j + 1], zj = pos[3 * j + 2], zq = Z[j];
+  double fx = 0, fy = 0, fz = 0, en = 0;
+  const double two_a_sqrtpi = 2.0 * alpha * 0.56418958354775628695;
+  for (int k = threadIdx.x; k < nions; k += blockDim.x) {
+    if (k == j) continue;
+    double dx = xj - pos[3 * k], dy = yj - pos[3 * k + 1], dz = zj - pos[3 * k + 2];
+    dx -= Lx * rint(dx / Lx); dy -= Ly * rint(dy / Ly); dz -= Lz * rint(dz / Lz);
+    const double r2 = dx * dx + dy * dy + dz * dz, r = sqrt(r2);
+    const double e = erfc(alpha * r) / r;
+    const double q = zq * Z[k];
+    en += 0.5 * q * e;
+    const double fr = q * (e + two_a_sqrtpi * exp(-alpha * alpha * r2)) / r2;
+    fx += fr * dx; fy += fr * dy; fz += fr * dz;
+  }
+  double v[4] = {fx, fy, fz, en};
+  const int op[4] = {0, 0, 0, 0};
+  block_reduce<4>(v, op, s_red);
+  if (threadIdx.x == 0) { F_pp[3 * j] = v[0]; F_pp[3 * j + 1] = v[1]; F_pp[3 * j + 2] = v[2]; e_pp[j] = v[3]; }
+}
+
+// U_ii = U_pp + U_pm + U_je (Eq. 40-44); single block, fixed order.
+__global__ void __launch_bounds__(256) ewald_finish_kernel(const double *__restrict__ e_pp, const double *__restrict__ Z,
+                                                           int nions, double alpha, double vol, DevScalars *sc) {
+  __shared__ double s_red[3 * 32];
+  double a = 0, q = 0, q2 = 0;
+  for (int j = threadIdx.x; j < nions; j += blockDim.x) { a += e_pp[j]; q += Z[j]; q2 += Z[j] * Z[j]; }
+  double v[3] = {a, q, q2};
+  const int op[3] = {0, 0, 0};
+  block_reduce<3>(v, op, s_red);
+  if (threadIdx.x == 0) {
+    const double upm = 0.5 * sc->U_pm_sum / vol - alpha * 0.56418958354775628695 * v[2];
+    const double uje = -ARCHE_PI * v[1] * v[1] / (2.0 * alpha * alpha * vol);
+    sc->U_pp = v[0];
+    sc->U_ii = v[0] + upm + uje;
+  }
+}
+
+// Forces.  F_j = -(2 pi/|Omega|) Z_j sum_k k Im( W(k) exp(-2 pi i k.r_j) ),
+//   W(k) = v(k) conj(nhat_a(k)) + V_alpha(k) conj(S_Z(k))   [electron-ion Eq. 56 + Ewald reciprocal Eq. 47].
+// Block = FC_THREADS ions x one slab of (ky,kz) rows; W rows are staged in shared memory.
+constexpr int FC_THREADS = 128;
+constexpr int FC_NXMAX = 1024;
+__global__ void __launch_bounds__(FC_THREADS) force_kernel(
+    GridGeom G, int nions, int rows_per_slab, const double2 *__restrict__ ax_ij /*[ix][j]*/,
+    const double2 *__restrict__ by_ij, const double2 *__restrict__ cz_ij, const double *__restrict__ vps,
+    const double *__restrict__ va, const double2 *__restrict__ nh_a, const double2 *__restrict__ S,
+    double *__restrict__ F_part /*[slab][j][3]*/) {
+  extern __shared__ double2 s_w[];  // [2][nx]: W and kx*W
+  double2 *s_W = s_w, *s_kW = s_w + G.nx;
+  const int j = blockIdx.x * FC_THREADS + threadIdx.x;
+  const long long nrows = (long long)G.ny * G.nz;
+  const long long r0 = (long long)blockIdx.y * rows_per_slab;
+  const long long r1 = min(nrows, r0 + rows_per_slab);
+  double fx = 0, fy = 0, fz = 0;
+  for (long long row = r0; row < r1; ++row) {
+    const int iy = (int)(row % G.ny), iz = (int)(row / G.ny);
+    __syncthreads();
+    for (int ix = threadIdx.x; ix < G.nx; ix += FC_THREADS) {
+      const long long g = row * G.nx + ix;
+      const double2 n = nh_a[g], s = S[g];
+      const double v = vps[g], a = va[g];
+      const double2 w = make_double2(v * n.x + a * s.x, -(v * n.y + a * s.y));
+      s_W[ix] = w;
+      const double kx = G.kx[ix];
+      s_kW[ix] = make_double2(kx * w.x, kx * w.y);
+    }
+    __syncthreads();
+    if (j < nions) {
+      double2 P = make_double2(0, 0), Q = make_double2(0, 0);
+      for (int ix = 0; ix < G.nx; ++ix) {
+        const double2 a = ax_ij[(long long)ix * nions + j];
+        const double2 w = s_W[ix], kw = s_kW[ix];
+        P.x = fma(w.x, a.x, fma(-w.y, a.y, P.x)); P.y = fma(w.x, a.y, fma(w.y, a.x, P.y));
+        Q.x = fma(kw.x, a.x, fma(-kw.y, a.y, Q.x)); Q.y = fma(kw.x, a.y, fma(kw.y, a.x, Q.y));
+      }
+      const double2 b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
+      const double2 bc = make_double2(b.x * c.x - b.y * c.y, b.x * c.y + b.y * c.x);
+      const double imP = P.x * bc.y + P.y * bc.x, imQ = Q.x * bc.y + Q.y * bc.x;
+      fx += imQ; fy += G.ky[iy] * imP; fz += G.kz[iz] * imP;
+    }
+  }
+  if (j < nions) {
+    double *o = F_part + ((size_t)blockIdx.y * nions + j) * 3;
+    o[0] = fx; o[1] = fy; o[2] = fz;
+  }
+}
+
+__global__ void force_finish_kernel(int nions, int nslabs, const double *__restrict__ F_part, const double *__restrict__ F_pp,
+                                    const double *__restrict__ Z, double pref /* -2 pi/|Omega| */, double *__restrict__ F) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= 3 * nions) return;
+  double a = 0.0;
+  for (int s = 0; s < nslabs; ++s) a += F_part[(size_t)s * nions * 3 + e];
+  F[e] = pref * Z[e / 3] * a + F_pp[e];
+}
+
+// velocity Verlet pieces (reading D2)
+__global__ void kick_drift_kernel(double *__restrict__ pos, double *__restrict__ vel, const double *__restrict__ F,
+                                  const double *__restrict__ mass, double dt, int nions, int drift) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= 3 * nions) return;
+  const double v = vel[e] + 0.5 * dt * F[e] / mass[e / 3];
+  vel[e] = v;
+  if (drift) pos[e] += dt * v;
+}
+
+__global__ void __launch_bounds__(256) kinetic_kernel(const double *__restrict__ vel, const double *__restrict__ mass,
+                                                      int nions, DevScalars *sc) {
+  __shared__ double s_red[32];
+  double a = 0.0;
+  for (int e = threadIdx.x; e < 3 * nions; e += blockDim.x) a += 0.5 * mass[e / 3] * vel[e] * vel[e];  // Eq. 36
+  double v[1] = {a};
+  const int op[1] = {0};
+  block_reduce<1>(v, op, s_red);
+  if (threadIdx.x == 0) sc->K_i = v[0];
+}
+
+}  // namespace arche

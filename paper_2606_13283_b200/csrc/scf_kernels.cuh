@@ -1,0 +1,327 @@
+// scf_kernels.cuh -- SCF-iteration kernels and the functors fused into the FFT passes.
+// Steps S1..S7 of DESIGN.md: potential assembly in G-space, real-part + V_xc epilogue,
+// device-side Newton-in-bracket for mu (Eq. 19), density + local reductions, G-space reductions, mixing.
+#pragma once
+#include "common.cuh"
+#include "fd.cuh"
+#include "fft.cuh"
+
+namespace arche {
+
+// All scalars of one solve live in this device struct; the host reads it back once per SCF iteration.
+struct DevScalars {
+  // S2 epilogue
+  double vmin, vmax, vsum;
+  // S3 state
+  double mu, mu_lo, mu_hi, N_last, dNdmu_last;
+  int mu_done, mu_evals, mu_have_prev, pad0;
+  // S4
+  double K, dn2, na2, F0, Ke, Exc;
+  // S5
+  double U, EH, Eie;
+  // S6/S7
+  double w, F_total, F_prev, dn_rel;
+  int iter, converged, mu_evals_total, pad1;
+  // per-MD-step
+  double U_pp, U_pm_sum, U_ii, init_sum, init_scale, K_i;
+};
+
+struct ScfConst {
+  double kT, cTF, Ne, vol, dV, eta0, E_ie0;
+  int xc, mix_mode, mix_warmup, pad;
+  double mix_w_fixed, tol_F, tol_dn;
+};
+
+// Perdew-Zunger 1981 LDA (unpolarised), Hartree units; restated from the publication (reading D5).
+__device__ __forceinline__ void xc_pz81(double n, double &eps, double &v) {
+  if (!(n > 0.0)) { eps = 0.0; v = 0.0; return; }
+  const double cx = 0.73855876638202240588;  // (3/4) (3/pi)^(1/3)
+  const double n13 = cbrt(n);
+  const double ex = -cx * n13;
+  const double rs = 0.62035049089940001667 / n13;  // (3/(4 pi))^(1/3) n^(-1/3)
+  double ec, vc;
+  if (rs >= 1.0) {
+    const double g = -0.1423, b1 = 1.0529, b2 = 0.3334;
+    const double sq = sqrt(rs), den = 1.0 + b1 * sq + b2 * rs;
+    ec = g / den;
+    vc = ec * (1.0 + (7.0 / 6.0) * b1 * sq + (4.0 / 3.0) * b2 * rs) / den;
+  } else {
+    const double A = 0.0311, B = -0.048, C = 0.0020, D = -0.0116;
+    const double l = log(rs);
+    ec = A * l + B + C * rs * l + D * rs;
+    vc = A * l + (B - A / 3.0) + (2.0 / 3.0) * C * rs * l + (2.0 * D - C) / 3.0 * rs;
+  }
+  eps = ex + ec;
+  v = (4.0 / 3.0) * ex + vc;
+}
+
+// ---- S1: Vhat(k) = nhat_i(k)/(pi k^2) + Vhat_ie(k), 0 at k = 0 (Eq. 12, 14) ------------------------------
+struct LoadPotentialG {
+  const double2 *nh_i, *vh_ie;
+  const double *kx2, *ky2, *kz2;
+  __device__ __forceinline__ void operator()(long long idx, int ix, int iy, int iz, double &re, double &im) const {
+    const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
+    if (k2 == 0.0) { re = 0.0; im = 0.0; return; }
+    const double inv = 1.0 / (ARCHE_PI * k2);
+    const double2 a = nh_i[idx], b = vh_ie[idx];
+    re = fma(a.x, inv, b.x); im = fma(a.y, inv, b.y);
+  }
+};
+
+// ---- S2: V_i = Re(IFFT)/|Omega| + V_xc(n_i); min/max/sum of V_i; the last block opens the mu bracket ------
+struct StoreVi {
+  double *V_i;
+  const double *n_i;
+  DevScalars *sc;
+  double *partials;
+  unsigned int *counter;
+  double inv_vol, kT_eta0;
+  int xc;
+  double acc_min, acc_max, acc_sum;
+  __device__ __forceinline__ void store(long long idx, int, int, int, double re, double) {
+    double v = re * inv_vol;
+    if (xc) { double e, vx; xc_pz81(n_i[idx], e, vx); v += vx; }
+    V_i[idx] = v;
+    acc_min = fmin(acc_min, v); acc_max = fmax(acc_max, v); acc_sum += v;
+  }
+  __device__ __forceinline__ void finish(double *smem) {
+    double v[3] = {acc_min, acc_max, acc_sum};
+    const int op[3] = {1, 2, 0};
+    if (grid_reduce<3>(v, op, partials, counter, smem) && threadIdx.x == 0) {
+      const double *t = smem + 3 * 32;
+      sc->vmin = t[0]; sc->vmax = t[1]; sc->vsum = t[2];
+      // bracket of the root of Eq. 19: N(mu) is increasing and eta0 solves the flat-potential problem
+      const double lo = t[0] + kT_eta0, hi = t[1] + kT_eta0;
+      const double pad = 1e-12 * (fabs(lo) + fabs(hi) + fabs(kT_eta0));
+      sc->mu_lo = lo - pad; sc->mu_hi = hi + pad;
+      sc->mu_done = 0; sc->mu_evals = 0;
+    }
+  }
+};
+
+// first guess of mu once the bracket is known (separate tiny kernel keeps StoreVi free of grid-size knowledge)
+__global__ void mu_guess_kernel(DevScalars *sc, double ng, double kT_eta0) {
+  double mu0 = sc->mu_have_prev ? sc->mu : sc->vsum / ng + kT_eta0;  // reading D1
+  if (!(mu0 > sc->mu_lo && mu0 < sc->mu_hi)) mu0 = 0.5 * (sc->mu_lo + sc->mu_hi);
+  if (sc->mu_hi - sc->mu_lo <= 4e-16 * fmax(fabs(sc->mu_lo), fabs(sc->mu_hi))) {
+    mu0 = 0.5 * (sc->mu_lo + sc->mu_hi); sc->mu_done = 1;  // flat potential: the bracket is the answer
+  }
+  sc->mu = mu0;
+}
+
+// ---- S3: one Newton-in-bracket pass: N(mu) and dN/dmu over the grid; the last block updates mu -----------
+__global__ void __launch_bounds__(256) mu_pass_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
+                                                      DevScalars *sc, const double *__restrict__ fdtab,
+                                                      double *partials, unsigned int *counter, int last_pass) {
+  __shared__ double s_tab[kFdTabDoubles];
+  __shared__ double s_red[2 * 32 + 2];
+  if (sc->mu_done) return;
+  fd_load_tables(s_tab, fdtab);
+  __syncthreads();
+  const double mu = sc->mu, inv_kT = 1.0 / C.kT;
+  double s1 = 0.0, s0 = 0.0;
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
+    double im12, i12, d;
+    fd_eval<3>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
+    s1 += i12; s0 += im12;
+  }
+  double v[2] = {s1, s0};
+  const int op[2] = {0, 0};
+  if (grid_reduce<2>(v, op, partials, counter, s_red) && threadIdx.x == 0) {
+    const double N = C.cTF * C.dV * s_red[64], dN = C.cTF * C.dV * 0.5 * s_red[65] * inv_kT;
+    const double f = N - C.Ne;
+    sc->N_last = N; sc->dNdmu_last = dN;
+    sc->mu_evals += 1; sc->mu_evals_total += 1;
+    double lo = sc->mu_lo, hi = sc->mu_hi;
+    if (fabs(f) <= 1e-14 * C.Ne || last_pass) {
+      sc->mu_done = 1;
+    } else {
+      if (f > 0.0) hi = mu; else lo = mu;
+      double mu_new = mu - f / dN;
+      if (!(mu_new > lo && mu_new < hi)) mu_new = 0.5 * (lo + hi);
+      if (fabs(mu_new - mu) <= 2e-16 * fmax(fabs(mu), C.kT)) sc->mu_done = 1;
+      sc->mu_lo = lo; sc->mu_hi = hi; sc->mu = mu_new;
+      if (sc->mu_done) sc->mu = mu;  // keep the evaluated point
+    }
+  }
+}
+
+// ---- S4: n_a, chi, Delta n and the local reductions K, ||dn||^2, ||n_a||^2, F0, K_e, E_xc ------------------
+__global__ void __launch_bounds__(256) density_kernel(const double *__restrict__ V_i, const double *__restrict__ n_i,
+                                                      double *__restrict__ n_a, long long ng, ScfConst C,
+                                                      DevScalars *sc, const double *__restrict__ fdtab,
+                                                      double *partials, unsigned int *counter) {
+  __shared__ double s_tab[kFdTabDoubles];
+  __shared__ double s_red[6 * 32 + 6];
+  fd_load_tables(s_tab, fdtab);
+  __syncthreads();
+  const double mu = sc->mu, inv_kT = 1.0 / C.kT;
+  double sK = 0, sdn2 = 0, sna2 = 0, sF0 = 0, sKe = 0, sExc = 0;
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
+    const double eta = (mu - V_i[g]) * inv_kT;
+    double im12, i12, i32;
+    fd_eval<7>(s_tab, eta, im12, i12, i32);
+    const double na = C.cTF * i12;                    // Eq. 9
+    const double chi = C.cTF * 0.5 * im12 * inv_kT;   // dn_a/dmu
+    const double dn = n_i[g] - na;
+    n_a[g] = na;
+    if (chi > 0.0) sK += dn * dn / chi;               // Eq. 31
+    sdn2 += dn * dn; sna2 += na * na;
+    sF0 += eta * i12 - (2.0 / 3.0) * i32;             // f_0/(kT cTF), from Eq. 38-39
+    sKe += i32;                                       // Eq. 38
+    if (C.xc) { double e, vx; xc_pz81(na, e, vx); sExc += na * e; }
+  }
+  double v[6] = {sK, sdn2, sna2, sF0, sKe, sExc};
+  const int op[6] = {0, 0, 0, 0, 0, 0};
+  if (grid_reduce<6>(v, op, partials, counter, s_red) && threadIdx.x == 0) {
+    const double *t = s_red + 6 * 32;
+    sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
+    sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
+  }
+}
+
+// ---- S5: forward FFT of the real n_a; epilogue scales by dV, stores nhat_a, reduces U, E_H, E_ie ----------
+struct LoadReal {
+  const double *src;
+  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
+    re = src[idx]; im = 0.0;
+  }
+};
+
+struct StoreNhatA {
+  double2 *nh_a;
+  const double2 *nh_i, *vh_ie;
+  const double *kx2, *ky2, *kz2;
+  DevScalars *sc;
+  double *partials;
+  unsigned int *counter;
+  ScfConst C;
+  double aU, aEH, aEie;
+  __device__ __forceinline__ void store(long long idx, int ix, int iy, int iz, double re, double im) {
+    re *= C.dV; im *= C.dV;
+    nh_a[idx] = make_double2(re, im);
+    const double2 b = vh_ie[idx];
+    aEie += re * b.x + im * b.y;                       // Re conj(nhat_a) Vhat_ie
+    const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
+    if (k2 != 0.0) {
+      const double inv = 1.0 / (ARCHE_PI * k2);
+      const double2 a = nh_i[idx];
+      const double dr = a.x - re, di = a.y - im;
+      aU += (dr * dr + di * di) * inv;                 // Eq. 30
+      aEH += (re * re + im * im) * inv;                // Eq. 53
+    }
+  }
+  __device__ __forceinline__ void finish(double *smem) {
+    double v[3] = {aU, aEH, aEie};
+    const int op[3] = {0, 0, 0};
+    if (grid_reduce<3>(v, op, partials, counter, smem) && threadIdx.x == 0) {
+      const double *t = smem + 3 * 32;
+      const double U = t[0] / C.vol, EH = 0.5 * t[1] / C.vol, Eie = t[2] / C.vol;
+      sc->U = U; sc->EH = EH; sc->Eie = Eie;
+      const int it = sc->iter + 1;
+      const double K = sc->K;
+      double w;
+      if (C.mix_mode == 1 && it > C.mix_warmup) w = (K + U > 0.0) ? U / (K + U) : 0.0;   // w = U/(K+U)
+      else w = C.mix_w_fixed;
+      const double F = sc->F0 + sc->Exc + EH + Eie + C.E_ie0 + sc->U_ii;
+      const double dn_rel = sqrt(sc->dn2 / sc->na2);
+      sc->converged = (it >= 2 && fabs(F - sc->F_total) < C.tol_F && dn_rel < C.tol_dn) ? 1 : 0;
+      sc->F_prev = sc->F_total; sc->F_total = F; sc->w = w; sc->dn_rel = dn_rel; sc->iter = it;
+      sc->mu_have_prev = 1;
+    }
+  }
+};
+
+// ---- S6: n_o = n_a + w (n_i - n_a) in real and reciprocal space --------------------------------
+__global__ void __launch_bounds__(256) mix_kernel(double *__restrict__ n_i, const double *__restrict__ n_a,
+                                                  double2 *__restrict__ nh_i, const double2 *__restrict__ nh_a,
+                                                  long long ng, const DevScalars *sc) {
+  const double w = sc->w;
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
+    const double na = n_a[g];
+    n_i[g] = fma(w, n_i[g] - na, na);
+    const double2 a = nh_a[g], b = nh_i[g];
+    nh_i[g] = make_double2(fma(w, b.x - a.x, a.x), fma(w, b.y - a.y, a.y));
+  }
+}
+
+// ---- input density: uniform or one-center profile (reading A10) ------------------------
+__global__ void set_uniform_kernel(double *n_i, double2 *nh_i, long long ng, double n0, double Ne) {
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
+    n_i[g] = n0;
+    nh_i[g] = make_double2(g == 0 ? Ne : 0.0, 0.0);
+  }
+}
+
+// ghat = nhat_a conj(S)/max(|S|^2, eps Q^2)
+__global__ void g_store_kernel(double2 *__restrict__ gh, const double2 *__restrict__ nh_a, const double2 *__restrict__ S,
+                               long long ng, double epsS) {
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
+    const double2 s = S[g], a = nh_a[g];
+    const double inv = 1.0 / fmax(s.x * s.x + s.y * s.y, epsS);
+    gh[g] = make_double2((a.x * s.x + a.y * s.y) * inv, (a.y * s.x - a.x * s.y) * inv);
+  }
+}
+
+struct LoadSG {  // nhat_i = S_Z^{new} ghat^{old} (Eq. 20)
+  const double2 *S, *gh;
+  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
+    const double2 s = S[idx], g = gh[idx];
+    re = s.x * g.x - s.y * g.y; im = s.x * g.y + s.y * g.x;
+  }
+};
+
+struct StoreClip {  // n_i = max(Re/|Omega|, floor), accumulates sum n_i
+  double *n_i;
+  DevScalars *sc;
+  double *partials;
+  unsigned int *counter;
+  double inv_vol, floor_n, Ne, dV, acc;
+  __device__ __forceinline__ void store(long long idx, int, int, int, double re, double) {
+    double v = fmax(re * inv_vol, floor_n);
+    n_i[idx] = v; acc += v;
+  }
+  __device__ __forceinline__ void finish(double *smem) {
+    double v[1] = {acc};
+    const int op[1] = {0};
+    if (grid_reduce<1>(v, op, partials, counter, smem) && threadIdx.x == 0) {
+      sc->init_sum = smem[32] * dV;
+      sc->init_scale = Ne / (smem[32] * dV);
+    }
+  }
+};
+
+struct LoadRealScaled {  // reads n_i, rescales to N_e, writes it back and feeds the forward FFT
+  double *n_i;
+  const DevScalars *sc;
+  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
+    const double v = n_i[idx] * sc->init_scale;
+    n_i[idx] = v; re = v; im = 0.0;
+  }
+};
+
+struct StoreScaled {
+  double2 *dst;
+  double scale;
+  __device__ __forceinline__ void store(long long idx, int, int, int, double re, double im) {
+    dst[idx] = make_double2(re * scale, im * scale);
+  }
+  __device__ __forceinline__ void finish(double *) {}
+};
+
+__global__ void copy_real_kernel(double *dst, const double *src, long long n) {
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < n; g += (long long)gridDim.x * blockDim.x) dst[g] = src[g];
+}
+
+__global__ void fermi_dirac_kernel(int twice_j, const double *eta, double *out, size_t n, const double *fdtab) {
+  __shared__ double s_tab[kFdTabDoubles];
+  fd_load_tables(s_tab, fdtab);
+  __syncthreads();
+  for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < n; g += (size_t)gridDim.x * blockDim.x) {
+    double a, b, c;
+    fd_eval<7>(s_tab, eta[g], a, b, c);
+    out[g] = twice_j == -1 ? a : (twice_j == 1 ? b : c);
+  }
+}
+
+}  // namespace arche

@@ -1,0 +1,164 @@
+"""GPU-vs-oracle parity through the C ABI (run on the B200 box: pytest -m gpu).
+
+Tolerances (BASELINE.json north_star): relative 1e-10 on density and free energy, 1e-8 on forces.
+Index/flag quantities (iteration counts under scf_fixed_iter) must be equal.
+"""
+import numpy as np
+import pytest
+
+import arche_inputs as ai
+
+pytestmark = pytest.mark.gpu
+
+TOL_N = 1e-10
+TOL_F = 1e-10
+TOL_FORCE = 1e-8
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test run without a CUDA device")
+    return torch
+
+
+def _gpu(cfg, **kw):
+    from paper_2606_13283_b200 import Arche
+    return Arche(cfg, **kw)
+
+
+def _rel(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def test_fermi_dirac_parity(orc, torch_cuda):
+    cfg = ai.make_small()
+    g = _gpu(cfg)
+    eta = np.concatenate([np.linspace(-60, 0, 301), np.linspace(0, 20, 801), np.linspace(20, 400, 401),
+                          [-0.0, 1e-300, 19.999999999, 20.0, 20.000000001, 2.0, 4.0, 7.0, 10.0, 14.0]])
+    for tj in (-1, 1, 3):
+        got = g.fermi_dirac(tj, eta).cpu().numpy()
+        ref = orc.fd(tj, eta)
+        assert np.abs(got / ref - 1).max() < 2e-14, tj
+
+
+@pytest.mark.parametrize("shape", [(4, 4, 4), (8, 12, 16), (24, 16, 36), (32, 32, 32), (48, 64, 96), (16, 18, 128)])
+def test_fft3d_parity(orc, torch_cuda, shape):
+    torch = torch_cuda
+    nz, ny, nx = shape
+    cfg = ai.make_small(grid=(nx, ny, nz))
+    g = _gpu(cfg)
+    rng = np.random.default_rng(nx + 7 * ny + 13 * nz)
+    a = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+    for sign in (-1, +1):
+        got = g.fft3d(torch.as_tensor(a), sign).cpu().numpy()
+        ref = orc.fft3d(a, sign)
+        assert np.abs(got - ref).max() < 1e-13 * np.abs(ref).max() * np.log2(a.size)
+
+
+def test_structure_factor_and_ionic_potential(orc, torch_cuda):
+    cfg = ai.make_small(n_ions=7, L=9.0, grid=(24, 16, 12), cell=[9.0, 7.0, 6.0], seed=3)
+    cfg["Z"] = np.array([3.0, 1.0, 2.0, 3.0, 1.5, 3.0, 0.5])
+    g = _gpu(cfg); o = orc.Oracle(cfg)
+    pos = cfg["pos"] + cfg["cell"] * np.array([2, -1, 0])          # unwrapped positions are legal
+    g.scf_begin(pos); o.scf_begin(pos)
+    for name in ("S_Z", "Vhat_ie"):
+        assert _rel(g.get_complex(name).cpu().numpy(), o.get_complex(name)) < 1e-12
+
+
+@pytest.mark.parametrize("xc", [0, 1])
+def test_single_scf_iteration(orc, torch_cuda, xc):
+    cfg = ai.make_small(n_ions=4, L=8.0, grid=(16, 12, 24), T_eV=10.0, seed=8)
+    g = _gpu(cfg, xc=xc); o = orc.Oracle(cfg, xc=xc)
+    g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
+    for it in range(3):
+        rg = g.scf_iter(); ro = o.scf_iter()
+        assert _rel(g.get_real("V_i").cpu().numpy(), o.get_real("V_i")) < 1e-11
+        assert _rel(g.get_real("n_a").cpu().numpy(), o.get_real("n_a")) < TOL_N
+        assert _rel(g.get_real("n_i").cpu().numpy(), o.get_real("n_i")) < TOL_N
+        assert _rel(g.get_complex("nhat_a").cpu().numpy(), o.get_complex("nhat_a")) < TOL_N
+        for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "E_ie0", "U_ii", "K_e", "w_last"):
+            assert abs(rg[k] - ro[k]) <= TOL_F * max(1.0, abs(ro[k])), (it, k, rg[k], ro[k])
+        assert abs(rg["U_mix"] / ro["U_mix"] - 1) < 1e-9 and abs(rg["K_mix"] / ro["K_mix"] - 1) < 1e-9
+        assert rg["scf_iters"] == ro["scf_iters"] == it + 1
+    dV = float(np.prod(cfg["cell"]) / np.prod(cfg["grid"]))
+    assert abs(g.get_real("n_a").sum().item() * dV - cfg["Z"].sum()) < 1e-12 * cfg["Z"].sum()   # neutrality
+
+
+def _solve_pair(orc, cfg, **kw):
+    o = orc.Oracle(cfg, **kw)
+    ro = o.scf_solve(cfg["pos"])
+    assert ro["converged"] == 1
+    g = _gpu(cfg, scf_fixed_iter=ro["scf_iters"], **kw)      # replay the same number of iterations (reading D4)
+    rg = g.scf_solve(cfg["pos"])
+    return g, o, rg, ro
+
+
+def test_converged_solve_and_forces(orc, torch_cuda):
+    cfg = ai.make_small(n_ions=5, L=9.0, grid=(24, 16, 18), cell=[9.0, 7.5, 8.0], T_eV=10.0, seed=9)
+    g, o, rg, ro = _solve_pair(orc, cfg, scf_tol_dn=1e-11, init_mode=0)
+    assert rg["scf_iters"] == ro["scf_iters"]
+    assert _rel(g.get_real("n_a").cpu().numpy(), o.get_real("n_a")) < TOL_N
+    assert abs(rg["F_total"] - ro["F_total"]) < TOL_F * abs(ro["F_total"])
+    Fg = g.forces().cpu().numpy(); Fo = o.forces()
+    assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max()
+    # the GPU's own stop rule ends at the same iteration
+    g2 = _gpu(cfg, scf_tol_dn=1e-11, init_mode=0)
+    r2 = g2.scf_solve(cfg["pos"])
+    assert r2["converged"] == 1 and abs(r2["scf_iters"] - ro["scf_iters"]) <= 1
+    assert _rel(g.get_complex("ghat").cpu().numpy(), o.get_complex("ghat")) < 1e-8
+
+
+def test_c1_md_trajectory(orc, torch_cuda):
+    """BASELINE.json config 1: 16 Al ions, 32^3, T = 10 eV, 5 velocity-Verlet steps of 0.5 fs."""
+    torch = torch_cuda
+    cfg = ai.make_config("c1")
+    kw = dict(scf_tol_F=1e-10, scf_tol_dn=1e-9, scf_max_iter=300)
+    o = orc.Oracle(cfg, **kw)
+    g = _gpu(cfg, **kw)
+    po = cfg["pos"].copy(); vo = cfg["vel"].copy()
+    pg = torch.as_tensor(cfg["pos"].copy(), device="cuda"); vg = torch.as_tensor(cfg["vel"].copy(), device="cuda")
+    for step in range(cfg["n_steps"]):
+        ro = o.md_step(cfg["dt"], po, vo)
+        rg = g.md_step(cfg["dt"], pg, vg)
+        assert abs(rg["scf_iters"] - ro["scf_iters"]) <= 1, step
+        assert abs(rg["F_total"] - ro["F_total"]) < 1e-9 * abs(ro["F_total"])
+        assert abs(rg["K_i"] - ro["K_i"]) < 1e-9 * abs(ro["K_i"])
+        assert np.abs(pg.cpu().numpy() - po).max() < 1e-9
+        Fo = o.forces(); Fg = g.forces().cpu().numpy()
+        assert np.abs(Fg - Fo).max() < 1e-6 * np.abs(Fo).max()    # free stop rule: residual-limited, not round-off
+    # host-buffer variant gives the same step as the device-pointer one
+    g2 = _gpu(cfg, **kw)
+    ph = cfg["pos"].copy(); vh = cfg["vel"].copy(); Fh = np.zeros_like(ph)
+    g3 = _gpu(cfg, **kw)
+    pd = torch.as_tensor(cfg["pos"].copy(), device="cuda"); vd = torch.as_tensor(cfg["vel"].copy(), device="cuda")
+    g2.md_step_host(cfg["dt"], ph, vh, Fh); g3.md_step(cfg["dt"], pd, vd)
+    assert np.array_equal(ph, pd.cpu().numpy()) and np.array_equal(Fh, g3.forces().cpu().numpy())
+
+
+def test_uniform_gas_and_edge_cases(orc, torch_cuda):
+    from paper_2606_13283_b200 import ArcheError
+    cfg = dict(cell=[5.0, 6.0, 7.0], grid=[8, 12, 16], Z=np.zeros(0), mass=np.zeros(0), kT=0.4)
+    g = _gpu(cfg, n_electrons=9.0); o = orc.Oracle(cfg, n_electrons=9.0)
+    g.scf_begin(np.zeros((0, 3))); o.scf_begin(np.zeros((0, 3)))
+    rg = g.scf_iter(); ro = o.scf_iter()
+    assert abs(rg["mu"] - ro["mu"]) < 1e-12 and abs(rg["F_total"] - ro["F_total"]) < 1e-11
+    assert np.abs(g.get_real("n_a").cpu().numpy() - 9.0 / 210.0).max() < 1e-15
+    with pytest.raises(ArcheError):
+        _gpu(dict(cfg, grid=[7, 12, 16]), n_electrons=9.0)        # 7 is not 2^a 3^b
+    c2 = ai.make_small()
+    g2 = _gpu(c2)
+    with pytest.raises(ArcheError):
+        g2.forces()                                                 # before any solve
+
+
+def test_determinism(orc, torch_cuda):
+    cfg = ai.make_small(n_ions=4, L=8.0, grid=(16, 16, 16), seed=12)
+    r = []
+    for _ in range(2):
+        g = _gpu(cfg, scf_fixed_iter=6)
+        res = g.scf_solve(cfg["pos"])
+        r.append((res["F_total"], res["mu"], g.get_real("n_a").cpu().numpy(), g.forces().cpu().numpy()))
+    assert r[0][0] == r[1][0] and r[0][1] == r[1][1]
+    assert np.array_equal(r[0][2], r[1][2]) and np.array_equal(r[0][3], r[1][3])
