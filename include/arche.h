@@ -113,6 +113,14 @@ int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta, double *d_
 /* number of kernels this context has launched so far (for bench.py's gpu_launches) */
 long long arche_launch_count(const arche_ctx *c);
 
+/* Per-kernel-class timing with CUDA events on params.stream (adds ~2 event records per launch; off by default).
+ * Classes: 0 inverse-FFT z pass with the G-space potential prologue (S1), 1 FFT y passes, 2 inverse-FFT x pass with
+ * the V_i epilogue (S2), 3 mu passes (S3), 4 density kernel (S4), 5 forward-FFT x pass reading the real n_a,
+ * 6 forward-FFT z pass with the G-space reductions (S5), 7 mixing (S6), 8 structure factor (P1,P2), 9 force sum (P5),
+ * 10 Ewald pair kernel, 11 other.  arche_profile_get returns the summed milliseconds and launch count of a class. */
+int arche_profile_enable(arche_ctx *c, int on);
+int arche_profile_get(arche_ctx *c, int cls, double *h_ms_total, long long *h_launches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -19,7 +19,7 @@ __all__ = ["Arche", "ArcheError", "load", "SYMBOLS", "Params", "Result"]
 SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_last_error", "arche_scf_solve",
            "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_md_step",
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
-           "arche_fermi_dirac", "arche_launch_count"]
+           "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
 
@@ -78,6 +78,8 @@ def load(rebuild_if_stale: bool = True):
     L.arche_fft3d.argtypes = [vp, dp, dp, dp, C.c_int]
     L.arche_fermi_dirac.argtypes = [vp, C.c_int, dp, dp, C.c_size_t]
     L.arche_launch_count.argtypes = [vp]; L.arche_launch_count.restype = C.c_longlong
+    L.arche_profile_enable.argtypes = [vp, C.c_int]
+    L.arche_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     _lib = L
     return L
 
@@ -224,6 +226,20 @@ class Arche:
         t = self.torch
         e = self._dev(eta); out = t.empty_like(e)
         self._check(self.lib.arche_fermi_dirac(self._h, int(twice_j), e.data_ptr(), out.data_ptr(), e.numel()))
+        return out
+
+    PROFILE_CLASSES = ("fft_inv_z_potential", "fft_y", "fft_inv_x_vi", "mu_pass", "density", "fft_fwd_x_real",
+                       "fft_fwd_z_reduce", "mix", "structure_factor", "force", "ewald_pp", "other")
+
+    def profile_enable(self, on: bool = True):
+        self._check(self.lib.arche_profile_enable(self._h, int(on)))
+
+    def profile_get(self) -> dict:
+        out = {}
+        for i, name in enumerate(self.PROFILE_CLASSES):
+            ms, n = C.c_double(), C.c_longlong()
+            self._check(self.lib.arche_profile_get(self._h, i, C.byref(ms), C.byref(n)))
+            out[name] = (ms.value, n.value)
         return out
 
     def launch_count(self) -> int:

@@ -21,6 +21,10 @@ using namespace arche;
 namespace {
 
 constexpr int kMuMaxPasses = 12;
+constexpr int kProfPairs = 512;
+// kernel classes for arche_profile_get
+enum ProfClass { PC_FFT_INV_Z = 0, PC_FFT_Y, PC_FFT_INV_X, PC_MU, PC_DENSITY, PC_FFT_FWD_X, PC_FFT_FWD_Z, PC_MIX,
+                 PC_SFAC, PC_FORCE, PC_EWALD, PC_OTHER, kProfClasses };
 constexpr int kEwBlocks = 148 * 8;
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -90,6 +94,13 @@ struct arche_ctx {
   DevScalars *h_sc;  // pinned
   bool have_g, have_solution, have_forces;
   long long launches;
+  // optional per-kernel-class timing (CUDA events on c->stream), see arche_profile_*
+  bool prof;
+  int prof_pending;
+  cudaEvent_t prof_ev[2 * kProfPairs];
+  int prof_cls[kProfPairs];
+  double prof_ms[kProfClasses];
+  long long prof_cnt[kProfClasses];
   char err[256];
 };
 
@@ -105,6 +116,27 @@ int fail(arche_ctx *c, int code, const char *what, cudaError_t e = cudaSuccess) 
     if (e__ != cudaSuccess) return fail(c, ARCHE_ECUDA, #call, e__);         \
   } while (0)
 #define LAUNCHED(c) do { ++(c)->launches; CK(cudaGetLastError()); } while (0)
+
+void prof_harvest(arche_ctx *c) {  // call after a stream synchronise
+  for (int k = 0; k < c->prof_pending; ++k) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->prof_ev[2 * k], c->prof_ev[2 * k + 1]) == cudaSuccess) {
+      c->prof_ms[c->prof_cls[k]] += ms; c->prof_cnt[c->prof_cls[k]] += 1;
+    }
+  }
+  c->prof_pending = 0;
+}
+struct ProfScope {  // records an event pair around the launches issued in its lifetime
+  arche_ctx *c; int k;
+  ProfScope(arche_ctx *ctx, int cls) : c(ctx), k(-1) {
+    if (!c->prof) return;
+    if (c->prof_pending == kProfPairs) { cudaStreamSynchronize(c->stream); prof_harvest(c); }
+    k = c->prof_pending++;
+    c->prof_cls[k] = cls;
+    cudaEventRecord(c->prof_ev[2 * k], c->stream);
+  }
+  ~ProfScope() { if (k >= 0) cudaEventRecord(c->prof_ev[2 * k + 1], c->stream); }
+};
 
 int fft_tile_blocks(int axis, int n, int nx, int ny, int nz) {
   int L = fft_pick_L(axis, n, nx, ny, nz);
@@ -181,6 +213,7 @@ extern "C" long long arche_launch_count(const arche_ctx *c) { return c ? c->laun
 extern "C" void arche_destroy(arche_ctx *c) {
   if (!c) return;
   if (c->h_sc) cudaFreeHost(c->h_sc);
+  for (int k = 0; k < 2 * kProfPairs; ++k) if (c->prof_ev[k]) cudaEventDestroy(c->prof_ev[k]);
   delete c;
 }
 
@@ -270,26 +303,33 @@ namespace {
 
 // inverse: axis order z, y, x (the x pass writes the real field contiguously)
 template <class LoadOp, class StoreOp>
-int fft3d_inverse(arche_ctx *c, LoadOp ld, StoreOp st) {
+int fft3d_inverse(arche_ctx *c, LoadOp ld, StoreOp st, int cls_first = PC_OTHER, int cls_last = PC_OTHER) {
   const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
-  CK((fft_launch_pass<2, true>(c->plan[2], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches;
-  CK((fft_launch_pass<1, true>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches;
-  CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches;
+  { ProfScope ps(c, cls_first);
+    CK((fft_launch_pass<2, true>(c->plan[2], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
+  { ProfScope ps(c, cls_first == PC_OTHER ? PC_OTHER : PC_FFT_Y);
+    CK((fft_launch_pass<1, true>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
+  { ProfScope ps(c, cls_last);
+    CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
   return ARCHE_OK;
 }
 // forward: axis order x, y, z
 template <class LoadOp, class StoreOp>
-int fft3d_forward(arche_ctx *c, LoadOp ld, StoreOp st) {
+int fft3d_forward(arche_ctx *c, LoadOp ld, StoreOp st, int cls_first = PC_OTHER, int cls_last = PC_OTHER) {
   const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
-  CK((fft_launch_pass<0, false>(c->plan[0], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches;
-  CK((fft_launch_pass<1, false>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches;
-  CK((fft_launch_pass<2, false>(c->plan[2], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches;
+  { ProfScope ps(c, cls_first);
+    CK((fft_launch_pass<0, false>(c->plan[0], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
+  { ProfScope ps(c, cls_first == PC_OTHER ? PC_OTHER : PC_FFT_Y);
+    CK((fft_launch_pass<1, false>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
+  { ProfScope ps(c, cls_last);
+    CK((fft_launch_pass<2, false>(c->plan[2], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
   return ARCHE_OK;
 }
 
 int read_scalars(arche_ctx *c) {
   CK(cudaMemcpyAsync(c->h_sc, c->sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, c->stream));
   CK(cudaStreamSynchronize(c->stream));
+  if (c->prof) prof_harvest(c);
   return ARCHE_OK;
 }
 
@@ -315,28 +355,31 @@ int scf_iteration(arche_ctx *c) {
   sv.V_i = c->V_i; sv.n_i = c->n_i; sv.sc = c->sc; sv.partials = c->partials; sv.counter = c->counter;
   sv.inv_vol = 1.0 / G.vol; sv.kT_eta0 = C.kT * C.eta0; sv.xc = C.xc;
   sv.acc_min = 1.0e308; sv.acc_max = -1.0e308; sv.acc_sum = 0.0;
-  int rc = fft3d_inverse(c, LoadPotentialG{c->nh_i, c->vh_ie, c->kx2, c->ky2, c->kz2}, sv);
+  int rc = fft3d_inverse(c, LoadPotentialG{c->nh_i, c->vh_ie, c->kx2, c->ky2, c->kz2}, sv, PC_FFT_INV_Z, PC_FFT_INV_X);
   if (rc) return rc;
   // S3
   mu_guess_kernel<<<1, 1, 0, c->stream>>>(c->sc, (double)c->ng, C.kT * C.eta0);
   LAUNCHED(c);
   for (int pass = 0; pass < kMuMaxPasses; ++pass) {
+    ProfScope ps(c, PC_MU);
     mu_pass_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->V_i, c->ng, C, c->sc, c->fdtab, c->partials, c->counter,
                                                      pass == kMuMaxPasses - 1);
     LAUNCHED(c);
   }
   // S4
+  { ProfScope ps(c, PC_DENSITY);
   density_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->V_i, c->n_i, c->n_a, c->ng, C, c->sc, c->fdtab, c->partials, c->counter);
-  LAUNCHED(c);
+  LAUNCHED(c); }
   // S5 (+ w, F, stop flags in the epilogue's last block)
   StoreNhatA sn;
   sn.nh_a = c->nh_a; sn.nh_i = c->nh_i; sn.vh_ie = c->vh_ie; sn.kx2 = c->kx2; sn.ky2 = c->ky2; sn.kz2 = c->kz2;
   sn.sc = c->sc; sn.partials = c->partials; sn.counter = c->counter; sn.C = C; sn.aU = sn.aEH = sn.aEie = 0.0;
-  rc = fft3d_forward(c, LoadReal{c->n_a}, sn);
+  rc = fft3d_forward(c, LoadReal{c->n_a}, sn, PC_FFT_FWD_X, PC_FFT_FWD_Z);
   if (rc) return rc;
   // S6
+  { ProfScope ps(c, PC_MIX);
   mix_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->n_a, c->nh_i, c->nh_a, c->ng, c->sc);
-  LAUNCHED(c);
+  LAUNCHED(c); }
   c->have_solution = true;
   c->have_forces = false;
   return ARCHE_OK;
@@ -354,9 +397,10 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 1, G.Ly, G.ny, ni, c->by_ij, nullptr); LAUNCHED(c);
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 2, G.Lz, G.nz, ni, c->cz_ij, nullptr); LAUNCHED(c);
     dim3 sg((unsigned)(((long long)G.ny * G.nz + SF_ROWS - 1) / SF_ROWS), (unsigned)((G.nx + SF_THREADS - 1) / SF_THREADS));
+    { ProfScope ps(c, PC_SFAC);
     structure_factor_kernel<<<sg, SF_THREADS, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S,
                                                               c->vh_ie, c->partials, c->counter, c->sc);
-    LAUNCHED(c);
+    LAUNCHED(c); }
     ewald_pp_kernel<<<ni, 128, 0, c->stream>>>(c->pos, c->Z, ni, G.Lx, G.Ly, G.Lz, c->alpha, c->F_pp, c->e_pp); LAUNCHED(c);
     ewald_finish_kernel<<<1, 256, 0, c->stream>>>(c->e_pp, c->Z, ni, c->alpha, G.vol, c->sc); LAUNCHED(c);
   } else {
@@ -414,9 +458,10 @@ int compute_forces(arche_ctx *c) {
   if (ni == 0) { c->have_forces = true; return ARCHE_OK; }
   const GridGeom &G = c->G;
   dim3 fg((unsigned)((ni + FC_THREADS - 1) / FC_THREADS), (unsigned)c->force_slabs);
+  { ProfScope ps(c, PC_FORCE);
   force_kernel<<<fg, FC_THREADS, 2 * G.nx * sizeof(double2), c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij,
                                                                         c->cz_ij, c->vps, c->va, c->nh_a, c->S, c->F_part);
-  LAUNCHED(c);
+  LAUNCHED(c); }
   force_finish_kernel<<<(3 * ni + 127) / 128, 128, 0, c->stream>>>(ni, c->force_slabs, c->F_part, c->F_pp, c->Z,
                                                                    -2.0 * ARCHE_PI / G.vol, c->F);
   LAUNCHED(c);
@@ -546,5 +591,24 @@ extern "C" int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta,
   int blocks = (int)((n + 255) / 256 < (size_t)kEwBlocks ? (n + 255) / 256 : kEwBlocks);
   fermi_dirac_kernel<<<blocks, 256, 0, c->stream>>>(twice_j, d_eta, d_out, n, c->fdtab);
   LAUNCHED(c);
+  return ARCHE_OK;
+}
+
+extern "C" int arche_profile_enable(arche_ctx *c, int on) {
+  if (!c) return ARCHE_EINVAL;
+  if (on && !c->prof_ev[0])
+    for (int k = 0; k < 2 * kProfPairs; ++k) CK(cudaEventCreate(&c->prof_ev[k]));
+  CK(cudaStreamSynchronize(c->stream));
+  prof_harvest(c);
+  c->prof = on != 0;
+  if (on) { memset(c->prof_ms, 0, sizeof(c->prof_ms)); memset(c->prof_cnt, 0, sizeof(c->prof_cnt)); }
+  return ARCHE_OK;
+}
+
+extern "C" int arche_profile_get(arche_ctx *c, int cls, double *h_ms_total, long long *h_launches) {
+  if (!c || cls < 0 || cls >= kProfClasses || !h_ms_total || !h_launches) return ARCHE_EINVAL;
+  CK(cudaStreamSynchronize(c->stream));
+  prof_harvest(c);
+  *h_ms_total = c->prof_ms[cls]; *h_launches = c->prof_cnt[cls];
   return ARCHE_OK;
 }
