@@ -341,6 +341,7 @@ struct oracle_ctx {
   double *F_ii;
   double mu;
   int have_g, have_solution, have_forces;
+  int warmup_eff; /* mix_warmup applies only to a uniform start (reading A11) */
   oracle_result last;
 };
 
@@ -455,7 +456,9 @@ int oracle_scf_begin(oracle_ctx *c, const double *pos) {
     double sc = c->Ne / tot;
     for (size_t g = 0; g < c->ng; ++g) c->n_i[g] *= sc;
     forward_real(c, c->n_i, c->nh_i);
+    c->warmup_eff = 0;
   } else {
+    c->warmup_eff = c->p.mix_warmup;
     double n0 = c->Ne / c->vol; /* PAPER.md:223 */
     for (size_t g = 0; g < c->ng; ++g) { c->n_i[g] = n0; c->nh_i[g] = 0.0; }
     c->nh_i[0] = c->Ne;
@@ -570,7 +573,7 @@ int oracle_scf_iter(oracle_ctx *c, oracle_result *out) {
   /* S6: mixing n_o = n_a + w (n_i - n_a), w = U/(K+U) */
   int it = c->last.scf_iters + 1;
   double w;
-  if (c->p.mix_mode == 1 && it > c->p.mix_warmup) w = (K + U > 0.0) ? U / (K + U) : 0.0;
+  if (c->p.mix_mode == 1 && it > c->warmup_eff) w = (K + U > 0.0) ? U / (K + U) : 0.0;
   else w = c->p.mix_w_fixed;
   for (size_t g = 0; g < ng; ++g) {
     c->n_i[g] = c->n_a[g] + w * (c->n_i[g] - c->n_a[g]);

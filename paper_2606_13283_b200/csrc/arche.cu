@@ -416,7 +416,9 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     if (rc) return rc;
     rc = fft3d_forward(c, LoadRealScaled{c->n_i, c->sc}, StoreScaled{c->nh_i, G.dV});
     if (rc) return rc;
+    c->C.mix_warmup = 0;  // profile start: mu fluctuations are small from the first iteration (reading A11)
   } else {
+    c->C.mix_warmup = c->p.mix_warmup;
     set_uniform_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->nh_i, c->ng, c->C.Ne / G.vol, c->C.Ne);
     LAUNCHED(c);
   }
