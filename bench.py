@@ -26,10 +26,10 @@ import arche_inputs as ai  # noqa: E402
 
 # stop rule used for throughput (BASELINE.json: 1e-10 Ha on the free energy; the density criterion of reading D4 is
 # set to 1e-8 for throughput runs, stated in config)
-TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000)
+TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000, mix_warmup=3, mix_w_fixed=0.95)
 # SCF iterations per MD step of each workload under TOL, measured on the GPU path (used only to express the
 # oracle's bounded sample in MD steps/s)
-ITERS_PER_STEP = {"c1": 20.0, "c2": 20.0, "c3": 8.0, "c4": 200.0}
+ITERS_PER_STEP = {"c1": 32.0, "c2": 155.0, "c3": 20.0, "c4": 1000.0}
 
 # algorithmic HBM bytes per grid point and launch of each kernel class
 BYTES_PER_POINT = {"fft_inv_z_potential": 48, "fft_y": 32, "fft_inv_x_vi": 32, "mu_pass": 8, "density": 24,

@@ -165,7 +165,7 @@ class Oracle:
     """SCF/MD context (mirrors the C-ABI of the product, with host arrays)."""
 
     def __init__(self, cfg: dict, **over):
-        p = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=0,
+        p = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=3,
                  scf_tol_F=1e-10, scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0,
                  ewald_alpha=0.0, n_electrons=0.0)
         for k in p:

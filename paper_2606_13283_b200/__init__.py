@@ -84,7 +84,7 @@ def load(rebuild_if_stale: bool = True):
     return L
 
 
-_DEFAULTS = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=0, scf_tol_F=1e-10,
+_DEFAULTS = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=3, scf_tol_F=1e-10,
                  scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0, ewald_alpha=0.0, n_electrons=0.0)
 
 

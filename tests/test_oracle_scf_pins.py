@@ -142,7 +142,7 @@ def test_more_mixing_single_mode_closed_form(orc):
     kT = 0.3; cell = np.array([8.0, 8.0, 8.0]); N = 8
     cfg = dict(cell=cell, grid=[N, N, N], Z=np.zeros(0), mass=np.zeros(0), kT=kT)
     Ne = 10.0; n0 = Ne / 512.0
-    o = orc.Oracle(cfg, n_electrons=Ne, xc=0)
+    o = orc.Oracle(cfg, n_electrons=Ne, xc=0, mix_warmup=0)
     o.scf_begin(np.zeros((0, 3)))
     x = np.arange(N) * 1.0
     zz, yy, xx = np.meshgrid(x, x, x, indexing="ij")
