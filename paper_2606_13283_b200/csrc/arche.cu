@@ -79,6 +79,7 @@ struct arche_ctx {
   double alpha, Q;
   FftAxisPlan plan[3];
   int red_blocks;  // capacity of the partials buffer (blocks)
+  int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
   int force_slabs, force_rows_per_slab;
   // device arrays (all inside the caller's workspace)
@@ -177,7 +178,7 @@ void derive_sizes(arche_ctx *c) {
   for (int a = 0; a < 3; ++a) { int b = fft_tile_blocks(a, c->p.grid[a], nx, ny, nz); if (b > rb) rb = b; }
   long long sfb = ((long long)ny * nz + SF_ROWS - 1) / SF_ROWS * ((nx + SF_THREADS - 1) / SF_THREADS);
   if (sfb > rb) rb = (int)sfb;
-  c->red_blocks = rb + 8;
+  c->red_blocks = rb + 8 + 2 * kEwBlocks;  // + room for the mu kernel's [2][grid][2] + [grid][6] partials
   const long long rows = (long long)ny * nz;
   const int tiles = (c->nions + FC_THREADS - 1) / FC_THREADS;
   int slabs = tiles > 0 ? (148 * 4 + tiles - 1) / tiles : 1;
@@ -257,6 +258,16 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     double rc = 0.5 * fmin(G.Lx, fmin(G.Ly, G.Lz));
     double kc = fmin(nx / (2.0 * G.Lx), fmin(ny / (2.0 * G.Ly), nz / (2.0 * G.Lz)));
     c->alpha = p->ewald_alpha > 0.0 ? p->ewald_alpha : sqrt(ARCHE_PI * kc / rc);
+  }
+  {  // cooperative grid: all blocks must be co-resident
+    int dev = 0, sms = 0, per_sm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_density_kernel, 256, 0));
+    long long gmax = (long long)sms * per_sm, want = (c->ng + 255) / 256;
+    if (gmax > kEwBlocks) gmax = kEwBlocks;
+    c->mu_grid = (int)(want < gmax ? want : gmax);
+    if (c->mu_grid < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
   }
   // ---- per-axis tables: k, k^2, twiddles (long double on the host)
   const int dims[3] = {nx, ny, nz};
@@ -357,19 +368,14 @@ int scf_iteration(arche_ctx *c) {
   sv.acc_min = 1.0e308; sv.acc_max = -1.0e308; sv.acc_sum = 0.0;
   int rc = fft3d_inverse(c, LoadPotentialG{c->nh_i, c->vh_ie, c->kx2, c->ky2, c->kz2}, sv, PC_FFT_INV_Z, PC_FFT_INV_X);
   if (rc) return rc;
-  // S3
-  mu_guess_kernel<<<1, 1, 0, c->stream>>>(c->sc, (double)c->ng, C.kT * C.eta0);
-  LAUNCHED(c);
-  for (int pass = 0; pass < kMuMaxPasses; ++pass) {
-    ProfScope ps(c, PC_MU);
-    mu_pass_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->V_i, c->ng, C, c->sc, c->fdtab, c->partials, c->counter,
-                                                     pass == kMuMaxPasses - 1);
-    LAUNCHED(c);
-  }
-  // S4
-  { ProfScope ps(c, PC_DENSITY);
-  density_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->V_i, c->n_i, c->n_a, c->ng, C, c->sc, c->fdtab, c->partials, c->counter);
-  LAUNCHED(c); }
+  // S3 + S4: one persistent cooperative kernel (Newton passes separated by grid barriers, then the density pass)
+  { ProfScope ps(c, PC_MU);
+    const double *aV = c->V_i, *an = c->n_i; double *ana = c->n_a; long long ang = c->ng; ScfConst aC = C;
+    DevScalars *asc = c->sc; const double *atab = c->fdtab; double *apart = c->partials; unsigned int *acnt = c->counter;
+    int amax = kMuMaxPasses;
+    void *args[] = {&aV, &an, &ana, &ang, &aC, &asc, &atab, &apart, &acnt, &amax};
+    CK(cudaLaunchCooperativeKernel((const void *)mu_density_kernel, dim3(c->mu_grid), dim3(256), args, 0, c->stream));
+    ++c->launches; }
   // S5 (+ w, F, stop flags in the epilogue's last block)
   StoreNhatA sn;
   sn.nh_a = c->nh_a; sn.nh_i = c->nh_i; sn.vh_ie = c->vh_ie; sn.kx2 = c->kx2; sn.ky2 = c->ky2; sn.kz2 = c->kz2;

@@ -5,6 +5,7 @@
 #include "common.cuh"
 #include "fd.cuh"
 #include "fft.cuh"
+#include <cooperative_groups.h>
 
 namespace arche {
 
@@ -177,6 +178,107 @@ __global__ void __launch_bounds__(256) density_kernel(const double *__restrict__
     const double *t = s_red + 6 * 32;
     sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
     sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
+  }
+}
+
+// ---- S3+S4 fused: persistent cooperative kernel.  Newton-in-bracket passes for mu separated by one grid-wide
+// barrier each (every block re-sums all block partials in the same fixed order, so all blocks take the same
+// Newton step without a second barrier), then the density pass at the converged mu.  On small grids the V_i
+// values of a thread stay in registers across the passes.
+constexpr int kMuCache = 4;
+__global__ void __launch_bounds__(256) mu_density_kernel(const double *__restrict__ V_i, const double *__restrict__ n_i,
+                                                         double *__restrict__ n_a, long long ng, ScfConst C,
+                                                         DevScalars *sc, const double *__restrict__ fdtab,
+                                                         double *partials, unsigned int *counter, int max_pass) {
+  namespace cg = cooperative_groups;
+  cg::grid_group grid = cg::this_grid();
+  __shared__ double s_tab[kFdTabDoubles];
+  __shared__ double s_red[6 * 32 + 6];
+  __shared__ double s_bc[2];
+  fd_load_tables(s_tab, fdtab);
+  __syncthreads();
+  const double inv_kT = 1.0 / C.kT, kT_eta0 = C.kT * C.eta0;
+  const long long nthreads = (long long)gridDim.x * blockDim.x, tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool cached = ng <= nthreads * kMuCache;
+  double vc[kMuCache];
+  if (cached) {
+#pragma unroll
+    for (int q = 0; q < kMuCache; ++q) { long long g = tid + q * nthreads; vc[q] = g < ng ? V_i[g] : 0.0; }
+  }
+  // bracket and first guess (identical in every block; reading D1)
+  double lo = sc->mu_lo, hi = sc->mu_hi;
+  double mu = sc->mu_have_prev ? sc->mu : sc->vsum / (double)ng + kT_eta0;
+  if (!(mu > lo && mu < hi)) mu = 0.5 * (lo + hi);
+  bool done = false;
+  if (hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi))) { mu = 0.5 * (lo + hi); done = true; }
+  int evals = 0;
+  double *pp = partials;                       // [2][gridDim.x][2]
+  double *pd = partials + 4 * (size_t)gridDim.x;  // density partials [gridDim.x][6]
+  for (int pass = 0; pass < max_pass && !done; ++pass) {
+    double s1 = 0.0, s0 = 0.0;
+    if (cached) {
+#pragma unroll
+      for (int q = 0; q < kMuCache; ++q) {
+        if (tid + q * nthreads < ng) {
+          double im12, i12, d;
+          fd_eval<3>(s_tab, (mu - vc[q]) * inv_kT, im12, i12, d);
+          s1 += i12; s0 += im12;
+        }
+      }
+    } else {
+      for (long long g = tid; g < ng; g += nthreads) {
+        double im12, i12, d;
+        fd_eval<3>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
+        s1 += i12; s0 += im12;
+      }
+    }
+    double v[2] = {s1, s0};
+    const int op[2] = {0, 0};
+    block_reduce<2>(v, op, s_red);
+    double *buf = pp + (size_t)(pass & 1) * 2 * gridDim.x;
+    if (threadIdx.x == 0) { buf[2 * blockIdx.x] = v[0]; buf[2 * blockIdx.x + 1] = v[1]; }
+    grid.sync();
+    double a[2] = {0.0, 0.0};
+    for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) { a[0] += __ldcg(&buf[2 * b]); a[1] += __ldcg(&buf[2 * b + 1]); }
+    block_reduce<2>(a, op, s_red);
+    if (threadIdx.x == 0) { s_bc[0] = a[0]; s_bc[1] = a[1]; }
+    __syncthreads();
+    const double N = C.cTF * C.dV * s_bc[0], dN = C.cTF * C.dV * 0.5 * s_bc[1] * inv_kT;
+    __syncthreads();
+    const double f = N - C.Ne;
+    ++evals;
+    if (fabs(f) <= 1e-14 * C.Ne || pass == max_pass - 1) {
+      done = true;
+    } else {
+      if (f > 0.0) hi = mu; else lo = mu;
+      double mu_new = mu - f / dN;
+      if (!(mu_new > lo && mu_new < hi)) mu_new = 0.5 * (lo + hi);
+      if (fabs(mu_new - mu) <= 2e-16 * fmax(fabs(mu), C.kT)) done = true; else mu = mu_new;
+    }
+  }
+  // density pass at mu
+  double sK = 0, sdn2 = 0, sna2 = 0, sF0 = 0, sKe = 0, sExc = 0;
+  for (long long g = tid; g < ng; g += nthreads) {
+    const double eta = (mu - V_i[g]) * inv_kT;
+    double im12, i12, i32;
+    fd_eval<7>(s_tab, eta, im12, i12, i32);
+    const double na = C.cTF * i12;
+    const double chi = C.cTF * 0.5 * im12 * inv_kT;
+    const double dn = n_i[g] - na;
+    n_a[g] = na;
+    if (chi > 0.0) sK += dn * dn / chi;
+    sdn2 += dn * dn; sna2 += na * na;
+    sF0 += eta * i12 - (2.0 / 3.0) * i32;
+    sKe += i32;
+    if (C.xc) { double e, vx; xc_pz81(na, e, vx); sExc += na * e; }
+  }
+  double v6[6] = {sK, sdn2, sna2, sF0, sKe, sExc};
+  const int op6[6] = {0, 0, 0, 0, 0, 0};
+  if (grid_reduce<6>(v6, op6, pd, counter, s_red) && threadIdx.x == 0) {
+    const double *t = s_red + 6 * 32;
+    sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
+    sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
+    sc->mu = mu; sc->mu_lo = lo; sc->mu_hi = hi; sc->mu_done = 1; sc->mu_evals = evals; sc->mu_evals_total += evals;
   }
 }
 
