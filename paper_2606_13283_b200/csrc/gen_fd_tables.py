@@ -2,29 +2,33 @@
 """Generate fd_tables.h: piecewise polynomial fits of the Fermi-Dirac integrals
 I_j(eta) = int_0^inf t^j/(exp(t-eta)+1) dt, j = -1/2, 1/2, 3/2 (Eq. 9), for the CUDA path.
 
-Run by hand (needs mpmath; ~3 minutes):  python paper_2606_13283_b200/csrc/gen_fd_tables.py
+Run by hand (needs mpmath; a few minutes on 8 cores):  python paper_2606_13283_b200/csrc/gen_fd_tables.py
 The generated header is committed, so building the library needs no mpmath.
 
 Method (own fits; no published coefficient table is used; nothing here is shared with oracle/):
   reference values: I_j(eta) = -Gamma(j+1) Li_{j+1}(-e^eta) with mpmath at 40 digits;
-  region A (eta <= 0):      I_j = x * P(t),   x = e^eta, segments in x on [0,1]   (P absorbs Gamma(j+1));
-  region B (0 < eta < ETA_C): I_j = P(t),     segments in eta with integer break points;
-  region C (eta >= ETA_C):  I_j = eta^(j+1) * P(t), t from u = 1/eta^2 on [0, 1/ETA_C^2] (P absorbs 1/(j+1)).
-Each P is the Chebyshev interpolant of degree FD_NC-1 converted to monomials in t in [-1,1] (Horner on
-the device).  The script checks every segment in simulated double precision against mpmath and fails if
-the relative error exceeds 1e-15.
+  segment 0          (eta <= ETA_A):        I_j = x * P(t), x = e^eta on [0, e^ETA_A]   (P absorbs Gamma(j+1));
+  segments 1..NB     (ETA_A < eta < ETA_C): I_j = P(t), uniform segments of width W in eta (direct index, no search);
+  segment NB+1       (eta >= ETA_C):        I_j = eta^(j+1) * P(t), t from u = 1/eta^2 on [0, 1/ETA_C^2].
+The poles of the Fermi function sit at eta +- i pi, so a Chebyshev interpolant on a segment of half-width h
+converges like rho^-n with rho = pi/h + sqrt((pi/h)^2 + 1): W = 0.5 gives rho = 25 and degree 11 reaches 1e-16.
+Each P is the Chebyshev interpolant of degree FD_NC-1 converted to monomials in t in [-1,1] (Horner on the
+device: 11 FMAs per function).  The script checks every segment in simulated double precision against mpmath
+and fails if the relative error exceeds 1e-15.
 """
 import os
 import sys
+from multiprocessing import Pool
 
 import mpmath as mp
 import numpy as np
 
 mp.mp.dps = 40
-NC = 22
-XA = [0.0, 1.0]                                  # region A break points in x = e^eta
-EB = [0, 2, 4, 7, 10, 14, 20]                    # region B break points in eta (integers)
-ETA_C = EB[-1]
+NC = 12
+ETA_A = -2.0
+ETA_C = 40.0
+W = 0.5
+NB = int(round((ETA_C - ETA_A) / W))
 TJ = (-1, 1, 3)
 
 
@@ -42,7 +46,6 @@ def cheb_to_mono(f, n):
         s = sum(fv[i] * mp.cos(mp.pi * m * (i + mp.mpf(1) / 2) / n) for i in range(n))
         c.append(2 * s / n)
     c[0] /= 2
-    # T_0 = 1, T_1 = t, T_{k+1} = 2 t T_k - T_{k-1}
     T = [[mp.mpf(1)], [mp.mpf(0), mp.mpf(1)]]
     for k in range(2, n):
         a = [mp.mpf(0)] + [2 * x for x in T[k - 1]]
@@ -62,76 +65,85 @@ def horner_f64(co, t):
     return acc
 
 
-def main():
-    segs = []       # (kind, center, invhalf, {tj: coefs})
-    for a, b in zip(XA[:-1], XA[1:]):
-        c, h = (a + b) / 2, (b - a) / 2
-        co = {}
-        for tj in TJ:
-            j = mp.mpf(tj) / 2
-            def f(t, tj=tj, c=c, h=h):
-                x = mp.mpf(c) + mp.mpf(h) * t
-                return I(tj, mp.log(x)) / x if x > 0 else mp.gamma(mp.mpf(tj) / 2 + 1)
-            co[tj] = cheb_to_mono(f, NC)
-        segs.append(("A", c, 1.0 / h, co))
-    for a, b in zip(EB[:-1], EB[1:]):
-        c, h = (a + b) / 2, (b - a) / 2
-        co = {tj: cheb_to_mono(lambda t, tj=tj: I(tj, mp.mpf(c) + mp.mpf(h) * t), NC) for tj in TJ}
-        segs.append(("B", c, 1.0 / h, co))
-    um = mp.mpf(1) / ETA_C ** 2
+def seg_geometry(s):
+    """(kind, centre, 1/halfwidth) of segment s in its own variable"""
+    if s == 0:
+        xa = float(mp.exp(ETA_A))
+        return "A", xa / 2, 2 / xa
+    if s == NB + 1:
+        um = 1.0 / ETA_C ** 2
+        return "C", um / 2, 2 / um
+    return "B", ETA_A + W * (s - 1) + W / 2, 2 / W
+
+
+def fit_segment(s):
+    mp.mp.dps = 40
+    kind, c, ih = seg_geometry(s)
     co = {}
     for tj in TJ:
         j = mp.mpf(tj) / 2
-        def f(t, tj=tj, j=j):
-            u = um * (t + 1) / 2
-            eta = 1 / mp.sqrt(u)
-            return I(tj, eta) / eta ** (j + 1)
+        if kind == "A":
+            def f(t):
+                x = mp.mpf(c) + t / mp.mpf(ih)
+                return I(tj, mp.log(x)) / x if x > 0 else mp.gamma(j + 1)
+        elif kind == "B":
+            def f(t):
+                return I(tj, mp.mpf(c) + t / mp.mpf(ih))
+        else:
+            def f(t):
+                u = mp.mpf(c) + t / mp.mpf(ih)
+                if u <= 0:
+                    return 1 / (j + 1)
+                eta = 1 / mp.sqrt(u)
+                return I(tj, eta) / eta ** (j + 1)
         co[tj] = cheb_to_mono(f, NC)
-    segs.append(("C", float(um / 2), float(2 / um), co))
-
-    # ---- verification in simulated double precision
-    rng = np.random.default_rng(1)
+    # verification in simulated double precision
+    rng = np.random.default_rng(1000 + s)
     worst = 0.0
-    for kind, c, ih, co in segs:
-        for tj in TJ:
-            cf = [float(x) for x in co[tj]]
-            for t in np.concatenate([rng.uniform(-1, 1, 60), [-1.0, 1.0, 0.0]]):
-                v = c + t / ih
-                if kind == "A":
-                    if v <= 0:
-                        continue
-                    eta = mp.log(mp.mpf(float(v))); val = np.float64(v) * horner_f64(cf, (np.float64(v) - c) * ih)
-                elif kind == "B":
-                    eta = mp.mpf(float(v)); val = horner_f64(cf, (np.float64(v) - c) * ih)
-                else:
-                    if v <= 1e-7:
-                        continue
-                    eta = 1 / mp.sqrt(mp.mpf(float(v)))
-                    val = horner_f64(cf, (np.float64(v) - c) * ih) * float(eta ** (mp.mpf(tj) / 2 + 1))
-                err = abs(mp.mpf(float(val)) / I(tj, eta) - 1)
-                worst = max(worst, float(err))
-        print(kind, c, "worst so far %.2e" % worst, file=sys.stderr)
-    assert worst < 1e-15, worst
+    for tj in TJ:
+        cf = [float(x) for x in co[tj]]
+        for t in np.concatenate([rng.uniform(-1, 1, 24), [-1.0, 1.0, 0.0]]):
+            v = np.float64(c) + np.float64(t) / np.float64(ih)
+            tt = (v - np.float64(c)) * np.float64(ih)
+            if kind == "A":
+                if v <= 0:
+                    continue
+                eta = mp.log(mp.mpf(float(v))); val = v * horner_f64(cf, tt)
+            elif kind == "B":
+                eta = mp.mpf(float(v)); val = horner_f64(cf, tt)
+            else:
+                if v <= 1e-9:
+                    continue
+                eta = 1 / mp.sqrt(mp.mpf(float(v)))
+                val = horner_f64(cf, tt) * float(eta ** (mp.mpf(tj) / 2 + 1))
+            worst = max(worst, float(abs(mp.mpf(float(val)) / I(tj, eta) - 1)))
+    return s, {tj: [mp.nstr(x, 19, min_fixed=0, max_fixed=0) for x in co[tj]] for tj in TJ}, worst
 
+
+def main():
+    with Pool(os.cpu_count()) as pool:
+        res = pool.map(fit_segment, range(NB + 2), chunksize=1)
+    res.sort()
+    worst = max(r[2] for r in res)
+    print("max rel err %.2e" % worst, file=sys.stderr)
+    assert worst < 1e-15, worst
     out = os.path.join(os.path.dirname(os.path.abspath(__file__)), "fd_tables.h")
     with open(out, "w") as fh:
         fh.write("// GENERATED by gen_fd_tables.py -- do not edit.  Piecewise fits of I_{-1/2}, I_{1/2}, I_{3/2}\n")
         fh.write("// (PAPER.md:124).  Max relative error of the double-precision Horner evaluation vs mpmath: %.2e\n" % worst)
-        fh.write("#pragma once\n#define FD_NC %d\n#define FD_NSEG %d\n#define FD_NA %d\n#define FD_NB %d\n#define FD_ETA_C %d\n"
-                 % (NC, len(segs), len(XA) - 1, len(EB) - 1, ETA_C))
-        fh.write("static const double FD_XA_BREAK[FD_NA + 1] = {%s};\n" % ", ".join(repr(float(x)) for x in XA))
-        emap = []
-        for e in range(ETA_C):
-            emap.append(len(XA) - 1 + max(i for i, a in enumerate(EB[:-1]) if a <= e))
-        fh.write("static const int FD_ETA_SEG[FD_ETA_C] = {%s};\n" % ", ".join(str(x) for x in emap))
-        fh.write("static const double FD_CENTER[FD_NSEG] = {%s};\n" % ", ".join(repr(float(s[1])) for s in segs))
-        fh.write("static const double FD_INVHALF[FD_NSEG] = {%s};\n" % ", ".join(repr(float(s[2])) for s in segs))
-        fh.write("// [segment][function: -1/2, 1/2, 3/2][monomial power]\n")
-        fh.write("static const double FD_COEF[FD_NSEG][3][FD_NC] = {\n")
-        for kind, c, ih, co in segs:
-            fh.write("  { // region %s centre %r\n" % (kind, float(c)))
-            for tj in TJ:
-                fh.write("    {%s},\n" % ", ".join(mp.nstr(x, 19, min_fixed=0, max_fixed=0) for x in co[tj]))
+        fh.write("#pragma once\n#define FD_NC %d\n#define FD_NB %d\n#define FD_NSEG %d\n" % (NC, NB, NB + 2))
+        fh.write("#define FD_ETA_A %r\n#define FD_ETA_C %r\n#define FD_INV_W %r\n" % (ETA_A, ETA_C, 1.0 / W))
+        ka, ca, iha = seg_geometry(0)
+        kc, cc, ihc = seg_geometry(NB + 1)
+        fh.write("#define FD_A_CENTER %r\n#define FD_A_INVHALF %r\n#define FD_C_CENTER %r\n#define FD_C_INVHALF %r\n"
+                 % (ca, iha, cc, ihc))
+        fh.write("// [function: -1/2, 1/2, 3/2][segment][monomial power]; segment 0 = region A, 1..FD_NB = region B,\n")
+        fh.write("// FD_NB+1 = region C\n")
+        fh.write("static const double FD_COEF[3][FD_NSEG][FD_NC] = {\n")
+        for tj in TJ:
+            fh.write("  { // I_{%d/2}\n" % tj)
+            for s, co, _ in res:
+                fh.write("    {%s},\n" % ", ".join(co[tj]))
             fh.write("  },\n")
         fh.write("};\n")
     print("wrote", out, "max rel err %.2e" % worst)
