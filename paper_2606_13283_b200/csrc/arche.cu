@@ -41,13 +41,11 @@ struct Carver {  // carves 256-byte aligned arrays out of the caller's workspace
 
 // host evaluation of the same fits (only for eta0 = I_{1/2}^{-1}(Ne/(|Omega| cTF)), once per init)
 double fd_half_host(double eta) {
-  int seg; double v, pre;
-  if (eta <= 0.0) { double x = exp(eta); seg = 0; for (int a = 1; a < FD_NA; ++a) seg += (x > FD_XA_BREAK[a]); v = x; pre = x; }
-  else if (eta < (double)FD_ETA_C) { seg = FD_ETA_SEG[(int)eta]; v = eta; pre = 1.0; }
-  else { seg = FD_NSEG - 1; v = 1.0 / (eta * eta); pre = sqrt(eta) * eta; }
-  double t = (v - FD_CENTER[seg]) * FD_INVHALF[seg], a = FD_COEF[seg][1][FD_NC - 1];
-  for (int i = FD_NC - 2; i >= 0; --i) a = fma(a, t, FD_COEF[seg][1][i]);
-  return a * pre;
+  int seg; double t, p0, p1, p2;
+  fd_locate(eta, seg, t, p0, p1, p2);
+  double a = FD_COEF[1][seg][FD_NC - 1];
+  for (int i = FD_NC - 2; i >= 0; --i) a = fma(a, t, FD_COEF[1][seg][i]);
+  return a * p1;
 }
 double fd_half_inverse_host(double y) {
   double lo = log(y / 0.88622692545275801365), hi = pow(1.5 * y, 2.0 / 3.0) + 2.0;
@@ -84,7 +82,10 @@ struct arche_ctx {
   int force_slabs, force_rows_per_slab;
   // device arrays (all inside the caller's workspace)
   double *n_i, *n_a, *V_i, *vps, *va;
-  double2 *nh_i, *nh_a, *vh_ie, *S, *gh, *work;
+  double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
+  long long nh;      // P*ny*nz
+  int nxh, P;
+  bool mix_pending;  // S6 of the last iteration not yet applied to n_i / nhat_i (fused into the next S1/S2)
   double *kx, *ky, *kz, *kx2, *ky2, *kz2;
   double2 *tw[3];
   double2 *ax_ij, *ax_ji, *by_ij, *cz_ij;
@@ -149,10 +150,12 @@ size_t layout(arche_ctx *c, char *base) {
   Carver w{base, 0};
   const size_t ng = (size_t)c->ng, ni = (size_t)(c->nions > 0 ? c->nions : 1);
   const int nx = c->p.grid[0], ny = c->p.grid[1], nz = c->p.grid[2];
+  const size_t nh = (size_t)c->nh;
   c->n_i = w.take<double>(ng); c->n_a = w.take<double>(ng); c->V_i = w.take<double>(ng);
-  c->vps = w.take<double>(ng); c->va = w.take<double>(ng);
-  c->nh_i = w.take<double2>(ng); c->nh_a = w.take<double2>(ng); c->vh_ie = w.take<double2>(ng);
-  c->S = w.take<double2>(ng); c->gh = w.take<double2>(ng); c->work = w.take<double2>(ng);
+  c->vps = w.take<double>(nh); c->va = w.take<double>(nh);
+  c->nh_i = w.take<double2>(nh); c->nh_a = w.take<double2>(nh); c->vh_ie = w.take<double2>(nh);
+  c->S = w.take<double2>(nh); c->S2 = w.take<double2>(nh); c->gh = w.take<double2>(nh); c->gh2 = w.take<double2>(nh);
+  c->work = w.take<double2>(nh);
   c->kx = w.take<double>(nx); c->ky = w.take<double>(ny); c->kz = w.take<double>(nz);
   c->kx2 = w.take<double>(nx); c->ky2 = w.take<double>(ny); c->kz2 = w.take<double>(nz);
   c->tw[0] = w.take<double2>(nx); c->tw[1] = w.take<double2>(ny); c->tw[2] = w.take<double2>(nz);
@@ -172,11 +175,15 @@ size_t layout(arche_ctx *c, char *base) {
 void derive_sizes(arche_ctx *c) {
   const int nx = c->p.grid[0], ny = c->p.grid[1], nz = c->p.grid[2];
   c->ng = (long long)nx * ny * nz;
+  c->nxh = nx / 2 + 1;
+  c->P = (c->nxh + 7) / 8 * 8;
+  c->nh = (long long)c->P * ny * nz;
   c->nions = c->p.n_ions;
   c->ew_grid = (int)((c->ng + 255) / 256 < kEwBlocks ? (c->ng + 255) / 256 : kEwBlocks);
   int rb = c->ew_grid;
-  for (int a = 0; a < 3; ++a) { int b = fft_tile_blocks(a, c->p.grid[a], nx, ny, nz); if (b > rb) rb = b; }
-  long long sfb = ((long long)ny * nz + SF_ROWS - 1) / SF_ROWS * ((nx + SF_THREADS - 1) / SF_THREADS);
+  for (int a = 1; a < 3; ++a) { int b = fft_tile_blocks(a, c->p.grid[a], c->P, ny, nz); if (b > rb) rb = b; }
+  { int b = fft_real_blocks(nx, ny, nz); if (b > rb) rb = b; }
+  long long sfb = ((long long)ny * nz + SF_ROWS - 1) / SF_ROWS * ((c->P + SF_THREADS - 1) / SF_THREADS);
   if (sfb > rb) rb = (int)sfb;
   c->red_blocks = rb + 8 + 2 * kEwBlocks;  // + room for the mu kernel's [2][grid][2] + [grid][6] partials
   const long long rows = (long long)ny * nz;
@@ -236,7 +243,7 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   if (e != cudaSuccess) { delete c; return ARCHE_ECUDA; }
   // ---- geometry and constants
   GridGeom &G = c->G;
-  G.nx = nx; G.ny = ny; G.nz = nz; G.ng = c->ng;
+  G.nx = nx; G.ny = ny; G.nz = nz; G.ng = c->ng; G.nxh = c->nxh; G.P = c->P; G.nh = c->nh;
   G.Lx = p->cell[0]; G.Ly = p->cell[1]; G.Lz = p->cell[2];
   G.vol = G.Lx * G.Ly * G.Lz; G.dV = G.vol / (double)c->ng;
   G.kx = c->kx; G.ky = c->ky; G.kz = c->kz; G.kx2 = c->kx2; G.ky2 = c->ky2; G.kz2 = c->kz2;
@@ -263,7 +270,7 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     int dev = 0, sms = 0, per_sm = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_density_kernel, 256, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, 0));
     long long gmax = (long long)sms * per_sm, want = (c->ng + 255) / 256;
     if (gmax > kEwBlocks) gmax = kEwBlocks;
     c->mu_grid = (int)(want < gmax ? want : gmax);
@@ -312,28 +319,28 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
 // =============================================================================================
 namespace {
 
-// inverse: axis order z, y, x (the x pass writes the real field contiguously)
+// inverse (half spectrum -> real field): axis order z, y, x; the x pass is the c2r pass and writes the real field
 template <class LoadOp, class StoreOp>
 int fft3d_inverse(arche_ctx *c, LoadOp ld, StoreOp st, int cls_first = PC_OTHER, int cls_last = PC_OTHER) {
-  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
   { ProfScope ps(c, cls_first);
-    CK((fft_launch_pass<2, true>(c->plan[2], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((fft_launch_pass<2, true>(c->plan[2], P, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
   { ProfScope ps(c, cls_first == PC_OTHER ? PC_OTHER : PC_FFT_Y);
-    CK((fft_launch_pass<1, true>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((fft_launch_pass<1, true>(c->plan[1], P, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
   { ProfScope ps(c, cls_last);
-    CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
+    CK((fft_launch_real_x<true>(c->plan[0], nx, ny, nz, P, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
   return ARCHE_OK;
 }
-// forward: axis order x, y, z
+// forward (real field -> half spectrum): axis order x (r2c), y, z
 template <class LoadOp, class StoreOp>
 int fft3d_forward(arche_ctx *c, LoadOp ld, StoreOp st, int cls_first = PC_OTHER, int cls_last = PC_OTHER) {
-  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
   { ProfScope ps(c, cls_first);
-    CK((fft_launch_pass<0, false>(c->plan[0], nx, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((fft_launch_real_x<false>(c->plan[0], nx, ny, nz, P, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
   { ProfScope ps(c, cls_first == PC_OTHER ? PC_OTHER : PC_FFT_Y);
-    CK((fft_launch_pass<1, false>(c->plan[1], nx, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((fft_launch_pass<1, false>(c->plan[1], P, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
   { ProfScope ps(c, cls_last);
-    CK((fft_launch_pass<2, false>(c->plan[2], nx, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
+    CK((fft_launch_pass<2, false>(c->plan[2], P, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
   return ARCHE_OK;
 }
 
@@ -355,37 +362,51 @@ void fill_result(const arche_ctx *c, arche_result *r) {
 
 // forward transform of the real input density into nhat_i (scaled by dV)
 int input_density_to_g(arche_ctx *c) {
-  return fft3d_forward(c, LoadReal{c->n_i}, StoreScaled{c->nh_i, c->G.dV});
+  return fft3d_forward(c, LoadReal{c->n_i}, StoreScaled{c->nh_i, c->G.dV, c->nxh});
+}
+
+// applies a pending S6 step to n_i / nhat_i (normally fused into the next iteration's S1/S2 passes)
+int flush_mix(arche_ctx *c) {
+  if (!c->mix_pending) return ARCHE_OK;
+  ProfScope ps(c, PC_MIX);
+  mix_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->n_a, c->nh_i, c->nh_a, c->ng, c->nh, c->sc);
+  LAUNCHED(c);
+  c->mix_pending = false;
+  return ARCHE_OK;
 }
 
 int scf_iteration(arche_ctx *c) {
   const GridGeom &G = c->G;
   const ScfConst &C = c->C;
-  // S1 + S2
+  const int mix = c->mix_pending ? 1 : 0;
+  // S1 + S2 (+ the pending S6 of the previous iteration, + the first mu evaluation)
+  LoadPotentialG lp;
+  lp.nh_i = c->nh_i; lp.nh_a = c->nh_a; lp.vh_ie = c->vh_ie; lp.kx2 = c->kx2; lp.ky2 = c->ky2; lp.kz2 = c->kz2;
+  lp.sc = c->sc; lp.nxh = c->nxh; lp.mix = mix; lp.w = 1.0;
   StoreVi sv;
-  sv.V_i = c->V_i; sv.n_i = c->n_i; sv.sc = c->sc; sv.partials = c->partials; sv.counter = c->counter;
-  sv.inv_vol = 1.0 / G.vol; sv.kT_eta0 = C.kT * C.eta0; sv.xc = C.xc;
-  sv.acc_min = 1.0e308; sv.acc_max = -1.0e308; sv.acc_sum = 0.0;
-  int rc = fft3d_inverse(c, LoadPotentialG{c->nh_i, c->vh_ie, c->kx2, c->ky2, c->kz2}, sv, PC_FFT_INV_Z, PC_FFT_INV_X);
+  sv.V_i = c->V_i; sv.n_i = c->n_i; sv.n_a = c->n_a; sv.sc = c->sc; sv.partials = c->partials; sv.counter = c->counter;
+  sv.fdtab = c->fdtab; sv.inv_vol = 1.0 / G.vol; sv.kT_eta0 = C.kT * C.eta0; sv.inv_kT = 1.0 / C.kT; sv.xc = C.xc; sv.mix = mix;
+  int rc = fft3d_inverse(c, lp, sv, PC_FFT_INV_Z, PC_FFT_INV_X);
   if (rc) return rc;
-  // S3 + S4: one persistent cooperative kernel (Newton passes separated by grid barriers, then the density pass)
+  c->mix_pending = false;
+  // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
   { ProfScope ps(c, PC_MU);
-    const double *aV = c->V_i, *an = c->n_i; double *ana = c->n_a; long long ang = c->ng; ScfConst aC = C;
-    DevScalars *asc = c->sc; const double *atab = c->fdtab; double *apart = c->partials; unsigned int *acnt = c->counter;
+    const double *aV = c->V_i; long long ang = c->ng; ScfConst aC = C;
+    DevScalars *asc = c->sc; const double *atab = c->fdtab; double *apart = c->partials;
     int amax = kMuMaxPasses;
-    void *args[] = {&aV, &an, &ana, &ang, &aC, &asc, &atab, &apart, &acnt, &amax};
-    CK(cudaLaunchCooperativeKernel((const void *)mu_density_kernel, dim3(c->mu_grid), dim3(256), args, 0, c->stream));
+    void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax};
+    CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, 0, c->stream));
     ++c->launches; }
-  // S5 (+ w, F, stop flags in the epilogue's last block)
+  // S4 (fused into the r2c x pass) + S5 (+ w, F, stop flags in the z-pass epilogue's last block)
+  LoadDensity ldn;
+  ldn.V_i = c->V_i; ldn.n_i = c->n_i; ldn.n_a = c->n_a; ldn.sc = c->sc; ldn.partials = c->partials; ldn.counter = c->counter;
+  ldn.fdtab = c->fdtab; ldn.C = C;
   StoreNhatA sn;
   sn.nh_a = c->nh_a; sn.nh_i = c->nh_i; sn.vh_ie = c->vh_ie; sn.kx2 = c->kx2; sn.ky2 = c->ky2; sn.kz2 = c->kz2;
-  sn.sc = c->sc; sn.partials = c->partials; sn.counter = c->counter; sn.C = C; sn.aU = sn.aEH = sn.aEie = 0.0;
-  rc = fft3d_forward(c, LoadReal{c->n_a}, sn, PC_FFT_FWD_X, PC_FFT_FWD_Z);
+  sn.sc = c->sc; sn.partials = c->partials; sn.counter = c->counter; sn.C = C; sn.H.nx = G.nx; sn.H.nxh = c->nxh;
+  rc = fft3d_forward(c, ldn, sn, PC_DENSITY, PC_FFT_FWD_Z);
   if (rc) return rc;
-  // S6
-  { ProfScope ps(c, PC_MIX);
-  mix_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->n_a, c->nh_i, c->nh_a, c->ng, c->sc);
-  LAUNCHED(c); }
+  c->mix_pending = true;   // S6 is applied by the next iteration's S1/S2 passes, or by flush_mix()
   c->have_solution = true;
   c->have_forces = false;
   return ARCHE_OK;
@@ -402,30 +423,34 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 0, G.Lx, G.nx, ni, c->ax_ij, c->ax_ji); LAUNCHED(c);
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 1, G.Ly, G.ny, ni, c->by_ij, nullptr); LAUNCHED(c);
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 2, G.Lz, G.nz, ni, c->cz_ij, nullptr); LAUNCHED(c);
-    dim3 sg((unsigned)(((long long)G.ny * G.nz + SF_ROWS - 1) / SF_ROWS), (unsigned)((G.nx + SF_THREADS - 1) / SF_THREADS));
+    dim3 sg((unsigned)(((long long)G.ny * G.nz + SF_ROWS - 1) / SF_ROWS), (unsigned)((c->P + SF_THREADS - 1) / SF_THREADS));
     { ProfScope ps(c, PC_SFAC);
     structure_factor_kernel<<<sg, SF_THREADS, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S,
-                                                              c->vh_ie, c->partials, c->counter, c->sc);
+                                                              c->S2, c->vh_ie, c->partials, c->counter, c->sc);
+    LAUNCHED(c);
+    structure_factor_nyquist_kernel<<<c->ew_grid, 128, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va,
+                                                                       c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc);
     LAUNCHED(c); }
     ewald_pp_kernel<<<ni, 128, 0, c->stream>>>(c->pos, c->Z, ni, G.Lx, G.Ly, G.Lz, c->alpha, c->F_pp, c->e_pp); LAUNCHED(c);
     ewald_finish_kernel<<<1, 256, 0, c->stream>>>(c->e_pp, c->Z, ni, c->alpha, G.vol, c->sc); LAUNCHED(c);
   } else {
-    CK(cudaMemsetAsync(c->S, 0, c->ng * sizeof(double2), c->stream));
-    CK(cudaMemsetAsync(c->vh_ie, 0, c->ng * sizeof(double2), c->stream));
+    CK(cudaMemsetAsync(c->S, 0, c->nh * sizeof(double2), c->stream));
+    CK(cudaMemsetAsync(c->S2, 0, c->nh * sizeof(double2), c->stream));
+    CK(cudaMemsetAsync(c->vh_ie, 0, c->nh * sizeof(double2), c->stream));
   }
   // P4: input density
   if (c->p.init_mode == 1 && c->have_g && ni > 0) {
     StoreClip sk;
     sk.n_i = c->n_i; sk.sc = c->sc; sk.partials = c->partials; sk.counter = c->counter;
     sk.inv_vol = 1.0 / G.vol; sk.floor_n = 1e-3 * c->C.Ne / G.vol; sk.Ne = c->C.Ne; sk.dV = G.dV; sk.acc = 0.0;
-    int rc = fft3d_inverse(c, LoadSG{c->S, c->gh}, sk);
+    int rc = fft3d_inverse(c, LoadSG{c->S, c->S2, c->gh, c->gh2, c->nxh}, sk);
     if (rc) return rc;
-    rc = fft3d_forward(c, LoadRealScaled{c->n_i, c->sc}, StoreScaled{c->nh_i, G.dV});
+    rc = fft3d_forward(c, LoadRealScaled{c->n_i, c->sc, 1.0}, StoreScaled{c->nh_i, G.dV, c->nxh});
     if (rc) return rc;
     c->C.mix_warmup = 0;  // profile start: mu fluctuations are small from the first iteration (reading A11)
   } else {
     c->C.mix_warmup = c->p.mix_warmup;
-    set_uniform_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->nh_i, c->ng, c->C.Ne / G.vol, c->C.Ne);
+    set_uniform_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->n_i, c->nh_i, c->ng, c->nh, c->C.Ne / G.vol, c->C.Ne);
     LAUNCHED(c);
   }
   // reset per-solve scalars (iter, F_total, converged); mu and U_ii persist
@@ -434,6 +459,7 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
   CK(cudaMemsetAsync(&c->sc->mu_evals_total, 0, sizeof(int), c->stream));
   c->have_solution = false;
   c->have_forces = false;
+  c->mix_pending = false;  // a new input density replaces any unapplied mixing step
   return ARCHE_OK;
 }
 
@@ -453,7 +479,7 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   }
   // P6: one-center profile of this step's converged density (reading A10)
   if (c->nions > 0) {
-    g_store_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->gh, c->nh_a, c->S, c->ng, 1e-8 * c->Q * c->Q);
+    g_store_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->gh, c->gh2, c->nh_a, c->S, c->S2, c->nh, 1e-8 * c->Q * c->Q);
     LAUNCHED(c);
     c->have_g = true;
   }
@@ -467,8 +493,8 @@ int compute_forces(arche_ctx *c) {
   const GridGeom &G = c->G;
   dim3 fg((unsigned)((ni + FC_THREADS - 1) / FC_THREADS), (unsigned)c->force_slabs);
   { ProfScope ps(c, PC_FORCE);
-  force_kernel<<<fg, FC_THREADS, 2 * G.nx * sizeof(double2), c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij,
-                                                                        c->cz_ij, c->vps, c->va, c->nh_a, c->S, c->F_part);
+  force_kernel<<<fg, FC_THREADS, 2 * c->nxh * sizeof(double2), c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij,
+                                                                          c->cz_ij, c->vps, c->va, c->nh_a, c->S, c->S2, c->F_part);
   LAUNCHED(c); }
   force_finish_kernel<<<(3 * ni + 127) / 128, 128, 0, c->stream>>>(ni, c->force_slabs, c->F_part, c->F_pp, c->Z,
                                                                    -2.0 * ARCHE_PI / G.vol, c->F);
@@ -500,6 +526,7 @@ extern "C" int arche_scf_iter(arche_ctx *c, arche_result *h_out) {
 extern "C" int arche_set_input_density(arche_ctx *c, const double *d_n) {
   if (!c || !d_n) return ARCHE_EINVAL;
   CK(cudaMemcpyAsync(c->n_i, d_n, c->ng * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  c->mix_pending = false;
   return input_density_to_g(c);
 }
 
@@ -563,15 +590,24 @@ extern "C" int arche_get_real(arche_ctx *c, int which, double *d_dst) {
   if (!c || !d_dst) return ARCHE_EINVAL;
   const double *src = which == 0 ? c->n_a : which == 1 ? c->n_i : which == 2 ? c->V_i : nullptr;
   if (!src) return ARCHE_EINVAL;
+  if (which == 1) { int rc = flush_mix(c); if (rc) return rc; }
   CK(cudaMemcpyAsync(d_dst, src, c->ng * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
   return ARCHE_OK;
 }
 extern "C" int arche_get_complex(arche_ctx *c, int which, double *d_dst) {
   if (!c || !d_dst) return ARCHE_EINVAL;
-  const double2 *src = which == 0 ? c->nh_a : which == 1 ? c->vh_ie : which == 2 ? c->S : which == 3 ? c->gh
-                       : which == 4 ? c->nh_i : nullptr;
-  if (!src) return ARCHE_EINVAL;
-  CK(cudaMemcpyAsync(d_dst, src, c->ng * sizeof(double2), cudaMemcpyDeviceToDevice, c->stream));
+  // the library keeps half spectra; the read-back is the full [nz][ny][nx] array on the literal index set of P:142
+  const double2 *src, *src2; const double *scale = nullptr;
+  switch (which) {
+    case 0: src = src2 = c->nh_a; break;
+    case 1: src = c->S; src2 = c->S2; scale = c->vps; break;   // Vhat_ie = v(k) S_Z(k)
+    case 2: src = c->S; src2 = c->S2; break;
+    case 3: src = c->gh; src2 = c->gh2; break;
+    case 4: { int rc = flush_mix(c); if (rc) return rc; src = src2 = c->nh_i; break; }
+    default: return ARCHE_EINVAL;
+  }
+  expand_half_kernel<<<c->ew_grid, 256, 0, c->stream>>>((double2 *)d_dst, src, src2, scale, c->G.nx, c->G.ny, c->G.nz, c->P);
+  LAUNCHED(c);
   return ARCHE_OK;
 }
 extern "C" int arche_get_density(arche_ctx *c, double *d_n) { return arche_get_real(c, 0, d_n); }

@@ -14,7 +14,8 @@ constexpr int kRedBlocksMax = 2048;
 
 struct GridGeom {
   int nx, ny, nz;
-  long long ng;
+  int nxh, P;                     // half spectrum: nxh = nx/2+1 stored columns, row pitch P (multiple of 8)
+  long long ng, nh;               // real points nx*ny*nz; half-spectrum elements P*ny*nz
   double Lx, Ly, Lz, vol, dV;
   const double *kx, *ky, *kz;     // k components per storage index, device
   const double *kx2, *ky2, *kz2;  // squares

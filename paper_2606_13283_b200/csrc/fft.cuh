@@ -111,24 +111,32 @@ __device__ __forceinline__ void fft_stage(const double *__restrict__ sre, const 
 }
 
 // Plain complex array load / store functors.
+// Functor protocol (all passes): begin() once per thread at kernel start; load: operator()(idx, ix, iy, iz, re, im)
+// (complex) or load_real(idx, ix, iy, iz); store(idx, ix, iy, iz, re, im) or store_real(idx, ix, iy, iz, v);
+// finish(smem) once per block at the end (grid reductions; smem = the tile buffer, free by then).
 struct LoadComplex {
   const double2 *src;
-  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
+  __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) {
     double2 v = src[idx]; re = v.x; im = v.y;
   }
+  __device__ __forceinline__ void finish(double *) {}
 };
 struct StoreComplex {
   double2 *dst;
+  __device__ __forceinline__ void begin() {}
   __device__ __forceinline__ void store(long long idx, int, int, int, double re, double im) { dst[idx] = make_double2(re, im); }
   __device__ __forceinline__ void finish(double *) {}
 };
 
 template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, LoadOp ld, StoreOp st_in) {
+__global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, LoadOp ld_in, StoreOp st_in) {
   extern __shared__ double smem[];
   const int N = P.plan.n, L = P.L;
   double *b0re = smem, *b0im = smem + (size_t)L * N, *b1re = smem + 2 * (size_t)L * N, *b1im = smem + 3 * (size_t)L * N;
   StoreOp st = st_in;
+  LoadOp ld = ld_in;
+  ld.begin(); st.begin();
   // tile geometry
   const long long nxny = (long long)P.nx * P.ny;
   long long tile_base;
@@ -198,6 +206,113 @@ __global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, LoadOp
     if (INVERSE) st.store(idx, ix, iy, iz, sim[a], sre[a]); else st.store(idx, ix, iy, iz, sre[a], sim[a]);
   }
   __syncthreads();
+  ld.finish(smem);
+  st.finish(smem);
+}
+
+// ---- x passes on real data (half spectrum) ---------------------------------------------------------
+// The real field [nz][ny][nx] transforms to the half spectrum [nz][ny][P] (ix = 0..nx/2 stored, row pitch P >= nx/2+1,
+// columns ix >= nx/2+1 are zero padding).  Two real lines a, b are packed as z = a + i b, one complex FFT of
+// length nx gives Z, and A(k) = (Z(k) + conj Z(N-k))/2, B(k) = (Z(k) - conj Z(N-k))/(2i) are the two half spectra.
+// The inverse builds Z = A + i B (completed by Hermitian symmetry) and one complex inverse FFT returns a = Re z,
+// b = Im z.  A block owns LP line pairs; stages run in shared memory ([pair][i] layout).
+struct FftRealPass {
+  FftAxisPlan plan;
+  int nx, ny, nz;
+  int P;    // row pitch of the half spectrum (complex elements)
+  int LP;   // line pairs per block
+};
+
+__device__ __forceinline__ void fft_run_stages_x(const FftAxisPlan &plan, int LP, double *&sre, double *&sim, double *&dre,
+                                                 double *&dim) {
+  const int N = plan.n;
+  int Ns = 1;
+  for (int s = 0; s < plan.nstages; ++s) {
+    const int R = plan.radix[s];
+    if (R == 8) fft_stage<8, 0>(sre, sim, dre, dim, N, Ns, LP, plan.tw);
+    else if (R == 4) fft_stage<4, 0>(sre, sim, dre, dim, N, Ns, LP, plan.tw);
+    else if (R == 3) fft_stage<3, 0>(sre, sim, dre, dim, N, Ns, LP, plan.tw);
+    else fft_stage<2, 0>(sre, sim, dre, dim, N, Ns, LP, plan.tw);
+    __syncthreads();
+    double *t;
+    t = sre; sre = dre; dre = t;
+    t = sim; sim = dim; dim = t;
+    Ns *= R;
+  }
+}
+
+// forward: real lines -> half spectrum.  LoadOp: double load_real(idx, ix, iy, iz); StoreOp: store(idx, ix, iy, iz, re, im)
+template <class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(kFftThreads) fft_r2c_x_kernel(FftRealPass P, LoadOp ld_in, StoreOp st_in) {
+  extern __shared__ double smem[];
+  const int N = P.plan.n, LP = P.LP, nxh = N / 2 + 1;
+  double *sre = smem, *sim = smem + (size_t)LP * N, *dre = smem + 2 * (size_t)LP * N, *dim = smem + 3 * (size_t)LP * N;
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  ld.begin(); st.begin();
+  const long long nl = (long long)P.ny * P.nz;
+  const long long line_base = (long long)blockIdx.x * LP * 2;
+  for (int e = threadIdx.x; e < 2 * LP * N; e += blockDim.x) {  // consecutive lines, contiguous in memory
+    const int i = e % N, q = e / N;                              // q = line within the tile (pair q/2, member q%2)
+    const long long line = line_base + q;
+    double v = 0.0;
+    if (line < nl) v = ld.load_real(line * N + i, i, (int)(line % P.ny), (int)(line / P.ny));
+    if (q & 1) sim[(q >> 1) * N + i] = v; else sre[(q >> 1) * N + i] = v;
+  }
+  __syncthreads();
+  fft_run_stages_x(P.plan, LP, sre, sim, dre, dim);
+  for (int e = threadIdx.x; e < 2 * LP * P.P; e += blockDim.x) {
+    const int k = e % P.P, q = e / P.P, pr = q >> 1;
+    const long long line = line_base + q;
+    if (line >= nl) continue;
+    double re = 0.0, im = 0.0;
+    if (k < nxh) {
+      const int mk = k == 0 ? 0 : N - k;
+      const double zr = sre[pr * N + k], zi = sim[pr * N + k], mr = sre[pr * N + mk], mi = sim[pr * N + mk];
+      if (q & 1) { re = 0.5 * (zi + mi); im = -0.5 * (zr - mr); }   // B(k)
+      else { re = 0.5 * (zr + mr); im = 0.5 * (zi - mi); }          // A(k)
+    }
+    st.store(line * P.P + k, k, (int)(line % P.ny), (int)(line / P.ny), re, im);
+  }
+  __syncthreads();
+  ld.finish(smem);
+  st.finish(smem);
+}
+
+// inverse: half spectrum -> real lines (unnormalised).  LoadOp: operator()(idx, ix, iy, iz, re, im);
+// StoreOp: store_real(idx, ix, iy, iz, v)
+template <class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(kFftThreads) fft_c2r_x_kernel(FftRealPass P, LoadOp ld_in, StoreOp st_in) {
+  extern __shared__ double smem[];
+  const int N = P.plan.n, LP = P.LP, nxh = N / 2 + 1;
+  double *sre = smem, *sim = smem + (size_t)LP * N, *dre = smem + 2 * (size_t)LP * N, *dim = smem + 3 * (size_t)LP * N;
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  ld.begin(); st.begin();
+  const long long nl = (long long)P.ny * P.nz;
+  const long long line_base = (long long)blockIdx.x * LP * 2;
+  for (int e = threadIdx.x; e < LP * nxh; e += blockDim.x) {
+    const int k = e % nxh, pr = e / nxh;
+    const long long la = line_base + 2 * pr, lb = la + 1;
+    double ar = 0.0, ai = 0.0, br = 0.0, bi = 0.0;
+    if (la < nl) ld(la * P.P + k, k, (int)(la % P.ny), (int)(la / P.ny), ar, ai);
+    if (lb < nl) ld(lb * P.P + k, k, (int)(lb % P.ny), (int)(lb / P.ny), br, bi);
+    // conj(Z(k)), Z = A + i B  (inverse transform = conj . forward . conj)
+    sre[pr * N + k] = ar - bi; sim[pr * N + k] = -(ai + br);
+    const int mk = N - k;
+    if (k > 0 && mk >= nxh) { sre[pr * N + mk] = ar + bi; sim[pr * N + mk] = ai - br; }  // conj(conj A + i conj B)
+  }
+  __syncthreads();
+  fft_run_stages_x(P.plan, LP, sre, sim, dre, dim);
+  for (int e = threadIdx.x; e < 2 * LP * N; e += blockDim.x) {
+    const int i = e % N, q = e / N;
+    const long long line = line_base + q;
+    if (line >= nl) continue;
+    const double v = (q & 1) ? -sim[(q >> 1) * N + i] : sre[(q >> 1) * N + i];
+    st.store_real(line * N + i, i, (int)(line % P.ny), (int)(line / P.ny), v);
+  }
+  __syncthreads();
+  ld.finish(smem);
   st.finish(smem);
 }
 
@@ -234,7 +349,7 @@ static inline cudaError_t fft_launch_pass(const FftAxisPlan &plan, int nx, int n
   P.L = fft_pick_L(AXIS, plan.n, nx, ny, nz);
   long long blocks = AXIS == 0 ? (long long)ny * nz / P.L : (AXIS == 1 ? (long long)nz * (nx / P.L) : (long long)ny * (nx / P.L));
   size_t smem = 4 * sizeof(double) * (size_t)P.L * plan.n;
-  if (smem < 1024) smem = 1024;  // room for the reduction scratch used by StoreOp::finish
+  if (smem < 4096) smem = 4096;  // room for the reduction scratch used by finish()
   auto kern = fft_pass_kernel<AXIS, INVERSE, LoadOp, StoreOp>;
   static bool attr_set = false;
   if (!attr_set) {
@@ -244,6 +359,49 @@ static inline cudaError_t fft_launch_pass(const FftAxisPlan &plan, int nx, int n
   }
   if (blocks_out) *blocks_out = (int)blocks;
   kern<<<(unsigned)blocks, kFftThreads, smem, stream>>>(P, ld, st);
+  return cudaGetLastError();
+}
+
+static inline int fft_pick_LP(int n, long long lines) {
+  const int max_elems = 3072;  // 4 arrays * 8 B * LP*N <= 96 KB
+  const long long pairs = (lines + 1) / 2;
+  int LP = 1;
+  while (LP * 2 * n <= max_elems && LP * 2 <= pairs && LP < 32) LP *= 2;
+  return LP;
+}
+static inline int fft_real_blocks(int n, int ny, int nz) {
+  const long long lines = (long long)ny * nz, pairs = (lines + 1) / 2;
+  const int LP = fft_pick_LP(n, lines);
+  return (int)((pairs + LP - 1) / LP);
+}
+
+template <bool INVERSE, class LoadOp, class StoreOp>
+static inline cudaError_t fft_launch_real_x(const FftAxisPlan &plan, int nx, int ny, int nz, int pitch, LoadOp ld, StoreOp st,
+                                            cudaStream_t stream) {
+  FftRealPass P;
+  P.plan = plan; P.nx = nx; P.ny = ny; P.nz = nz; P.P = pitch;
+  P.LP = fft_pick_LP(nx, (long long)ny * nz);
+  const int blocks = fft_real_blocks(nx, ny, nz);
+  size_t smem = 4 * sizeof(double) * (size_t)P.LP * plan.n;
+  if (smem < 4096) smem = 4096;
+  static bool attr_set = false;
+  if constexpr (INVERSE) {
+    auto kern = fft_c2r_x_kernel<LoadOp, StoreOp>;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    kern<<<blocks, kFftThreads, smem, stream>>>(P, ld, st);
+  } else {
+    auto kern = fft_r2c_x_kernel<LoadOp, StoreOp>;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    kern<<<blocks, kFftThreads, smem, stream>>>(P, ld, st);
+  }
   return cudaGetLastError();
 }
 

@@ -26,11 +26,14 @@ __global__ void phase_table_kernel(const double *__restrict__ pos, int comp, dou
   }
 }
 
-// reciprocal-space form factors that depend only on the cell: Ashcroft v(k) = -cos(2 pi k rc)/(pi k^2) (per unit
-// charge, 0 at k=0) and the Ewald kernel V_alpha(k) = exp(-(pi k/alpha)^2)/(pi k^2) (Eq. 43).
+// reciprocal-space form factors that depend only on the cell, on the half spectrum [nz][ny][P]: Ashcroft
+// v(k) = -cos(2 pi k rc)/(pi k^2) (per unit charge, 0 at k=0) and the Ewald kernel
+// V_alpha(k) = exp(-(pi k/alpha)^2)/(pi k^2) (Eq. 43).  Zero in the padding columns.
 __global__ void form_factor_kernel(GridGeom G, double rc, double alpha, double *__restrict__ vps, double *__restrict__ va) {
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < G.ng; g += (long long)gridDim.x * blockDim.x) {
-    const int ix = (int)(g % G.nx), iy = (int)((g / G.nx) % G.ny), iz = (int)(g / ((long long)G.nx * G.ny));
+  const long long nh = (long long)G.P * G.ny * G.nz;
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < nh; g += (long long)gridDim.x * blockDim.x) {
+    const int ix = (int)(g % G.P), iy = (int)((g / G.P) % G.ny), iz = (int)(g / ((long long)G.P * G.ny));
+    if (ix >= G.nxh) { vps[g] = 0.0; va[g] = 0.0; continue; }
     const double k2 = G.kx2[ix] + G.ky2[iy] + G.kz2[iz];
     if (k2 == 0.0) { vps[g] = 0.0; va[g] = 0.0; continue; }
     const double k = sqrt(k2);
@@ -39,17 +42,18 @@ __global__ void form_factor_kernel(GridGeom G, double rc, double alpha, double *
   }
 }
 
-// S_Z(k) = sum_j Z_j a_j(kx) b_j(ky) c_j(kz).  A block owns SF_ROWS (ky,kz) rows and a chunk of kx; the ion sum is
-// tiled: d_j = Z_j b_j c_j for SF_JT ions of every row is staged in shared memory, a_j(kx) streams coalesced.
-// Epilogue: Vhat_ie = v(k) S (Eq. 14) and the Ewald reciprocal energy sum of Eq. 42.
+// S_Z(k) = sum_j Z_j a_j(kx) b_j(ky) c_j(kz) on the half spectrum.  A block owns SF_ROWS (ky,kz) rows and a chunk of
+// kx; the ion sum is tiled: d_j = Z_j b_j c_j for SF_JT ions of every row is staged in shared memory, a_j(kx)
+// streams coalesced.  Epilogue: Vhat_ie = v(k) S (Eq. 14) and the Ewald reciprocal energy sum of Eq. 42 with the
+// half-spectrum weights; S2 = S (the Nyquist planes are corrected by structure_factor_nyquist_kernel).
 constexpr int SF_ROWS = 4;
 constexpr int SF_JT = 128;
 constexpr int SF_THREADS = 128;
 __global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
     GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ji /*[j][ix]*/,
     const double2 *__restrict__ by_ij /*[iy][j]*/, const double2 *__restrict__ cz_ij /*[iz][j]*/,
-    const double *__restrict__ vps, const double *__restrict__ va, double2 *__restrict__ S, double2 *__restrict__ vh_ie,
-    double *partials, unsigned int *counter, DevScalars *sc) {
+    const double *__restrict__ vps, const double *__restrict__ va, double2 *__restrict__ S, double2 *__restrict__ S2,
+    double2 *__restrict__ vh_ie, double *partials, unsigned int *counter, DevScalars *sc) {
   __shared__ double2 s_d[SF_ROWS][SF_JT];
   __shared__ double s_red[32 + 1];
   const long long nrows = (long long)G.ny * G.nz;
@@ -73,7 +77,7 @@ __global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
       s_d[r][jj] = d;
     }
     __syncthreads();
-    if (ix < G.nx) {
+    if (ix < G.nxh) {
       const int jn = min(SF_JT, nions - j0);
       for (int jj = 0; jj < jn; ++jj) {
         const double2 a = ax_ji[(long long)(j0 + jj) * G.nx + ix];
@@ -87,23 +91,27 @@ __global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
     }
   }
   double epm = 0.0;
-  if (ix < G.nx) {
+  if (ix < G.P) {
+    const double wt = (ix == 0 || 2 * ix == G.nx) ? 1.0 : 2.0;
 #pragma unroll
     for (int r = 0; r < SF_ROWS; ++r) {
       const long long row = row0 + r;
       if (row < nrows) {
-        const long long g = row * G.nx + ix;
-        S[g] = acc[r];
-        const double v = vps[g];
-        vh_ie[g] = make_double2(v * acc[r].x, v * acc[r].y);
-        epm += va[g] * (acc[r].x * acc[r].x + acc[r].y * acc[r].y);
+        const long long g = row * G.P + ix;
+        if (ix < G.nxh) {
+          S[g] = acc[r]; S2[g] = acc[r];
+          const double v = vps[g];
+          vh_ie[g] = make_double2(v * acc[r].x, v * acc[r].y);
+          epm += wt * va[g] * (acc[r].x * acc[r].x + acc[r].y * acc[r].y);
+        } else {
+          S[g] = make_double2(0.0, 0.0); S2[g] = make_double2(0.0, 0.0); vh_ie[g] = make_double2(0.0, 0.0);
+        }
       }
     }
   }
   // deterministic grid sum of the Ewald reciprocal term (2D grid flattened)
   double v[1] = {epm};
   const int op[1] = {0};
-  // grid_reduce uses blockIdx.x/gridDim.x: emulate a flat grid
   block_reduce<1>(v, op, s_red);
   __shared__ bool s_last;
   const unsigned int nblk = gridDim.x * gridDim.y, bid = blockIdx.y * gridDim.x + blockIdx.x;
@@ -121,6 +129,54 @@ __global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
     block_reduce<1>(w, op, s_red);
     if (threadIdx.x == 0) { sc->U_pm_sum = w[0]; *counter = 0u; }
   }
+}
+
+// Nyquist planes (reading A6).  With the literal index set of P:142 a Nyquist component is +N/2, whose mirror -N/2 is
+// not on the grid, so S_Z is not Hermitian there.  For every stored point with a Nyquist component this kernel forms
+// S2 = S_Z(k''), k'' = k with every Nyquist component flipped to -N/2 (phase-table entries conjugated), and
+//   Vhat_ie <- v(k) (S + S2)/2, the Hermitian part, whose half-spectrum inverse equals the real part of the full
+//   inverse transform of v(k) S_Z(k);  sum conj(nhat) Vhat_ie over the half spectrum then equals Re sum over the full
+//   literal set.  It also corrects the Ewald reciprocal energy for the mirrored halves of the y/z Nyquist rows.
+// Points are enumerated as: list A = rows with iy or iz Nyquist (all ix < nxh), list B = column ix = nx/2 of the
+// remaining rows.  One thread per point, direct sum over the ions (O(N_i N^2) work).
+__global__ void __launch_bounds__(128) structure_factor_nyquist_kernel(
+    GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ji, const double2 *__restrict__ by_ij,
+    const double2 *__restrict__ cz_ij, const double *__restrict__ vps, const double *__restrict__ va,
+    const double2 *__restrict__ S, double2 *__restrict__ S2, double2 *__restrict__ vh_ie, double *partials,
+    unsigned int *counter, DevScalars *sc) {
+  __shared__ double s_red[32 + 1 + 1];
+  const int nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
+  const int nyq_x = (G.nx % 2 == 0) ? G.nx / 2 : -1;
+  const long long nrows = (long long)G.ny * G.nz;
+  const long long total = nrows * G.nxh;     // simple enumeration: every stored point tests itself
+  double corr = 0.0;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
+    const int ix = (int)(e % G.nxh);
+    const long long row = e / G.nxh;
+    const int iy = (int)(row % G.ny), iz = (int)(row / G.ny);
+    const bool fy = iy == nyq_y, fz = iz == nyq_z, fx = ix == nyq_x;
+    if (!(fx || fy || fz)) continue;
+    double sr = 0.0, si = 0.0;
+    for (int j = 0; j < nions; ++j) {
+      double2 a = ax_ji[(long long)j * G.nx + ix], b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
+      if (fx) a.y = -a.y;
+      if (fy) b.y = -b.y;
+      if (fz) c.y = -c.y;
+      const double z = Z[j];
+      const double bcx = b.x * c.x - b.y * c.y, bcy = b.x * c.y + b.y * c.x;
+      sr += z * (a.x * bcx - a.y * bcy); si += z * (a.x * bcy + a.y * bcx);
+    }
+    const long long g = row * G.P + ix;
+    const double2 s = S[g];
+    S2[g] = make_double2(sr, si);
+    const double v = vps[g];
+    vh_ie[g] = make_double2(0.5 * v * (s.x + sr), 0.5 * v * (s.y + si));
+    // interior columns were counted twice with |S|^2; the mirrored half carries |S2|^2 instead
+    if (ix != 0 && !fx) corr += va[g] * ((sr * sr + si * si) - (s.x * s.x + s.y * s.y));
+  }
+  double v[1] = {corr};
+  const int op[1] = {0};
+  if (grid_reduce<1>(v, op, partials, counter, s_red) && threadIdx.x == 0) sc->U_pm_fix = s_red[32];
 }
 
 // Ewald short-range part (Eq. 41, 46) with the minimum-image convention: one block per ion j.
@@ -159,55 +215,70 @@ __global__ void __launch_bounds__(256) ewald_finish_kernel(const double *__restr
   const int op[3] = {0, 0, 0};
   block_reduce<3>(v, op, s_red);
   if (threadIdx.x == 0) {
-    const double upm = 0.5 * sc->U_pm_sum / vol - alpha * 0.56418958354775628695 * v[2];
+    const double upm = 0.5 * (sc->U_pm_sum + sc->U_pm_fix) / vol - alpha * 0.56418958354775628695 * v[2];
     const double uje = -ARCHE_PI * v[1] * v[1] / (2.0 * alpha * alpha * vol);
     sc->U_pp = v[0];
     sc->U_ii = v[0] + upm + uje;
   }
 }
 
-// Forces.  F_j = -(2 pi/|Omega|) Z_j sum_k k Im( W(k) exp(-2 pi i k.r_j) ),
-//   W(k) = v(k) conj(nhat_a(k)) + V_alpha(k) conj(S_Z(k))   [electron-ion Eq. 56 + Ewald reciprocal Eq. 47].
-// Block = FC_THREADS ions x one slab of (ky,kz) rows; W rows are staged in shared memory.
+// Forces.  F_j = -(2 pi/|Omega|) Z_j sum_k k Im( W(k) exp(-2 pi i k.r_j) ) over the literal index set of P:142,
+//   W(k) = v(k) conj(nhat_a(k)) + V_alpha(k) conj(S_Z(k))   [electron-ion Eq. 56 + Ewald reciprocal Eq. 47],
+// evaluated on the half spectrum: the term of a point and of its mirror are equal, so interior columns
+// (0 < ix < nx/2) count twice and the self-mirrored columns ix = 0, nx/2 once.  On a row with a Nyquist ky or kz the
+// mirror of (kx, +N/2, kz) is (-kx, -N/2, -kz), which the literal set replaces by (-kx, +N/2, -kz): such rows are
+// summed as two variants, the literal one and (interior columns only) the one with the Nyquist component flipped
+// (conjugated phase-table entry, S2 instead of S, -N/2 in the k factor).
+// Block = FC_THREADS ions x one slab of (ky,kz) rows; the weighted W rows are staged in shared memory.
 constexpr int FC_THREADS = 128;
-constexpr int FC_NXMAX = 1024;
 __global__ void __launch_bounds__(FC_THREADS) force_kernel(
     GridGeom G, int nions, int rows_per_slab, const double2 *__restrict__ ax_ij /*[ix][j]*/,
     const double2 *__restrict__ by_ij, const double2 *__restrict__ cz_ij, const double *__restrict__ vps,
     const double *__restrict__ va, const double2 *__restrict__ nh_a, const double2 *__restrict__ S,
-    double *__restrict__ F_part /*[slab][j][3]*/) {
-  extern __shared__ double2 s_w[];  // [2][nx]: W and kx*W
-  double2 *s_W = s_w, *s_kW = s_w + G.nx;
+    const double2 *__restrict__ S2, double *__restrict__ F_part /*[slab][j][3]*/) {
+  extern __shared__ double2 s_w[];  // [2][nxh]: W and kx*W
+  double2 *s_W = s_w, *s_kW = s_w + G.nxh;
   const int j = blockIdx.x * FC_THREADS + threadIdx.x;
   const long long nrows = (long long)G.ny * G.nz;
   const long long r0 = (long long)blockIdx.y * rows_per_slab;
   const long long r1 = min(nrows, r0 + rows_per_slab);
+  const int nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
   double fx = 0, fy = 0, fz = 0;
   for (long long row = r0; row < r1; ++row) {
     const int iy = (int)(row % G.ny), iz = (int)(row / G.ny);
-    __syncthreads();
-    for (int ix = threadIdx.x; ix < G.nx; ix += FC_THREADS) {
-      const long long g = row * G.nx + ix;
-      const double2 n = nh_a[g], s = S[g];
-      const double v = vps[g], a = va[g];
-      const double2 w = make_double2(v * n.x + a * s.x, -(v * n.y + a * s.y));
-      s_W[ix] = w;
-      const double kx = G.kx[ix];
-      s_kW[ix] = make_double2(kx * w.x, kx * w.y);
-    }
-    __syncthreads();
-    if (j < nions) {
-      double2 P = make_double2(0, 0), Q = make_double2(0, 0);
-      for (int ix = 0; ix < G.nx; ++ix) {
-        const double2 a = ax_ij[(long long)ix * nions + j];
-        const double2 w = s_W[ix], kw = s_kW[ix];
-        P.x = fma(w.x, a.x, fma(-w.y, a.y, P.x)); P.y = fma(w.x, a.y, fma(w.y, a.x, P.y));
-        Q.x = fma(kw.x, a.x, fma(-kw.y, a.y, Q.x)); Q.y = fma(kw.x, a.y, fma(kw.y, a.x, Q.y));
+    const bool ny_row = iy == nyq_y || iz == nyq_z;
+    for (int var = 0; var < (ny_row ? 2 : 1); ++var) {
+      __syncthreads();
+      for (int ix = threadIdx.x; ix < G.nxh; ix += FC_THREADS) {
+        const long long g = row * G.P + ix;
+        const bool edge = ix == 0 || 2 * ix == G.nx;
+        const double wt = edge ? (var == 0 ? 1.0 : 0.0) : (ny_row ? 1.0 : 2.0);
+        const double2 n = nh_a[g], s = var == 0 ? S[g] : S2[g];
+        const double v = vps[g], a = va[g];
+        const double2 w = make_double2(wt * (v * n.x + a * s.x), -wt * (v * n.y + a * s.y));
+        s_W[ix] = w;
+        const double kx = G.kx[ix];
+        s_kW[ix] = make_double2(kx * w.x, kx * w.y);
       }
-      const double2 b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
-      const double2 bc = make_double2(b.x * c.x - b.y * c.y, b.x * c.y + b.y * c.x);
-      const double imP = P.x * bc.y + P.y * bc.x, imQ = Q.x * bc.y + Q.y * bc.x;
-      fx += imQ; fy += G.ky[iy] * imP; fz += G.kz[iz] * imP;
+      __syncthreads();
+      if (j < nions) {
+        double2 P = make_double2(0, 0), Q = make_double2(0, 0);
+        for (int ix = 0; ix < G.nxh; ++ix) {
+          const double2 a = ax_ij[(long long)ix * nions + j];
+          const double2 w = s_W[ix], kw = s_kW[ix];
+          P.x = fma(w.x, a.x, fma(-w.y, a.y, P.x)); P.y = fma(w.x, a.y, fma(w.y, a.x, P.y));
+          Q.x = fma(kw.x, a.x, fma(-kw.y, a.y, Q.x)); Q.y = fma(kw.x, a.y, fma(kw.y, a.x, Q.y));
+        }
+        double2 b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
+        double ky = G.ky[iy], kz = G.kz[iz];
+        if (var == 1) {
+          if (iy == nyq_y) { b.y = -b.y; ky = -ky; }
+          if (iz == nyq_z) { c.y = -c.y; kz = -kz; }
+        }
+        const double2 bc = make_double2(b.x * c.x - b.y * c.y, b.x * c.y + b.y * c.x);
+        const double imP = P.x * bc.y + P.y * bc.x, imQ = Q.x * bc.y + Q.y * bc.x;
+        fx += imQ; fy += ky * imP; fz += kz * imP;
+      }
     }
   }
   if (j < nions) {

@@ -14,7 +14,7 @@ struct DevScalars {
   // S2 epilogue
   double vmin, vmax, vsum;
   // S3 state
-  double mu, mu_lo, mu_hi, N_last, dNdmu_last;
+  double mu, mu_lo, mu_hi, N_last, dNdmu, n0sum;
   int mu_done, mu_evals, mu_have_prev, pad0;
   // S4
   double K, dn2, na2, F0, Ke, Exc;
@@ -24,7 +24,7 @@ struct DevScalars {
   double w, F_total, F_prev, dn_rel;
   int iter, converged, mu_evals_total, pad1;
   // per-MD-step
-  double U_pp, U_pm_sum, U_ii, init_sum, init_scale, K_i;
+  double U_pp, U_pm_sum, U_pm_fix, U_ii, init_sum, init_scale, K_i;
 };
 
 struct ScfConst {
@@ -56,148 +56,98 @@ __device__ __forceinline__ void xc_pz81(double n, double &eps, double &v) {
   v = (4.0 / 3.0) * ex + vc;
 }
 
-// ---- S1: Vhat(k) = nhat_i(k)/(pi k^2) + Vhat_ie(k), 0 at k = 0 (Eq. 12, 14) ------------------------------
+// Half-spectrum conventions (fft.cuh): G-space arrays are [nz][ny][P], ix = 0..nx/2 stored.  A sum over the full
+// reciprocal grid is sum_half wt(ix) (...), wt = 1 on the self-mirrored columns ix = 0 and (even nx) ix = nx/2, else 2.
+struct HalfGeom {
+  int nx, nxh;  // nxh = nx/2 + 1
+  __device__ __forceinline__ double wt(int ix) const { return (ix == 0 || 2 * ix == nx) ? 1.0 : 2.0; }
+};
+
+// ---- S1: Vhat(k) = nhat_i(k)/(pi k^2) + Vhat_ie(k), 0 at k = 0 (Eq. 12, 14).  When a mixing step is pending the
+// new input density nhat_i <- nhat_a + w (nhat_i - nhat_a) (S6) is formed here and written back.
 struct LoadPotentialG {
-  const double2 *nh_i, *vh_ie;
+  double2 *nh_i;
+  const double2 *nh_a, *vh_ie;
   const double *kx2, *ky2, *kz2;
-  __device__ __forceinline__ void operator()(long long idx, int ix, int iy, int iz, double &re, double &im) const {
+  const DevScalars *sc;
+  int nxh, mix;
+  double w;
+  __device__ __forceinline__ void begin() { w = mix ? sc->w : 1.0; }
+  __device__ __forceinline__ void operator()(long long idx, int ix, int iy, int iz, double &re, double &im) {
+    if (ix >= nxh) { re = 0.0; im = 0.0; return; }
+    double2 a = nh_i[idx];
+    if (mix) {
+      const double2 na = nh_a[idx];
+      a = make_double2(fma(w, a.x - na.x, na.x), fma(w, a.y - na.y, na.y));
+      nh_i[idx] = a;
+    }
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 == 0.0) { re = 0.0; im = 0.0; return; }
     const double inv = 1.0 / (ARCHE_PI * k2);
-    const double2 a = nh_i[idx], b = vh_ie[idx];
+    const double2 b = vh_ie[idx];
     re = fma(a.x, inv, b.x); im = fma(a.y, inv, b.y);
   }
+  __device__ __forceinline__ void finish(double *) {}
 };
 
-// ---- S2: V_i = Re(IFFT)/|Omega| + V_xc(n_i); min/max/sum of V_i; the last block opens the mu bracket ------
+// ---- S2: V_i = IFFT/|Omega| + V_xc(n_i); min/max/sum of V_i; the last block opens the mu bracket.  A pending
+// mixing step forms the real-space n_i here (S6).  When a previous mu exists the first Newton evaluation
+// sum I_{1/2}((mu_prev - V_i)/kT) is taken in the same pass (S3).
 struct StoreVi {
-  double *V_i;
-  const double *n_i;
+  double *V_i, *n_i;
+  const double *n_a;
   DevScalars *sc;
   double *partials;
   unsigned int *counter;
-  double inv_vol, kT_eta0;
-  int xc;
-  double acc_min, acc_max, acc_sum;
-  __device__ __forceinline__ void store(long long idx, int, int, int, double re, double) {
+  const double *fdtab;
+  double inv_vol, kT_eta0, inv_kT;
+  int xc, mix;
+  double w, mu0, acc_min, acc_max, acc_sum, acc_n;
+  int have_mu;
+  __device__ __forceinline__ void begin() {
+    w = mix ? sc->w : 1.0;
+    have_mu = sc->mu_have_prev; mu0 = sc->mu;
+    acc_min = 1.0e308; acc_max = -1.0e308; acc_sum = 0.0; acc_n = 0.0;
+  }
+  __device__ __forceinline__ void store_real(long long idx, int, int, int, double re) {
     double v = re * inv_vol;
-    if (xc) { double e, vx; xc_pz81(n_i[idx], e, vx); v += vx; }
+    double ni = n_i[idx];
+    if (mix) { const double na = n_a[idx]; ni = fma(w, ni - na, na); n_i[idx] = ni; }
+    if (xc) { double e, vx; xc_pz81(ni, e, vx); v += vx; }
     V_i[idx] = v;
     acc_min = fmin(acc_min, v); acc_max = fmax(acc_max, v); acc_sum += v;
+    if (have_mu) { double a, b, c; fd_eval<2>(fdtab, (mu0 - v) * inv_kT, a, b, c); acc_n += b; }
   }
   __device__ __forceinline__ void finish(double *smem) {
-    double v[3] = {acc_min, acc_max, acc_sum};
-    const int op[3] = {1, 2, 0};
-    if (grid_reduce<3>(v, op, partials, counter, smem) && threadIdx.x == 0) {
-      const double *t = smem + 3 * 32;
-      sc->vmin = t[0]; sc->vmax = t[1]; sc->vsum = t[2];
+    double v[4] = {acc_min, acc_max, acc_sum, acc_n};
+    const int op[4] = {1, 2, 0, 0};
+    if (grid_reduce<4>(v, op, partials, counter, smem) && threadIdx.x == 0) {
+      const double *t = smem + 4 * 32;
+      sc->vmin = t[0]; sc->vmax = t[1]; sc->vsum = t[2]; sc->n0sum = t[3];
       // bracket of the root of Eq. 19: N(mu) is increasing and eta0 solves the flat-potential problem
       const double lo = t[0] + kT_eta0, hi = t[1] + kT_eta0;
       const double pad = 1e-12 * (fabs(lo) + fabs(hi) + fabs(kT_eta0));
       sc->mu_lo = lo - pad; sc->mu_hi = hi + pad;
-      sc->mu_done = 0; sc->mu_evals = 0;
     }
   }
 };
 
-// first guess of mu once the bracket is known (separate tiny kernel keeps StoreVi free of grid-size knowledge)
-__global__ void mu_guess_kernel(DevScalars *sc, double ng, double kT_eta0) {
-  double mu0 = sc->mu_have_prev ? sc->mu : sc->vsum / ng + kT_eta0;  // reading D1
-  if (!(mu0 > sc->mu_lo && mu0 < sc->mu_hi)) mu0 = 0.5 * (sc->mu_lo + sc->mu_hi);
-  if (sc->mu_hi - sc->mu_lo <= 4e-16 * fmax(fabs(sc->mu_lo), fabs(sc->mu_hi))) {
-    mu0 = 0.5 * (sc->mu_lo + sc->mu_hi); sc->mu_done = 1;  // flat potential: the bracket is the answer
-  }
-  sc->mu = mu0;
-}
-
-// ---- S3: one Newton-in-bracket pass: N(mu) and dN/dmu over the grid; the last block updates mu -----------
-__global__ void __launch_bounds__(256) mu_pass_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
-                                                      DevScalars *sc, const double *__restrict__ fdtab,
-                                                      double *partials, unsigned int *counter, int last_pass) {
-  __shared__ double s_tab[kFdTabDoubles];
-  __shared__ double s_red[2 * 32 + 2];
-  if (sc->mu_done) return;
-  fd_load_tables(s_tab, fdtab);
-  __syncthreads();
-  const double mu = sc->mu, inv_kT = 1.0 / C.kT;
-  double s1 = 0.0, s0 = 0.0;
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
-    double im12, i12, d;
-    fd_eval<3>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
-    s1 += i12; s0 += im12;
-  }
-  double v[2] = {s1, s0};
-  const int op[2] = {0, 0};
-  if (grid_reduce<2>(v, op, partials, counter, s_red) && threadIdx.x == 0) {
-    const double N = C.cTF * C.dV * s_red[64], dN = C.cTF * C.dV * 0.5 * s_red[65] * inv_kT;
-    const double f = N - C.Ne;
-    sc->N_last = N; sc->dNdmu_last = dN;
-    sc->mu_evals += 1; sc->mu_evals_total += 1;
-    double lo = sc->mu_lo, hi = sc->mu_hi;
-    if (fabs(f) <= 1e-14 * C.Ne || last_pass) {
-      sc->mu_done = 1;
-    } else {
-      if (f > 0.0) hi = mu; else lo = mu;
-      double mu_new = mu - f / dN;
-      if (!(mu_new > lo && mu_new < hi)) mu_new = 0.5 * (lo + hi);
-      if (fabs(mu_new - mu) <= 2e-16 * fmax(fabs(mu), C.kT)) sc->mu_done = 1;
-      sc->mu_lo = lo; sc->mu_hi = hi; sc->mu = mu_new;
-      if (sc->mu_done) sc->mu = mu;  // keep the evaluated point
-    }
-  }
-}
-
-// ---- S4: n_a, chi, Delta n and the local reductions K, ||dn||^2, ||n_a||^2, F0, K_e, E_xc ------------------
-__global__ void __launch_bounds__(256) density_kernel(const double *__restrict__ V_i, const double *__restrict__ n_i,
-                                                      double *__restrict__ n_a, long long ng, ScfConst C,
-                                                      DevScalars *sc, const double *__restrict__ fdtab,
-                                                      double *partials, unsigned int *counter) {
-  __shared__ double s_tab[kFdTabDoubles];
-  __shared__ double s_red[6 * 32 + 6];
-  fd_load_tables(s_tab, fdtab);
-  __syncthreads();
-  const double mu = sc->mu, inv_kT = 1.0 / C.kT;
-  double sK = 0, sdn2 = 0, sna2 = 0, sF0 = 0, sKe = 0, sExc = 0;
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
-    const double eta = (mu - V_i[g]) * inv_kT;
-    double im12, i12, i32;
-    fd_eval<7>(s_tab, eta, im12, i12, i32);
-    const double na = C.cTF * i12;                    // Eq. 9
-    const double chi = C.cTF * 0.5 * im12 * inv_kT;   // dn_a/dmu
-    const double dn = n_i[g] - na;
-    n_a[g] = na;
-    if (chi > 0.0) sK += dn * dn / chi;               // Eq. 31
-    sdn2 += dn * dn; sna2 += na * na;
-    sF0 += eta * i12 - (2.0 / 3.0) * i32;             // f_0/(kT cTF), from Eq. 38-39
-    sKe += i32;                                       // Eq. 38
-    if (C.xc) { double e, vx; xc_pz81(na, e, vx); sExc += na * e; }
-  }
-  double v[6] = {sK, sdn2, sna2, sF0, sKe, sExc};
-  const int op[6] = {0, 0, 0, 0, 0, 0};
-  if (grid_reduce<6>(v, op, partials, counter, s_red) && threadIdx.x == 0) {
-    const double *t = s_red + 6 * 32;
-    sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
-    sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
-  }
-}
-
-// ---- S3+S4 fused: persistent cooperative kernel.  Newton-in-bracket passes for mu separated by one grid-wide
-// barrier each (every block re-sums all block partials in the same fixed order, so all blocks take the same
-// Newton step without a second barrier), then the density pass at the converged mu.  On small grids the V_i
-// values of a thread stay in registers across the passes.
+// ---- S3: mu from charge neutrality (Eq. 19), persistent cooperative kernel.  Newton-type iteration kept inside
+// the bracket (reading D1): the first evaluation comes from the S2 pass when a previous mu exists (slope = dN/dmu of
+// the previous density pass), later slopes are secants; one grid-wide barrier per evaluation.  Every block re-sums
+// all block partials in the same fixed order, so all blocks take the same step.  On small grids the V_i values of a
+// thread stay in registers across the passes.
 constexpr int kMuCache = 4;
-__global__ void __launch_bounds__(256) mu_density_kernel(const double *__restrict__ V_i, const double *__restrict__ n_i,
-                                                         double *__restrict__ n_a, long long ng, ScfConst C,
-                                                         DevScalars *sc, const double *__restrict__ fdtab,
-                                                         double *partials, unsigned int *counter, int max_pass) {
+__global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
+                                                       DevScalars *sc, const double *__restrict__ fdtab,
+                                                       double *partials, int max_pass) {
   namespace cg = cooperative_groups;
   cg::grid_group grid = cg::this_grid();
   __shared__ double s_tab[kFdTabDoubles];
-  __shared__ double s_red[6 * 32 + 6];
+  __shared__ double s_red[2 * 32 + 2];
   __shared__ double s_bc[2];
   fd_load_tables(s_tab, fdtab);
-  __syncthreads();
-  const double inv_kT = 1.0 / C.kT, kT_eta0 = C.kT * C.eta0;
+  const double inv_kT = 1.0 / C.kT, kT_eta0 = C.kT * C.eta0, scaleN = C.cTF * C.dV;
   const long long nthreads = (long long)gridDim.x * blockDim.x, tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const bool cached = ng <= nthreads * kMuCache;
   double vc[kMuCache];
@@ -205,89 +155,120 @@ __global__ void __launch_bounds__(256) mu_density_kernel(const double *__restric
 #pragma unroll
     for (int q = 0; q < kMuCache; ++q) { long long g = tid + q * nthreads; vc[q] = g < ng ? V_i[g] : 0.0; }
   }
-  // bracket and first guess (identical in every block; reading D1)
+  __syncthreads();
   double lo = sc->mu_lo, hi = sc->mu_hi;
-  double mu = sc->mu_have_prev ? sc->mu : sc->vsum / (double)ng + kT_eta0;
-  if (!(mu > lo && mu < hi)) mu = 0.5 * (lo + hi);
-  bool done = false;
-  if (hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi))) { mu = 0.5 * (lo + hi); done = true; }
+  const int have_prev = sc->mu_have_prev;
+  double mu, f = 0.0, slope = 0.0;
+  bool have_f = false, done = false;
   int evals = 0;
-  double *pp = partials;                       // [2][gridDim.x][2]
-  double *pd = partials + 4 * (size_t)gridDim.x;  // density partials [gridDim.x][6]
+  if (hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi))) { mu = 0.5 * (lo + hi); done = true; }  // flat potential
+  else if (have_prev) { mu = sc->mu; f = scaleN * sc->n0sum - C.Ne; slope = sc->dNdmu; have_f = slope > 0.0; evals = have_f; }
+  else mu = sc->vsum / (double)ng + kT_eta0;
+  if (!done && !have_f && !(mu > lo && mu < hi)) mu = 0.5 * (lo + hi);
+  double mu_prev = mu, f_prev = 0.0;
+  bool have_prev_pt = false;
   for (int pass = 0; pass < max_pass && !done; ++pass) {
-    double s1 = 0.0, s0 = 0.0;
-    if (cached) {
+    if (!have_f) {
+      const bool want_slope = !(slope > 0.0);
+      double s1 = 0.0, s0 = 0.0;
+      if (cached) {
 #pragma unroll
-      for (int q = 0; q < kMuCache; ++q) {
-        if (tid + q * nthreads < ng) {
-          double im12, i12, d;
-          fd_eval<3>(s_tab, (mu - vc[q]) * inv_kT, im12, i12, d);
+        for (int q = 0; q < kMuCache; ++q) {
+          if (tid + q * nthreads < ng) {
+            double im12 = 0.0, i12, d;
+            if (want_slope) fd_eval<3>(s_tab, (mu - vc[q]) * inv_kT, im12, i12, d);
+            else fd_eval<2>(s_tab, (mu - vc[q]) * inv_kT, im12, i12, d);
+            s1 += i12; s0 += im12;
+          }
+        }
+      } else {
+        for (long long g = tid; g < ng; g += nthreads) {
+          double im12 = 0.0, i12, d;
+          if (want_slope) fd_eval<3>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
+          else fd_eval<2>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
           s1 += i12; s0 += im12;
         }
       }
-    } else {
-      for (long long g = tid; g < ng; g += nthreads) {
-        double im12, i12, d;
-        fd_eval<3>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
-        s1 += i12; s0 += im12;
-      }
+      double v[2] = {s1, s0};
+      const int op[2] = {0, 0};
+      block_reduce<2>(v, op, s_red);
+      double *buf = partials + (size_t)(pass & 1) * 2 * gridDim.x;
+      if (threadIdx.x == 0) { buf[2 * blockIdx.x] = v[0]; buf[2 * blockIdx.x + 1] = v[1]; }
+      grid.sync();
+      double a[2] = {0.0, 0.0};
+      for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) { a[0] += __ldcg(&buf[2 * b]); a[1] += __ldcg(&buf[2 * b + 1]); }
+      block_reduce<2>(a, op, s_red);
+      if (threadIdx.x == 0) { s_bc[0] = a[0]; s_bc[1] = a[1]; }
+      __syncthreads();
+      f = scaleN * s_bc[0] - C.Ne;
+      if (want_slope) slope = scaleN * 0.5 * s_bc[1] * inv_kT;                                    // dN/dmu (I_j' = j I_{j-1})
+      else if (have_prev_pt && mu != mu_prev) { const double sct = (f - f_prev) / (mu - mu_prev); if (sct > 0.0) slope = sct; }
+      __syncthreads();
+      ++evals;
     }
-    double v[2] = {s1, s0};
-    const int op[2] = {0, 0};
-    block_reduce<2>(v, op, s_red);
-    double *buf = pp + (size_t)(pass & 1) * 2 * gridDim.x;
-    if (threadIdx.x == 0) { buf[2 * blockIdx.x] = v[0]; buf[2 * blockIdx.x + 1] = v[1]; }
-    grid.sync();
-    double a[2] = {0.0, 0.0};
-    for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) { a[0] += __ldcg(&buf[2 * b]); a[1] += __ldcg(&buf[2 * b + 1]); }
-    block_reduce<2>(a, op, s_red);
-    if (threadIdx.x == 0) { s_bc[0] = a[0]; s_bc[1] = a[1]; }
-    __syncthreads();
-    const double N = C.cTF * C.dV * s_bc[0], dN = C.cTF * C.dV * 0.5 * s_bc[1] * inv_kT;
-    __syncthreads();
-    const double f = N - C.Ne;
-    ++evals;
-    if (fabs(f) <= 1e-14 * C.Ne || pass == max_pass - 1) {
-      done = true;
-    } else {
-      if (f > 0.0) hi = mu; else lo = mu;
-      double mu_new = mu - f / dN;
-      if (!(mu_new > lo && mu_new < hi)) mu_new = 0.5 * (lo + hi);
-      if (fabs(mu_new - mu) <= 2e-16 * fmax(fabs(mu), C.kT)) done = true; else mu = mu_new;
-    }
+    have_f = false;
+    if (fabs(f) <= 1e-14 * C.Ne || pass == max_pass - 1) { done = true; break; }
+    if (f > 0.0) hi = fmin(hi, mu); else lo = fmax(lo, mu);
+    double mu_new = mu - f / slope;
+    if (!(mu_new > lo && mu_new < hi)) mu_new = 0.5 * (lo + hi);
+    if (fabs(mu_new - mu) <= 2e-16 * fmax(fabs(mu), C.kT)) { done = true; break; }
+    mu_prev = mu; f_prev = f; have_prev_pt = true;
+    mu = mu_new;
   }
-  // density pass at mu
-  double sK = 0, sdn2 = 0, sna2 = 0, sF0 = 0, sKe = 0, sExc = 0;
-  for (long long g = tid; g < ng; g += nthreads) {
-    const double eta = (mu - V_i[g]) * inv_kT;
-    double im12, i12, i32;
-    fd_eval<7>(s_tab, eta, im12, i12, i32);
-    const double na = C.cTF * i12;
-    const double chi = C.cTF * 0.5 * im12 * inv_kT;
-    const double dn = n_i[g] - na;
-    n_a[g] = na;
-    if (chi > 0.0) sK += dn * dn / chi;
-    sdn2 += dn * dn; sna2 += na * na;
-    sF0 += eta * i12 - (2.0 / 3.0) * i32;
-    sKe += i32;
-    if (C.xc) { double e, vx; xc_pz81(na, e, vx); sExc += na * e; }
-  }
-  double v6[6] = {sK, sdn2, sna2, sF0, sKe, sExc};
-  const int op6[6] = {0, 0, 0, 0, 0, 0};
-  if (grid_reduce<6>(v6, op6, pd, counter, s_red) && threadIdx.x == 0) {
-    const double *t = s_red + 6 * 32;
-    sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
-    sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
-    sc->mu = mu; sc->mu_lo = lo; sc->mu_hi = hi; sc->mu_done = 1; sc->mu_evals = evals; sc->mu_evals_total += evals;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    sc->mu = mu; sc->mu_lo = lo; sc->mu_hi = hi; sc->mu_evals = evals; sc->mu_evals_total += evals; sc->N_last = f + C.Ne;
   }
 }
 
-// ---- S5: forward FFT of the real n_a; epilogue scales by dV, stores nhat_a, reduces U, E_H, E_ie ----------
+// ---- S4 fused into the forward x pass: n_a, chi and the local reductions K, ||dn||^2, ||n_a||^2, F0, K_e, E_xc,
+// dN/dmu are formed while the real lines of n_a are loaded for the transform; n_a is also stored (mixing needs it).
+struct LoadDensity {
+  const double *V_i, *n_i;
+  double *n_a;
+  DevScalars *sc;
+  double *partials;
+  unsigned int *counter;
+  const double *fdtab;
+  ScfConst C;
+  double mu, inv_kT, sK, sdn2, sna2, sF0, sKe, sExc, sChi;
+  __device__ __forceinline__ void begin() {
+    mu = sc->mu; inv_kT = 1.0 / C.kT;
+    sK = sdn2 = sna2 = sF0 = sKe = sExc = sChi = 0.0;
+  }
+  __device__ __forceinline__ double load_real(long long g, int, int, int) {
+    const double eta = (mu - V_i[g]) * inv_kT;
+    double im12, i12, i32;
+    fd_eval<7>(fdtab, eta, im12, i12, i32);
+    const double na = C.cTF * i12;                    // Eq. 9
+    const double chi = C.cTF * 0.5 * im12 * inv_kT;   // dn_a/dmu
+    const double dn = n_i[g] - na;
+    n_a[g] = na;
+    if (chi > 0.0) sK += dn * dn / chi;               // Eq. 31
+    sdn2 += dn * dn; sna2 += na * na; sChi += chi;
+    sF0 += eta * i12 - (2.0 / 3.0) * i32;             // f_0/(kT cTF), from Eq. 38-39
+    sKe += i32;                                       // Eq. 38
+    if (C.xc) { double e, vx; xc_pz81(na, e, vx); sExc += na * e; }
+    return na;
+  }
+  __device__ __forceinline__ void finish(double *smem) {
+    double v[7] = {sK, sdn2, sna2, sF0, sKe, sExc, sChi};
+    const int op[7] = {0, 0, 0, 0, 0, 0, 0};
+    if (grid_reduce<7>(v, op, partials, counter, smem) && threadIdx.x == 0) {
+      const double *t = smem + 7 * 32;
+      sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
+      sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
+      sc->dNdmu = t[6] * C.dV;
+    }
+  }
+};
+
+// ---- S5: forward FFT of the real n_a; the z-pass epilogue scales by dV, stores nhat_a, reduces U, E_H, E_ie ------
 struct LoadReal {
   const double *src;
-  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
-    re = src[idx]; im = 0.0;
-  }
+  __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) { re = src[idx]; im = 0.0; }
+  __device__ __forceinline__ double load_real(long long idx, int, int, int) { return src[idx]; }
+  __device__ __forceinline__ void finish(double *) {}
 };
 
 struct StoreNhatA {
@@ -298,19 +279,23 @@ struct StoreNhatA {
   double *partials;
   unsigned int *counter;
   ScfConst C;
+  HalfGeom H;
   double aU, aEH, aEie;
+  __device__ __forceinline__ void begin() { aU = aEH = aEie = 0.0; }
   __device__ __forceinline__ void store(long long idx, int ix, int iy, int iz, double re, double im) {
+    if (ix >= H.nxh) { nh_a[idx] = make_double2(0.0, 0.0); return; }
     re *= C.dV; im *= C.dV;
     nh_a[idx] = make_double2(re, im);
+    const double wt = H.wt(ix);
     const double2 b = vh_ie[idx];
-    aEie += re * b.x + im * b.y;                       // Re conj(nhat_a) Vhat_ie
+    aEie += wt * (re * b.x + im * b.y);                  // Re conj(nhat_a) Vhat_ie
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 != 0.0) {
-      const double inv = 1.0 / (ARCHE_PI * k2);
+      const double inv = wt / (ARCHE_PI * k2);
       const double2 a = nh_i[idx];
       const double dr = a.x - re, di = a.y - im;
-      aU += (dr * dr + di * di) * inv;                 // Eq. 30
-      aEH += (re * re + im * im) * inv;                // Eq. 53
+      aU += (dr * dr + di * di) * inv;                   // Eq. 30
+      aEH += (re * re + im * im) * inv;                  // Eq. 53
     }
   }
   __device__ __forceinline__ void finish(double *smem) {
@@ -334,52 +319,67 @@ struct StoreNhatA {
   }
 };
 
-// ---- S6: n_o = n_a + w (n_i - n_a) in real and reciprocal space --------------------------------
+// ---- S6: n_o = n_a + w (n_i - n_a) in real and reciprocal space.  Inside the SCF loop this is fused into
+// the next iteration's S1/S2 passes; this kernel materialises a pending step when n_i is read back.
 __global__ void __launch_bounds__(256) mix_kernel(double *__restrict__ n_i, const double *__restrict__ n_a,
                                                   double2 *__restrict__ nh_i, const double2 *__restrict__ nh_a,
-                                                  long long ng, const DevScalars *sc) {
+                                                  long long ng, long long nh, const DevScalars *sc) {
   const double w = sc->w;
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
+  const long long stride = (long long)gridDim.x * blockDim.x, t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  for (long long g = t0; g < ng; g += stride) {
     const double na = n_a[g];
     n_i[g] = fma(w, n_i[g] - na, na);
+  }
+  for (long long g = t0; g < nh; g += stride) {
     const double2 a = nh_a[g], b = nh_i[g];
     nh_i[g] = make_double2(fma(w, b.x - a.x, a.x), fma(w, b.y - a.y, a.y));
   }
 }
 
 // ---- input density: uniform or one-center profile (reading A10) ------------------------
-__global__ void set_uniform_kernel(double *n_i, double2 *nh_i, long long ng, double n0, double Ne) {
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
-    n_i[g] = n0;
-    nh_i[g] = make_double2(g == 0 ? Ne : 0.0, 0.0);
-  }
+__global__ void set_uniform_kernel(double *n_i, double2 *nh_i, long long ng, long long nh, double n0, double Ne) {
+  const long long stride = (long long)gridDim.x * blockDim.x, t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  for (long long g = t0; g < ng; g += stride) n_i[g] = n0;
+  for (long long g = t0; g < nh; g += stride) nh_i[g] = make_double2(g == 0 ? Ne : 0.0, 0.0);
 }
 
-// ghat = nhat_a conj(S)/max(|S|^2, eps Q^2)
-__global__ void g_store_kernel(double2 *__restrict__ gh, const double2 *__restrict__ nh_a, const double2 *__restrict__ S,
-                               long long ng, double epsS) {
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
-    const double2 s = S[g], a = nh_a[g];
-    const double inv = 1.0 / fmax(s.x * s.x + s.y * s.y, epsS);
+// ghat = nhat_a conj(S)/max(|S|^2, eps Q^2) and the same with the Nyquist-flipped S2 (ion_kernels.cuh)
+__global__ void g_store_kernel(double2 *__restrict__ gh, double2 *__restrict__ gh2, const double2 *__restrict__ nh_a,
+                               const double2 *__restrict__ S, const double2 *__restrict__ S2, long long nh, double epsS) {
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < nh; g += (long long)gridDim.x * blockDim.x) {
+    const double2 a = nh_a[g];
+    double2 s = S[g];
+    double inv = 1.0 / fmax(s.x * s.x + s.y * s.y, epsS);
     gh[g] = make_double2((a.x * s.x + a.y * s.y) * inv, (a.y * s.x - a.x * s.y) * inv);
+    s = S2[g];
+    inv = 1.0 / fmax(s.x * s.x + s.y * s.y, epsS);
+    gh2[g] = make_double2((a.x * s.x + a.y * s.y) * inv, (a.y * s.x - a.x * s.y) * inv);
   }
 }
 
-struct LoadSG {  // nhat_i = S_Z^{new} ghat^{old} (Eq. 20)
-  const double2 *S, *gh;
-  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
-    const double2 s = S[idx], g = gh[idx];
-    re = s.x * g.x - s.y * g.y; im = s.x * g.y + s.y * g.x;
+// nhat_i = S_Z^{new} ghat^{old} (Eq. 20) symmetrised so that the half-spectrum inverse returns the real part of the
+// full inverse transform (reading A6): X_sym = (S ghat + S2 ghat2)/2, equal to S ghat off the Nyquist planes.
+struct LoadSG {
+  const double2 *S, *S2, *gh, *gh2;
+  int nxh;
+  __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void operator()(long long idx, int ix, int, int, double &re, double &im) {
+    if (ix >= nxh) { re = 0.0; im = 0.0; return; }
+    const double2 s = S[idx], g = gh[idx], s2 = S2[idx], g2 = gh2[idx];
+    re = 0.5 * ((s.x * g.x - s.y * g.y) + (s2.x * g2.x - s2.y * g2.y));
+    im = 0.5 * ((s.x * g.y + s.y * g.x) + (s2.x * g2.y + s2.y * g2.x));
   }
+  __device__ __forceinline__ void finish(double *) {}
 };
 
-struct StoreClip {  // n_i = max(Re/|Omega|, floor), accumulates sum n_i
+struct StoreClip {  // n_i = max(IFFT/|Omega|, floor), accumulates sum n_i
   double *n_i;
   DevScalars *sc;
   double *partials;
   unsigned int *counter;
   double inv_vol, floor_n, Ne, dV, acc;
-  __device__ __forceinline__ void store(long long idx, int, int, int, double re, double) {
+  __device__ __forceinline__ void begin() { acc = 0.0; }
+  __device__ __forceinline__ void store_real(long long idx, int, int, int, double re) {
     double v = fmax(re * inv_vol, floor_n);
     n_i[idx] = v; acc += v;
   }
@@ -396,23 +396,53 @@ struct StoreClip {  // n_i = max(Re/|Omega|, floor), accumulates sum n_i
 struct LoadRealScaled {  // reads n_i, rescales to N_e, writes it back and feeds the forward FFT
   double *n_i;
   const DevScalars *sc;
-  __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) const {
-    const double v = n_i[idx] * sc->init_scale;
-    n_i[idx] = v; re = v; im = 0.0;
-  }
-};
-
-struct StoreScaled {
-  double2 *dst;
   double scale;
-  __device__ __forceinline__ void store(long long idx, int, int, int, double re, double im) {
-    dst[idx] = make_double2(re * scale, im * scale);
+  __device__ __forceinline__ void begin() { scale = sc->init_scale; }
+  __device__ __forceinline__ double load_real(long long idx, int, int, int) {
+    const double v = n_i[idx] * scale;
+    n_i[idx] = v;
+    return v;
   }
   __device__ __forceinline__ void finish(double *) {}
 };
 
-__global__ void copy_real_kernel(double *dst, const double *src, long long n) {
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < n; g += (long long)gridDim.x * blockDim.x) dst[g] = src[g];
+struct StoreScaled {  // half spectrum, scaled; zero in the padding columns
+  double2 *dst;
+  double scale;
+  int nxh;
+  __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void store(long long idx, int ix, int, int, double re, double im) {
+    dst[idx] = ix < nxh ? make_double2(re * scale, im * scale) : make_double2(0.0, 0.0);
+  }
+  __device__ __forceinline__ void finish(double *) {}
+};
+
+struct StoreRealPlain {
+  double *dst;
+  __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void store_real(long long idx, int, int, int, double v) { dst[idx] = v; }
+  __device__ __forceinline__ void finish(double *) {}
+};
+
+// Full-spectrum view [nz][ny][nx] of a half-spectrum array for read-back: ix <= nx/2 copies src, the rest is
+// conj(src2[mirror]) (src2 = src for DFT-Hermitian fields, the Nyquist-flipped companion for S_Z and ghat);
+// `scale` (optional, half-spectrum real array) multiplies the result (Vhat_ie = v(k) S_Z(k)).
+__global__ void expand_half_kernel(double2 *__restrict__ dst, const double2 *__restrict__ src, const double2 *__restrict__ src2,
+                                   const double *__restrict__ scale, int nx, int ny, int nz, int P) {
+  const long long ng = (long long)nx * ny * nz;
+  const int nxh = nx / 2 + 1;
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < ng; g += (long long)gridDim.x * blockDim.x) {
+    const int ix = (int)(g % nx), iy = (int)((g / nx) % ny), iz = (int)(g / ((long long)nx * ny));
+    double2 v;
+    long long h;
+    if (ix < nxh) { h = ((long long)iz * ny + iy) * P + ix; v = src[h]; }
+    else {
+      h = ((long long)((nz - iz) % nz) * ny + (ny - iy) % ny) * P + (nx - ix);
+      v = src2[h]; v.y = -v.y;
+    }
+    if (scale) { const double sfac = scale[h]; v.x *= sfac; v.y *= sfac; }
+    dst[g] = v;
+  }
 }
 
 __global__ void fermi_dirac_kernel(int twice_j, const double *eta, double *out, size_t n, const double *fdtab) {
