@@ -108,6 +108,13 @@ int arche_get_density(arche_ctx *c, double *d_n); /* = arche_get_real(c, 0, d_n)
 /* 3D complex FFT, unnormalised, out-of-place or in-place (d_in == d_out allowed); sign = -1 forward, +1 inverse.
  * d_scratch: 16*Nx*Ny*Nz bytes. */
 int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, double *d_scratch, int sign);
+/* The transform pair the SCF itself uses: real field [Nz][Ny][Nx] <-> half spectrum, through the r2c / c2r x passes and
+ * the y/z passes (register two-stage kernels for N in {32,64,128,192,256,384}, generic radix kernels otherwise).
+ * forward: d_full_out receives the full unnormalised spectrum [Nz][Ny][Nx] complex (the stored half expanded by
+ * Hermitian symmetry); inverse: d_full_in must be Hermitian (only ix <= Nx/2 is read), d_real_out receives the
+ * unnormalised inverse transform.  Both use the context's FFT scratch array. */
+int arche_rfft3d_forward(arche_ctx *c, const double *d_real_in, double *d_full_out);
+int arche_rfft3d_inverse(arche_ctx *c, const double *d_full_in, double *d_real_out);
 /* I_j(eta) for twice_j in {-1,1,3} on n device values */
 int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta, double *d_out, size_t n);
 /* number of kernels this context has launched so far (for bench.py's gpu_launches) */

@@ -19,6 +19,7 @@ __all__ = ["Arche", "ArcheError", "load", "SYMBOLS", "Params", "Result"]
 SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_last_error", "arche_scf_solve",
            "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_md_step",
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
+           "arche_rfft3d_forward", "arche_rfft3d_inverse",
            "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
@@ -76,6 +77,8 @@ def load(rebuild_if_stale: bool = True):
     L.arche_get_complex.argtypes = [vp, C.c_int, dp]
     L.arche_get_density.argtypes = [vp, dp]
     L.arche_fft3d.argtypes = [vp, dp, dp, dp, C.c_int]
+    L.arche_rfft3d_forward.argtypes = [vp, dp, dp]
+    L.arche_rfft3d_inverse.argtypes = [vp, dp, dp]
     L.arche_fermi_dirac.argtypes = [vp, C.c_int, dp, dp, C.c_size_t]
     L.arche_launch_count.argtypes = [vp]; L.arche_launch_count.restype = C.c_longlong
     L.arche_profile_enable.argtypes = [vp, C.c_int]
@@ -220,6 +223,22 @@ class Arche:
         a = a.to(device=self.device, dtype=t.complex128).contiguous()
         out = t.empty_like(a); scratch = t.empty_like(a)
         self._check(self.lib.arche_fft3d(self._h, a.data_ptr(), out.data_ptr(), scratch.data_ptr(), int(sign)))
+        return out
+
+    def rfft3d_forward(self, a):
+        """real [nz,ny,nx] -> full unnormalised complex spectrum, through the SCF's own r2c passes"""
+        t = self.torch
+        a = a.to(device=self.device, dtype=t.float64).contiguous()
+        out = t.empty(self.shape, dtype=t.complex128, device=self.device)
+        self._check(self.lib.arche_rfft3d_forward(self._h, a.data_ptr(), out.data_ptr()))
+        return out
+
+    def rfft3d_inverse(self, ahat):
+        """Hermitian complex spectrum [nz,ny,nx] -> real unnormalised inverse transform (c2r passes)"""
+        t = self.torch
+        ahat = ahat.to(device=self.device, dtype=t.complex128).contiguous()
+        out = t.empty(self.shape, dtype=t.float64, device=self.device)
+        self._check(self.lib.arche_rfft3d_inverse(self._h, ahat.data_ptr(), out.data_ptr()))
         return out
 
     def fermi_dirac(self, twice_j: int, eta):

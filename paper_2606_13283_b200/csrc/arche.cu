@@ -5,6 +5,7 @@
 
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -13,6 +14,7 @@
 #include "common.cuh"
 #include "fd.cuh"
 #include "fft.cuh"
+#include "fft_fast.cuh"
 #include "ion_kernels.cuh"
 #include "scf_kernels.cuh"
 
@@ -85,6 +87,7 @@ struct arche_ctx {
   double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
   long long nh;      // P*ny*nz
   int nxh, P;
+  bool use_fast;     // register two-stage FFT passes where the axis length has a plan (ARCHE_FFT_GENERIC=1 disables)
   bool mix_pending;  // S6 of the last iteration not yet applied to n_i / nhat_i (fused into the next S1/S2)
   double *kx, *ky, *kz, *kx2, *ky2, *kz2;
   double2 *tw[3];
@@ -235,6 +238,7 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   c->p = *p;
   c->stream = (cudaStream_t)p->stream;
   derive_sizes(c);
+  { const char *e = getenv("ARCHE_FFT_GENERIC"); c->use_fast = !(e && e[0] == '1'); }
   size_t need = layout(c, nullptr);
   if (!p->d_workspace || p->workspace_bytes < need || ((uintptr_t)p->d_workspace & 255)) { delete c; return ARCHE_ENOMEM; }
   layout(c, (char *)p->d_workspace);
@@ -319,28 +323,44 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
 // =============================================================================================
 namespace {
 
+// one y or z pass over the half spectrum: register two-stage kernel for the production sizes, generic kernel otherwise
+template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
+cudaError_t pass_yz(arche_ctx *c, LoadOp ld, StoreOp st) {
+  const int ny = c->G.ny, nz = c->G.nz, P = c->P, n = AXIS == 1 ? ny : nz;
+  FastGeom fg{c->G.nx, ny, nz, P, c->tw[AXIS]};
+  cudaError_t e = c->use_fast ? fft_launch_yz_fast<AXIS, INVERSE>(n, fg, ld, st, c->stream) : cudaErrorNotSupported;
+  if (e == cudaErrorNotSupported) e = fft_launch_pass<AXIS, INVERSE>(c->plan[AXIS], P, ny, nz, ld, st, c->stream);
+  return e;
+}
+template <bool INVERSE, class LoadOp, class StoreOp>
+cudaError_t pass_x(arche_ctx *c, LoadOp ld, StoreOp st) {
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
+  FastGeom fg{nx, ny, nz, P, c->tw[0]};
+  cudaError_t e = c->use_fast ? fft_launch_x_fast<INVERSE>(nx, fg, ld, st, c->stream) : cudaErrorNotSupported;
+  if (e == cudaErrorNotSupported) e = fft_launch_real_x<INVERSE>(c->plan[0], nx, ny, nz, P, ld, st, c->stream);
+  return e;
+}
+
 // inverse (half spectrum -> real field): axis order z, y, x; the x pass is the c2r pass and writes the real field
 template <class LoadOp, class StoreOp>
 int fft3d_inverse(arche_ctx *c, LoadOp ld, StoreOp st, int cls_first = PC_OTHER, int cls_last = PC_OTHER) {
-  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
   { ProfScope ps(c, cls_first);
-    CK((fft_launch_pass<2, true>(c->plan[2], P, ny, nz, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((pass_yz<2, true>(c, ld, StoreComplex{c->work}))); ++c->launches; }
   { ProfScope ps(c, cls_first == PC_OTHER ? PC_OTHER : PC_FFT_Y);
-    CK((fft_launch_pass<1, true>(c->plan[1], P, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((pass_yz<1, true>(c, LoadComplex{c->work}, StoreComplex{c->work}))); ++c->launches; }
   { ProfScope ps(c, cls_last);
-    CK((fft_launch_real_x<true>(c->plan[0], nx, ny, nz, P, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
+    CK((pass_x<true>(c, LoadComplex{c->work}, st))); ++c->launches; }
   return ARCHE_OK;
 }
 // forward (real field -> half spectrum): axis order x (r2c), y, z
 template <class LoadOp, class StoreOp>
 int fft3d_forward(arche_ctx *c, LoadOp ld, StoreOp st, int cls_first = PC_OTHER, int cls_last = PC_OTHER) {
-  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
   { ProfScope ps(c, cls_first);
-    CK((fft_launch_real_x<false>(c->plan[0], nx, ny, nz, P, ld, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((pass_x<false>(c, ld, StoreComplex{c->work}))); ++c->launches; }
   { ProfScope ps(c, cls_first == PC_OTHER ? PC_OTHER : PC_FFT_Y);
-    CK((fft_launch_pass<1, false>(c->plan[1], P, ny, nz, LoadComplex{c->work}, StoreComplex{c->work}, c->stream))); ++c->launches; }
+    CK((pass_yz<1, false>(c, LoadComplex{c->work}, StoreComplex{c->work}))); ++c->launches; }
   { ProfScope ps(c, cls_last);
-    CK((fft_launch_pass<2, false>(c->plan[2], P, ny, nz, LoadComplex{c->work}, st, c->stream))); ++c->launches; }
+    CK((pass_yz<2, false>(c, LoadComplex{c->work}, st))); ++c->launches; }
   return ARCHE_OK;
 }
 
@@ -627,6 +647,22 @@ extern "C" int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, doub
     CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz, LoadComplex{w}, StoreComplex{o}, c->stream))); ++c->launches;
   }
   return ARCHE_OK;
+}
+
+extern "C" int arche_rfft3d_forward(arche_ctx *c, const double *d_real_in, double *d_full_out) {
+  if (!c || !d_real_in || !d_full_out) return ARCHE_EINVAL;
+  int rc = fft3d_forward(c, LoadReal{d_real_in}, StoreComplex{c->work});
+  if (rc) return rc;
+  expand_half_kernel<<<c->ew_grid, 256, 0, c->stream>>>((double2 *)d_full_out, c->work, c->work, nullptr, c->G.nx, c->G.ny, c->G.nz, c->P);
+  LAUNCHED(c);
+  return ARCHE_OK;
+}
+
+extern "C" int arche_rfft3d_inverse(arche_ctx *c, const double *d_full_in, double *d_real_out) {
+  if (!c || !d_full_in || !d_real_out) return ARCHE_EINVAL;
+  compress_half_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->work, (const double2 *)d_full_in, c->G.nx, c->G.ny, c->G.nz, c->P);
+  LAUNCHED(c);
+  return fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{d_real_out});
 }
 
 extern "C" int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta, double *d_out, size_t n) {

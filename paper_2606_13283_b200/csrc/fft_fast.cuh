@@ -1,0 +1,356 @@
+// fft_fast.cuh -- two-stage register FFT passes for the production grid sizes (N = R1*R2 in {32, 64, 128, 192, 256, 384}).
+//
+// Every thread holds one radix-R butterfly (R up to 24) in registers; a 1D transform of length N = R1*R2 is
+//   stage 1:  y[j1*R1 + t'] = DFT_R1{ x[j1 + t*R2] }_t                      j1 in [0,R2)     (no twiddles)
+//   stage 2:  X[j2 + t'*R1] = DFT_R2{ W_N^(t*j2) y[j2 + t*R1] }_t            j2 in [0,R1)
+// with exactly one exchange through shared memory between the stages (Stockham autosort, natural order in and out).
+//   y/z passes: a block owns 8 consecutive x columns (128-byte rows) and all N points of the axis; stage 1 reads global
+//               memory straight into registers, stage 2 stores straight from registers (one smem round trip in total).
+//   x passes:   real <-> half-spectrum (see fft.cuh): a block owns LP pairs of contiguous real lines; the pointwise
+//               prologue/epilogue functors run on all threads, two lines of a pair per thread (one 16-byte smem word).
+// The inverse transform is conj . forward . conj.  Butterflies larger than 4 are Cooley-Tukey compositions in
+// registers with compile-time twiddles (table of cos(2 pi k/48)).
+#pragma once
+#include <type_traits>
+
+#include "fft.cuh"
+
+namespace arche {
+
+// ---- compile-time twiddles -------------------------------------------------------------------------------
+__host__ __device__ constexpr double cos48_quarter(int k) {  // cos(2 pi k/48), k = 0..12
+  constexpr double t[13] = {1.0, 0.99144486137381041114, 0.96592582628906828675, 0.92387953251128675613,
+                            0.86602540378443864676, 0.79335334029123516458, 0.7071067811865475244,
+                            0.60876142900872063942, 0.5, 0.38268343236508977173, 0.25881904510252076235,
+                            0.13052619222005159155, 0.0};
+  return t[k];
+}
+__host__ __device__ constexpr double cos48(int k) {
+  k = ((k % 48) + 48) % 48;
+  if (k > 24) k = 48 - k;
+  return k > 12 ? -cos48_quarter(24 - k) : cos48_quarter(k);
+}
+__host__ __device__ constexpr double sin48(int k) { return cos48(k + 36); }  // sin(t) = cos(t - 90 deg)
+
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+  return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
+}
+
+// v * exp(-2 pi i NUM/DEN), DEN | 48
+template <int NUM, int DEN>
+__device__ __forceinline__ double2 twid(double2 v) {
+  constexpr int k = ((NUM % DEN) + DEN) % DEN * (48 / DEN);  // angle = 2 pi k/48
+  if constexpr (k == 0) return v;
+  else if constexpr (k == 12) return make_double2(v.y, -v.x);   // * (-i)
+  else if constexpr (k == 24) return make_double2(-v.x, -v.y);
+  else if constexpr (k == 36) return make_double2(-v.y, v.x);   // * (+i)
+  else if constexpr (k == 6) { constexpr double c = cos48(6); return make_double2(c * (v.x + v.y), c * (v.y - v.x)); }
+  else if constexpr (k == 18) { constexpr double c = cos48(6); return make_double2(c * (v.y - v.x), -c * (v.x + v.y)); }
+  else if constexpr (k == 30) { constexpr double c = cos48(6); return make_double2(-c * (v.x + v.y), c * (v.x - v.y)); }
+  else if constexpr (k == 42) { constexpr double c = cos48(6); return make_double2(c * (v.x - v.y), c * (v.x + v.y)); }
+  else { constexpr double c = cos48(k), s = sin48(k); return make_double2(fma(v.x, c, v.y * s), fma(v.y, c, -v.x * s)); }
+}
+
+// ---- in-register DFTs (forward, natural order in and out) ------------------------------------------------
+template <int R> struct Dft;
+template <> struct Dft<2> {
+  static __device__ __forceinline__ void run(double2 (&v)[2]) { const double2 a = v[0]; v[0] = cadd(a, v[1]); v[1] = csub(a, v[1]); }
+};
+template <> struct Dft<3> {
+  static __device__ __forceinline__ void run(double2 (&v)[3]) {
+    constexpr double h = 0.86602540378443864676;
+    const double2 s = cadd(v[1], v[2]), d = csub(v[1], v[2]);
+    const double2 m = make_double2(v[0].x - 0.5 * s.x, v[0].y - 0.5 * s.y);
+    v[0] = cadd(v[0], s);
+    v[1] = make_double2(m.x + h * d.y, m.y - h * d.x);
+    v[2] = make_double2(m.x - h * d.y, m.y + h * d.x);
+  }
+};
+template <> struct Dft<4> {
+  static __device__ __forceinline__ void run(double2 (&v)[4]) {
+    const double2 a = cadd(v[0], v[2]), b = csub(v[0], v[2]), c = cadd(v[1], v[3]), d = csub(v[1], v[3]);
+    v[0] = cadd(a, c); v[2] = csub(a, c);
+    v[1] = make_double2(b.x + d.y, b.y - d.x);   // b - i d
+    v[3] = make_double2(b.x - d.y, b.y + d.x);   // b + i d
+  }
+};
+template <int I, int N, class F>
+__device__ __forceinline__ void static_for(F &&f) {
+  if constexpr (I < N) { f(std::integral_constant<int, I>{}); static_for<I + 1, N>(f); }
+}
+// R = A*B (n = A n2 + n1, k = B k1 + k2): DFT_B over the stride-A subsequences, twiddle W_R^(n1 k2), DFT_A over the
+// contiguous groups, transpose to natural order
+template <int A, int B>
+__device__ __forceinline__ void dft_ct(double2 (&v)[A * B]) {
+  constexpr int R = A * B;
+  static_for<0, A>([&](auto n1c) {
+    constexpr int n1 = decltype(n1c)::value;
+    double2 t[B];
+    static_for<0, B>([&](auto n2c) { constexpr int n2 = decltype(n2c)::value; t[n2] = v[A * n2 + n1]; });
+    Dft<B>::run(t);
+    static_for<0, B>([&](auto k2c) { constexpr int k2 = decltype(k2c)::value; v[A * k2 + n1] = twid<n1 * k2, R>(t[k2]); });
+  });
+  double2 o[R];
+  static_for<0, B>([&](auto k2c) {
+    constexpr int k2 = decltype(k2c)::value;
+    double2 t[A];
+    static_for<0, A>([&](auto n1c) { constexpr int n1 = decltype(n1c)::value; t[n1] = v[A * k2 + n1]; });
+    Dft<A>::run(t);
+    static_for<0, A>([&](auto k1c) { constexpr int k1 = decltype(k1c)::value; o[B * k1 + k2] = t[k1]; });
+  });
+  static_for<0, R>([&](auto ic) { constexpr int i = decltype(ic)::value; v[i] = o[i]; });
+}
+template <> struct Dft<6> { static __device__ __forceinline__ void run(double2 (&v)[6]) { dft_ct<2, 3>(v); } };
+template <> struct Dft<8> { static __device__ __forceinline__ void run(double2 (&v)[8]) { dft_ct<2, 4>(v); } };
+template <> struct Dft<12> { static __device__ __forceinline__ void run(double2 (&v)[12]) { dft_ct<3, 4>(v); } };
+template <> struct Dft<16> { static __device__ __forceinline__ void run(double2 (&v)[16]) { dft_ct<4, 4>(v); } };
+template <> struct Dft<24> { static __device__ __forceinline__ void run(double2 (&v)[24]) { dft_ct<3, 8>(v); } };
+
+// ---- plans -----------------------------------------------------------------------------------------------
+template <int N> struct FastPlan { static constexpr bool ok = false; static constexpr int R1 = 1, R2 = 1; };
+template <> struct FastPlan<32> { static constexpr bool ok = true; static constexpr int R1 = 4, R2 = 8; };
+template <> struct FastPlan<64> { static constexpr bool ok = true; static constexpr int R1 = 8, R2 = 8; };
+template <> struct FastPlan<128> { static constexpr bool ok = true; static constexpr int R1 = 8, R2 = 16; };
+template <> struct FastPlan<192> { static constexpr bool ok = true; static constexpr int R1 = 12, R2 = 16; };
+template <> struct FastPlan<256> { static constexpr bool ok = true; static constexpr int R1 = 16, R2 = 16; };
+template <> struct FastPlan<384> { static constexpr bool ok = true; static constexpr int R1 = 16, R2 = 24; };
+static inline bool fft_fast_size(int n) { return n == 32 || n == 64 || n == 128 || n == 192 || n == 256 || n == 384; }
+
+struct FastGeom {
+  int nx, ny, nz, P;        // real grid and half-spectrum pitch
+  const double2 *tw;        // exp(-2 pi i a/N) of the transformed axis
+};
+
+constexpr int kFastL = 8;   // columns per y/z tile (128-byte rows)
+template <int N> __host__ __device__ constexpr int fast_threads_yz() {
+  return kFastL * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
+}
+
+// ---- y / z pass over the half spectrum [nz][ny][P] -------------------------------------------------------
+template <int N, int AXIS, bool INVERSE, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, TH = fast_threads_yz<N>(), JS = TH / kFastL;
+  extern __shared__ double smem_raw[];
+  double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [N][8]
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  ld.begin(); st.begin();
+  const int l = threadIdx.x % kFastL, jj = threadIdx.x / kFastL;
+  const int xt = G.P / kFastL;
+  const int fixed = blockIdx.x / xt, ix = (blockIdx.x % xt) * kFastL + l;   // fixed = iz (AXIS 1) or iy (AXIS 2)
+  const long long stride = AXIS == 1 ? G.P : (long long)G.P * G.ny;
+  const long long base = (AXIS == 1 ? (long long)fixed * G.ny * G.P : (long long)fixed * G.P) + ix;
+  // stage 1: global -> registers -> shared
+  for (int j1 = jj; j1 < R2; j1 += JS) {
+    double2 v[R1];
+#pragma unroll
+    for (int t = 0; t < R1; ++t) {
+      const int i = j1 + t * R2;
+      ld(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, v[t].y);
+      if (INVERSE) v[t].y = -v[t].y;
+    }
+    Dft<R1>::run(v);
+#pragma unroll
+    for (int t = 0; t < R1; ++t) buf[(j1 * R1 + t) * kFastL + l] = v[t];
+  }
+  __syncthreads();
+  // stage 2: shared -> registers -> global
+  for (int j2 = jj; j2 < R1; j2 += JS) {
+    double2 v[R2];
+#pragma unroll
+    for (int t = 0; t < R2; ++t) v[t] = buf[(j2 + t * R1) * kFastL + l];
+#pragma unroll
+    for (int t = 1; t < R2; ++t) v[t] = cmul(v[t], __ldg(&G.tw[t * j2]));
+    Dft<R2>::run(v);
+#pragma unroll
+    for (int t = 0; t < R2; ++t) {
+      const int i = j2 + t * R1;
+      st.store(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, INVERSE ? -v[t].y : v[t].y);
+    }
+  }
+  __syncthreads();
+  ld.finish(smem_raw);
+  st.finish(smem_raw);
+}
+
+// ---- x passes: real lines <-> half spectrum ---------------------------------------------------------------
+constexpr int kFastLP = 8;  // line pairs per block
+template <int N> __host__ __device__ constexpr int fast_threads_x() {
+  return kFastLP * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
+}
+template <int N> __host__ __device__ constexpr int fast_row_x() { return N + N / FastPlan<N>::R1; }   // padded smem row (elements)
+template <int N> __device__ __forceinline__ int fast_pos(int i) { return i + i / FastPlan<N>::R1; }
+
+// the two stages on the block's LP complex lines held in shared memory (in place)
+template <int N>
+__device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *__restrict__ tw) {
+  constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, ROW = fast_row_x<N>();
+  {
+    const int p = threadIdx.x / R2, j1 = threadIdx.x % R2;
+    const bool act = threadIdx.x < kFastLP * R2;
+    double2 v[R1];
+    if (act) {
+#pragma unroll
+      for (int t = 0; t < R1; ++t) v[t] = buf[p * ROW + fast_pos<N>(j1 + t * R2)];
+      Dft<R1>::run(v);
+    }
+    __syncthreads();
+    if (act) {
+#pragma unroll
+      for (int t = 0; t < R1; ++t) buf[p * ROW + j1 * (R1 + 1) + t] = v[t];   // = fast_pos(j1*R1 + t)
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x < kFastLP * R1) {
+    const int p = threadIdx.x / R1, j2 = threadIdx.x % R1;
+    double2 v[R2];
+#pragma unroll
+    for (int t = 0; t < R2; ++t) v[t] = buf[p * ROW + j2 + t * (R1 + 1)];       // = fast_pos(j2 + t*R1)
+#pragma unroll
+    for (int t = 1; t < R2; ++t) v[t] = cmul(v[t], __ldg(&tw[t * j2]));
+    Dft<R2>::run(v);
+#pragma unroll
+    for (int t = 0; t < R2; ++t) buf[p * ROW + j2 + t * (R1 + 1)] = v[t];
+  }
+  __syncthreads();
+}
+
+template <int N, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(fast_threads_x<N>()) fft_r2c_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  constexpr int TH = fast_threads_x<N>(), ROW = fast_row_x<N>(), NXH = N / 2 + 1;
+  extern __shared__ double smem_raw[];
+  double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  ld.begin(); st.begin();
+  const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
+  for (int e = threadIdx.x; e < kFastLP * N; e += TH) {
+    const int p = e / N, i = e % N;
+    const long long la = line0 + 2 * p, lb = la + 1;
+    const double a = ld.load_real(la * N + i, i, (int)(la % G.ny), (int)(la / G.ny));
+    const double b = ld.load_real(lb * N + i, i, (int)(lb % G.ny), (int)(lb / G.ny));
+    buf[p * ROW + fast_pos<N>(i)] = make_double2(a, b);
+  }
+  __syncthreads();
+  fast_stages_x<N>(buf, G.tw);
+  for (int e = threadIdx.x; e < kFastLP * G.P; e += TH) {
+    const int p = e / G.P, k = e % G.P;
+    const long long la = line0 + 2 * p, lb = la + 1;
+    double2 A = make_double2(0.0, 0.0), B = A;
+    if (k < NXH) {
+      const double2 z = buf[p * ROW + fast_pos<N>(k)], m = buf[p * ROW + fast_pos<N>(k == 0 ? 0 : N - k)];
+      A = make_double2(0.5 * (z.x + m.x), 0.5 * (z.y - m.y));
+      B = make_double2(0.5 * (z.y + m.y), -0.5 * (z.x - m.x));
+    }
+    st.store(la * G.P + k, k, (int)(la % G.ny), (int)(la / G.ny), A.x, A.y);
+    st.store(lb * G.P + k, k, (int)(lb % G.ny), (int)(lb / G.ny), B.x, B.y);
+  }
+  __syncthreads();
+  ld.finish(smem_raw);
+  st.finish(smem_raw);
+}
+
+template <int N, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  constexpr int TH = fast_threads_x<N>(), ROW = fast_row_x<N>(), NXH = N / 2 + 1;
+  extern __shared__ double smem_raw[];
+  double2 *buf = reinterpret_cast<double2 *>(smem_raw);
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  ld.begin(); st.begin();
+  const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
+  for (int e = threadIdx.x; e < kFastLP * NXH; e += TH) {
+    const int p = e / NXH, k = e % NXH;
+    const long long la = line0 + 2 * p, lb = la + 1;
+    double2 A, B;
+    ld(la * G.P + k, k, (int)(la % G.ny), (int)(la / G.ny), A.x, A.y);
+    ld(lb * G.P + k, k, (int)(lb % G.ny), (int)(lb / G.ny), B.x, B.y);
+    buf[p * ROW + fast_pos<N>(k)] = make_double2(A.x - B.y, -(A.y + B.x));              // conj(A + i B)
+    if (k > 0 && 2 * k < N) buf[p * ROW + fast_pos<N>(N - k)] = make_double2(A.x + B.y, A.y - B.x);  // conj(conj A + i conj B)
+  }
+  __syncthreads();
+  fast_stages_x<N>(buf, G.tw);
+  for (int e = threadIdx.x; e < kFastLP * N; e += TH) {
+    const int p = e / N, i = e % N;
+    const long long la = line0 + 2 * p, lb = la + 1;
+    const double2 z = buf[p * ROW + fast_pos<N>(i)];
+    st.store_real(la * N + i, i, (int)(la % G.ny), (int)(la / G.ny), z.x);
+    st.store_real(lb * N + i, i, (int)(lb % G.ny), (int)(lb / G.ny), -z.y);
+  }
+  __syncthreads();
+  ld.finish(smem_raw);
+  st.finish(smem_raw);
+}
+
+// ---- host dispatch ------------------------------------------------------------------------------------------
+template <int N, int AXIS, bool INVERSE, class LoadOp, class StoreOp>
+static inline cudaError_t fft_launch_yz_fast_n(const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
+  auto kern = fft_yz_fast_kernel<N, AXIS, INVERSE, LoadOp, StoreOp>;
+  size_t smem = sizeof(double2) * N * kFastL;
+  if (smem < 4096) smem = 4096;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const unsigned blocks = (unsigned)((AXIS == 1 ? G.nz : G.ny) * (G.P / kFastL));
+  kern<<<blocks, fast_threads_yz<N>(), smem, stream>>>(G, ld, st);
+  return cudaGetLastError();
+}
+// returns cudaErrorNotSupported when the axis length has no fast plan (caller falls back to the generic pass)
+template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
+static inline cudaError_t fft_launch_yz_fast(int n, const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
+  switch (n) {
+    case 32: return fft_launch_yz_fast_n<32, AXIS, INVERSE>(G, ld, st, stream);
+    case 64: return fft_launch_yz_fast_n<64, AXIS, INVERSE>(G, ld, st, stream);
+    case 128: return fft_launch_yz_fast_n<128, AXIS, INVERSE>(G, ld, st, stream);
+    case 192: return fft_launch_yz_fast_n<192, AXIS, INVERSE>(G, ld, st, stream);
+    case 256: return fft_launch_yz_fast_n<256, AXIS, INVERSE>(G, ld, st, stream);
+    case 384: return fft_launch_yz_fast_n<384, AXIS, INVERSE>(G, ld, st, stream);
+    default: return cudaErrorNotSupported;
+  }
+}
+
+template <int N, bool INVERSE, class LoadOp, class StoreOp>
+static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
+  size_t smem = sizeof(double2) * kFastLP * fast_row_x<N>();
+  if (smem < 4096) smem = 4096;
+  const unsigned blocks = (unsigned)((long long)G.ny * G.nz / (2 * kFastLP));
+  static bool attr_set = false;
+  if constexpr (INVERSE) {
+    auto kern = fft_c2r_fast_kernel<N, LoadOp, StoreOp>;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    kern<<<blocks, fast_threads_x<N>(), smem, stream>>>(G, ld, st);
+  } else {
+    auto kern = fft_r2c_fast_kernel<N, LoadOp, StoreOp>;
+    if (!attr_set) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+      if (e != cudaSuccess) return e;
+      attr_set = true;
+    }
+    kern<<<blocks, fast_threads_x<N>(), smem, stream>>>(G, ld, st);
+  }
+  return cudaGetLastError();
+}
+template <bool INVERSE, class LoadOp, class StoreOp>
+static inline cudaError_t fft_launch_x_fast(int n, const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
+  if (((long long)G.ny * G.nz) % (2 * kFastLP) != 0) return cudaErrorNotSupported;
+  switch (n) {
+    case 32: return fft_launch_x_fast_n<32, INVERSE>(G, ld, st, stream);
+    case 64: return fft_launch_x_fast_n<64, INVERSE>(G, ld, st, stream);
+    case 128: return fft_launch_x_fast_n<128, INVERSE>(G, ld, st, stream);
+    case 192: return fft_launch_x_fast_n<192, INVERSE>(G, ld, st, stream);
+    case 256: return fft_launch_x_fast_n<256, INVERSE>(G, ld, st, stream);
+    case 384: return fft_launch_x_fast_n<384, INVERSE>(G, ld, st, stream);
+    default: return cudaErrorNotSupported;
+  }
+}
+
+}  // namespace arche

@@ -445,6 +445,17 @@ __global__ void expand_half_kernel(double2 *__restrict__ dst, const double2 *__r
   }
 }
 
+// half <- the stored columns of a full [nz][ny][nx] complex array (zero padding columns)
+__global__ void compress_half_kernel(double2 *__restrict__ dst, const double2 *__restrict__ src, int nx, int ny, int nz, int P) {
+  const long long nh = (long long)P * ny * nz;
+  const int nxh = nx / 2 + 1;
+  for (long long h = (long long)blockIdx.x * blockDim.x + threadIdx.x; h < nh; h += (long long)gridDim.x * blockDim.x) {
+    const int ix = (int)(h % P);
+    const long long row = h / P;
+    dst[h] = ix < nxh ? src[row * nx + ix] : make_double2(0.0, 0.0);
+  }
+}
+
 __global__ void fermi_dirac_kernel(int twice_j, const double *eta, double *out, size_t n, const double *fdtab) {
   __shared__ double s_tab[kFdTabDoubles];
   fd_load_tables(s_tab, fdtab);
