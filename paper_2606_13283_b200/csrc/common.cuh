@@ -21,6 +21,10 @@ struct GridGeom {
   const double *kx2, *ky2, *kz2;  // squares
 };
 
+// L2 prefetch of the 128-byte line holding *p: the fused passes request every operand line of a tile up front, so
+// the later (register-limited, partly serialised) loads find their data in L2 instead of paying HBM latency each
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -113,10 +113,12 @@ __device__ __forceinline__ void fft_stage(const double *__restrict__ sre, const 
 // Plain complex array load / store functors.
 // Functor protocol (all passes): begin() once per thread at kernel start; load: operator()(idx, ix, iy, iz, re, im)
 // (complex) or load_real(idx, ix, iy, iz); store(idx, ix, iy, iz, re, im) or store_real(idx, ix, iy, iz, v);
-// finish(smem) once per block at the end (grid reductions; smem = the tile buffer, free by then).
+// finish(smem) once per block at the end (grid reductions; smem = the tile buffer, free by then);
+// prefetch(idx): L2 prefetch of the operand lines the functor will touch at element idx (fast passes only).
 struct LoadComplex {
   const double2 *src;
   __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(src + idx); }
   __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) {
     double2 v = src[idx]; re = v.x; im = v.y;
   }
@@ -125,6 +127,7 @@ struct LoadComplex {
 struct StoreComplex {
   double2 *dst;
   __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long) const {}
   __device__ __forceinline__ void store(long long idx, int, int, int, double re, double im) { dst[idx] = make_double2(re, im); }
   __device__ __forceinline__ void finish(double *) {}
 };

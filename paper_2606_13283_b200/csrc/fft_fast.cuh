@@ -142,6 +142,14 @@ __global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastG
   const int fixed = blockIdx.x / xt, ix = (blockIdx.x % xt) * kFastL + l;   // fixed = iz (AXIS 1) or iy (AXIS 2)
   const long long stride = AXIS == 1 ? G.P : (long long)G.P * G.ny;
   const long long base = (AXIS == 1 ? (long long)fixed * G.ny * G.P : (long long)fixed * G.P) + ix;
+  if (l == 0) {  // one lane per 128-byte row: request every operand line of the tile now
+    for (int j1 = jj; j1 < R2; j1 += JS)
+#pragma unroll
+      for (int t = 0; t < R1; ++t) ld.prefetch(base + (j1 + t * R2) * stride);
+    for (int j2 = jj; j2 < R1; j2 += JS)
+#pragma unroll
+      for (int t = 0; t < R2; ++t) st.prefetch(base + (j2 + t * R1) * stride);
+  }
   // stage 1: global -> registers -> shared
   for (int j1 = jj; j1 < R2; j1 += JS) {
     double2 v[R1];
@@ -226,11 +234,12 @@ __global__ void __launch_bounds__(fast_threads_x<N>()) fft_r2c_fast_kernel(FastG
   StoreOp st = st_in;
   ld.begin(); st.begin();
   const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
+  for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
   for (int e = threadIdx.x; e < kFastLP * N; e += TH) {
     const int p = e / N, i = e % N;
     const long long la = line0 + 2 * p, lb = la + 1;
-    const double a = ld.load_real(la * N + i, i, (int)(la % G.ny), (int)(la / G.ny));
-    const double b = ld.load_real(lb * N + i, i, (int)(lb % G.ny), (int)(lb / G.ny));
+    double a, b;
+    ld.load_real2(la * N + i, lb * N + i, a, b);
     buf[p * ROW + fast_pos<N>(i)] = make_double2(a, b);
   }
   __syncthreads();
@@ -261,6 +270,8 @@ __global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastG
   StoreOp st = st_in;
   ld.begin(); st.begin();
   const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
+  for (int e = threadIdx.x * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile
+  for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) st.prefetch(line0 * N + e);    // operands of the epilogue
   for (int e = threadIdx.x; e < kFastLP * NXH; e += TH) {
     const int p = e / NXH, k = e % NXH;
     const long long la = line0 + 2 * p, lb = la + 1;
@@ -276,8 +287,7 @@ __global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastG
     const int p = e / N, i = e % N;
     const long long la = line0 + 2 * p, lb = la + 1;
     const double2 z = buf[p * ROW + fast_pos<N>(i)];
-    st.store_real(la * N + i, i, (int)(la % G.ny), (int)(la / G.ny), z.x);
-    st.store_real(lb * N + i, i, (int)(lb % G.ny), (int)(lb / G.ny), -z.y);
+    st.store_real2(la * N + i, lb * N + i, z.x, -z.y);
   }
   __syncthreads();
   ld.finish(smem_raw);

@@ -73,6 +73,10 @@ struct LoadPotentialG {
   int nxh, mix;
   double w;
   __device__ __forceinline__ void begin() { w = mix ? sc->w : 1.0; }
+  __device__ __forceinline__ void prefetch(long long idx) const {
+    prefetch_l2(nh_i + idx); prefetch_l2(vh_ie + idx);
+    if (mix) prefetch_l2(nh_a + idx);
+  }
   __device__ __forceinline__ void operator()(long long idx, int ix, int iy, int iz, double &re, double &im) {
     if (ix >= nxh) { re = 0.0; im = 0.0; return; }
     double2 a = nh_i[idx];
@@ -109,6 +113,10 @@ struct StoreVi {
     have_mu = sc->mu_have_prev; mu0 = sc->mu;
     acc_min = 1.0e308; acc_max = -1.0e308; acc_sum = 0.0; acc_n = 0.0;
   }
+  __device__ __forceinline__ void prefetch(long long idx) const {
+    prefetch_l2(n_i + idx);
+    if (mix) prefetch_l2(n_a + idx);
+  }
   __device__ __forceinline__ void store_real(long long idx, int, int, int, double re) {
     double v = re * inv_vol;
     double ni = n_i[idx];
@@ -117,6 +125,28 @@ struct StoreVi {
     V_i[idx] = v;
     acc_min = fmin(acc_min, v); acc_max = fmax(acc_max, v); acc_sum += v;
     if (have_mu) { double a, b, c; fd_eval<2>(fdtab, (mu0 - v) * inv_kT, a, b, c); acc_n += b; }
+  }
+  // two elements at once (the two lines of an x-pass pair): interleaves the two Fermi-Dirac evaluations
+  __device__ __forceinline__ void store_real2(long long ia, long long ib, double ra, double rb) {
+    double v[2] = {ra * inv_vol, rb * inv_vol};
+    double ni[2] = {n_i[ia], n_i[ib]};
+    if (mix) {
+      const double na0 = n_a[ia], na1 = n_a[ib];
+      ni[0] = fma(w, ni[0] - na0, na0); ni[1] = fma(w, ni[1] - na1, na1);
+      n_i[ia] = ni[0]; n_i[ib] = ni[1];
+    }
+    if (xc) {
+      double e, vx;
+      xc_pz81(ni[0], e, vx); v[0] += vx;
+      xc_pz81(ni[1], e, vx); v[1] += vx;
+    }
+    V_i[ia] = v[0]; V_i[ib] = v[1];
+    acc_min = fmin(acc_min, fmin(v[0], v[1])); acc_max = fmax(acc_max, fmax(v[0], v[1])); acc_sum += v[0]; acc_sum += v[1];
+    if (have_mu) {
+      double eta[2] = {(mu0 - v[0]) * inv_kT, (mu0 - v[1]) * inv_kT}, a[2], b[2], c[2];
+      fd_eval_multi<2, 2>(fdtab, eta, a, b, c);
+      acc_n += b[0]; acc_n += b[1];
+    }
   }
   __device__ __forceinline__ void finish(double *smem) {
     double v[4] = {acc_min, acc_max, acc_sum, acc_n};
@@ -138,6 +168,18 @@ struct StoreVi {
 // all block partials in the same fixed order, so all blocks take the same step.  On small grids the V_i values of a
 // thread stay in registers across the passes.
 constexpr int kMuCache = 4;
+// sum of I_{1/2} (and I_{-1/2} when SLOPE) over four potentials at once
+template <bool SLOPE>
+__device__ __forceinline__ void mu_accumulate4(const double *tab, const double (&v)[4], const bool (&ok)[4], double mu,
+                                               double inv_kT, double &s1, double &s0) {
+  double eta[4], im12[4] = {0.0, 0.0, 0.0, 0.0}, i12[4], d[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) eta[q] = ok[q] ? (mu - v[q]) * inv_kT : 1.0;
+  fd_eval_multi<SLOPE ? 3 : 2, 4>(tab, eta, im12, i12, d);
+#pragma unroll
+  for (int q = 0; q < 4; ++q) if (ok[q]) { s1 += i12[q]; s0 += im12[q]; }
+}
+
 __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
                                                        DevScalars *sc, const double *__restrict__ fdtab,
                                                        double *partials, int max_pass) {
@@ -172,21 +214,18 @@ __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict_
       const bool want_slope = !(slope > 0.0);
       double s1 = 0.0, s0 = 0.0;
       if (cached) {
+        bool ok[4];
 #pragma unroll
-        for (int q = 0; q < kMuCache; ++q) {
-          if (tid + q * nthreads < ng) {
-            double im12 = 0.0, i12, d;
-            if (want_slope) fd_eval<3>(s_tab, (mu - vc[q]) * inv_kT, im12, i12, d);
-            else fd_eval<2>(s_tab, (mu - vc[q]) * inv_kT, im12, i12, d);
-            s1 += i12; s0 += im12;
-          }
-        }
+        for (int q = 0; q < 4; ++q) ok[q] = tid + q * nthreads < ng;
+        if (want_slope) mu_accumulate4<true>(s_tab, vc, ok, mu, inv_kT, s1, s0);
+        else mu_accumulate4<false>(s_tab, vc, ok, mu, inv_kT, s1, s0);
       } else {
-        for (long long g = tid; g < ng; g += nthreads) {
-          double im12 = 0.0, i12, d;
-          if (want_slope) fd_eval<3>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
-          else fd_eval<2>(s_tab, (mu - V_i[g]) * inv_kT, im12, i12, d);
-          s1 += i12; s0 += im12;
+        for (long long g0 = tid; g0 < ng; g0 += 4 * nthreads) {
+          double vv[4]; bool ok[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) { const long long g = g0 + q * nthreads; ok[q] = g < ng; vv[q] = ok[q] ? V_i[g] : 0.0; }
+          if (want_slope) mu_accumulate4<true>(s_tab, vv, ok, mu, inv_kT, s1, s0);
+          else mu_accumulate4<false>(s_tab, vv, ok, mu, inv_kT, s1, s0);
         }
       }
       double v[2] = {s1, s0};
@@ -235,6 +274,7 @@ struct LoadDensity {
     mu = sc->mu; inv_kT = 1.0 / C.kT;
     sK = sdn2 = sna2 = sF0 = sKe = sExc = sChi = 0.0;
   }
+  __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(V_i + idx); prefetch_l2(n_i + idx); }
   __device__ __forceinline__ double load_real(long long g, int, int, int) {
     const double eta = (mu - V_i[g]) * inv_kT;
     double im12, i12, i32;
@@ -249,6 +289,26 @@ struct LoadDensity {
     sKe += i32;                                       // Eq. 38
     if (C.xc) { double e, vx; xc_pz81(na, e, vx); sExc += na * e; }
     return na;
+  }
+  __device__ __forceinline__ void load_real2(long long ia, long long ib, double &ra, double &rb) {
+    const long long g[2] = {ia, ib};
+    double eta[2] = {(mu - V_i[ia]) * inv_kT, (mu - V_i[ib]) * inv_kT}, im12[2], i12[2], i32[2];
+    const double ni[2] = {n_i[ia], n_i[ib]};
+    fd_eval_multi<7, 2>(fdtab, eta, im12, i12, i32);
+    double na[2];
+#pragma unroll
+    for (int m = 0; m < 2; ++m) {
+      na[m] = C.cTF * i12[m];
+      const double chi = C.cTF * 0.5 * im12[m] * inv_kT;
+      const double dn = ni[m] - na[m];
+      n_a[g[m]] = na[m];
+      if (chi > 0.0) sK += dn * dn / chi;
+      sdn2 += dn * dn; sna2 += na[m] * na[m]; sChi += chi;
+      sF0 += eta[m] * i12[m] - (2.0 / 3.0) * i32[m];
+      sKe += i32[m];
+      if (C.xc) { double e, vx; xc_pz81(na[m], e, vx); sExc += na[m] * e; }
+    }
+    ra = na[0]; rb = na[1];
   }
   __device__ __forceinline__ void finish(double *smem) {
     double v[7] = {sK, sdn2, sna2, sF0, sKe, sExc, sChi};
@@ -266,8 +326,10 @@ struct LoadDensity {
 struct LoadReal {
   const double *src;
   __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(src + idx); }
   __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) { re = src[idx]; im = 0.0; }
   __device__ __forceinline__ double load_real(long long idx, int, int, int) { return src[idx]; }
+  __device__ __forceinline__ void load_real2(long long ia, long long ib, double &ra, double &rb) { ra = src[ia]; rb = src[ib]; }
   __device__ __forceinline__ void finish(double *) {}
 };
 
@@ -282,6 +344,7 @@ struct StoreNhatA {
   HalfGeom H;
   double aU, aEH, aEie;
   __device__ __forceinline__ void begin() { aU = aEH = aEie = 0.0; }
+  __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(vh_ie + idx); prefetch_l2(nh_i + idx); }
   __device__ __forceinline__ void store(long long idx, int ix, int iy, int iz, double re, double im) {
     if (ix >= H.nxh) { nh_a[idx] = make_double2(0.0, 0.0); return; }
     re *= C.dV; im *= C.dV;
@@ -363,6 +426,9 @@ struct LoadSG {
   const double2 *S, *S2, *gh, *gh2;
   int nxh;
   __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long idx) const {
+    prefetch_l2(S + idx); prefetch_l2(S2 + idx); prefetch_l2(gh + idx); prefetch_l2(gh2 + idx);
+  }
   __device__ __forceinline__ void operator()(long long idx, int ix, int, int, double &re, double &im) {
     if (ix >= nxh) { re = 0.0; im = 0.0; return; }
     const double2 s = S[idx], g = gh[idx], s2 = S2[idx], g2 = gh2[idx];
@@ -379,9 +445,13 @@ struct StoreClip {  // n_i = max(IFFT/|Omega|, floor), accumulates sum n_i
   unsigned int *counter;
   double inv_vol, floor_n, Ne, dV, acc;
   __device__ __forceinline__ void begin() { acc = 0.0; }
+  __device__ __forceinline__ void prefetch(long long) const {}
   __device__ __forceinline__ void store_real(long long idx, int, int, int, double re) {
     double v = fmax(re * inv_vol, floor_n);
     n_i[idx] = v; acc += v;
+  }
+  __device__ __forceinline__ void store_real2(long long ia, long long ib, double ra, double rb) {
+    store_real(ia, 0, 0, 0, ra); store_real(ib, 0, 0, 0, rb);
   }
   __device__ __forceinline__ void finish(double *smem) {
     double v[1] = {acc};
@@ -398,10 +468,14 @@ struct LoadRealScaled {  // reads n_i, rescales to N_e, writes it back and feeds
   const DevScalars *sc;
   double scale;
   __device__ __forceinline__ void begin() { scale = sc->init_scale; }
+  __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(n_i + idx); }
   __device__ __forceinline__ double load_real(long long idx, int, int, int) {
     const double v = n_i[idx] * scale;
     n_i[idx] = v;
     return v;
+  }
+  __device__ __forceinline__ void load_real2(long long ia, long long ib, double &ra, double &rb) {
+    ra = load_real(ia, 0, 0, 0); rb = load_real(ib, 0, 0, 0);
   }
   __device__ __forceinline__ void finish(double *) {}
 };
@@ -411,6 +485,7 @@ struct StoreScaled {  // half spectrum, scaled; zero in the padding columns
   double scale;
   int nxh;
   __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long) const {}
   __device__ __forceinline__ void store(long long idx, int ix, int, int, double re, double im) {
     dst[idx] = ix < nxh ? make_double2(re * scale, im * scale) : make_double2(0.0, 0.0);
   }
@@ -420,7 +495,9 @@ struct StoreScaled {  // half spectrum, scaled; zero in the padding columns
 struct StoreRealPlain {
   double *dst;
   __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long) const {}
   __device__ __forceinline__ void store_real(long long idx, int, int, int, double v) { dst[idx] = v; }
+  __device__ __forceinline__ void store_real2(long long ia, long long ib, double ra, double rb) { dst[ia] = ra; dst[ib] = rb; }
   __device__ __forceinline__ void finish(double *) {}
 };
 
