@@ -12,6 +12,7 @@ Method (own fits; no published coefficient table is used; nothing here is shared
   segment NB+1       (eta >= ETA_C):        I_j = eta^(j+1) * P(t), t from u = 1/eta^2 on [0, 1/ETA_C^2].
 The poles of the Fermi function sit at eta +- i pi, so a Chebyshev interpolant on a segment of half-width h
 converges like rho^-n with rho = pi/h + sqrt((pi/h)^2 + 1): W = 0.5 gives rho = 25 and degree 11 reaches 1e-16.
+Region B reaches down to eta = -24 so that hot, dilute plasmas (eta << 0) never pay for an exp() per grid point.
 Each P is the Chebyshev interpolant of degree FD_NC-1 converted to monomials in t in [-1,1] (Horner on the
 device: 11 FMAs per function).  The script checks every segment in simulated double precision against mpmath
 and fails if the relative error exceeds 1e-15.
@@ -25,7 +26,7 @@ import numpy as np
 
 mp.mp.dps = 40
 NC = 12
-ETA_A = -2.0
+ETA_A = -24.0
 ETA_C = 40.0
 W = 0.5
 NB = int(round((ETA_C - ETA_A) / W))
