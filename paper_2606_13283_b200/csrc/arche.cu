@@ -275,9 +275,12 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, 0));
-    long long gmax = (long long)sms * per_sm, want = (c->ng + 255) / 256;
-    if (gmax > kEwBlocks) gmax = kEwBlocks;
-    c->mu_grid = (int)(want < gmax ? want : gmax);
+    // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
+    if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
+    const long long cache_pts = (long long)sms * 256 * kMuCache;
+    long long blocks = c->ng <= cache_pts ? sms : (long long)sms * (per_sm < 3 ? per_sm : 3);
+    const long long want = (c->ng + 255) / 256;
+    c->mu_grid = (int)(want < blocks ? want : blocks);
     if (c->mu_grid < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
   }
   // ---- per-axis tables: k, k^2, twiddles (long double on the host)

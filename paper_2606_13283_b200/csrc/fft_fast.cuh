@@ -185,9 +185,9 @@ __global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastG
 
 // ---- x passes: real lines <-> half spectrum ---------------------------------------------------------------
 constexpr int kFastLP = 8;  // line pairs per block
-template <int N> __host__ __device__ constexpr int fast_threads_x() {
-  return kFastLP * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
-}
+// 256 threads: the FFT stages need only LP*max(R1,R2) <= 192 of them, the pointwise prologue/epilogue (Fermi-Dirac
+// integrals, XC) uses all
+template <int N> __host__ __device__ constexpr int fast_threads_x() { return 256; }
 template <int N> __host__ __device__ constexpr int fast_row_x() { return N + N / FastPlan<N>::R1; }   // padded smem row (elements)
 template <int N> __device__ __forceinline__ int fast_pos(int i) { return i + i / FastPlan<N>::R1; }
 

@@ -167,7 +167,7 @@ struct StoreVi {
 // the previous density pass), later slopes are secants; one grid-wide barrier per evaluation.  Every block re-sums
 // all block partials in the same fixed order, so all blocks take the same step.  On small grids the V_i values of a
 // thread stay in registers across the passes.
-constexpr int kMuCache = 4;
+constexpr int kMuCache = 8;
 // sum of I_{1/2} (and I_{-1/2} when SLOPE) over four potentials at once
 template <bool SLOPE>
 __device__ __forceinline__ void mu_accumulate4(const double *tab, const double (&v)[4], const bool (&ok)[4], double mu,
@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict_
   double lo = sc->mu_lo, hi = sc->mu_hi;
   const int have_prev = sc->mu_have_prev;
   double mu, f = 0.0, slope = 0.0;
-  bool have_f = false, done = false;
+  bool have_f = false, done = false, slope_fresh = false;   // slope_fresh: exact or secant (not the previous iteration's)
   int evals = 0;
   if (hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi))) { mu = 0.5 * (lo + hi); done = true; }  // flat potential
   else if (have_prev) { mu = sc->mu; f = scaleN * sc->n0sum - C.Ne; slope = sc->dNdmu; have_f = slope > 0.0; evals = have_f; }
@@ -214,11 +214,15 @@ __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict_
       const bool want_slope = !(slope > 0.0);
       double s1 = 0.0, s0 = 0.0;
       if (cached) {
-        bool ok[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) ok[q] = tid + q * nthreads < ng;
-        if (want_slope) mu_accumulate4<true>(s_tab, vc, ok, mu, inv_kT, s1, s0);
-        else mu_accumulate4<false>(s_tab, vc, ok, mu, inv_kT, s1, s0);
+        for (int h = 0; h < kMuCache; h += 4) {
+          bool ok[4]; double vv[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) { ok[q] = tid + (h + q) * nthreads < ng; vv[q] = vc[h + q]; }
+          if (!ok[0]) break;
+          if (want_slope) mu_accumulate4<true>(s_tab, vv, ok, mu, inv_kT, s1, s0);
+          else mu_accumulate4<false>(s_tab, vv, ok, mu, inv_kT, s1, s0);
+        }
       } else {
         for (long long g0 = tid; g0 < ng; g0 += 4 * nthreads) {
           double vv[4]; bool ok[4];
@@ -240,8 +244,8 @@ __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict_
       if (threadIdx.x == 0) { s_bc[0] = a[0]; s_bc[1] = a[1]; }
       __syncthreads();
       f = scaleN * s_bc[0] - C.Ne;
-      if (want_slope) slope = scaleN * 0.5 * s_bc[1] * inv_kT;                                    // dN/dmu (I_j' = j I_{j-1})
-      else if (have_prev_pt && mu != mu_prev) { const double sct = (f - f_prev) / (mu - mu_prev); if (sct > 0.0) slope = sct; }
+      if (want_slope) { slope = scaleN * 0.5 * s_bc[1] * inv_kT; slope_fresh = true; }           // dN/dmu (I_j' = j I_{j-1})
+      else if (have_prev_pt && mu != mu_prev) { const double sct = (f - f_prev) / (mu - mu_prev); if (sct > 0.0) { slope = sct; slope_fresh = true; } }
       __syncthreads();
       ++evals;
     }
@@ -251,6 +255,13 @@ __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict_
     double mu_new = mu - f / slope;
     if (!(mu_new > lo && mu_new < hi)) mu_new = 0.5 * (lo + hi);
     if (fabs(mu_new - mu) <= 2e-16 * fmax(fabs(mu), C.kT)) { done = true; break; }
+    // With an exact or secant slope the residual after the step is ~ f (f''/2f') max(|step|, |previous step|)
+    // <= |f| max(step)/kT (I_{-1/2}'/I_{-1/2} <= 1/2 per kT): when that is below the tolerance the step is taken
+    // without another pass over the grid (the density pass that follows evaluates at the accepted mu).
+    if (slope_fresh) {
+      const double st = fmax(fabs(mu_new - mu), have_prev_pt ? fabs(mu - mu_prev) : 0.0);
+      if (fabs(f) * st * inv_kT <= 2e-15 * C.Ne) { mu = mu_new; f = 0.0; done = true; break; }
+    }
     mu_prev = mu; f_prev = f; have_prev_pt = true;
     mu = mu_new;
   }
