@@ -32,16 +32,25 @@ TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000, mix_warmup=3, mi
 ITERS_PER_STEP = {"c1": 32.0, "c2": 155.0, "c3": 20.0, "c4": 1000.0}
 
 # algorithmic HBM bytes per grid point and launch of each kernel class
-def bytes_per_point(nx):
+def bytes_per_point(nx, fused=True):
     """algorithmic HBM bytes per REAL grid point and launch of each kernel class; a half-spectrum complex array costs
     h = 16*P/nx bytes per real point (P = padded row pitch of the nx/2+1 stored columns)"""
     h = 16.0 * ((nx // 2 + 1 + 7) // 8 * 8) / nx
-    return {"fft_inv_z_potential": 5 * h,      # read nhat_i, nhat_a, Vhat_ie; write nhat_i (fused mixing), work
-            "fft_y": 2 * h,                    # read + write work
-            "fft_inv_x_vi": h + 32,            # read work, n_i, n_a; write n_i (fused mixing), V_i
-            "mu_pass": 8,                      # per evaluation of N(mu): read V_i (L2/register-cached on small grids)
-            "density": 24 + h,                 # read V_i, n_i; write n_a, work (r2c x pass with the density prologue)
-            "fft_fwd_z_reduce": 4 * h,         # read work, nhat_i, Vhat_ie; write nhat_a
+    if fused:
+        return {"fft_inv_z_potential": 5 * h,  # read nhat_i, nhat_a, Vhat_ie; write nhat_i (fused mixing), work
+                "fft_y": 2 * h,                # read + write work
+                "fft_inv_x_vi": h + 32,        # read work, n_i, n_a; write n_i (fused mixing), V_i
+                "mu_pass": 8,                  # per evaluation of N(mu): read V_i (L2/register-cached on small grids)
+                "density": 24 + h,             # read V_i, n_i; write n_a, work (r2c x pass with the density prologue)
+                "fft_fwd_z_reduce": 4 * h,     # read work, nhat_i, Vhat_ie; write nhat_a
+                "mix": 16 + 3 * h}
+    return {"potential_g": 5 * h,              # streaming: read nhat_i, nhat_a, Vhat_ie; write nhat_i, work
+            "fft_inv_z_potential": 2 * h, "fft_y": 2 * h, "fft_inv_x_vi": h + 8,      # plain passes
+            "vi_r": 40,                        # read V_H, n_i, n_a; write n_i, V_i
+            "mu_pass": 8,
+            "density_r": 24,                   # read V_i, n_i; write n_a
+            "fft_fwd_x_real": 8 + h, "fft_fwd_z_reduce": 2 * h,                        # plain passes
+            "reduce_g": 3 * h,                 # read nhat_a, nhat_i, Vhat_ie
             "mix": 16 + 3 * h}
 
 
@@ -217,7 +226,7 @@ def main():
         return
     peak, peak_src = peaks()
     ng = g.ng
-    BYTES_PER_POINT = bytes_per_point(g.grid[0])
+    BYTES_PER_POINT = bytes_per_point(g.grid[0], g.is_fused())
     tot_prof = sum(v[0] for v in prof.values()) or 1.0
     dom = max((k for k in prof if k in BYTES_PER_POINT), key=lambda k: prof[k][0])
     dom_ms, dom_n = prof[dom]

@@ -124,8 +124,12 @@ long long arche_launch_count(const arche_ctx *c);
  * Classes: 0 inverse-FFT z pass with the G-space potential prologue (S1), 1 FFT y passes, 2 inverse-FFT x pass with
  * the V_i epilogue (S2), 3 mu passes (S3), 4 density kernel (S4), 5 forward-FFT x pass reading the real n_a,
  * 6 forward-FFT z pass with the G-space reductions (S5), 7 mixing (S6), 8 structure factor (P1,P2), 9 force sum (P5),
- * 10 Ewald pair kernel, 11 other.  arche_profile_get returns the summed milliseconds and launch count of a class. */
+ * 10 Ewald pair kernel, 11 other.  On grids beyond the L2 the pointwise work runs as streaming kernels around plain
+ * passes (arche_is_fused() == 0): 12 G-space potential assembly + mixing (S1/S6), 13 V_i assembly + XC + first mu
+ * evaluation (S2), 14 density and local reductions (S4), 15 G-space reductions (S5); classes 0, 2, 5, 6 are then the
+ * plain passes and 4 is unused.  arche_profile_get returns the summed milliseconds and launch count of a class. */
 int arche_profile_enable(arche_ctx *c, int on);
+int arche_is_fused(const arche_ctx *c);
 int arche_profile_get(arche_ctx *c, int cls, double *h_ms_total, long long *h_launches);
 
 #ifdef __cplusplus

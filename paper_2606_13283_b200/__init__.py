@@ -20,7 +20,7 @@ SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_la
            "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_md_step",
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
            "arche_rfft3d_forward", "arche_rfft3d_inverse",
-           "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get"]
+           "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
 
@@ -82,6 +82,7 @@ def load(rebuild_if_stale: bool = True):
     L.arche_fermi_dirac.argtypes = [vp, C.c_int, dp, dp, C.c_size_t]
     L.arche_launch_count.argtypes = [vp]; L.arche_launch_count.restype = C.c_longlong
     L.arche_profile_enable.argtypes = [vp, C.c_int]
+    L.arche_is_fused.argtypes = [vp]
     L.arche_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     _lib = L
     return L
@@ -248,7 +249,11 @@ class Arche:
         return out
 
     PROFILE_CLASSES = ("fft_inv_z_potential", "fft_y", "fft_inv_x_vi", "mu_pass", "density", "fft_fwd_x_real",
-                       "fft_fwd_z_reduce", "mix", "structure_factor", "force", "ewald_pp", "other")
+                       "fft_fwd_z_reduce", "mix", "structure_factor", "force", "ewald_pp", "other",
+                       "potential_g", "vi_r", "density_r", "reduce_g")
+
+    def is_fused(self) -> bool:
+        return bool(self.lib.arche_is_fused(self._h))
 
     def profile_enable(self, on: bool = True):
         self._check(self.lib.arche_profile_enable(self._h, int(on)))

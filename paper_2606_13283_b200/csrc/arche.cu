@@ -26,7 +26,7 @@ constexpr int kMuMaxPasses = 12;
 constexpr int kProfPairs = 512;
 // kernel classes for arche_profile_get
 enum ProfClass { PC_FFT_INV_Z = 0, PC_FFT_Y, PC_FFT_INV_X, PC_MU, PC_DENSITY, PC_FFT_FWD_X, PC_FFT_FWD_Z, PC_MIX,
-                 PC_SFAC, PC_FORCE, PC_EWALD, PC_OTHER, kProfClasses };
+                 PC_SFAC, PC_FORCE, PC_EWALD, PC_OTHER, PC_POT_G, PC_VI_R, PC_DENS_R, PC_RED_G, kProfClasses };
 constexpr int kEwBlocks = 148 * 8;
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -87,6 +87,7 @@ struct arche_ctx {
   double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
   long long nh;      // P*ny*nz
   int nxh, P;
+  bool fuse;         // pointwise work fused into the FFT passes (grids that live in L2) or streamed around plain passes
   bool use_fast;     // register two-stage FFT passes where the axis length has a plan (ARCHE_FFT_GENERIC=1 disables)
   bool mix_pending;  // S6 of the last iteration not yet applied to n_i / nhat_i (fused into the next S1/S2)
   double *kx, *ky, *kz, *kx2, *ky2, *kz2;
@@ -239,6 +240,11 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   c->stream = (cudaStream_t)p->stream;
   derive_sizes(c);
   { const char *e = getenv("ARCHE_FFT_GENERIC"); c->use_fast = !(e && e[0] == '1'); }
+  {  // fused passes while the iteration's working set (3 real + 4 half-spectrum fields) stays well inside the 126 MB L2
+    const char *e = getenv("ARCHE_FUSE");
+    const double ws = 24.0 * (double)c->ng + 64.0 * (double)c->nh;
+    c->fuse = e ? e[0] == '1' : (ws <= 96.0e6 || (c->ng & 1));
+  }
   size_t need = layout(c, nullptr);
   if (!p->d_workspace || p->workspace_bytes < need || ((uintptr_t)p->d_workspace & 255)) { delete c; return ARCHE_ENOMEM; }
   layout(c, (char *)p->d_workspace);
@@ -402,6 +408,7 @@ int scf_iteration(arche_ctx *c) {
   const GridGeom &G = c->G;
   const ScfConst &C = c->C;
   const int mix = c->mix_pending ? 1 : 0;
+  const int pg = c->ew_grid * 2;   // streaming kernels: 16 blocks per SM
   // S1 + S2 (+ the pending S6 of the previous iteration, + the first mu evaluation)
   LoadPotentialG lp;
   lp.nh_i = c->nh_i; lp.nh_a = c->nh_a; lp.vh_ie = c->vh_ie; lp.kx2 = c->kx2; lp.ky2 = c->ky2; lp.kz2 = c->kz2;
@@ -409,8 +416,18 @@ int scf_iteration(arche_ctx *c) {
   StoreVi sv;
   sv.V_i = c->V_i; sv.n_i = c->n_i; sv.n_a = c->n_a; sv.sc = c->sc; sv.partials = c->partials; sv.counter = c->counter;
   sv.fdtab = c->fdtab; sv.inv_vol = 1.0 / G.vol; sv.kT_eta0 = C.kT * C.eta0; sv.inv_kT = 1.0 / C.kT; sv.xc = C.xc; sv.mix = mix;
-  int rc = fft3d_inverse(c, lp, sv, PC_FFT_INV_Z, PC_FFT_INV_X);
-  if (rc) return rc;
+  int rc;
+  if (c->fuse) {
+    rc = fft3d_inverse(c, lp, sv, PC_FFT_INV_Z, PC_FFT_INV_X);
+    if (rc) return rc;
+  } else {
+    { ProfScope ps(c, PC_POT_G);
+      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(lp, StoreComplex{c->work}, c->P, G.ny, c->nh); LAUNCHED(c); }
+    rc = fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{c->V_i}, PC_FFT_INV_Z, PC_FFT_INV_X);
+    if (rc) return rc;
+    { ProfScope ps(c, PC_VI_R);
+      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng); LAUNCHED(c); }
+  }
   c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
   { ProfScope ps(c, PC_MU);
@@ -420,15 +437,25 @@ int scf_iteration(arche_ctx *c) {
     void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax};
     CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, 0, c->stream));
     ++c->launches; }
-  // S4 (fused into the r2c x pass) + S5 (+ w, F, stop flags in the z-pass epilogue's last block)
+  // S4 + S5 (+ w, F, stop flags in the last block of the G-space reduction)
   LoadDensity ldn;
   ldn.V_i = c->V_i; ldn.n_i = c->n_i; ldn.n_a = c->n_a; ldn.sc = c->sc; ldn.partials = c->partials; ldn.counter = c->counter;
   ldn.fdtab = c->fdtab; ldn.C = C;
   StoreNhatA sn;
   sn.nh_a = c->nh_a; sn.nh_i = c->nh_i; sn.vh_ie = c->vh_ie; sn.kx2 = c->kx2; sn.ky2 = c->ky2; sn.kz2 = c->kz2;
   sn.sc = c->sc; sn.partials = c->partials; sn.counter = c->counter; sn.C = C; sn.H.nx = G.nx; sn.H.nxh = c->nxh;
-  rc = fft3d_forward(c, ldn, sn, PC_DENSITY, PC_FFT_FWD_Z);
-  if (rc) return rc;
+  sn.prestored = c->fuse ? 0 : 1;
+  if (c->fuse) {
+    rc = fft3d_forward(c, ldn, sn, PC_DENSITY, PC_FFT_FWD_Z);
+    if (rc) return rc;
+  } else {
+    { ProfScope ps(c, PC_DENS_R);
+      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng); LAUNCHED(c); }
+    rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
+    if (rc) return rc;
+    { ProfScope ps(c, PC_RED_G);
+      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(LoadComplex{c->nh_a}, sn, c->P, G.ny, c->nh); LAUNCHED(c); }
+  }
   c->mix_pending = true;   // S6 is applied by the next iteration's S1/S2 passes, or by flush_mix()
   c->have_solution = true;
   c->have_forces = false;
@@ -676,6 +703,8 @@ extern "C" int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta,
   LAUNCHED(c);
   return ARCHE_OK;
 }
+
+extern "C" int arche_is_fused(const arche_ctx *c) { return c && c->fuse ? 1 : 0; }
 
 extern "C" int arche_profile_enable(arche_ctx *c, int on) {
   if (!c) return ARCHE_EINVAL;

@@ -353,13 +353,13 @@ struct StoreNhatA {
   unsigned int *counter;
   ScfConst C;
   HalfGeom H;
+  int prestored;   // 1: the value is already scaled and stored in nh_a (streaming reduction after a plain z pass)
   double aU, aEH, aEie;
   __device__ __forceinline__ void begin() { aU = aEH = aEie = 0.0; }
   __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(vh_ie + idx); prefetch_l2(nh_i + idx); }
   __device__ __forceinline__ void store(long long idx, int ix, int iy, int iz, double re, double im) {
-    if (ix >= H.nxh) { nh_a[idx] = make_double2(0.0, 0.0); return; }
-    re *= C.dV; im *= C.dV;
-    nh_a[idx] = make_double2(re, im);
+    if (ix >= H.nxh) { if (!prestored) nh_a[idx] = make_double2(0.0, 0.0); return; }
+    if (!prestored) { re *= C.dV; im *= C.dV; nh_a[idx] = make_double2(re, im); }
     const double wt = H.wt(ix);
     const double2 b = vh_ie[idx];
     aEie += wt * (re * b.x + im * b.y);                  // Re conj(nhat_a) Vhat_ie
@@ -511,6 +511,50 @@ struct StoreRealPlain {
   __device__ __forceinline__ void store_real2(long long ia, long long ib, double ra, double rb) { dst[ia] = ra; dst[ib] = rb; }
   __device__ __forceinline__ void finish(double *) {}
 };
+
+// ---- streaming forms of the pointwise work (large grids) -----------------------------------------------------
+// On grids beyond the L2 the fused prologues/epilogues above run inside FFT tiles at two blocks per SM, which is too
+// little parallelism for their extra operand streams (z passes) and their Fermi-Dirac/XC arithmetic (x passes).
+// There the same functors run in these grid-stride kernels at full occupancy, around plain FFT passes.
+struct StoreNull {
+  __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void store_real2(long long, long long, double, double) {}
+  __device__ __forceinline__ void finish(double *) {}
+};
+
+template <class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp st_in, int P, int ny, long long nh) {
+  __shared__ double s_red[kMaxRed * 33];
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  ld.begin(); st.begin();
+  for (long long h = (long long)blockIdx.x * blockDim.x + threadIdx.x; h < nh; h += (long long)gridDim.x * blockDim.x) {
+    const int ix = (int)(h % P);
+    const long long row = h / P;
+    double re, im;
+    ld(h, ix, (int)(row % ny), (int)(row / ny), re, im);
+    st.store(h, ix, (int)(row % ny), (int)(row / ny), re, im);
+  }
+  ld.finish(s_red);
+  st.finish(s_red);
+}
+
+// real fields, two elements per thread and step (the functors interleave their two Fermi-Dirac evaluations); ng even
+template <class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(256) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng) {
+  __shared__ double s_red[kMaxRed * 33];
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  ld.begin(); st.begin();
+  const long long half = ng / 2;
+  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < half; g += (long long)gridDim.x * blockDim.x) {
+    double a, b;
+    ld.load_real2(g, g + half, a, b);
+    st.store_real2(g, g + half, a, b);
+  }
+  ld.finish(s_red);
+  st.finish(s_red);
+}
 
 // Full-spectrum view [nz][ny][nx] of a half-spectrum array for read-back: ix <= nx/2 copies src, the rest is
 // conj(src2[mirror]) (src2 = src for DFT-Hermitian fields, the Nyquist-flipped companion for S_Z and ghat);
