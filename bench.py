@@ -29,7 +29,7 @@ import arche_inputs as ai  # noqa: E402
 TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000, mix_warmup=3, mix_w_fixed=0.95)
 # SCF iterations per MD step of each workload under TOL, measured on the GPU path (used only to express the
 # oracle's bounded sample in MD steps/s)
-ITERS_PER_STEP = {"c1": 32.0, "c2": 155.0, "c3": 20.0, "c4": 1000.0}
+ITERS_PER_STEP = {"c1": 32.0, "c2": 162.0, "c3": 20.0, "c4": 1000.0}
 
 # algorithmic HBM bytes per grid point and launch of each kernel class
 def bytes_per_point(nx, fused=True):
@@ -52,6 +52,31 @@ def bytes_per_point(nx, fused=True):
             "fft_fwd_x_real": 8 + h, "fft_fwd_z_reduce": 2 * h,                        # plain passes
             "reduce_g": 3 * h,                 # read nhat_a, nhat_i, Vhat_ie
             "mix": 16 + 3 * h}
+
+
+# fp64 work per grid point of the arithmetic-bound classes, counted from the kernels (an FMA = 2 flops): one
+# Fermi-Dirac function = 11 FMA Horner + ~8 flops to locate the segment; PZ81 = cbrt + log or sqrt + 2 divisions
+# ~ 90 flops; the reductions ~ 20.
+FLOPS_PER_POINT = {"mu_pass": 32, "density": 3 * 30 + 90 + 20, "density_r": 3 * 30 + 90 + 20, "vi_r": 30 + 90 + 10,
+                   "fft_inv_x_vi": 30 + 90 + 10}     # fft_inv_x_vi carries the V_i epilogue only in the fused form
+# fp64 vector peak of one B200: 148 SMs x 64 FMA lanes x 2 flops x 1.965 GHz
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+
+def roofline_entry(name, ms_per_launch, ng, bpp, peak_gbs, peak_src, evals_per_launch=1.0):
+    """roofline object of one kernel class: HBM bytes for the streaming/FFT classes, fp64 flops for the
+    arithmetic-bound ones (whichever bound is the higher fraction is the binding one and is reported)"""
+    t = ms_per_launch * 1e-3
+    hbm = bpp.get(name, 0.0) * evals_per_launch * ng / t / 1e9 if t > 0 else 0.0
+    out = {"bound": "hbm", "kernel": name, "achieved": hbm, "peak": peak_gbs, "unit": "GB/s",
+           "frac": hbm / peak_gbs, "traffic": None, "peak_source": peak_src}
+    if name in FLOPS_PER_POINT and t > 0 and not (name == "fft_inv_x_vi" and "vi_r" in bpp):
+        tf = FLOPS_PER_POINT[name] * evals_per_launch * ng / t / 1e12
+        if tf / FP64_PEAK_TFLOPS > out["frac"]:
+            out = {"bound": "alu", "kernel": name, "achieved": tf, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                   "frac": tf / FP64_PEAK_TFLOPS, "traffic": None,
+                   "peak_source": "derived: 148 SMs x 64 fp64 FMA lanes x 2 x 1.965 GHz", "hbm_gbs": hbm}
+    return out
 
 
 def peaks():
@@ -98,20 +123,23 @@ class ClockSampler:
                 "reasons": sorted(self.reasons)}
 
 
-def oracle_sample(cfg, workload, iters=2):
+def oracle_sample(cfg, workload, iters=2, iters_per_step=None):
     """bounded oracle sample: `iters` SCF iterations of the workload from the uniform density + the ion-grid work"""
     import oracle
     o = oracle.Oracle(cfg, **TOL)
     t0 = time.perf_counter(); o.scf_begin(cfg["pos"]); t_ion = time.perf_counter() - t0
+    t0 = time.perf_counter(); o.scf_iter(); t_first = time.perf_counter() - t0
+    iters = max(iters, min(40, int(15.0 / max(t_first, 1e-3))))     # about 15 s of CPU work in total
     t0 = time.perf_counter()
     for _ in range(iters):
         o.scf_iter()
     t_it = (time.perf_counter() - t0) / iters
     t0 = time.perf_counter(); o.forces(); t_force = time.perf_counter() - t0
-    step_s = ITERS_PER_STEP[workload] * t_it + t_ion + t_force
+    ips = iters_per_step or ITERS_PER_STEP[workload]
+    step_s = ips * t_it + t_ion + t_force
     return dict(value=1.0 / step_s, unit="md_steps/s", cores=oracle.lib().oracle_num_threads(), kind="oracle",
                 sample=f"{iters} SCF iterations ({t_it:.2f} s each) + structure factor/Ewald ({t_ion:.2f} s) + forces "
-                       f"({t_force:.2f} s) of {workload}; MD step extrapolated with {ITERS_PER_STEP[workload]:.0f} "
+                       f"({t_force:.2f} s) of {workload}; MD step extrapolated with {ips:.0f} "
                        f"iterations/step", scf_iters_per_s=1.0 / t_it)
 
 
@@ -142,6 +170,84 @@ def workload_config(cfg, name):
             "l2": "flushed between timed steps (256 MiB write); the 64^3 working set (36 MB) is L2-resident within a step"}
 
 
+def replica_config(cfg, rank, world):
+    """N > 1 runs independent replicas: same recipe, rank-dependent thermal displacement"""
+    if world > 1:
+        rng = np.random.default_rng(1000 + rank)
+        cfg = dict(cfg)
+        cfg["pos"] = np.mod(cfg["pos"] + 0.05 * rng.standard_normal(cfg["pos"].shape), cfg["cell"])
+    return cfg
+
+
+def max_over_ranks(values, device=None):
+    """element-wise MAX of a list of floats over all ranks of the default process group (NCCL on GPUs, gloo in tests)"""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def run_iteration_sweep(args):
+    """BASELINE.json configs[4]: single-SCF-iteration and force throughput on the 2000-ion cell for one grid size.
+    Prints one JSON line with the per-class roofline numbers (CUDA events around every launch of a class)."""
+    import torch
+    from paper_2606_13283_b200 import Arche
+    cfg = ai.make_config("c5", grid=args.grid)
+    g = Arche(cfg, **TOL)
+    pos = torch.as_tensor(cfg["pos"], device="cuda")
+    g.scf_begin(pos)
+    for _ in range(max(args.warmup, 3)):
+        g.scf_iter()
+    g.forces()
+    torch.cuda.synchronize()
+    K = args.steps
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    with ClockSampler(0) as cs:
+        e0.record(g.stream)
+        for _ in range(K):
+            r = g.scf_iter()
+        e1.record(g.stream); torch.cuda.synchronize()
+    it_ms = e0.elapsed_time(e1) / K
+    ev0 = r["mu_evals"]
+    g.profile_enable(True)
+    g.scf_begin(pos)
+    for _ in range(K):
+        r = g.scf_iter()
+    g.forces()
+    prof = g.profile_get()
+    g.profile_enable(False)
+    evals_per_iter = r["mu_evals"] / K
+    peak, peak_src = peaks()
+    bpp = bytes_per_point(args.grid, g.is_fused())
+    rl = {}
+    for k, (ms, n) in prof.items():
+        if not n:
+            continue
+        per = (evals_per_iter - 1.0) if k == "mu_pass" else 1.0   # one evaluation per iteration rides in the S2 pass
+        if k in bpp or k in FLOPS_PER_POINT:
+            e = roofline_entry(k, ms / n, g.ng, bpp, peak, peak_src, max(per, 1e-9))
+            rl[k] = {"ms": round(ms / n, 4), "bound": e["bound"], "achieved": round(e["achieved"], 2), "unit": e["unit"],
+                     "frac": round(e["frac"], 3)}
+        else:
+            rl[k] = {"ms": round(ms / n, 4)}
+    hbm_classes = [k for k in rl if rl[k].get("bound") == "hbm"]
+    tot_b = sum(bpp[k] * g.ng * prof[k][1] for k in hbm_classes)
+    tot_t = sum(prof[k][0] for k in hbm_classes) * 1e-3
+    line = {"metric": "scf_iterations_per_s", "value": 1e3 / it_ms, "unit": "scf_iterations/s", "n_gpus": 1, "steps": K,
+            "warmup": max(args.warmup, 3), "ms_per_step": it_ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"c5: 2000 Al ions, cubic cell {cfg['cell'][0]:.4f} bohr, grid {args.grid}^3, T=50 eV; "
+                                   f"one SCF iteration from the uniform start, forces on the resulting density",
+                       "l2": "fields larger than L2 for grids >= 192^3" if args.grid >= 192 else "L2-resident grid",
+                       "fused": g.is_fused()},
+            "grid_points_per_s": g.ng / it_ms * 1e3, "mu_evals_per_iter": evals_per_iter, "clocks": cs.summary(),
+            "hbm_classes_aggregate_gbs": tot_b / tot_t / 1e9 if tot_t > 0 else None, "hbm_peak_gbs": peak,
+            "kernels": rl}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -150,7 +256,11 @@ def main():
     ap.add_argument("--workload", default="c2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--grid", type=int, default=0, help="with --workload c5: grid size of the single-iteration sweep point")
     args = ap.parse_args()
+    if args.workload == "c5":
+        args.grid = args.grid or 256
+        return run_iteration_sweep(args)
     cfg = ai.make_config(args.workload)
     if args.impl == "reference":
         return run_reference(args, cfg)
@@ -164,9 +274,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     torch.cuda.set_device(local)
     dev = f"cuda:{local}"
-    if world > 1:  # independent replica: same recipe, rank-dependent thermal noise
-        rng = np.random.default_rng(1000 + rank)
-        cfg["pos"] = np.mod(cfg["pos"] + 0.05 * rng.standard_normal(cfg["pos"].shape), cfg["cell"])
+    cfg = replica_config(cfg, rank, world)
     g = Arche(cfg, device=dev, **TOL)
     stream = g.stream
     pos = torch.as_tensor(cfg["pos"].copy(), device=dev); vel = torch.as_tensor(cfg["vel"].copy(), device=dev)
@@ -181,14 +289,15 @@ def main():
 
     def timed_steps(K, step_fn):
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-        iters = 0
+        iters = 0; evals = 0
         for a, b in ev:
             flush.fill_(1)                      # evict L2 between timed steps
             a.record(stream)
             r = step_fn()
             b.record(stream)
-            iters += r["scf_iters"]
+            iters += r["scf_iters"]; evals += r["mu_evals"]
         torch.cuda.synchronize()
+        timed_steps.mu_evals = evals
         return sum(a.elapsed_time(b) for a, b in ev) * 1e-3, iters
 
     # ---- device-resident arm
@@ -198,6 +307,7 @@ def main():
     l0 = g.launch_count()
     with ClockSampler(local) as cs:
         t_dev, iters = timed_steps(args.steps, lambda: g.md_step(dt, pos, vel))
+    mu_evals = timed_steps.mu_evals
     launches = g.launch_count() - l0
     barrier()
     # ---- end-to-end arm: host buffers through the C ABI (H2D of positions/velocities, D2H of positions/velocities/forces)
@@ -216,10 +326,7 @@ def main():
     prof = g.profile_get()
     g.profile_enable(False)
 
-    times = torch.tensor([t_dev, t_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    t_dev_max, t_e2e_max = times.tolist()
+    t_dev_max, t_e2e_max = max_over_ranks([t_dev, t_e2e], device=dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -228,12 +335,24 @@ def main():
     ng = g.ng
     BYTES_PER_POINT = bytes_per_point(g.grid[0], g.is_fused())
     tot_prof = sum(v[0] for v in prof.values()) or 1.0
-    dom = max((k for k in prof if k in BYTES_PER_POINT), key=lambda k: prof[k][0])
-    dom_ms, dom_n = prof[dom]
-    ach = BYTES_PER_POINT[dom] * ng / (dom_ms / dom_n * 1e-3) / 1e9 if dom_n else 0.0
+    evals_per_iter = mu_evals / max(iters, 1)
+    rl = {}
+    for k, v in prof.items():
+        if v[1] and (k in BYTES_PER_POINT or k in FLOPS_PER_POINT):
+            per = max(evals_per_iter - 1.0, 1e-9) if k == "mu_pass" else 1.0
+            rl[k] = roofline_entry(k, v[0] / v[1], ng, BYTES_PER_POINT, peak, peak_src, per)
+    dom = max(rl, key=lambda k: prof[k][0])
     kernels = {k: {"ms_total": round(v[0], 4), "launches": v[1], "share": round(v[0] / tot_prof, 4),
-                   "gbs": round(BYTES_PER_POINT[k] * ng / (v[0] / v[1] * 1e-3) / 1e9, 1) if k in BYTES_PER_POINT and v[1] else None}
+                   "us_per_launch": round(1e3 * v[0] / v[1], 2),
+                   **({"bound": rl[k]["bound"], "achieved": round(rl[k]["achieved"], 2), "unit": rl[k]["unit"],
+                       "frac": round(rl[k]["frac"], 4)} if k in rl else {})}
                for k, v in prof.items() if v[1]}
+    roof = dict(rl[dom])
+    roof["share_of_step"] = round(prof[dom][0] / tot_prof, 4)
+    roof["note"] = ("the 64^3 fields of this workload are L2-resident and every launch lasts 7-25 us: the kernels are "
+                    "latency-bound, so neither fraction is high; the large-grid rooflines are in profiles/ "
+                    "(bench.py --workload c5 --grid N)")
+    roof["measured"] = "CUDA events around each launch of the class in a second pass of the same steps"
     line = {"metric": "md_steps_per_s", "value": world * args.steps / t_dev_max, "unit": "md_steps/s",
             "n_gpus": world, "steps": args.steps, "warmup": W, "ms_per_step": 1e3 * t_dev_max / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -243,13 +362,9 @@ def main():
             "e2e": {"value": world * args.steps / t_e2e_max, "unit": "md_steps/s",
                     "h2d_bytes_per_step": 2 * 3 * g.n_ions * 8, "d2h_bytes_per_step": 3 * 3 * g.n_ions * 8 + 136},
             "gpu_launches": int(launches),
-            "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                         "traffic": None, "peak_source": peak_src,
-                         "note": "64^3 fields are L2-resident: HBM fraction reported as the contract asks, flagged",
-                         "measured": "CUDA events around each launch of the class in a second pass of the same steps"},
-            "kernels": kernels}
+            "mu_evals_per_iter": evals_per_iter, "roofline": roof, "kernels": kernels}
     if not args.no_cpu_baseline:
-        line["cpu_baseline"] = oracle_sample(cfg, args.workload, iters=2)
+        line["cpu_baseline"] = oracle_sample(cfg, args.workload, iters=2, iters_per_step=iters / args.steps)
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

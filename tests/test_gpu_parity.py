@@ -86,10 +86,19 @@ def test_structure_factor_and_ionic_potential(orc, torch_cuda):
         assert _rel(g.get_complex(name).cpu().numpy(), o.get_complex(name)) < 1e-12
 
 
+@pytest.fixture(params=["fused", "streamed"])
+def pointwise_mode(request, monkeypatch):
+    """both forms of the pointwise work: fused into the FFT passes (default on L2-resident grids) and streaming
+    kernels around plain passes (default on large grids); ARCHE_FUSE is read by arche_scf_init"""
+    monkeypatch.setenv("ARCHE_FUSE", "1" if request.param == "fused" else "0")
+    return request.param
+
+
 @pytest.mark.parametrize("xc", [0, 1])
-def test_single_scf_iteration(orc, torch_cuda, xc):
+def test_single_scf_iteration(orc, torch_cuda, xc, pointwise_mode):
     cfg = ai.make_small(n_ions=4, L=8.0, grid=(16, 12, 24), T_eV=10.0, seed=8)
     g = _gpu(cfg, xc=xc); o = orc.Oracle(cfg, xc=xc)
+    assert g.is_fused() == (pointwise_mode == "fused")
     g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
     for it in range(3):
         rg = g.scf_iter(); ro = o.scf_iter()
@@ -114,7 +123,32 @@ def _solve_pair(orc, cfg, **kw):
     return g, o, rg, ro
 
 
-def test_converged_solve_and_forces(orc, torch_cuda):
+@pytest.mark.parametrize("name,iters", [("c2", 3), ("c3", 2)])
+def test_full_size_configs_iterations_and_forces(orc, torch_cuda, name, iters):
+    """BASELINE.json configs[1] (128 ions, 64^3: fused passes, register FFT kernels) and configs[2] (256 ions, 128^3:
+    streamed pointwise kernels) at their full sizes and in the launch configuration bench.py times: a few SCF
+    iterations from the uniform start, every field and scalar against the oracle, then the forces on that density."""
+    cfg = ai.make_config(name)
+    kw = dict(mix_warmup=3, mix_w_fixed=0.95)
+    g = _gpu(cfg, **kw); o = orc.Oracle(cfg, **kw)
+    assert g.is_fused() == (name == "c2")
+    g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
+    for name_c in ("S_Z", "Vhat_ie"):
+        assert _rel(g.get_complex(name_c).cpu().numpy(), o.get_complex(name_c)) < 1e-11
+    for it in range(iters):
+        rg = g.scf_iter(); ro = o.scf_iter()
+        for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "U_ii", "K_e", "w_last"):
+            assert abs(rg[k] - ro[k]) <= TOL_F * max(1.0, abs(ro[k])), (it, k, rg[k], ro[k])
+    assert _rel(g.get_real("n_a").cpu().numpy(), o.get_real("n_a")) < TOL_N
+    assert _rel(g.get_real("n_i").cpu().numpy(), o.get_real("n_i")) < TOL_N
+    assert _rel(g.get_complex("nhat_a").cpu().numpy(), o.get_complex("nhat_a")) < TOL_N
+    Fg = g.forces().cpu().numpy(); Fo = o.forces()
+    assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max()
+    dV = float(np.prod(cfg["cell"]) / np.prod(cfg["grid"]))
+    assert abs(g.get_real("n_a").sum().item() * dV - cfg["Z"].sum()) < 1e-12 * cfg["Z"].sum()
+
+
+def test_converged_solve_and_forces(orc, torch_cuda, pointwise_mode):
     cfg = ai.make_small(n_ions=5, L=9.0, grid=(24, 16, 18), cell=[9.0, 7.5, 8.0], T_eV=10.0, seed=9)
     g, o, rg, ro = _solve_pair(orc, cfg, scf_tol_dn=1e-11, init_mode=0)
     assert rg["scf_iters"] == ro["scf_iters"]
