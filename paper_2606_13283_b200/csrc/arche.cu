@@ -23,6 +23,7 @@ using namespace arche;
 namespace {
 
 constexpr int kMuMaxPasses = 12;
+constexpr int kScfBatch = 6;      // SCF iterations launched between two reads of the device scalars
 constexpr int kProfPairs = 512;
 // kernel classes for arche_profile_get
 enum ProfClass { PC_FFT_INV_Z = 0, PC_FFT_Y, PC_FFT_INV_X, PC_MU, PC_DENSITY, PC_FFT_FWD_X, PC_FFT_FWD_Z, PC_MIX,
@@ -87,6 +88,7 @@ struct arche_ctx {
   double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
   long long nh;      // P*ny*nz
   int nxh, P;
+  const int *stop;   // device flag handed to the kernels of speculatively launched iterations (nullptr: never skip)
   bool fuse;         // pointwise work fused into the FFT passes (grids that live in L2) or streamed around plain passes
   bool use_fast;     // register two-stage FFT passes where the axis length has a plan (ARCHE_FFT_GENERIC=1 disables)
   bool mix_pending;  // S6 of the last iteration not yet applied to n_i / nhat_i (fused into the next S1/S2)
@@ -336,17 +338,17 @@ namespace {
 template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
 cudaError_t pass_yz(arche_ctx *c, LoadOp ld, StoreOp st) {
   const int ny = c->G.ny, nz = c->G.nz, P = c->P, n = AXIS == 1 ? ny : nz;
-  FastGeom fg{c->G.nx, ny, nz, P, c->tw[AXIS]};
+  FastGeom fg{c->G.nx, ny, nz, P, c->tw[AXIS], c->stop};
   cudaError_t e = c->use_fast ? fft_launch_yz_fast<AXIS, INVERSE>(n, fg, ld, st, c->stream) : cudaErrorNotSupported;
-  if (e == cudaErrorNotSupported) e = fft_launch_pass<AXIS, INVERSE>(c->plan[AXIS], P, ny, nz, ld, st, c->stream);
+  if (e == cudaErrorNotSupported) { c->plan[AXIS].stop = c->stop; e = fft_launch_pass<AXIS, INVERSE>(c->plan[AXIS], P, ny, nz, ld, st, c->stream); }
   return e;
 }
 template <bool INVERSE, class LoadOp, class StoreOp>
 cudaError_t pass_x(arche_ctx *c, LoadOp ld, StoreOp st) {
   const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
-  FastGeom fg{nx, ny, nz, P, c->tw[0]};
+  FastGeom fg{nx, ny, nz, P, c->tw[0], c->stop};
   cudaError_t e = c->use_fast ? fft_launch_x_fast<INVERSE>(nx, fg, ld, st, c->stream) : cudaErrorNotSupported;
-  if (e == cudaErrorNotSupported) e = fft_launch_real_x<INVERSE>(c->plan[0], nx, ny, nz, P, ld, st, c->stream);
+  if (e == cudaErrorNotSupported) { c->plan[0].stop = c->stop; e = fft_launch_real_x<INVERSE>(c->plan[0], nx, ny, nz, P, ld, st, c->stream); }
   return e;
 }
 
@@ -422,19 +424,19 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_POT_G);
-      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(lp, StoreComplex{c->work}, c->P, G.ny, c->nh); LAUNCHED(c); }
+      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(lp, StoreComplex{c->work}, c->P, G.ny, c->nh, c->stop); LAUNCHED(c); }
     rc = fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{c->V_i}, PC_FFT_INV_Z, PC_FFT_INV_X);
     if (rc) return rc;
     { ProfScope ps(c, PC_VI_R);
-      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng); LAUNCHED(c); }
+      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop); LAUNCHED(c); }
   }
   c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
   { ProfScope ps(c, PC_MU);
     const double *aV = c->V_i; long long ang = c->ng; ScfConst aC = C;
     DevScalars *asc = c->sc; const double *atab = c->fdtab; double *apart = c->partials;
-    int amax = kMuMaxPasses;
-    void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax};
+    int amax = kMuMaxPasses; const int *astop = c->stop;
+    void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax, &astop};
     CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, 0, c->stream));
     ++c->launches; }
   // S4 + S5 (+ w, F, stop flags in the last block of the G-space reduction)
@@ -450,11 +452,11 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_DENS_R);
-      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng); LAUNCHED(c); }
+      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop); LAUNCHED(c); }
     rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
     if (rc) return rc;
     { ProfScope ps(c, PC_RED_G);
-      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(LoadComplex{c->nh_a}, sn, c->P, G.ny, c->nh); LAUNCHED(c); }
+      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(LoadComplex{c->nh_a}, sn, c->P, G.ny, c->nh, c->stop); LAUNCHED(c); }
   }
   c->mix_pending = true;   // S6 is applied by the next iteration's S1/S2 passes, or by flush_mix()
   c->have_solution = true;
@@ -519,13 +521,23 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   const int fixed = c->p.scf_fixed_iter;
   const int maxit = fixed > 0 ? fixed : (c->p.scf_max_iter > 0 ? c->p.scf_max_iter : 200);
   bool conv = false;
-  for (int it = 0; it < maxit; ++it) {
-    rc = scf_iteration(c);
-    if (rc) return rc;
+  // Iterations are launched in batches without a host round trip; once the S5 epilogue has set the stop flag the
+  // kernels of the remaining iterations of the batch return at once, so the state stays that of the converged
+  // iteration.  Parity replays (scf_fixed_iter) run every iteration.
+  const int batch = fixed > 0 ? maxit : kScfBatch;
+  for (int it = 0; it < maxit && !conv;) {
+    c->stop = fixed > 0 ? nullptr : &c->sc->converged;
+    const int n = it + batch <= maxit ? batch : maxit - it;
+    for (int b = 0; b < n; ++b) {
+      rc = scf_iteration(c);
+      if (rc) { c->stop = nullptr; return rc; }
+    }
+    c->stop = nullptr;
+    it += n;
     rc = read_scalars(c);
     if (rc) return rc;
     if (!isfinite(c->h_sc->F_total) || !isfinite(c->h_sc->mu)) return fail(c, ARCHE_ENAN, "non-finite free energy or mu");
-    if (fixed <= 0 && c->h_sc->converged) { conv = true; break; }
+    if (fixed <= 0 && c->h_sc->converged) conv = true;
   }
   // P6: one-center profile of this step's converged density (reading A10)
   if (c->nions > 0) {
@@ -665,6 +677,7 @@ extern "C" int arche_get_density(arche_ctx *c, double *d_n) { return arche_get_r
 extern "C" int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, double *d_scratch, int sign) {
   if (!c || !d_in || !d_out || !d_scratch || (sign != 1 && sign != -1)) return ARCHE_EINVAL;
   const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  for (int a = 0; a < 3; ++a) c->plan[a].stop = nullptr;
   double2 *w = (double2 *)d_scratch, *o = (double2 *)d_out;
   const double2 *in = (const double2 *)d_in;
   if (sign < 0) {

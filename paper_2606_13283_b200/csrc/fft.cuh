@@ -23,6 +23,7 @@ struct FftAxisPlan {
   int nstages;
   int radix[kFftMaxStages];
   const double2 *tw;  // device, [n], exp(-2 pi i a / n)
+  const int *stop;    // optional device flag: when set and non-zero the pass is skipped (speculative SCF launches)
 };
 
 struct FftPass {
@@ -139,6 +140,7 @@ __global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, LoadOp
   double *b0re = smem, *b0im = smem + (size_t)L * N, *b1re = smem + 2 * (size_t)L * N, *b1im = smem + 3 * (size_t)L * N;
   StoreOp st = st_in;
   LoadOp ld = ld_in;
+  if (P.plan.stop && *P.plan.stop) return;
   ld.begin(); st.begin();
   // tile geometry
   const long long nxny = (long long)P.nx * P.ny;
@@ -252,6 +254,7 @@ __global__ void __launch_bounds__(kFftThreads) fft_r2c_x_kernel(FftRealPass P, L
   double *sre = smem, *sim = smem + (size_t)LP * N, *dre = smem + 2 * (size_t)LP * N, *dim = smem + 3 * (size_t)LP * N;
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  if (P.plan.stop && *P.plan.stop) return;
   ld.begin(); st.begin();
   const long long nl = (long long)P.ny * P.nz;
   const long long line_base = (long long)blockIdx.x * LP * 2;
@@ -291,6 +294,7 @@ __global__ void __launch_bounds__(kFftThreads) fft_c2r_x_kernel(FftRealPass P, L
   double *sre = smem, *sim = smem + (size_t)LP * N, *dre = smem + 2 * (size_t)LP * N, *dim = smem + 3 * (size_t)LP * N;
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  if (P.plan.stop && *P.plan.stop) return;
   ld.begin(); st.begin();
   const long long nl = (long long)P.ny * P.nz;
   const long long line_base = (long long)blockIdx.x * LP * 2;
@@ -321,7 +325,7 @@ __global__ void __launch_bounds__(kFftThreads) fft_c2r_x_kernel(FftRealPass P, L
 
 // ---- host side ------------------------------------------------------------------------------
 static inline bool fft_make_plan(int n, const double2 *d_tw, FftAxisPlan *p) {
-  p->n = n; p->tw = d_tw; p->nstages = 0;
+  p->n = n; p->tw = d_tw; p->nstages = 0; p->stop = nullptr;
   int m = n;
   // radix-3 factors first (small Ns => no twiddles on the odd radix), then 8s, then the 4/2 remainder
   while (m % 3 == 0) { p->radix[p->nstages++] = 3; m /= 3; }

@@ -121,6 +121,7 @@ static inline bool fft_fast_size(int n) { return n == 32 || n == 64 || n == 128 
 struct FastGeom {
   int nx, ny, nz, P;        // real grid and half-spectrum pitch
   const double2 *tw;        // exp(-2 pi i a/N) of the transformed axis
+  const int *stop;          // optional device flag: non-zero skips the pass
 };
 
 constexpr int kFastL = 8;   // columns per y/z tile (128-byte rows)
@@ -136,6 +137,7 @@ __global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastG
   double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [N][8]
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   const int l = threadIdx.x % kFastL, jj = threadIdx.x / kFastL;
   const int xt = G.P / kFastL;
@@ -232,6 +234,7 @@ __global__ void __launch_bounds__(fast_threads_x<N>()) fft_r2c_fast_kernel(FastG
   double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
   for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
@@ -268,6 +271,7 @@ __global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastG
   double2 *buf = reinterpret_cast<double2 *>(smem_raw);
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
   for (int e = threadIdx.x * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile

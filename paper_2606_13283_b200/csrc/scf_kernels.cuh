@@ -182,8 +182,9 @@ __device__ __forceinline__ void mu_accumulate4(const double *tab, const double (
 
 __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
                                                        DevScalars *sc, const double *__restrict__ fdtab,
-                                                       double *partials, int max_pass) {
+                                                       double *partials, int max_pass, const int *stop) {
   namespace cg = cooperative_groups;
+  if (stop && *stop) return;   // uniform over the grid: no block reaches a barrier
   cg::grid_group grid = cg::this_grid();
   __shared__ double s_tab[kFdTabDoubles];
   __shared__ double s_red[2 * 32 + 2];
@@ -523,8 +524,10 @@ struct StoreNull {
 };
 
 template <class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp st_in, int P, int ny, long long nh) {
+__global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp st_in, int P, int ny, long long nh,
+                                                          const int *stop) {
   __shared__ double s_red[kMaxRed * 33];
+  if (stop && *stop) return;
   LoadOp ld = ld_in;
   StoreOp st = st_in;
   ld.begin(); st.begin();
@@ -541,8 +544,9 @@ __global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp 
 
 // real fields, two elements per thread and step (the functors interleave their two Fermi-Dirac evaluations); ng even
 template <class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(256) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng) {
+__global__ void __launch_bounds__(256) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng, const int *stop) {
   __shared__ double s_red[kMaxRed * 33];
+  if (stop && *stop) return;
   LoadOp ld = ld_in;
   StoreOp st = st_in;
   ld.begin(); st.begin();
