@@ -17,6 +17,7 @@
 #include "fft_fast.cuh"
 #include "ion_kernels.cuh"
 #include "scf_kernels.cuh"
+#include "scf_persistent.cuh"
 
 using namespace arche;
 
@@ -88,6 +89,8 @@ struct arche_ctx {
   double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
   long long nh;      // P*ny*nz
   int nxh, P;
+  bool persist;      // whole solve in one cooperative launch (scf_persistent.cuh): fused form, 32^3 / 64^3 grids
+  int sm_count;
   const int *stop;   // device flag handed to the kernels of speculatively launched iterations (nullptr: never skip)
   bool fuse;         // pointwise work fused into the FFT passes (grids that live in L2) or streamed around plain passes
   bool use_fast;     // register two-stage FFT passes where the axis length has a plan (ARCHE_FFT_GENERIC=1 disables)
@@ -246,6 +249,8 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     const char *e = getenv("ARCHE_FUSE");
     const double ws = 24.0 * (double)c->ng + 64.0 * (double)c->nh;
     c->fuse = e ? e[0] == '1' : (ws <= 96.0e6 || (c->ng & 1));
+    const char *pe = getenv("ARCHE_PERSIST");
+    c->persist = c->fuse && c->use_fast && !(pe && pe[0] == '0');
   }
   size_t need = layout(c, nullptr);
   if (!p->d_workspace || p->workspace_bytes < need || ((uintptr_t)p->d_workspace & 255)) { delete c; return ARCHE_ENOMEM; }
@@ -285,6 +290,7 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, 0));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
+    c->sm_count = sms;
     const long long cache_pts = (long long)sms * 256 * kMuCache;
     long long blocks = c->ng <= cache_pts ? sms : (long long)sms * (per_sm < 3 ? per_sm : 3);
     const long long want = (c->ng + 255) / 256;
@@ -480,7 +486,7 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     structure_factor_kernel<<<sg, SF_THREADS, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S,
                                                               c->S2, c->vh_ie, c->partials, c->counter, c->sc);
     LAUNCHED(c);
-    structure_factor_nyquist_kernel<<<c->ew_grid, 128, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va,
+    structure_factor_nyquist_kernel<<<c->ew_grid, 128, 0, c->stream>>>(G, ni, c->Z, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,
                                                                        c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc);
     LAUNCHED(c); }
     ewald_pp_kernel<<<ni, 128, 0, c->stream>>>(c->pos, c->Z, ni, G.Lx, G.Ly, G.Lz, c->alpha, c->F_pp, c->e_pp); LAUNCHED(c);
@@ -521,9 +527,32 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   const int fixed = c->p.scf_fixed_iter;
   const int maxit = fixed > 0 ? fixed : (c->p.scf_max_iter > 0 ? c->p.scf_max_iter : 200);
   bool conv = false;
+  // L2-resident production grids: the whole solve in one cooperative launch (not while per-class profiling is on)
+  if (c->persist && !c->prof) {
+    PersistParams pp;
+    pp.n_i = c->n_i; pp.n_a = c->n_a; pp.V_i = c->V_i; pp.nh_i = c->nh_i; pp.nh_a = c->nh_a; pp.work = c->work;
+    pp.vh_ie = c->vh_ie; pp.kx2 = c->kx2; pp.ky2 = c->ky2; pp.kz2 = c->kz2;
+    pp.tw0 = c->tw[0]; pp.tw1 = c->tw[1]; pp.tw2 = c->tw[2];
+    pp.sc = c->sc; pp.partials = c->partials; pp.counter = c->counter; pp.fdtab = c->fdtab; pp.C = c->C;
+    pp.nxh = c->nxh; pp.P = c->P; pp.ng = c->ng; pp.inv_vol = 1.0 / c->G.vol;
+    pp.mix_first = c->mix_pending ? 1 : 0; pp.max_iters = maxit; pp.fixed = fixed > 0 ? 1 : 0; pp.mu_max_pass = kMuMaxPasses;
+    cudaError_t e = scf_persistent_launch(c->G.nx, c->G.ny, c->G.nz, pp, c->sm_count, c->stream);
+    if (e == cudaSuccess) {
+      ++c->launches;
+      c->mix_pending = true; c->have_solution = true; c->have_forces = false;
+      rc = read_scalars(c);
+      if (rc) return rc;
+      if (!isfinite(c->h_sc->F_total) || !isfinite(c->h_sc->mu)) return fail(c, ARCHE_ENAN, "non-finite free energy or mu");
+      conv = fixed <= 0 && c->h_sc->converged;
+      goto solved;
+    }
+    if (e != cudaErrorNotSupported) return fail(c, ARCHE_ECUDA, "scf_persistent_launch", e);
+    c->persist = false;   // no instantiation for this grid: per-pass form from now on
+  }
   // Iterations are launched in batches without a host round trip; once the S5 epilogue has set the stop flag the
   // kernels of the remaining iterations of the batch return at once, so the state stays that of the converged
   // iteration.  Parity replays (scf_fixed_iter) run every iteration.
+  {
   const int batch = fixed > 0 ? maxit : kScfBatch;
   for (int it = 0; it < maxit && !conv;) {
     c->stop = fixed > 0 ? nullptr : &c->sc->converged;
@@ -539,6 +568,8 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
     if (!isfinite(c->h_sc->F_total) || !isfinite(c->h_sc->mu)) return fail(c, ARCHE_ENAN, "non-finite free energy or mu");
     if (fixed <= 0 && c->h_sc->converged) conv = true;
   }
+  }
+solved:
   // P6: one-center profile of this step's converged density (reading A10)
   if (c->nions > 0) {
     g_store_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->gh, c->gh2, c->nh_a, c->S, c->S2, c->nh, 1e-8 * c->Q * c->Q);

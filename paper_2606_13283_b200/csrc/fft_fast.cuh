@@ -129,22 +129,23 @@ template <int N> __host__ __device__ constexpr int fast_threads_yz() {
   return kFastL * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
 }
 
+// barrier over a group of `count` threads (multiple of 32) of the block; id 0 with the whole block = __syncthreads()
+__device__ __forceinline__ void group_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+
 // ---- y / z pass over the half spectrum [nz][ny][P] -------------------------------------------------------
-template <int N, int AXIS, bool INVERSE, class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+// One tile (8 columns x N) by a group of fast_threads_yz<N>() threads: t = thread index within the group, buf = the
+// group's [N][8] shared buffer, bar = the group's barrier id.  Used by the per-pass kernel (group = block) and by the
+// persistent SCF kernel (several groups per block).
+template <int N, int AXIS, bool INVERSE, bool PREFETCH, class LoadOp, class StoreOp>
+__device__ __forceinline__ void fft_yz_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf, int t_in_group,
+                                            int bar) {
   constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, TH = fast_threads_yz<N>(), JS = TH / kFastL;
-  extern __shared__ double smem_raw[];
-  double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [N][8]
-  LoadOp ld = ld_in;
-  StoreOp st = st_in;
-  if (G.stop && *G.stop) return;
-  ld.begin(); st.begin();
-  const int l = threadIdx.x % kFastL, jj = threadIdx.x / kFastL;
+  const int l = t_in_group % kFastL, jj = t_in_group / kFastL;
   const int xt = G.P / kFastL;
-  const int fixed = blockIdx.x / xt, ix = (blockIdx.x % xt) * kFastL + l;   // fixed = iz (AXIS 1) or iy (AXIS 2)
+  const int fixed = tile / xt, ix = (tile % xt) * kFastL + l;   // fixed = iz (AXIS 1) or iy (AXIS 2)
   const long long stride = AXIS == 1 ? G.P : (long long)G.P * G.ny;
   const long long base = (AXIS == 1 ? (long long)fixed * G.ny * G.P : (long long)fixed * G.P) + ix;
-  if (l == 0) {  // one lane per 128-byte row: request every operand line of the tile now
+  if (PREFETCH && l == 0) {  // one lane per 128-byte row: request every operand line of the tile now
     for (int j1 = jj; j1 < R2; j1 += JS)
 #pragma unroll
       for (int t = 0; t < R1; ++t) ld.prefetch(base + (j1 + t * R2) * stride);
@@ -165,7 +166,7 @@ __global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastG
 #pragma unroll
     for (int t = 0; t < R1; ++t) buf[(j1 * R1 + t) * kFastL + l] = v[t];
   }
-  __syncthreads();
+  group_sync(bar, TH);
   // stage 2: shared -> registers -> global
   for (int j2 = jj; j2 < R1; j2 += JS) {
     double2 v[R2];
@@ -180,7 +181,17 @@ __global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastG
       st.store(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, INVERSE ? -v[t].y : v[t].y);
     }
   }
-  __syncthreads();
+  group_sync(bar, TH);
+}
+
+template <int N, int AXIS, bool INVERSE, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  extern __shared__ double smem_raw[];
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
+  ld.begin(); st.begin();
+  fft_yz_tile<N, AXIS, INVERSE, true>(G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw), threadIdx.x, 0);
   ld.finish(smem_raw);
   st.finish(smem_raw);
 }
@@ -227,17 +238,13 @@ __device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *__res
   __syncthreads();
 }
 
-template <int N, class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(fast_threads_x<N>()) fft_r2c_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+// one x tile (8 pairs of real lines) by the whole block (256 threads); buf = [LP][ROW] shared
+template <int N, bool PREFETCH, class LoadOp, class StoreOp>
+__device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf) {
   constexpr int TH = fast_threads_x<N>(), ROW = fast_row_x<N>(), NXH = N / 2 + 1;
-  extern __shared__ double smem_raw[];
-  double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
-  LoadOp ld = ld_in;
-  StoreOp st = st_in;
-  if (G.stop && *G.stop) return;
-  ld.begin(); st.begin();
-  const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
-  for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
+  const long long line0 = (long long)tile * (2 * kFastLP);
+  if (PREFETCH)
+    for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
   for (int e = threadIdx.x; e < kFastLP * N; e += TH) {
     const int p = e / N, i = e % N;
     const long long la = line0 + 2 * p, lb = la + 1;
@@ -260,22 +267,16 @@ __global__ void __launch_bounds__(fast_threads_x<N>()) fft_r2c_fast_kernel(FastG
     st.store(lb * G.P + k, k, (int)(lb % G.ny), (int)(lb / G.ny), B.x, B.y);
   }
   __syncthreads();
-  ld.finish(smem_raw);
-  st.finish(smem_raw);
 }
 
-template <int N, class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+template <int N, bool PREFETCH, class LoadOp, class StoreOp>
+__device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf) {
   constexpr int TH = fast_threads_x<N>(), ROW = fast_row_x<N>(), NXH = N / 2 + 1;
-  extern __shared__ double smem_raw[];
-  double2 *buf = reinterpret_cast<double2 *>(smem_raw);
-  LoadOp ld = ld_in;
-  StoreOp st = st_in;
-  if (G.stop && *G.stop) return;
-  ld.begin(); st.begin();
-  const long long line0 = (long long)blockIdx.x * (2 * kFastLP);
-  for (int e = threadIdx.x * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile
-  for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) st.prefetch(line0 * N + e);    // operands of the epilogue
+  const long long line0 = (long long)tile * (2 * kFastLP);
+  if (PREFETCH) {
+    for (int e = threadIdx.x * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile
+    for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) st.prefetch(line0 * N + e);    // operands of the epilogue
+  }
   for (int e = threadIdx.x; e < kFastLP * NXH; e += TH) {
     const int p = e / NXH, k = e % NXH;
     const long long la = line0 + 2 * p, lb = la + 1;
@@ -294,6 +295,28 @@ __global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastG
     st.store_real2(la * N + i, lb * N + i, z.x, -z.y);
   }
   __syncthreads();
+}
+
+template <int N, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(fast_threads_x<N>()) fft_r2c_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  extern __shared__ double smem_raw[];
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
+  ld.begin(); st.begin();
+  fft_r2c_tile<N, true>(G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw));
+  ld.finish(smem_raw);
+  st.finish(smem_raw);
+}
+
+template <int N, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  extern __shared__ double smem_raw[];
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
+  ld.begin(); st.begin();
+  fft_c2r_tile<N, true>(G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw));
   ld.finish(smem_raw);
   st.finish(smem_raw);
 }

@@ -137,28 +137,38 @@ __global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
 //   Vhat_ie <- v(k) (S + S2)/2, the Hermitian part, whose half-spectrum inverse equals the real part of the full
 //   inverse transform of v(k) S_Z(k);  sum conj(nhat) Vhat_ie over the half spectrum then equals Re sum over the full
 //   literal set.  It also corrects the Ewald reciprocal energy for the mirrored halves of the y/z Nyquist rows.
-// Points are enumerated as: list A = rows with iy or iz Nyquist (all ix < nxh), list B = column ix = nx/2 of the
-// remaining rows.  One thread per point, direct sum over the ions (O(N_i N^2) work).
+// Points: list A = rows with ky or kz Nyquist (all stored kx), list B = the column kx = nx/2 of the other rows.
+// One warp per point: the lanes stride over the ions (coalesced [k][j] tables), fixed-order shuffle reduction.
 __global__ void __launch_bounds__(128) structure_factor_nyquist_kernel(
-    GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ji, const double2 *__restrict__ by_ij,
-    const double2 *__restrict__ cz_ij, const double *__restrict__ vps, const double *__restrict__ va,
-    const double2 *__restrict__ S, double2 *__restrict__ S2, double2 *__restrict__ vh_ie, double *partials,
-    unsigned int *counter, DevScalars *sc) {
+    GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ij /*[ix][j]*/,
+    const double2 *__restrict__ by_ij, const double2 *__restrict__ cz_ij, const double *__restrict__ vps,
+    const double *__restrict__ va, const double2 *__restrict__ S, double2 *__restrict__ S2, double2 *__restrict__ vh_ie,
+    double *partials, unsigned int *counter, DevScalars *sc) {
   __shared__ double s_red[32 + 1 + 1];
   const int nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
   const int nyq_x = (G.nx % 2 == 0) ? G.nx / 2 : -1;
   const long long nrows = (long long)G.ny * G.nz;
-  const long long total = nrows * G.nxh;     // simple enumeration: every stored point tests itself
+  const int rowsA = (nyq_z >= 0 ? G.ny : 0) + (nyq_y >= 0 ? (nyq_z >= 0 ? G.nz - 1 : G.nz) : 0);
+  const long long nA = (long long)rowsA * G.nxh, total = nA + (nyq_x >= 0 ? nrows : 0);
+  const int lane = threadIdx.x & 31;
+  const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
   double corr = 0.0;
-  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (long long)gridDim.x * blockDim.x) {
-    const int ix = (int)(e % G.nxh);
-    const long long row = e / G.nxh;
-    const int iy = (int)(row % G.ny), iz = (int)(row / G.ny);
+  for (long long e = warp0; e < total; e += nwarps) {
+    int ix, iy, iz;
+    if (e < nA) {
+      const int ra = (int)(e / G.nxh);
+      ix = (int)(e % G.nxh);
+      if (nyq_z >= 0 && ra < G.ny) { iy = ra; iz = nyq_z; }
+      else { const int q = ra - (nyq_z >= 0 ? G.ny : 0); iy = nyq_y; iz = (nyq_z >= 0 && q >= nyq_z) ? q + 1 : q; }
+    } else {
+      const long long row = e - nA;
+      ix = nyq_x; iy = (int)(row % G.ny); iz = (int)(row / G.ny);
+      if (iy == nyq_y || iz == nyq_z) continue;   // already in list A
+    }
     const bool fy = iy == nyq_y, fz = iz == nyq_z, fx = ix == nyq_x;
-    if (!(fx || fy || fz)) continue;
     double sr = 0.0, si = 0.0;
-    for (int j = 0; j < nions; ++j) {
-      double2 a = ax_ji[(long long)j * G.nx + ix], b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
+    for (int j = lane; j < nions; j += 32) {
+      double2 a = ax_ij[(long long)ix * nions + j], b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
       if (fx) a.y = -a.y;
       if (fy) b.y = -b.y;
       if (fz) c.y = -c.y;
@@ -166,13 +176,16 @@ __global__ void __launch_bounds__(128) structure_factor_nyquist_kernel(
       const double bcx = b.x * c.x - b.y * c.y, bcy = b.x * c.y + b.y * c.x;
       sr += z * (a.x * bcx - a.y * bcy); si += z * (a.x * bcy + a.y * bcx);
     }
-    const long long g = row * G.P + ix;
-    const double2 s = S[g];
-    S2[g] = make_double2(sr, si);
-    const double v = vps[g];
-    vh_ie[g] = make_double2(0.5 * v * (s.x + sr), 0.5 * v * (s.y + si));
-    // interior columns were counted twice with |S|^2; the mirrored half carries |S2|^2 instead
-    if (ix != 0 && !fx) corr += va[g] * ((sr * sr + si * si) - (s.x * s.x + s.y * s.y));
+    sr = warp_sum(sr); si = warp_sum(si);
+    if (lane == 0) {
+      const long long g = ((long long)iz * G.ny + iy) * G.P + ix;
+      const double2 s = S[g];
+      S2[g] = make_double2(sr, si);
+      const double v = vps[g];
+      vh_ie[g] = make_double2(0.5 * v * (s.x + sr), 0.5 * v * (s.y + si));
+      // interior columns were counted twice with |S|^2; the mirrored half carries |S2|^2 instead
+      if (ix != 0 && !fx) corr += va[g] * ((sr * sr + si * si) - (s.x * s.x + s.y * s.y));
+    }
   }
   double v[1] = {corr};
   const int op[1] = {0};

@@ -180,16 +180,11 @@ __device__ __forceinline__ void mu_accumulate4(const double *tab, const double (
   for (int q = 0; q < 4; ++q) if (ok[q]) { s1 += i12[q]; s0 += im12[q]; }
 }
 
-__global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
-                                                       DevScalars *sc, const double *__restrict__ fdtab,
-                                                       double *partials, int max_pass, const int *stop) {
-  namespace cg = cooperative_groups;
-  if (stop && *stop) return;   // uniform over the grid: no block reaches a barrier
-  cg::grid_group grid = cg::this_grid();
-  __shared__ double s_tab[kFdTabDoubles];
-  __shared__ double s_red[2 * 32 + 2];
-  __shared__ double s_bc[2];
-  fd_load_tables(s_tab, fdtab);
+// s_tab: the Fermi-Dirac table in shared memory (already loaded and synchronised); s_red: [2*32+2]; s_bc: [2];
+// partials: [2][gridDim.x][2], not shared with any other reduction that may run concurrently
+__device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &grid, const double *__restrict__ V_i,
+                                             long long ng, const ScfConst &C, DevScalars *sc, const double *s_tab,
+                                             double *s_red, double *s_bc, double *partials, int max_pass) {
   const double inv_kT = 1.0 / C.kT, kT_eta0 = C.kT * C.eta0, scaleN = C.cTF * C.dV;
   const long long nthreads = (long long)gridDim.x * blockDim.x, tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const bool cached = ng <= nthreads * kMuCache;
@@ -269,6 +264,21 @@ __global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict_
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     sc->mu = mu; sc->mu_lo = lo; sc->mu_hi = hi; sc->mu_evals = evals; sc->mu_evals_total += evals; sc->N_last = f + C.Ne;
   }
+  return mu;   // identical in every thread of the grid
+}
+
+__global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
+                                                       DevScalars *sc, const double *__restrict__ fdtab,
+                                                       double *partials, int max_pass, const int *stop) {
+  namespace cg = cooperative_groups;
+  if (stop && *stop) return;   // uniform over the grid: no block reaches a barrier
+  cg::grid_group grid = cg::this_grid();
+  __shared__ double s_tab[kFdTabDoubles];
+  __shared__ double s_red[2 * 32 + 2];
+  __shared__ double s_bc[2];
+  fd_load_tables(s_tab, fdtab);
+  __syncthreads();
+  mu_solve_dev(grid, V_i, ng, C, sc, s_tab, s_red, s_bc, partials, max_pass);
 }
 
 // ---- S4 fused into the forward x pass: n_a, chi and the local reductions K, ||dn||^2, ||n_a||^2, F0, K_e, E_xc,

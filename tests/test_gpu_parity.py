@@ -148,6 +148,30 @@ def test_full_size_configs_iterations_and_forces(orc, torch_cuda, name, iters):
     assert abs(g.get_real("n_a").sum().item() * dV - cfg["Z"].sum()) < 1e-12 * cfg["Z"].sum()
 
 
+def test_c2_solve_in_one_cooperative_launch(orc, torch_cuda, monkeypatch):
+    """configs[1] through arche_scf_solve: on 32^3 / 64^3 grids the whole solve runs in one persistent cooperative
+    kernel (scf_persistent.cuh).  Ten iterations replayed against the oracle, and against the per-pass form."""
+    cfg = ai.make_config("c2")
+    kw = dict(mix_warmup=3, mix_w_fixed=0.95, scf_fixed_iter=10)
+    o = orc.Oracle(cfg, **kw); ro = o.scf_solve(cfg["pos"])
+    g = _gpu(cfg, **kw)
+    l0 = g.launch_count(); rg = g.scf_solve(cfg["pos"]); launches = g.launch_count() - l0
+    assert launches < 20, launches                       # per-MD-step kernels + ONE launch for the ten iterations
+    assert rg["scf_iters"] == ro["scf_iters"] == 10
+    na = g.get_real("n_a").cpu().numpy()
+    assert _rel(na, o.get_real("n_a")) < TOL_N
+    assert _rel(g.get_real("n_i").cpu().numpy(), o.get_real("n_i")) < TOL_N
+    for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "K_e", "w_last"):
+        assert abs(rg[k] - ro[k]) <= TOL_F * max(1.0, abs(ro[k])), (k, rg[k], ro[k])
+    Fg = g.forces().cpu().numpy(); Fo = o.forces()
+    assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max()
+    monkeypatch.setenv("ARCHE_PERSIST", "0")
+    g2 = _gpu(cfg, **kw)
+    l0 = g2.launch_count(); r2 = g2.scf_solve(cfg["pos"])
+    assert g2.launch_count() - l0 > 70                   # 7 launches per iteration
+    assert _rel(g2.get_real("n_a").cpu().numpy(), na) < 1e-13 and abs(r2["F_total"] - rg["F_total"]) < 1e-12 * abs(rg["F_total"])
+
+
 def test_converged_solve_and_forces(orc, torch_cuda, pointwise_mode):
     cfg = ai.make_small(n_ions=5, L=9.0, grid=(24, 16, 18), cell=[9.0, 7.5, 8.0], T_eV=10.0, seed=9)
     g, o, rg, ro = _solve_pair(orc, cfg, scf_tol_dn=1e-11, init_mode=0)
