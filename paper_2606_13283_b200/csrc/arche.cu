@@ -101,6 +101,7 @@ struct arche_ctx {
   double *Z, *mass, *pos, *F, *F_pp, *e_pp, *F_part, *vel_tmp;
   double *fdtab, *partials;
   unsigned int *counter;
+  unsigned long long *phase_ns;
   DevScalars *sc;
   DevScalars *h_sc;  // pinned
   bool have_g, have_solution, have_forces;
@@ -177,6 +178,7 @@ size_t layout(arche_ctx *c, char *base) {
   c->fdtab = w.take<double>(kFdTabDoubles);
   c->partials = w.take<double>((size_t)c->red_blocks * kMaxRed);
   c->counter = w.take<unsigned int>(64);
+  c->phase_ns = w.take<unsigned long long>(8);
   c->sc = w.take<DevScalars>(1);
   return w.off;
 }
@@ -527,21 +529,30 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   const int fixed = c->p.scf_fixed_iter;
   const int maxit = fixed > 0 ? fixed : (c->p.scf_max_iter > 0 ? c->p.scf_max_iter : 200);
   bool conv = false;
-  // L2-resident production grids: the whole solve in one cooperative launch (not while per-class profiling is on)
-  if (c->persist && !c->prof) {
+  // L2-resident production grids: the whole solve in one cooperative launch (with per-class profiling on, block 0
+  // times the phases with %globaltimer and the classes receive those times)
+  if (c->persist) {
     PersistParams pp;
+    pp.phase_ns = c->prof ? c->phase_ns : nullptr;
+    if (c->prof) CK(cudaMemsetAsync(c->phase_ns, 0, 8 * sizeof(unsigned long long), c->stream));
     pp.n_i = c->n_i; pp.n_a = c->n_a; pp.V_i = c->V_i; pp.nh_i = c->nh_i; pp.nh_a = c->nh_a; pp.work = c->work;
     pp.vh_ie = c->vh_ie; pp.kx2 = c->kx2; pp.ky2 = c->ky2; pp.kz2 = c->kz2;
     pp.tw0 = c->tw[0]; pp.tw1 = c->tw[1]; pp.tw2 = c->tw[2];
     pp.sc = c->sc; pp.partials = c->partials; pp.counter = c->counter; pp.fdtab = c->fdtab; pp.C = c->C;
     pp.nxh = c->nxh; pp.P = c->P; pp.ng = c->ng; pp.inv_vol = 1.0 / c->G.vol;
     pp.mix_first = c->mix_pending ? 1 : 0; pp.max_iters = maxit; pp.fixed = fixed > 0 ? 1 : 0; pp.mu_max_pass = kMuMaxPasses;
-    cudaError_t e = scf_persistent_launch(c->G.nx, c->G.ny, c->G.nz, pp, c->sm_count, c->stream);
+    cudaError_t e = scf_persistent_launch(c->G.nx, c->G.ny, c->G.nz, pp, c->sm_count * kPersistBlocksPerSM, c->stream);
     if (e == cudaSuccess) {
       ++c->launches;
       c->mix_pending = true; c->have_solution = true; c->have_forces = false;
       rc = read_scalars(c);
       if (rc) return rc;
+      if (c->prof) {
+        unsigned long long ns[8];
+        CK(cudaMemcpy(ns, c->phase_ns, sizeof(ns), cudaMemcpyDeviceToHost));
+        const int cls[7] = {PC_FFT_INV_Z, PC_FFT_Y, PC_FFT_INV_X, PC_MU, PC_DENSITY, PC_FFT_Y, PC_FFT_FWD_Z};
+        for (int k = 0; k < 7; ++k) { c->prof_ms[cls[k]] += 1e-6 * (double)ns[k]; c->prof_cnt[cls[k]] += (long long)ns[7]; }
+      }
       if (!isfinite(c->h_sc->F_total) || !isfinite(c->h_sc->mu)) return fail(c, ARCHE_ENAN, "non-finite free energy or mu");
       conv = fixed <= 0 && c->h_sc->converged;
       goto solved;

@@ -70,6 +70,31 @@ __device__ __forceinline__ void block_reduce(double (&v)[NQ], const int (&op)[NQ
   __syncthreads();
 }
 
+// Barrier-based form of the grid reduction for cooperative kernels: every block writes its partials, the caller
+// issues a grid barrier, then every block sums all partials in the same fixed order (no atomics, no last-block
+// serialisation; all blocks end up with identical totals).
+template <int NQ>
+__device__ __forceinline__ void block_partials(double (&v)[NQ], const int (&op)[NQ], double *smem /*[NQ*32]*/,
+                                               double *out /*[gridDim.x][NQ]*/) {
+  block_reduce<NQ>(v, op, smem);
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) out[(size_t)blockIdx.x * NQ + q] = v[q];
+  }
+}
+// totals valid in thread 0 (written to t[NQ] there); call after the grid barrier that follows block_partials
+template <int NQ>
+__device__ __forceinline__ void block_totals(const int (&op)[NQ], const double *in /*[gridDim.x][NQ]*/, double *smem,
+                                             double (&t)[NQ]) {
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) t[q] = op[q] == 0 ? 0.0 : (op[q] == 1 ? 1.0e308 : -1.0e308);
+  for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) t[q] = red_combine(t[q], __ldcg(&in[(size_t)b * NQ + q]), op[q]);
+  }
+  block_reduce<NQ>(t, op, smem);
+}
+
 // Grid-level deterministic reduction.  Every block calls this once with its per-thread values.
 // partials: [gridDim.x * NQ]; counter: zero before the launch (reset by the last block);
 // returns true in ALL threads of the last block, with the totals in `out` (shared memory, [NQ]).

@@ -117,6 +117,7 @@ __device__ __forceinline__ void fft_stage(const double *__restrict__ sre, const 
 // finish(smem) once per block at the end (grid reductions; smem = the tile buffer, free by then);
 // prefetch(idx): L2 prefetch of the operand lines the functor will touch at element idx (fast passes only).
 struct LoadComplex {
+  static constexpr bool kWriteBack = false;
   const double2 *src;
   __device__ __forceinline__ void begin() {}
   __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(src + idx); }
@@ -126,6 +127,7 @@ struct LoadComplex {
   __device__ __forceinline__ void finish(double *) {}
 };
 struct StoreComplex {
+  static constexpr bool kSplitStore = false;
   double2 *dst;
   __device__ __forceinline__ void begin() {}
   __device__ __forceinline__ void prefetch(long long) const {}

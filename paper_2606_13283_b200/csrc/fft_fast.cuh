@@ -156,11 +156,25 @@ __device__ __forceinline__ void fft_yz_tile(const FastGeom &G, LoadOp &ld, Store
   // stage 1: global -> registers -> shared
   for (int j1 = jj; j1 < R2; j1 += JS) {
     double2 v[R1];
+    if constexpr (LoadOp::kWriteBack && R1 <= 8) {
+      // a prologue that also updates its operand in place: all loads first, then the stores, so that the stores
+      // (which the compiler must assume to alias the next loads) do not serialise the load latencies
+      double2 wb[R1];
 #pragma unroll
-    for (int t = 0; t < R1; ++t) {
-      const int i = j1 + t * R2;
-      ld(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, v[t].y);
-      if (INVERSE) v[t].y = -v[t].y;
+      for (int t = 0; t < R1; ++t) {
+        const int i = j1 + t * R2;
+        ld.load_wb(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, v[t].y, wb[t]);
+        if (INVERSE) v[t].y = -v[t].y;
+      }
+#pragma unroll
+      for (int t = 0; t < R1; ++t) ld.store_wb(base + (j1 + t * R2) * stride, ix, wb[t]);
+    } else {
+#pragma unroll
+      for (int t = 0; t < R1; ++t) {
+        const int i = j1 + t * R2;
+        ld(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, v[t].y);
+        if (INVERSE) v[t].y = -v[t].y;
+      }
     }
     Dft<R1>::run(v);
 #pragma unroll
@@ -175,10 +189,22 @@ __device__ __forceinline__ void fft_yz_tile(const FastGeom &G, LoadOp &ld, Store
 #pragma unroll
     for (int t = 1; t < R2; ++t) v[t] = cmul(v[t], __ldg(&G.tw[t * j2]));
     Dft<R2>::run(v);
+    if constexpr (StoreOp::kSplitStore && R2 <= 8) {
+      // an epilogue that reads further operands: every load and reduction first, then the stores (see above)
 #pragma unroll
-    for (int t = 0; t < R2; ++t) {
-      const int i = j2 + t * R1;
-      st.store(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, INVERSE ? -v[t].y : v[t].y);
+      for (int t = 0; t < R2; ++t) {
+        const int i = j2 + t * R1;
+        if (INVERSE) v[t].y = -v[t].y;
+        st.accumulate(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t]);
+      }
+#pragma unroll
+      for (int t = 0; t < R2; ++t) st.put(base + (j2 + t * R1) * stride, v[t]);
+    } else {
+#pragma unroll
+      for (int t = 0; t < R2; ++t) {
+        const int i = j2 + t * R1;
+        st.store(base + i * stride, ix, AXIS == 1 ? i : fixed, AXIS == 1 ? fixed : i, v[t].x, INVERSE ? -v[t].y : v[t].y);
+      }
     }
   }
   group_sync(bar, TH);
@@ -239,9 +265,9 @@ __device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *__res
 }
 
 // one x tile (8 pairs of real lines) by the whole block (256 threads); buf = [LP][ROW] shared
-template <int N, bool PREFETCH, class LoadOp, class StoreOp>
+template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), class LoadOp, class StoreOp>
 __device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf) {
-  constexpr int TH = fast_threads_x<N>(), ROW = fast_row_x<N>(), NXH = N / 2 + 1;
+  constexpr int ROW = fast_row_x<N>(), NXH = N / 2 + 1;
   const long long line0 = (long long)tile * (2 * kFastLP);
   if (PREFETCH)
     for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
@@ -269,9 +295,9 @@ __device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, Stor
   __syncthreads();
 }
 
-template <int N, bool PREFETCH, class LoadOp, class StoreOp>
+template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), class LoadOp, class StoreOp>
 __device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf) {
-  constexpr int TH = fast_threads_x<N>(), ROW = fast_row_x<N>(), NXH = N / 2 + 1;
+  constexpr int ROW = fast_row_x<N>(), NXH = N / 2 + 1;
   const long long line0 = (long long)tile * (2 * kFastLP);
   if (PREFETCH) {
     for (int e = threadIdx.x * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile

@@ -66,6 +66,7 @@ struct HalfGeom {
 // ---- S1: Vhat(k) = nhat_i(k)/(pi k^2) + Vhat_ie(k), 0 at k = 0 (Eq. 12, 14).  When a mixing step is pending the
 // new input density nhat_i <- nhat_a + w (nhat_i - nhat_a) (S6) is formed here and written back.
 struct LoadPotentialG {
+  static constexpr bool kWriteBack = true;
   double2 *nh_i;
   const double2 *nh_a, *vh_ie;
   const double *kx2, *ky2, *kz2;
@@ -91,6 +92,23 @@ struct LoadPotentialG {
     const double2 b = vh_ie[idx];
     re = fma(a.x, inv, b.x); im = fma(a.y, inv, b.y);
   }
+  // the same without the in-place store: wb receives the mixed nhat_i, stored afterwards by store_wb
+  __device__ __forceinline__ void load_wb(long long idx, int ix, int iy, int iz, double &re, double &im, double2 &wb) {
+    re = 0.0; im = 0.0; wb = make_double2(0.0, 0.0);
+    if (ix >= nxh) return;
+    double2 a = nh_i[idx];
+    if (mix) {
+      const double2 na = nh_a[idx];
+      a = make_double2(fma(w, a.x - na.x, na.x), fma(w, a.y - na.y, na.y));
+    }
+    wb = a;
+    const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
+    if (k2 == 0.0) return;
+    const double inv = 1.0 / (ARCHE_PI * k2);
+    const double2 b = vh_ie[idx];
+    re = fma(a.x, inv, b.x); im = fma(a.y, inv, b.y);
+  }
+  __device__ __forceinline__ void store_wb(long long idx, int ix, double2 wb) { if (mix && ix < nxh) nh_i[idx] = wb; }
   __device__ __forceinline__ void finish(double *) {}
 };
 
@@ -151,14 +169,21 @@ struct StoreVi {
   __device__ __forceinline__ void finish(double *smem) {
     double v[4] = {acc_min, acc_max, acc_sum, acc_n};
     const int op[4] = {1, 2, 0, 0};
-    if (grid_reduce<4>(v, op, partials, counter, smem) && threadIdx.x == 0) {
-      const double *t = smem + 4 * 32;
-      sc->vmin = t[0]; sc->vmax = t[1]; sc->vsum = t[2]; sc->n0sum = t[3];
-      // bracket of the root of Eq. 19: N(mu) is increasing and eta0 solves the flat-potential problem
-      const double lo = t[0] + kT_eta0, hi = t[1] + kT_eta0;
-      const double pad = 1e-12 * (fabs(lo) + fabs(hi) + fabs(kT_eta0));
-      sc->mu_lo = lo - pad; sc->mu_hi = hi + pad;
-    }
+    if (grid_reduce<4>(v, op, partials, counter, smem) && threadIdx.x == 0) apply(smem + 4 * 32, kT_eta0, sc);
+  }
+  // grid totals {min, max, sum of V_i, sum I_{1/2}} -> scalars and the mu bracket
+  static __device__ __forceinline__ void apply(const double *t, double kT_eta0, DevScalars *sc) {
+    sc->vmin = t[0]; sc->vmax = t[1]; sc->vsum = t[2]; sc->n0sum = t[3];
+    // bracket of the root of Eq. 19: N(mu) is increasing and eta0 solves the flat-potential problem
+    const double lo = t[0] + kT_eta0, hi = t[1] + kT_eta0;
+    const double pad = 1e-12 * (fabs(lo) + fabs(hi) + fabs(kT_eta0));
+    sc->mu_lo = lo - pad; sc->mu_hi = hi + pad;
+  }
+  // persistent form: block partial sums only (the totals are taken by every block after the next grid barrier)
+  __device__ __forceinline__ void partial(double *smem, double *out /*[gridDim.x][4]*/) {
+    double v[4] = {acc_min, acc_max, acc_sum, acc_n};
+    const int op[4] = {1, 2, 0, 0};
+    block_partials<4>(v, op, smem, out);
   }
 };
 
@@ -181,10 +206,12 @@ __device__ __forceinline__ void mu_accumulate4(const double *tab, const double (
 }
 
 // s_tab: the Fermi-Dirac table in shared memory (already loaded and synchronised); s_red: [2*32+2]; s_bc: [2];
-// partials: [2][gridDim.x][2], not shared with any other reduction that may run concurrently
+// partials: [2][gridDim.x][2], not shared with any other reduction that may run concurrently; sc may be the global
+// scalar block (block 0 writes the result) or a per-block shared copy (sc_is_block_local: every block writes its own)
 __device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &grid, const double *__restrict__ V_i,
                                              long long ng, const ScfConst &C, DevScalars *sc, const double *s_tab,
-                                             double *s_red, double *s_bc, double *partials, int max_pass) {
+                                             double *s_red, double *s_bc, double *partials, int max_pass,
+                                             bool sc_is_block_local = false) {
   const double inv_kT = 1.0 / C.kT, kT_eta0 = C.kT * C.eta0, scaleN = C.cTF * C.dV;
   const long long nthreads = (long long)gridDim.x * blockDim.x, tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const bool cached = ng <= nthreads * kMuCache;
@@ -261,7 +288,7 @@ __device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &g
     mu_prev = mu; f_prev = f; have_prev_pt = true;
     mu = mu_new;
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
+  if ((sc_is_block_local || blockIdx.x == 0) && threadIdx.x == 0) {
     sc->mu = mu; sc->mu_lo = lo; sc->mu_hi = hi; sc->mu_evals = evals; sc->mu_evals_total += evals; sc->N_last = f + C.Ne;
   }
   return mu;   // identical in every thread of the grid
@@ -335,12 +362,17 @@ struct LoadDensity {
   __device__ __forceinline__ void finish(double *smem) {
     double v[7] = {sK, sdn2, sna2, sF0, sKe, sExc, sChi};
     const int op[7] = {0, 0, 0, 0, 0, 0, 0};
-    if (grid_reduce<7>(v, op, partials, counter, smem) && threadIdx.x == 0) {
-      const double *t = smem + 7 * 32;
-      sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
-      sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
-      sc->dNdmu = t[6] * C.dV;
-    }
+    if (grid_reduce<7>(v, op, partials, counter, smem) && threadIdx.x == 0) apply(smem + 7 * 32, C, sc);
+  }
+  static __device__ __forceinline__ void apply(const double *t, const ScfConst &C, DevScalars *sc) {
+    sc->K = t[0] * C.dV; sc->dn2 = t[1] * C.dV; sc->na2 = t[2] * C.dV;
+    sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
+    sc->dNdmu = t[6] * C.dV;
+  }
+  __device__ __forceinline__ void partial(double *smem, double *out /*[gridDim.x][7]*/) {
+    double v[7] = {sK, sdn2, sna2, sF0, sKe, sExc, sChi};
+    const int op[7] = {0, 0, 0, 0, 0, 0, 0};
+    block_partials<7>(v, op, smem, out);
   }
 };
 
@@ -356,6 +388,7 @@ struct LoadReal {
 };
 
 struct StoreNhatA {
+  static constexpr bool kSplitStore = true;
   double2 *nh_a;
   const double2 *nh_i, *vh_ie;
   const double *kx2, *ky2, *kz2;
@@ -383,11 +416,36 @@ struct StoreNhatA {
       aEH += (re * re + im * im) * inv;                  // Eq. 53
     }
   }
+  // split form of store(): accumulate() scales v in place and does every load and reduction, put() stores
+  __device__ __forceinline__ void accumulate(long long idx, int ix, int iy, int iz, double2 &v) {
+    if (ix >= H.nxh) { v = make_double2(0.0, 0.0); return; }
+    v.x *= C.dV; v.y *= C.dV;
+    const double wt = H.wt(ix);
+    const double2 b = vh_ie[idx];
+    aEie += wt * (v.x * b.x + v.y * b.y);
+    const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
+    if (k2 != 0.0) {
+      const double inv = wt / (ARCHE_PI * k2);
+      const double2 a = nh_i[idx];
+      const double dr = a.x - v.x, di = a.y - v.y;
+      aU += (dr * dr + di * di) * inv;
+      aEH += (v.x * v.x + v.y * v.y) * inv;
+    }
+  }
+  __device__ __forceinline__ void put(long long idx, double2 v) { nh_a[idx] = v; }
   __device__ __forceinline__ void finish(double *smem) {
     double v[3] = {aU, aEH, aEie};
     const int op[3] = {0, 0, 0};
-    if (grid_reduce<3>(v, op, partials, counter, smem) && threadIdx.x == 0) {
-      const double *t = smem + 3 * 32;
+    if (grid_reduce<3>(v, op, partials, counter, smem) && threadIdx.x == 0) apply(smem + 3 * 32, C, sc);
+  }
+  __device__ __forceinline__ void partial(double *smem, double *out /*[gridDim.x][3]*/) {
+    double v[3] = {aU, aEH, aEie};
+    const int op[3] = {0, 0, 0};
+    block_partials<3>(v, op, smem, out);
+  }
+  // grid totals {U, E_H, E_ie sums} -> energies, w (Eq. 30-31), free energy and the stop flag
+  static __device__ __forceinline__ void apply(const double *t, const ScfConst &C, DevScalars *sc) {
+    {
       const double U = t[0] / C.vol, EH = 0.5 * t[1] / C.vol, Eie = t[2] / C.vol;
       sc->U = U; sc->EH = EH; sc->Eie = Eie;
       const int it = sc->iter + 1;
@@ -445,6 +503,7 @@ __global__ void g_store_kernel(double2 *__restrict__ gh, double2 *__restrict__ g
 // nhat_i = S_Z^{new} ghat^{old} (Eq. 20) symmetrised so that the half-spectrum inverse returns the real part of the
 // full inverse transform (reading A6): X_sym = (S ghat + S2 ghat2)/2, equal to S ghat off the Nyquist planes.
 struct LoadSG {
+  static constexpr bool kWriteBack = false;
   const double2 *S, *S2, *gh, *gh2;
   int nxh;
   __device__ __forceinline__ void begin() {}
@@ -503,6 +562,7 @@ struct LoadRealScaled {  // reads n_i, rescales to N_e, writes it back and feeds
 };
 
 struct StoreScaled {  // half spectrum, scaled; zero in the padding columns
+  static constexpr bool kSplitStore = false;
   double2 *dst;
   double scale;
   int nxh;

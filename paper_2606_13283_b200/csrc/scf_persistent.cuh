@@ -35,11 +35,15 @@ struct PersistParams {
   int max_iters;   // iterations to run at most (exactly, when fixed)
   int fixed;       // 1: ignore the stop flag (parity replay)
   int mu_max_pass;
+  unsigned long long *phase_ns;   // optional [8]: nanoseconds per phase (7 phases incl. their barrier) + iteration count
 };
+
+constexpr int kPersistThreads = 256;     // measured on c2: 512 threads (one pair element per thread and x tile) is slower
+constexpr int kPersistBlocksPerSM = 1;   // measured on c2: 2 blocks/SM shortens the x phases but lengthens the barriers
 
 template <int NX, int NY, int NZ>
 constexpr size_t persist_smem_bytes() {
-  constexpr size_t gy = 256 / fast_threads_yz<NY>(), gz = 256 / fast_threads_yz<NZ>();
+  constexpr size_t gy = kPersistThreads / fast_threads_yz<NY>(), gz = kPersistThreads / fast_threads_yz<NZ>();
   constexpr size_t ty = gy * NY * kFastL * sizeof(double2), tz = gz * NZ * kFastL * sizeof(double2);
   constexpr size_t tx = (size_t)kFastLP * fast_row_x<NX>() * sizeof(double2);
   constexpr size_t tile = ty > tz ? (ty > tx ? ty : tx) : (tz > tx ? tz : tx);
@@ -48,14 +52,14 @@ constexpr size_t persist_smem_bytes() {
 
 template <int N, int AXIS, bool INVERSE, class LoadOp, class StoreOp>
 __device__ __forceinline__ void persist_yz_phase(const FastGeom &G, LoadOp &ld, StoreOp &st, double2 *tiles, int ntiles) {
-  constexpr int TH = fast_threads_yz<N>(), GR = 256 / TH;
+  constexpr int TH = fast_threads_yz<N>(), GR = kPersistThreads / TH;
   const int group = threadIdx.x / TH, t = threadIdx.x % TH;
   for (int tile = blockIdx.x + gridDim.x * group; tile < ntiles; tile += gridDim.x * GR)
     fft_yz_tile<N, AXIS, INVERSE, false>(G, ld, st, tile, tiles + (size_t)group * N * kFastL, t, 1 + group);
 }
 
 template <int NX, int NY, int NZ>
-__global__ void __launch_bounds__(256, 1) scf_persistent_kernel(PersistParams p) {
+__global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_persistent_kernel(PersistParams p) {
   namespace cg = cooperative_groups;
   cg::grid_group grid = cg::this_grid();
   extern __shared__ double smem[];
@@ -63,77 +67,120 @@ __global__ void __launch_bounds__(256, 1) scf_persistent_kernel(PersistParams p)
   double *s_red = s_tab + kFdTabDoubles;
   double *s_bc = s_red + kMaxRed * 33;
   double2 *tiles = reinterpret_cast<double2 *>(s_bc + 8);
+  // every block keeps its own copy of the scalar block in shared memory: the phase totals are taken by all blocks
+  // in the same fixed order after a grid barrier (block_partials / block_totals), so the copies stay identical and no
+  // block ever waits for another one's scalar result; block 0 writes the copy back at the end
+  __shared__ DevScalars s_sc;
+  if (threadIdx.x == 0) s_sc = *p.sc;
   fd_load_tables(s_tab, p.fdtab);
   __syncthreads();
+  DevScalars *const sc = &s_sc;
+  double *const part_vi = p.partials, *const part_dn = part_vi + (size_t)gridDim.x * 4,
+         *const part_g = part_dn + (size_t)gridDim.x * 7, *const part_mu = part_g + (size_t)gridDim.x * 3;
   const FastGeom Gx{NX, NY, NZ, p.P, p.tw0, nullptr}, Gy{NX, NY, NZ, p.P, p.tw1, nullptr}, Gz{NX, NY, NZ, p.P, p.tw2, nullptr};
   const int xtiles = NY * NZ / (2 * kFastLP), ytiles = NZ * (p.P / kFastL), ztiles = NY * (p.P / kFastL);
   int mix = p.mix_first;
+  const bool timing = p.phase_ns != nullptr && blockIdx.x == 0 && threadIdx.x == 0;
+  unsigned long long t_prev = 0;
+  auto lap = [&](int phase) {   // block 0 attributes the time since the previous lap (work + barrier) to `phase`
+    if (timing) {
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+      if (phase >= 0) p.phase_ns[phase] += t - t_prev;
+      t_prev = t;
+    }
+  };
+  lap(-1);
   for (int it = 0; it < p.max_iters; ++it) {
     // ---- S1 (+ pending S6 in G-space): inverse z pass
     {
       LoadPotentialG lp;
       lp.nh_i = p.nh_i; lp.nh_a = p.nh_a; lp.vh_ie = p.vh_ie; lp.kx2 = p.kx2; lp.ky2 = p.ky2; lp.kz2 = p.kz2;
-      lp.sc = p.sc; lp.nxh = p.nxh; lp.mix = mix;
+      lp.sc = sc; lp.nxh = p.nxh; lp.mix = mix;
       StoreComplex sw{p.work};
       lp.begin();
       persist_yz_phase<NZ, 2, true>(Gz, lp, sw, tiles, ztiles);
     }
     grid.sync();
+    lap(0);
     {
       LoadComplex lw{p.work};
       StoreComplex sw{p.work};
       persist_yz_phase<NY, 1, true>(Gy, lw, sw, tiles, ytiles);
     }
     grid.sync();
+    lap(1);
     // ---- S2 (+ pending S6 in real space, + first mu evaluation): c2r x pass
     {
       LoadComplex lw{p.work};
       StoreVi sv;
-      sv.V_i = p.V_i; sv.n_i = p.n_i; sv.n_a = p.n_a; sv.sc = p.sc; sv.partials = p.partials; sv.counter = p.counter;
+      sv.V_i = p.V_i; sv.n_i = p.n_i; sv.n_a = p.n_a; sv.sc = sc; sv.partials = nullptr; sv.counter = nullptr;
       sv.fdtab = s_tab; sv.inv_vol = p.inv_vol; sv.kT_eta0 = p.C.kT * p.C.eta0; sv.inv_kT = 1.0 / p.C.kT; sv.xc = p.C.xc;
       sv.mix = mix;
       sv.begin();
-      for (int tile = blockIdx.x; tile < xtiles; tile += gridDim.x) fft_c2r_tile<NX, false>(Gx, lw, sv, tile, tiles);
-      sv.finish(s_red);
+      for (int tile = blockIdx.x; tile < xtiles; tile += gridDim.x) fft_c2r_tile<NX, false, kPersistThreads>(Gx, lw, sv, tile, tiles);
+      sv.partial(s_red, part_vi);
     }
     grid.sync();
+    {
+      double t[4];
+      const int op[4] = {1, 2, 0, 0};
+      block_totals<4>(op, part_vi, s_red, t);
+      if (threadIdx.x == 0) StoreVi::apply(t, p.C.kT * p.C.eta0, sc);
+      __syncthreads();
+    }
+    lap(2);
     // ---- S3: mu (grid barriers inside, one per evaluation)
-    const double mu = mu_solve_dev(grid, p.V_i, p.ng, p.C, p.sc, s_tab, s_red, s_bc,
-                                   p.partials + (size_t)gridDim.x * kMaxRed, p.mu_max_pass);
+    const double mu = mu_solve_dev(grid, p.V_i, p.ng, p.C, sc, s_tab, s_red, s_bc, part_mu, p.mu_max_pass, true);
+    __syncthreads();
+    lap(3);
     // ---- S4: density prologue of the r2c x pass
     {
       LoadDensity ldn;
-      ldn.V_i = p.V_i; ldn.n_i = p.n_i; ldn.n_a = p.n_a; ldn.sc = p.sc; ldn.partials = p.partials; ldn.counter = p.counter;
+      ldn.V_i = p.V_i; ldn.n_i = p.n_i; ldn.n_a = p.n_a; ldn.sc = sc; ldn.partials = nullptr; ldn.counter = nullptr;
       ldn.fdtab = s_tab; ldn.C = p.C;
       StoreComplex sw{p.work};
       ldn.begin();
-      ldn.mu = mu;   // block 0's store to sc->mu may not be visible yet; every block holds the same value
-      for (int tile = blockIdx.x; tile < xtiles; tile += gridDim.x) fft_r2c_tile<NX, false>(Gx, ldn, sw, tile, tiles);
-      ldn.finish(s_red);
+      ldn.mu = mu;
+      for (int tile = blockIdx.x; tile < xtiles; tile += gridDim.x) fft_r2c_tile<NX, false, kPersistThreads>(Gx, ldn, sw, tile, tiles);
+      ldn.partial(s_red, part_dn);
     }
     grid.sync();
+    lap(4);
     {
       LoadComplex lw{p.work};
       StoreComplex sw{p.work};
       persist_yz_phase<NY, 1, false>(Gy, lw, sw, tiles, ytiles);
     }
     grid.sync();
+    lap(5);
     // ---- S5 (+ w, F, stop flag): forward z pass
     {
       LoadComplex lw{p.work};
       StoreNhatA sn;
       sn.nh_a = p.nh_a; sn.nh_i = p.nh_i; sn.vh_ie = p.vh_ie; sn.kx2 = p.kx2; sn.ky2 = p.ky2; sn.kz2 = p.kz2;
-      sn.sc = p.sc; sn.partials = p.partials; sn.counter = p.counter; sn.C = p.C; sn.H.nx = NX; sn.H.nxh = p.nxh;
+      sn.sc = sc; sn.partials = nullptr; sn.counter = nullptr; sn.C = p.C; sn.H.nx = NX; sn.H.nxh = p.nxh;
       sn.prestored = 0;
       sn.begin();
       persist_yz_phase<NZ, 2, false>(Gz, lw, sn, tiles, ztiles);
       __syncthreads();
-      sn.finish(s_red);
+      sn.partial(s_red, part_g);
     }
     grid.sync();
+    {  // totals of the density pass and of the G-space pass -> K, F0, ..., then U, E_H, E_ie, w, F and the stop flag
+      double t7[7], t3[3];
+      const int op7[7] = {0, 0, 0, 0, 0, 0, 0}, op3[3] = {0, 0, 0};
+      block_totals<7>(op7, part_dn, s_red, t7);
+      block_totals<3>(op3, part_g, s_red, t3);
+      if (threadIdx.x == 0) { LoadDensity::apply(t7, p.C, sc); StoreNhatA::apply(t3, p.C, sc); }
+      __syncthreads();
+    }
+    lap(6);
+    if (timing) p.phase_ns[7] += 1;
     mix = 1;
-    if (!p.fixed && __ldcg(&p.sc->converged)) break;
+    if (!p.fixed && sc->converged) break;
   }
+  if (blockIdx.x == 0 && threadIdx.x == 0) *p.sc = s_sc;
 }
 
 // launches the persistent solve when the grid has an instantiation; cudaErrorNotSupported otherwise
@@ -147,7 +194,7 @@ static inline cudaError_t scf_persistent_launch(int nx, int ny, int nz, const Pe
   if (e != cudaSuccess) return e;
   PersistParams pp = p;
   void *args[] = {&pp};
-  return cudaLaunchCooperativeKernel(kern, dim3(blocks), dim3(256), args, smem, stream);
+  return cudaLaunchCooperativeKernel(kern, dim3(blocks), dim3(kPersistThreads), args, smem, stream);
 }
 
 }  // namespace arche
