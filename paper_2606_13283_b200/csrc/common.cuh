@@ -75,24 +75,30 @@ __device__ __forceinline__ void block_reduce(double (&v)[NQ], const int (&op)[NQ
 // serialisation; all blocks end up with identical totals).
 template <int NQ>
 __device__ __forceinline__ void block_partials(double (&v)[NQ], const int (&op)[NQ], double *smem /*[NQ*32]*/,
-                                               double *out /*[gridDim.x][NQ]*/) {
+                                               double *out /*[gridDim.x][stride]*/, int stride = NQ, int offset = 0) {
   block_reduce<NQ>(v, op, smem);
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) out[(size_t)blockIdx.x * NQ + q] = v[q];
+    for (int q = 0; q < NQ; ++q) out[(size_t)blockIdx.x * stride + offset + q] = v[q];
   }
 }
-// totals valid in thread 0 (written to t[NQ] there); call after the grid barrier that follows block_partials
+// totals valid in thread 0 (written to t[NQ] there); call after the grid barrier that follows block_partials.
+// Warp q sums quantity q over the blocks (lane-strided, then one shuffle tree): one L2 round trip and no second
+// reduction level; needs NQ <= warps per block.
 template <int NQ>
 __device__ __forceinline__ void block_totals(const int (&op)[NQ], const double *in /*[gridDim.x][NQ]*/, double *smem,
                                              double (&t)[NQ]) {
-#pragma unroll
-  for (int q = 0; q < NQ; ++q) t[q] = op[q] == 0 ? 0.0 : (op[q] == 1 ? 1.0e308 : -1.0e308);
-  for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
-#pragma unroll
-    for (int q = 0; q < NQ; ++q) t[q] = red_combine(t[q], __ldcg(&in[(size_t)b * NQ + q]), op[q]);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  for (int q = wid; q < NQ; q += nw) {
+    double a = op[q] == 0 ? 0.0 : (op[q] == 1 ? 1.0e308 : -1.0e308);
+    for (unsigned int b = lane; b < gridDim.x; b += 32) a = red_combine(a, __ldcg(&in[(size_t)b * NQ + q]), op[q]);
+    a = warp_red(a, op[q]);
+    if (lane == 0) smem[q] = a;
   }
-  block_reduce<NQ>(t, op, smem);
+  __syncthreads();
+#pragma unroll
+  for (int q = 0; q < NQ; ++q) t[q] = smem[q];
+  __syncthreads();
 }
 
 // Grid-level deterministic reduction.  Every block calls this once with its per-thread values.

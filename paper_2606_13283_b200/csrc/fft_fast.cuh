@@ -187,7 +187,7 @@ __device__ __forceinline__ void fft_yz_tile(const FastGeom &G, LoadOp &ld, Store
 #pragma unroll
     for (int t = 0; t < R2; ++t) v[t] = buf[(j2 + t * R1) * kFastL + l];
 #pragma unroll
-    for (int t = 1; t < R2; ++t) v[t] = cmul(v[t], __ldg(&G.tw[t * j2]));
+    for (int t = 1; t < R2; ++t) v[t] = cmul(v[t], G.tw[t * j2]);
     Dft<R2>::run(v);
     if constexpr (StoreOp::kSplitStore && R2 <= 8) {
       // an epilogue that reads further operands: every load and reduction first, then the stores (see above)
@@ -230,57 +230,60 @@ template <int N> __host__ __device__ constexpr int fast_threads_x() { return 256
 template <int N> __host__ __device__ constexpr int fast_row_x() { return N + N / FastPlan<N>::R1; }   // padded smem row (elements)
 template <int N> __device__ __forceinline__ int fast_pos(int i) { return i + i / FastPlan<N>::R1; }
 
-// the two stages on the block's LP complex lines held in shared memory (in place)
-template <int N>
-__device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *__restrict__ tw) {
+// the two stages on the tile's LP complex lines held in shared memory (in place); t = thread index within the group
+// of TH threads that owns the tile, bar = the group's barrier id (0 with the whole block)
+template <int N, int TH>
+__device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *tw, int t, int bar) {
   constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, ROW = fast_row_x<N>();
+  static_assert(TH >= kFastLP * R1 && TH >= kFastLP * R2, "one butterfly per thread");
   {
-    const int p = threadIdx.x / R2, j1 = threadIdx.x % R2;
-    const bool act = threadIdx.x < kFastLP * R2;
+    const int p = t / R2, j1 = t % R2;
+    const bool act = t < kFastLP * R2;
     double2 v[R1];
     if (act) {
 #pragma unroll
-      for (int t = 0; t < R1; ++t) v[t] = buf[p * ROW + fast_pos<N>(j1 + t * R2)];
+      for (int q = 0; q < R1; ++q) v[q] = buf[p * ROW + fast_pos<N>(j1 + q * R2)];
       Dft<R1>::run(v);
     }
-    __syncthreads();
+    group_sync(bar, TH);
     if (act) {
 #pragma unroll
-      for (int t = 0; t < R1; ++t) buf[p * ROW + j1 * (R1 + 1) + t] = v[t];   // = fast_pos(j1*R1 + t)
+      for (int q = 0; q < R1; ++q) buf[p * ROW + j1 * (R1 + 1) + q] = v[q];   // = fast_pos(j1*R1 + q)
     }
   }
-  __syncthreads();
-  if (threadIdx.x < kFastLP * R1) {
-    const int p = threadIdx.x / R1, j2 = threadIdx.x % R1;
+  group_sync(bar, TH);
+  if (t < kFastLP * R1) {
+    const int p = t / R1, j2 = t % R1;
     double2 v[R2];
 #pragma unroll
-    for (int t = 0; t < R2; ++t) v[t] = buf[p * ROW + j2 + t * (R1 + 1)];       // = fast_pos(j2 + t*R1)
+    for (int q = 0; q < R2; ++q) v[q] = buf[p * ROW + j2 + q * (R1 + 1)];       // = fast_pos(j2 + q*R1)
 #pragma unroll
-    for (int t = 1; t < R2; ++t) v[t] = cmul(v[t], __ldg(&tw[t * j2]));
+    for (int q = 1; q < R2; ++q) v[q] = cmul(v[q], tw[q * j2]);
     Dft<R2>::run(v);
 #pragma unroll
-    for (int t = 0; t < R2; ++t) buf[p * ROW + j2 + t * (R1 + 1)] = v[t];
+    for (int q = 0; q < R2; ++q) buf[p * ROW + j2 + q * (R1 + 1)] = v[q];
   }
-  __syncthreads();
+  group_sync(bar, TH);
 }
 
 // one x tile (8 pairs of real lines) by the whole block (256 threads); buf = [LP][ROW] shared
 template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), class LoadOp, class StoreOp>
-__device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf) {
+__device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf,
+                                             int tg = threadIdx.x, int bar = 0) {
   constexpr int ROW = fast_row_x<N>(), NXH = N / 2 + 1;
   const long long line0 = (long long)tile * (2 * kFastLP);
   if (PREFETCH)
-    for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
-  for (int e = threadIdx.x; e < kFastLP * N; e += TH) {
+    for (int e = tg * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
+  for (int e = tg; e < kFastLP * N; e += TH) {
     const int p = e / N, i = e % N;
     const long long la = line0 + 2 * p, lb = la + 1;
     double a, b;
     ld.load_real2(la * N + i, lb * N + i, a, b);
     buf[p * ROW + fast_pos<N>(i)] = make_double2(a, b);
   }
-  __syncthreads();
-  fast_stages_x<N>(buf, G.tw);
-  for (int e = threadIdx.x; e < kFastLP * G.P; e += TH) {
+  group_sync(bar, TH);
+  fast_stages_x<N, TH>(buf, G.tw, tg, bar);
+  for (int e = tg; e < kFastLP * G.P; e += TH) {
     const int p = e / G.P, k = e % G.P;
     const long long la = line0 + 2 * p, lb = la + 1;
     double2 A = make_double2(0.0, 0.0), B = A;
@@ -292,18 +295,19 @@ __device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, Stor
     st.store(la * G.P + k, k, (int)(la % G.ny), (int)(la / G.ny), A.x, A.y);
     st.store(lb * G.P + k, k, (int)(lb % G.ny), (int)(lb / G.ny), B.x, B.y);
   }
-  __syncthreads();
+  group_sync(bar, TH);
 }
 
 template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), class LoadOp, class StoreOp>
-__device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf) {
+__device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf,
+                                             int tg = threadIdx.x, int bar = 0) {
   constexpr int ROW = fast_row_x<N>(), NXH = N / 2 + 1;
   const long long line0 = (long long)tile * (2 * kFastLP);
   if (PREFETCH) {
-    for (int e = threadIdx.x * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile
-    for (int e = threadIdx.x * 16; e < 2 * kFastLP * N; e += TH * 16) st.prefetch(line0 * N + e);    // operands of the epilogue
+    for (int e = tg * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile
+    for (int e = tg * 16; e < 2 * kFastLP * N; e += TH * 16) st.prefetch(line0 * N + e);    // operands of the epilogue
   }
-  for (int e = threadIdx.x; e < kFastLP * NXH; e += TH) {
+  for (int e = tg; e < kFastLP * NXH; e += TH) {
     const int p = e / NXH, k = e % NXH;
     const long long la = line0 + 2 * p, lb = la + 1;
     double2 A, B;
@@ -312,15 +316,15 @@ __device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, Stor
     buf[p * ROW + fast_pos<N>(k)] = make_double2(A.x - B.y, -(A.y + B.x));              // conj(A + i B)
     if (k > 0 && 2 * k < N) buf[p * ROW + fast_pos<N>(N - k)] = make_double2(A.x + B.y, A.y - B.x);  // conj(conj A + i conj B)
   }
-  __syncthreads();
-  fast_stages_x<N>(buf, G.tw);
-  for (int e = threadIdx.x; e < kFastLP * N; e += TH) {
+  group_sync(bar, TH);
+  fast_stages_x<N, TH>(buf, G.tw, tg, bar);
+  for (int e = tg; e < kFastLP * N; e += TH) {
     const int p = e / N, i = e % N;
     const long long la = line0 + 2 * p, lb = la + 1;
     const double2 z = buf[p * ROW + fast_pos<N>(i)];
     st.store_real2(la * N + i, lb * N + i, z.x, -z.y);
   }
-  __syncthreads();
+  group_sync(bar, TH);
 }
 
 template <int N, class LoadOp, class StoreOp>

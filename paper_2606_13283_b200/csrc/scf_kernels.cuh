@@ -369,10 +369,10 @@ struct LoadDensity {
     sc->F0 = t[3] * C.dV * C.kT * C.cTF; sc->Ke = t[4] * C.dV * C.kT * C.cTF; sc->Exc = t[5] * C.dV;
     sc->dNdmu = t[6] * C.dV;
   }
-  __device__ __forceinline__ void partial(double *smem, double *out /*[gridDim.x][7]*/) {
+  __device__ __forceinline__ void partial(double *smem, double *out /*[gridDim.x][stride]*/, int stride = 7, int offset = 0) {
     double v[7] = {sK, sdn2, sna2, sF0, sKe, sExc, sChi};
     const int op[7] = {0, 0, 0, 0, 0, 0, 0};
-    block_partials<7>(v, op, smem, out);
+    block_partials<7>(v, op, smem, out, stride, offset);
   }
 };
 
@@ -438,10 +438,10 @@ struct StoreNhatA {
     const int op[3] = {0, 0, 0};
     if (grid_reduce<3>(v, op, partials, counter, smem) && threadIdx.x == 0) apply(smem + 3 * 32, C, sc);
   }
-  __device__ __forceinline__ void partial(double *smem, double *out /*[gridDim.x][3]*/) {
+  __device__ __forceinline__ void partial(double *smem, double *out /*[gridDim.x][stride]*/, int stride = 3, int offset = 0) {
     double v[3] = {aU, aEH, aEie};
     const int op[3] = {0, 0, 0};
-    block_partials<3>(v, op, smem, out);
+    block_partials<3>(v, op, smem, out, stride, offset);
   }
   // grid totals {U, E_H, E_ie sums} -> energies, w (Eq. 30-31), free energy and the stop flag
   static __device__ __forceinline__ void apply(const double *t, const ScfConst &C, DevScalars *sc) {

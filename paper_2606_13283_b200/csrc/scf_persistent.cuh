@@ -45,9 +45,9 @@ template <int NX, int NY, int NZ>
 constexpr size_t persist_smem_bytes() {
   constexpr size_t gy = kPersistThreads / fast_threads_yz<NY>(), gz = kPersistThreads / fast_threads_yz<NZ>();
   constexpr size_t ty = gy * NY * kFastL * sizeof(double2), tz = gz * NZ * kFastL * sizeof(double2);
-  constexpr size_t tx = (size_t)kFastLP * fast_row_x<NX>() * sizeof(double2);
+  constexpr size_t tx = 2 * (size_t)kFastLP * fast_row_x<NX>() * sizeof(double2);   // two x tiles at a time
   constexpr size_t tile = ty > tz ? (ty > tx ? ty : tx) : (tz > tx ? tz : tx);
-  return (kFdTabDoubles + kMaxRed * 33 + 8) * sizeof(double) + tile;
+  return (kFdTabDoubles + 10 * 33 + 8 + 2 * (NX + NY + NZ) + (NX + NY + NZ)) * sizeof(double) + tile;
 }
 
 template <int N, int AXIS, bool INVERSE, class LoadOp, class StoreOp>
@@ -65,8 +65,13 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_pers
   extern __shared__ double smem[];
   double *s_tab = smem;
   double *s_red = s_tab + kFdTabDoubles;
-  double *s_bc = s_red + kMaxRed * 33;
-  double2 *tiles = reinterpret_cast<double2 *>(s_bc + 8);
+  double *s_bc = s_red + 10 * 33;
+  double2 *s_tw0 = reinterpret_cast<double2 *>(s_bc + 8), *s_tw1 = s_tw0 + NX, *s_tw2 = s_tw1 + NY;   // twiddles
+  double *s_kx2 = reinterpret_cast<double *>(s_tw2 + NZ), *s_ky2 = s_kx2 + NX, *s_kz2 = s_ky2 + NY;    // k^2 per axis
+  double2 *tiles = reinterpret_cast<double2 *>(s_kz2 + NZ);
+  for (int i = threadIdx.x; i < NX; i += blockDim.x) { s_tw0[i] = p.tw0[i]; s_kx2[i] = p.kx2[i]; }
+  for (int i = threadIdx.x; i < NY; i += blockDim.x) { s_tw1[i] = p.tw1[i]; s_ky2[i] = p.ky2[i]; }
+  for (int i = threadIdx.x; i < NZ; i += blockDim.x) { s_tw2[i] = p.tw2[i]; s_kz2[i] = p.kz2[i]; }
   // every block keeps its own copy of the scalar block in shared memory: the phase totals are taken by all blocks
   // in the same fixed order after a grid barrier (block_partials / block_totals), so the copies stay identical and no
   // block ever waits for another one's scalar result; block 0 writes the copy back at the end
@@ -75,9 +80,12 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_pers
   fd_load_tables(s_tab, p.fdtab);
   __syncthreads();
   DevScalars *const sc = &s_sc;
-  double *const part_vi = p.partials, *const part_dn = part_vi + (size_t)gridDim.x * 4,
-         *const part_g = part_dn + (size_t)gridDim.x * 7, *const part_mu = part_g + (size_t)gridDim.x * 3;
-  const FastGeom Gx{NX, NY, NZ, p.P, p.tw0, nullptr}, Gy{NX, NY, NZ, p.P, p.tw1, nullptr}, Gz{NX, NY, NZ, p.P, p.tw2, nullptr};
+  double *const part_vi = p.partials, *const part_dg = part_vi + (size_t)gridDim.x * 4,   // density 7 + G-space 3 per block
+         *const part_mu = part_dg + (size_t)gridDim.x * 10;
+  const FastGeom Gx{NX, NY, NZ, p.P, s_tw0, nullptr}, Gy{NX, NY, NZ, p.P, s_tw1, nullptr}, Gz{NX, NY, NZ, p.P, s_tw2, nullptr};
+  constexpr int XTH = kPersistThreads / 2;   // two x tiles per block at a time
+  const int xg = threadIdx.x / XTH, xt = threadIdx.x % XTH;
+  double2 *const xbuf = tiles + (size_t)xg * kFastLP * fast_row_x<NX>();
   const int xtiles = NY * NZ / (2 * kFastLP), ytiles = NZ * (p.P / kFastL), ztiles = NY * (p.P / kFastL);
   int mix = p.mix_first;
   const bool timing = p.phase_ns != nullptr && blockIdx.x == 0 && threadIdx.x == 0;
@@ -95,7 +103,7 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_pers
     // ---- S1 (+ pending S6 in G-space): inverse z pass
     {
       LoadPotentialG lp;
-      lp.nh_i = p.nh_i; lp.nh_a = p.nh_a; lp.vh_ie = p.vh_ie; lp.kx2 = p.kx2; lp.ky2 = p.ky2; lp.kz2 = p.kz2;
+      lp.nh_i = p.nh_i; lp.nh_a = p.nh_a; lp.vh_ie = p.vh_ie; lp.kx2 = s_kx2; lp.ky2 = s_ky2; lp.kz2 = s_kz2;
       lp.sc = sc; lp.nxh = p.nxh; lp.mix = mix;
       StoreComplex sw{p.work};
       lp.begin();
@@ -118,7 +126,9 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_pers
       sv.fdtab = s_tab; sv.inv_vol = p.inv_vol; sv.kT_eta0 = p.C.kT * p.C.eta0; sv.inv_kT = 1.0 / p.C.kT; sv.xc = p.C.xc;
       sv.mix = mix;
       sv.begin();
-      for (int tile = blockIdx.x; tile < xtiles; tile += gridDim.x) fft_c2r_tile<NX, false, kPersistThreads>(Gx, lw, sv, tile, tiles);
+      for (int tile = blockIdx.x + gridDim.x * xg; tile < xtiles; tile += 2 * gridDim.x)
+        fft_c2r_tile<NX, false, XTH>(Gx, lw, sv, tile, xbuf, xt, 1 + xg);
+      __syncthreads();
       sv.partial(s_red, part_vi);
     }
     grid.sync();
@@ -142,8 +152,10 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_pers
       StoreComplex sw{p.work};
       ldn.begin();
       ldn.mu = mu;
-      for (int tile = blockIdx.x; tile < xtiles; tile += gridDim.x) fft_r2c_tile<NX, false, kPersistThreads>(Gx, ldn, sw, tile, tiles);
-      ldn.partial(s_red, part_dn);
+      for (int tile = blockIdx.x + gridDim.x * xg; tile < xtiles; tile += 2 * gridDim.x)
+        fft_r2c_tile<NX, false, XTH>(Gx, ldn, sw, tile, xbuf, xt, 1 + xg);
+      __syncthreads();
+      ldn.partial(s_red, part_dg, 10, 0);
     }
     grid.sync();
     lap(4);
@@ -158,21 +170,20 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_pers
     {
       LoadComplex lw{p.work};
       StoreNhatA sn;
-      sn.nh_a = p.nh_a; sn.nh_i = p.nh_i; sn.vh_ie = p.vh_ie; sn.kx2 = p.kx2; sn.ky2 = p.ky2; sn.kz2 = p.kz2;
+      sn.nh_a = p.nh_a; sn.nh_i = p.nh_i; sn.vh_ie = p.vh_ie; sn.kx2 = s_kx2; sn.ky2 = s_ky2; sn.kz2 = s_kz2;
       sn.sc = sc; sn.partials = nullptr; sn.counter = nullptr; sn.C = p.C; sn.H.nx = NX; sn.H.nxh = p.nxh;
       sn.prestored = 0;
       sn.begin();
       persist_yz_phase<NZ, 2, false>(Gz, lw, sn, tiles, ztiles);
       __syncthreads();
-      sn.partial(s_red, part_g);
+      sn.partial(s_red, part_dg, 10, 7);
     }
     grid.sync();
     {  // totals of the density pass and of the G-space pass -> K, F0, ..., then U, E_H, E_ie, w, F and the stop flag
-      double t7[7], t3[3];
-      const int op7[7] = {0, 0, 0, 0, 0, 0, 0}, op3[3] = {0, 0, 0};
-      block_totals<7>(op7, part_dn, s_red, t7);
-      block_totals<3>(op3, part_g, s_red, t3);
-      if (threadIdx.x == 0) { LoadDensity::apply(t7, p.C, sc); StoreNhatA::apply(t3, p.C, sc); }
+      double t[10];
+      const int op[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+      block_totals<10>(op, part_dg, s_red, t);
+      if (threadIdx.x == 0) { LoadDensity::apply(t, p.C, sc); StoreNhatA::apply(t + 7, p.C, sc); }
       __syncthreads();
     }
     lap(6);
