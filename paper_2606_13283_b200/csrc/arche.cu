@@ -83,7 +83,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
-  int force_slabs, force_rows_per_slab;
+  int force_slabs, force_rows_per_slab, force_ipt;   // ions per thread of the force kernel's register tile
   // device arrays (all inside the caller's workspace)
   double *n_i, *n_a, *V_i, *vps, *va;
   double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
@@ -198,7 +198,8 @@ void derive_sizes(arche_ctx *c) {
   if (sfb > rb) rb = (int)sfb;
   c->red_blocks = rb + 8 + 2 * kEwBlocks;  // + room for the mu kernel's [2][grid][2] + [grid][6] partials
   const long long rows = (long long)ny * nz;
-  const int tiles = (c->nions + FC_THREADS - 1) / FC_THREADS;
+  c->force_ipt = c->nions >= 1024 ? 4 : (c->nions >= 256 ? 2 : 1);
+  const int tiles = (c->nions + FC_THREADS * c->force_ipt - 1) / (FC_THREADS * c->force_ipt);
   int slabs = tiles > 0 ? (148 * 4 + tiles - 1) / tiles : 1;
   if (slabs > rows) slabs = (int)rows;
   if (slabs < 1) slabs = 1;
@@ -595,10 +596,19 @@ int compute_forces(arche_ctx *c) {
   const int ni = c->nions;
   if (ni == 0) { c->have_forces = true; return ARCHE_OK; }
   const GridGeom &G = c->G;
-  dim3 fg((unsigned)((ni + FC_THREADS - 1) / FC_THREADS), (unsigned)c->force_slabs);
+  const int ipt = c->force_ipt, per_block = FC_THREADS * ipt;
+  dim3 fg((unsigned)((ni + per_block - 1) / per_block), (unsigned)c->force_slabs);
+  const size_t fsm = FC_RPT * c->nxh * sizeof(double2) + c->nxh * sizeof(double);
   { ProfScope ps(c, PC_FORCE);
-  force_kernel<<<fg, FC_THREADS, 2 * c->nxh * sizeof(double2), c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij,
-                                                                          c->cz_ij, c->vps, c->va, c->nh_a, c->S, c->S2, c->F_part);
+  if (ipt == 4)
+    force_kernel<4><<<fg, FC_THREADS, fsm, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,
+                                                        c->nh_a, c->S, c->S2, c->F_part);
+  else if (ipt == 2)
+    force_kernel<2><<<fg, FC_THREADS, fsm, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,
+                                                        c->nh_a, c->S, c->S2, c->F_part);
+  else
+    force_kernel<1><<<fg, FC_THREADS, fsm, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,
+                                                        c->nh_a, c->S, c->S2, c->F_part);
   LAUNCHED(c); }
   force_finish_kernel<<<(3 * ni + 127) / 128, 128, 0, c->stream>>>(ni, c->force_slabs, c->F_part, c->F_pp, c->Z,
                                                                    -2.0 * ARCHE_PI / G.vol, c->F);

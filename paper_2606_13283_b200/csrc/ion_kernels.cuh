@@ -242,61 +242,107 @@ __global__ void __launch_bounds__(256) ewald_finish_kernel(const double *__restr
 // mirror of (kx, +N/2, kz) is (-kx, -N/2, -kz), which the literal set replaces by (-kx, +N/2, -kz): such rows are
 // summed as two variants, the literal one and (interior columns only) the one with the Nyquist component flipped
 // (conjugated phase-table entry, S2 instead of S, -N/2 in the k factor).
-// Block = FC_THREADS ions x one slab of (ky,kz) rows; the weighted W rows are staged in shared memory.
+// Block = FC_THREADS*IPT ions x one slab of (ky,kz) rows.  Register tile: every thread owns IPT ions and works on FC_RPT
+// (virtual) rows at a time, so that one a_j(kx) load and one staged W(k) word feed FC_RPT resp. IPT complex products --
+// with one ion and one row per thread the kernel is bound by its shared-memory/L1 reads (measured 0.35 of fp64 peak),
+// not by the FMA pipe.  Per (ion, row, kx): t = W a_j, P += t, Q += kx t (8 fp64 instructions).
 constexpr int FC_THREADS = 128;
+constexpr int FC_RPT = 4;   // (virtual) rows in flight: every a_j(kx) word read from L2 feeds FC_RPT products
+template <int IPT>
 __global__ void __launch_bounds__(FC_THREADS) force_kernel(
     GridGeom G, int nions, int rows_per_slab, const double2 *__restrict__ ax_ij /*[ix][j]*/,
     const double2 *__restrict__ by_ij, const double2 *__restrict__ cz_ij, const double *__restrict__ vps,
     const double *__restrict__ va, const double2 *__restrict__ nh_a, const double2 *__restrict__ S,
     const double2 *__restrict__ S2, double *__restrict__ F_part /*[slab][j][3]*/) {
-  extern __shared__ double2 s_w[];  // [2][nxh]: W and kx*W
-  double2 *s_W = s_w, *s_kW = s_w + G.nxh;
-  const int j = blockIdx.x * FC_THREADS + threadIdx.x;
+  extern __shared__ double2 s_w[];  // [FC_RPT][nxh] weighted W of the rows in flight, then kx[nxh]
+  double *s_kx = reinterpret_cast<double *>(s_w + FC_RPT * G.nxh);
+  const int j0 = blockIdx.x * (FC_THREADS * IPT) + threadIdx.x;
   const long long nrows = (long long)G.ny * G.nz;
   const long long r0 = (long long)blockIdx.y * rows_per_slab;
   const long long r1 = min(nrows, r0 + rows_per_slab);
   const int nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
-  double fx = 0, fy = 0, fz = 0;
-  for (long long row = r0; row < r1; ++row) {
-    const int iy = (int)(row % G.ny), iz = (int)(row / G.ny);
-    const bool ny_row = iy == nyq_y || iz == nyq_z;
-    for (int var = 0; var < (ny_row ? 2 : 1); ++var) {
-      __syncthreads();
+  for (int ix = threadIdx.x; ix < G.nxh; ix += FC_THREADS) s_kx[ix] = G.kx[ix];
+  double fx[IPT], fy[IPT], fz[IPT];
+#pragma unroll
+  for (int q = 0; q < IPT; ++q) fx[q] = fy[q] = fz[q] = 0.0;
+  long long row = r0;
+  int var = 0;
+  while (row < r1) {
+    // take up to FC_RPT virtual rows (row, variant)
+    long long vrow[FC_RPT]; int vvar[FC_RPT]; bool vnyq[FC_RPT], vok[FC_RPT];
+#pragma unroll
+    for (int s = 0; s < FC_RPT; ++s) {
+      vok[s] = row < r1; vrow[s] = vok[s] ? row : r0; vvar[s] = var;
+      const int iy = (int)(vrow[s] % G.ny), iz = (int)(vrow[s] / G.ny);
+      vnyq[s] = iy == nyq_y || iz == nyq_z;
+      if (vok[s]) { if (vnyq[s] && var == 0) var = 1; else { ++row; var = 0; } }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int s = 0; s < FC_RPT; ++s) {
       for (int ix = threadIdx.x; ix < G.nxh; ix += FC_THREADS) {
-        const long long g = row * G.P + ix;
-        const bool edge = ix == 0 || 2 * ix == G.nx;
-        const double wt = edge ? (var == 0 ? 1.0 : 0.0) : (ny_row ? 1.0 : 2.0);
-        const double2 n = nh_a[g], s = var == 0 ? S[g] : S2[g];
-        const double v = vps[g], a = va[g];
-        const double2 w = make_double2(wt * (v * n.x + a * s.x), -wt * (v * n.y + a * s.y));
-        s_W[ix] = w;
-        const double kx = G.kx[ix];
-        s_kW[ix] = make_double2(kx * w.x, kx * w.y);
-      }
-      __syncthreads();
-      if (j < nions) {
-        double2 P = make_double2(0, 0), Q = make_double2(0, 0);
-        for (int ix = 0; ix < G.nxh; ++ix) {
-          const double2 a = ax_ij[(long long)ix * nions + j];
-          const double2 w = s_W[ix], kw = s_kW[ix];
-          P.x = fma(w.x, a.x, fma(-w.y, a.y, P.x)); P.y = fma(w.x, a.y, fma(w.y, a.x, P.y));
-          Q.x = fma(kw.x, a.x, fma(-kw.y, a.y, Q.x)); Q.y = fma(kw.x, a.y, fma(kw.y, a.x, Q.y));
+        double2 w = make_double2(0.0, 0.0);
+        if (vok[s]) {
+          const long long g = vrow[s] * G.P + ix;
+          const bool edge = ix == 0 || 2 * ix == G.nx;
+          const double wt = edge ? (vvar[s] == 0 ? 1.0 : 0.0) : (vnyq[s] ? 1.0 : 2.0);
+          const double2 n = nh_a[g], sf = vvar[s] == 0 ? S[g] : S2[g];
+          const double v = vps[g], a = va[g];
+          w = make_double2(wt * (v * n.x + a * sf.x), -wt * (v * n.y + a * sf.y));
         }
+        s_w[s * G.nxh + ix] = w;
+      }
+    }
+    __syncthreads();
+    double2 P[IPT][FC_RPT], Q[IPT][FC_RPT];
+#pragma unroll
+    for (int q = 0; q < IPT; ++q)
+#pragma unroll
+      for (int s = 0; s < FC_RPT; ++s) { P[q][s] = make_double2(0.0, 0.0); Q[q][s] = make_double2(0.0, 0.0); }
+    for (int ix = 0; ix < G.nxh; ++ix) {
+      double2 w[FC_RPT];
+#pragma unroll
+      for (int s = 0; s < FC_RPT; ++s) w[s] = s_w[s * G.nxh + ix];
+      const double kx = s_kx[ix];
+#pragma unroll
+      for (int q = 0; q < IPT; ++q) {
+        const int j = j0 + q * FC_THREADS;
+        const double2 a = j < nions ? ax_ij[(long long)ix * nions + j] : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int s = 0; s < FC_RPT; ++s) {
+          const double2 t = make_double2(fma(w[s].x, a.x, -w[s].y * a.y), fma(w[s].x, a.y, w[s].y * a.x));
+          P[q][s].x += t.x; P[q][s].y += t.y;
+          Q[q][s].x = fma(kx, t.x, Q[q][s].x); Q[q][s].y = fma(kx, t.y, Q[q][s].y);
+        }
+      }
+    }
+#pragma unroll
+    for (int s = 0; s < FC_RPT; ++s) {
+      if (!vok[s]) continue;
+      const int iy = (int)(vrow[s] % G.ny), iz = (int)(vrow[s] / G.ny);
+#pragma unroll
+      for (int q = 0; q < IPT; ++q) {
+        const int j = j0 + q * FC_THREADS;
+        if (j >= nions) continue;
         double2 b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
         double ky = G.ky[iy], kz = G.kz[iz];
-        if (var == 1) {
+        if (vvar[s] == 1) {
           if (iy == nyq_y) { b.y = -b.y; ky = -ky; }
           if (iz == nyq_z) { c.y = -c.y; kz = -kz; }
         }
         const double2 bc = make_double2(b.x * c.x - b.y * c.y, b.x * c.y + b.y * c.x);
-        const double imP = P.x * bc.y + P.y * bc.x, imQ = Q.x * bc.y + Q.y * bc.x;
-        fx += imQ; fy += ky * imP; fz += kz * imP;
+        const double imP = P[q][s].x * bc.y + P[q][s].y * bc.x, imQ = Q[q][s].x * bc.y + Q[q][s].y * bc.x;
+        fx[q] += imQ; fy[q] += ky * imP; fz[q] += kz * imP;
       }
     }
   }
-  if (j < nions) {
-    double *o = F_part + ((size_t)blockIdx.y * nions + j) * 3;
-    o[0] = fx; o[1] = fy; o[2] = fz;
+#pragma unroll
+  for (int q = 0; q < IPT; ++q) {
+    const int j = j0 + q * FC_THREADS;
+    if (j < nions) {
+      double *o = F_part + ((size_t)blockIdx.y * nions + j) * 3;
+      o[0] = fx[q]; o[1] = fy[q]; o[2] = fz[q];
+    }
   }
 }
 
