@@ -130,6 +130,9 @@ long long arche_launch_count(const arche_ctx *c);
  * plain passes and 4 is unused.  arche_profile_get returns the summed milliseconds and launch count of a class. */
 int arche_profile_enable(arche_ctx *c, int on);
 int arche_is_fused(const arche_ctx *c);
+/* 1 when arche_scf_solve runs the whole SCF loop in one persistent cooperative launch (fused form on 32^3 / 64^3 grids;
+ * the profile classes 0-6 then receive the phase times block 0 measures with %globaltimer) */
+int arche_is_persistent(const arche_ctx *c);
 int arche_profile_get(arche_ctx *c, int cls, double *h_ms_total, long long *h_launches);
 
 #ifdef __cplusplus

@@ -20,7 +20,7 @@ SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_la
            "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_md_step",
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
            "arche_rfft3d_forward", "arche_rfft3d_inverse",
-           "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused"]
+           "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused", "arche_is_persistent"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
 
@@ -83,6 +83,7 @@ def load(rebuild_if_stale: bool = True):
     L.arche_launch_count.argtypes = [vp]; L.arche_launch_count.restype = C.c_longlong
     L.arche_profile_enable.argtypes = [vp, C.c_int]
     L.arche_is_fused.argtypes = [vp]
+    L.arche_is_persistent.argtypes = [vp]
     L.arche_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     _lib = L
     return L
@@ -254,6 +255,9 @@ class Arche:
 
     def is_fused(self) -> bool:
         return bool(self.lib.arche_is_fused(self._h))
+
+    def is_persistent(self) -> bool:
+        return bool(self.lib.arche_is_persistent(self._h))
 
     def profile_enable(self, on: bool = True):
         self._check(self.lib.arche_profile_enable(self._h, int(on)))

@@ -771,6 +771,12 @@ extern "C" int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta,
 
 extern "C" int arche_is_fused(const arche_ctx *c) { return c && c->fuse ? 1 : 0; }
 
+extern "C" int arche_is_persistent(const arche_ctx *c) {
+  if (!c || !c->persist) return 0;
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  return (nx == ny && ny == nz && (nx == 32 || nx == 64)) ? 1 : 0;
+}
+
 extern "C" int arche_profile_enable(arche_ctx *c, int on) {
   if (!c) return ARCHE_EINVAL;
   if (on && !c->prof_ev[0])

@@ -114,6 +114,21 @@ def test_single_scf_iteration(orc, torch_cuda, xc, pointwise_mode):
     assert abs(g.get_real("n_a").sum().item() * dV - cfg["Z"].sum()) < 1e-12 * cfg["Z"].sum()   # neutrality
 
 
+@pytest.mark.parametrize("T_eV", [1.0, 100.0])
+def test_temperature_extremes(orc, torch_cuda, T_eV):
+    """degenerate (T = 1 eV: eta up to several hundred, asymptotic Fermi-Dirac region, vanishing density in the
+    classically forbidden cores) and hot dilute (T = 100 eV: eta << 0) plasmas, three iterations field by field"""
+    cfg = ai.make_small(n_ions=4, L=8.0, grid=(16, 16, 16), T_eV=T_eV, seed=21)
+    g = _gpu(cfg); o = orc.Oracle(cfg)
+    g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
+    for it in range(3):
+        rg = g.scf_iter(); ro = o.scf_iter()
+        assert _rel(g.get_real("V_i").cpu().numpy(), o.get_real("V_i")) < 1e-11
+        assert _rel(g.get_real("n_a").cpu().numpy(), o.get_real("n_a")) < TOL_N
+        for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "K_e", "w_last"):
+            assert abs(rg[k] - ro[k]) <= TOL_F * max(1.0, abs(ro[k])), (T_eV, it, k, rg[k], ro[k])
+
+
 def _solve_pair(orc, cfg, **kw):
     o = orc.Oracle(cfg, **kw)
     ro = o.scf_solve(cfg["pos"])
