@@ -34,18 +34,21 @@ struct ScfConst {
 };
 
 // Perdew-Zunger 1981 LDA (unpolarised), Hartree units; restated from the publication (reading D5).
+// One reciprocal cube root gives r_s and n^(1/3) (no division), one reciprocal serves eps_c and V_c on the r_s >= 1
+// branch; the branch is decided on r_s in fp64 exactly as in the oracle (reading A13).
 __device__ __forceinline__ void xc_pz81(double n, double &eps, double &v) {
   if (!(n > 0.0)) { eps = 0.0; v = 0.0; return; }
   const double cx = 0.73855876638202240588;  // (3/4) (3/pi)^(1/3)
-  const double n13 = cbrt(n);
+  const double r = rcbrt(n);
+  const double n13 = n * r * r;
   const double ex = -cx * n13;
-  const double rs = 0.62035049089940001667 / n13;  // (3/(4 pi))^(1/3) n^(-1/3)
+  const double rs = 0.62035049089940001667 * r;  // (3/(4 pi))^(1/3) n^(-1/3)
   double ec, vc;
   if (rs >= 1.0) {
     const double g = -0.1423, b1 = 1.0529, b2 = 0.3334;
-    const double sq = sqrt(rs), den = 1.0 + b1 * sq + b2 * rs;
-    ec = g / den;
-    vc = ec * (1.0 + (7.0 / 6.0) * b1 * sq + (4.0 / 3.0) * b2 * rs) / den;
+    const double sq = sqrt(rs), inv = __drcp_rn(1.0 + b1 * sq + b2 * rs);
+    ec = g * inv;
+    vc = ec * (1.0 + (7.0 / 6.0) * b1 * sq + (4.0 / 3.0) * b2 * rs) * inv;
   } else {
     const double A = 0.0311, B = -0.048, C = 0.0020, D = -0.0116;
     const double l = log(rs);
@@ -88,7 +91,7 @@ struct LoadPotentialG {
     }
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 == 0.0) { re = 0.0; im = 0.0; return; }
-    const double inv = 1.0 / (ARCHE_PI * k2);
+    const double inv = __drcp_rn(ARCHE_PI * k2);
     const double2 b = vh_ie[idx];
     re = fma(a.x, inv, b.x); im = fma(a.y, inv, b.y);
   }
@@ -104,7 +107,7 @@ struct LoadPotentialG {
     wb = a;
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 == 0.0) return;
-    const double inv = 1.0 / (ARCHE_PI * k2);
+    const double inv = __drcp_rn(ARCHE_PI * k2);
     const double2 b = vh_ie[idx];
     re = fma(a.x, inv, b.x); im = fma(a.y, inv, b.y);
   }
@@ -409,7 +412,7 @@ struct StoreNhatA {
     aEie += wt * (re * b.x + im * b.y);                  // Re conj(nhat_a) Vhat_ie
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 != 0.0) {
-      const double inv = wt / (ARCHE_PI * k2);
+      const double inv = wt * __drcp_rn(ARCHE_PI * k2);
       const double2 a = nh_i[idx];
       const double dr = a.x - re, di = a.y - im;
       aU += (dr * dr + di * di) * inv;                   // Eq. 30
@@ -425,7 +428,7 @@ struct StoreNhatA {
     aEie += wt * (v.x * b.x + v.y * b.y);
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 != 0.0) {
-      const double inv = wt / (ARCHE_PI * k2);
+      const double inv = wt * __drcp_rn(ARCHE_PI * k2);
       const double2 a = nh_i[idx];
       const double dr = a.x - v.x, di = a.y - v.y;
       aU += (dr * dr + di * di) * inv;
