@@ -419,7 +419,11 @@ int scf_iteration(arche_ctx *c) {
   const GridGeom &G = c->G;
   const ScfConst &C = c->C;
   const int mix = c->mix_pending ? 1 : 0;
-  const int pg = c->ew_grid * 2;   // streaming kernels: 16 blocks per SM
+  // streaming kernels: up to 16 blocks per SM, but at least 4 half-spectrum elements / 2 real pairs per thread (every
+  // block takes part in the closing grid reduction, so an over-sized grid only adds to its tail)
+  const int pmax = c->ew_grid * 2;
+  auto fit = [&](long long work) { long long b = (work + 255) / 256; return (int)(b < c->sm_count ? c->sm_count : (b > pmax ? pmax : b)); };
+  const int pg = fit(c->nh / 4), pr = fit(c->ng / 4);
   // S1 + S2 (+ the pending S6 of the previous iteration, + the first mu evaluation)
   LoadPotentialG lp;
   lp.nh_i = c->nh_i; lp.nh_a = c->nh_a; lp.vh_ie = c->vh_ie; lp.kx2 = c->kx2; lp.ky2 = c->ky2; lp.kz2 = c->kz2;
@@ -437,7 +441,7 @@ int scf_iteration(arche_ctx *c) {
     rc = fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{c->V_i}, PC_FFT_INV_Z, PC_FFT_INV_X);
     if (rc) return rc;
     { ProfScope ps(c, PC_VI_R);
-      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop); LAUNCHED(c); }
+      pointwise_r_kernel<<<pr, 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop); LAUNCHED(c); }
   }
   c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
@@ -461,7 +465,7 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_DENS_R);
-      pointwise_r_kernel<<<pg, 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop); LAUNCHED(c); }
+      pointwise_r_kernel<<<pr, 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop); LAUNCHED(c); }
     rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
     if (rc) return rc;
     { ProfScope ps(c, PC_RED_G);
