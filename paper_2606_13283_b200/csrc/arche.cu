@@ -328,6 +328,8 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   fd_pack_tables(tab.data());
   CK(cudaMemcpyAsync(c->fdtab, tab.data(), kFdTabDoubles * sizeof(double), cudaMemcpyHostToDevice, c->stream));
   CK(cudaMemsetAsync(c->counter, 0, 64 * sizeof(unsigned int), c->stream));
+  for (double2 *a : {c->S, c->S2, c->vh_ie, c->gh, c->gh2, c->nh_i, c->nh_a, c->work})   // padding columns stay zero
+    CK(cudaMemsetAsync(a, 0, (size_t)c->nh * sizeof(double2), c->stream));
   CK(cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream));
   CK(cudaMemsetAsync(c->F, 0, 3 * (c->nions > 0 ? c->nions : 1) * sizeof(double), c->stream));
   form_factor_kernel<<<c->ew_grid, 256, 0, c->stream>>>(G, p->psp_rc, c->alpha, c->vps, c->va);
@@ -488,13 +490,26 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 0, G.Lx, G.nx, ni, c->ax_ij, c->ax_ji); LAUNCHED(c);
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 1, G.Ly, G.ny, ni, c->by_ij, nullptr); LAUNCHED(c);
     phase_table_kernel<<<pb, 256, 0, c->stream>>>(c->pos, 2, G.Lz, G.nz, ni, c->cz_ij, nullptr); LAUNCHED(c);
-    dim3 sg((unsigned)(((long long)G.ny * G.nz + SF_ROWS - 1) / SF_ROWS), (unsigned)((c->P + SF_THREADS - 1) / SF_THREADS));
     { ProfScope ps(c, PC_SFAC);
-    structure_factor_kernel<<<sg, SF_THREADS, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S,
-                                                              c->S2, c->vh_ie, c->partials, c->counter, c->sc);
+    // register-tiled kernel when nx/2 splits into IXT columns per thread with whole warps, else the generic one
+    const int nxm = G.nx / 2;
+    const int ixt = (G.nx % 2 == 0 && ni >= 256) ? (nxm % 128 == 0 ? 4 : (nxm % 96 == 0 ? 3 : (nxm % 64 == 0 ? 2 : 0))) : 0;
+    int own_nyq_x = 0;
+    if (ixt) {
+      const unsigned blocks = (unsigned)(((long long)G.ny * G.nz + SF2_ROWS - 1) / SF2_ROWS);
+      const int txb = nxm / ixt;
+      if (ixt == 4) structure_factor_tiled_kernel<4><<<blocks, txb, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc);
+      else if (ixt == 3) structure_factor_tiled_kernel<3><<<blocks, txb, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc);
+      else structure_factor_tiled_kernel<2><<<blocks, txb, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc);
+      own_nyq_x = 1;
+    } else {
+      dim3 sg((unsigned)(((long long)G.ny * G.nz + SF_ROWS - 1) / SF_ROWS), (unsigned)((c->P + SF_THREADS - 1) / SF_THREADS));
+      structure_factor_kernel<<<sg, SF_THREADS, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S,
+                                                                c->S2, c->vh_ie, c->partials, c->counter, c->sc);
+    }
     LAUNCHED(c);
     structure_factor_nyquist_kernel<<<c->ew_grid, 128, 0, c->stream>>>(G, ni, c->Z, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,
-                                                                       c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc);
+                                                                       c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc, own_nyq_x);
     LAUNCHED(c); }
     ewald_pp_kernel<<<ni, 128, 0, c->stream>>>(c->pos, c->Z, ni, G.Lx, G.Ly, G.Lz, c->alpha, c->F_pp, c->e_pp); LAUNCHED(c);
     ewald_finish_kernel<<<1, 256, 0, c->stream>>>(c->e_pp, c->Z, ni, c->alpha, G.vol, c->sc); LAUNCHED(c);

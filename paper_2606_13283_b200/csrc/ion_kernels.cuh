@@ -131,6 +131,82 @@ __global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
   }
 }
 
+// Register-tiled form for the production grids (nx even, nx/2 a multiple of 32*IXT): every thread owns IXT kx columns x
+// 8 (ky,kz) rows, so that one a_j(kx) word feeds 8 products and one staged d_j word IXT products -- the kernel above
+// (1 column x 4 rows per thread) is bound by its broadcast shared-memory reads at 0.46 of the fp64 peak.  Covers
+// kx < nx/2; the column kx = nx/2 is left to structure_factor_nyquist_kernel (all of it lies on a Nyquist plane),
+// the padding columns stay zero from arche_scf_init.
+constexpr int SF2_ROWS = 8;
+constexpr int SF2_JT = 64;
+template <int IXT>
+__global__ void __launch_bounds__(256) structure_factor_tiled_kernel(
+    GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ji /*[j][ix]*/,
+    const double2 *__restrict__ by_ij /*[iy][j]*/, const double2 *__restrict__ cz_ij /*[iz][j]*/,
+    const double *__restrict__ vps, const double *__restrict__ va, double2 *__restrict__ S, double2 *__restrict__ S2,
+    double2 *__restrict__ vh_ie, double *partials, unsigned int *counter, DevScalars *sc) {
+  __shared__ double2 s_d[SF2_ROWS][SF2_JT];
+  __shared__ double s_red[32 + 1 + 1];
+  const long long nrows = (long long)G.ny * G.nz;
+  const long long row0 = (long long)blockIdx.x * SF2_ROWS;
+  const int txb = blockDim.x;   // = (nx/2)/IXT
+  double2 acc[IXT][SF2_ROWS];
+#pragma unroll
+  for (int q = 0; q < IXT; ++q)
+#pragma unroll
+    for (int r = 0; r < SF2_ROWS; ++r) acc[q][r] = make_double2(0.0, 0.0);
+  for (int j0 = 0; j0 < nions; j0 += SF2_JT) {
+    __syncthreads();
+    for (int e = threadIdx.x; e < SF2_ROWS * SF2_JT; e += txb) {
+      const int r = e / SF2_JT, jj = e % SF2_JT, j = j0 + jj;
+      const long long row = row0 + r;
+      double2 d = make_double2(0.0, 0.0);
+      if (j < nions && row < nrows) {
+        const int iy = (int)(row % G.ny), iz = (int)(row / G.ny);
+        const double2 b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
+        const double z = Z[j];
+        d = make_double2(z * (b.x * c.x - b.y * c.y), z * (b.x * c.y + b.y * c.x));
+      }
+      s_d[r][jj] = d;
+    }
+    __syncthreads();
+    const int jn = min(SF2_JT, nions - j0);
+    for (int jj = 0; jj < jn; ++jj) {
+      double2 a[IXT];
+#pragma unroll
+      for (int q = 0; q < IXT; ++q) a[q] = ax_ji[(long long)(j0 + jj) * G.nx + threadIdx.x + q * txb];
+#pragma unroll
+      for (int r = 0; r < SF2_ROWS; ++r) {
+        const double2 d = s_d[r][jj];
+#pragma unroll
+        for (int q = 0; q < IXT; ++q) {
+          acc[q][r].x = fma(a[q].x, d.x, fma(-a[q].y, d.y, acc[q][r].x));
+          acc[q][r].y = fma(a[q].x, d.y, fma(a[q].y, d.x, acc[q][r].y));
+        }
+      }
+    }
+  }
+  double epm = 0.0;
+#pragma unroll
+  for (int q = 0; q < IXT; ++q) {
+    const int ix = threadIdx.x + q * txb;
+    const double wt = ix == 0 ? 1.0 : 2.0;
+#pragma unroll
+    for (int r = 0; r < SF2_ROWS; ++r) {
+      const long long row = row0 + r;
+      if (row < nrows) {
+        const long long g = row * G.P + ix;
+        S[g] = acc[q][r]; S2[g] = acc[q][r];
+        const double v = vps[g];
+        vh_ie[g] = make_double2(v * acc[q][r].x, v * acc[q][r].y);
+        epm += wt * va[g] * (acc[q][r].x * acc[q][r].x + acc[q][r].y * acc[q][r].y);
+      }
+    }
+  }
+  double v[1] = {epm};
+  const int op[1] = {0};
+  if (grid_reduce<1>(v, op, partials, counter, s_red) && threadIdx.x == 0) sc->U_pm_sum = s_red[32];
+}
+
 // Nyquist planes (reading A6).  With the literal index set of P:142 a Nyquist component is +N/2, whose mirror -N/2 is
 // not on the grid, so S_Z is not Hermitian there.  For every stored point with a Nyquist component this kernel forms
 // S2 = S_Z(k''), k'' = k with every Nyquist component flipped to -N/2 (phase-table entries conjugated), and
@@ -142,8 +218,8 @@ __global__ void __launch_bounds__(SF_THREADS) structure_factor_kernel(
 __global__ void __launch_bounds__(128) structure_factor_nyquist_kernel(
     GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ij /*[ix][j]*/,
     const double2 *__restrict__ by_ij, const double2 *__restrict__ cz_ij, const double *__restrict__ vps,
-    const double *__restrict__ va, const double2 *__restrict__ S, double2 *__restrict__ S2, double2 *__restrict__ vh_ie,
-    double *partials, unsigned int *counter, DevScalars *sc) {
+    const double *__restrict__ va, double2 *S, double2 *__restrict__ S2, double2 *__restrict__ vh_ie,
+    double *partials, unsigned int *counter, DevScalars *sc, int own_nyq_x /* 1: the main kernel left kx = nx/2 to this one */) {
   __shared__ double s_red[32 + 1 + 1];
   const int nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
   const int nyq_x = (G.nx % 2 == 0) ? G.nx / 2 : -1;
@@ -166,19 +242,26 @@ __global__ void __launch_bounds__(128) structure_factor_nyquist_kernel(
       if (iy == nyq_y || iz == nyq_z) continue;   // already in list A
     }
     const bool fy = iy == nyq_y, fz = iz == nyq_z, fx = ix == nyq_x;
-    double sr = 0.0, si = 0.0;
+    const bool lit = own_nyq_x && fx;   // the literal S_Z of this point is computed here too
+    double sr = 0.0, si = 0.0, lr = 0.0, li = 0.0;
     for (int j = lane; j < nions; j += 32) {
       double2 a = ax_ij[(long long)ix * nions + j], b = by_ij[(long long)iy * nions + j], c = cz_ij[(long long)iz * nions + j];
+      const double z = Z[j];
+      if (lit) {
+        const double bcx = b.x * c.x - b.y * c.y, bcy = b.x * c.y + b.y * c.x;
+        lr += z * (a.x * bcx - a.y * bcy); li += z * (a.x * bcy + a.y * bcx);
+      }
       if (fx) a.y = -a.y;
       if (fy) b.y = -b.y;
       if (fz) c.y = -c.y;
-      const double z = Z[j];
       const double bcx = b.x * c.x - b.y * c.y, bcy = b.x * c.y + b.y * c.x;
       sr += z * (a.x * bcx - a.y * bcy); si += z * (a.x * bcy + a.y * bcx);
     }
     sr = warp_sum(sr); si = warp_sum(si);
+    if (lit) { lr = warp_sum(lr); li = warp_sum(li); }
     if (lane == 0) {
       const long long g = ((long long)iz * G.ny + iy) * G.P + ix;
+      if (lit) { S[g] = make_double2(lr, li); corr += va[g] * (lr * lr + li * li); }   // column weight 1 in Eq. 42
       const double2 s = S[g];
       S2[g] = make_double2(sr, si);
       const double v = vps[g];

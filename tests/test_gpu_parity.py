@@ -86,6 +86,21 @@ def test_structure_factor_and_ionic_potential(orc, torch_cuda):
         assert _rel(g.get_complex(name).cpu().numpy(), o.get_complex(name)) < 1e-12
 
 
+@pytest.mark.parametrize("grid", [(128, 16, 8), (192, 8, 8), (256, 8, 12), (384, 12, 8)])
+def test_structure_factor_register_tiled(orc, torch_cuda, grid):
+    """the register-tiled structure-factor kernel (2, 3 or 4 kx columns x 8 rows per thread, column kx = nx/2 left to
+    the Nyquist-plane kernel) on long-x cells with 256 ions: S_Z, V_ie and the Ewald energy against the oracle"""
+    cfg = ai.make_small(n_ions=256, grid=grid, cell=[40.0, 8.0, 8.0], seed=31, dmin=0.8)
+    cfg["Z"] = np.full(256, 0.25)                      # weak ions: a dense cell the oracle's quadrature handles quickly
+    g = _gpu(cfg); o = orc.Oracle(cfg)
+    g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
+    for name in ("S_Z", "Vhat_ie"):
+        assert _rel(g.get_complex(name).cpu().numpy(), o.get_complex(name)) < 1e-11
+    rg = g.scf_iter(); ro = o.scf_iter()
+    assert abs(rg["U_ii"] - ro["U_ii"]) < 1e-10 * abs(ro["U_ii"])
+    assert abs(rg["E_ie"] - ro["E_ie"]) < 1e-10 * abs(ro["E_ie"])
+
+
 @pytest.fixture(params=["fused", "streamed"])
 def pointwise_mode(request, monkeypatch):
     """both forms of the pointwise work: fused into the FFT passes (default on L2-resident grids) and streaming
