@@ -377,7 +377,8 @@ def main():
             "scf_iterations_per_s": world * iters / t_dev_max, "scf_iters_per_step": iters / args.steps,
             "clocks": cs.summary(),
             "e2e": {"value": world * args.steps / t_e2e_max, "unit": "md_steps/s",
-                    "h2d_bytes_per_step": 2 * 3 * g.n_ions * 8, "d2h_bytes_per_step": 3 * 3 * g.n_ions * 8 + 136},
+                    "h2d_bytes_per_step": 2 * 3 * g.n_ions * 8, "d2h_bytes_per_step": 3 * 3 * g.n_ions * 8 + 136,
+                    "scf_iters_per_step": iters_e2e / args.steps},
             "gpu_launches": int(launches),
             "mu_evals_per_iter": evals_per_iter, "roofline": roof, "kernels": kernels}
     if not args.no_cpu_baseline:

@@ -44,13 +44,14 @@ struct Carver {  // carves 256-byte aligned arrays out of the caller's workspace
 };
 
 // host evaluation of the same fits (only for eta0 = I_{1/2}^{-1}(Ne/(|Omega| cTF)), once per init)
-double fd_half_host(double eta) {
-  int seg; double t, p0, p1, p2;
-  fd_locate(eta, seg, t, p0, p1, p2);
-  double a = FD_COEF[1][seg][FD_NC - 1];
-  for (int i = FD_NC - 2; i >= 0; --i) a = fma(a, t, FD_COEF[1][seg][i]);
-  return a * p1;
+double fd_host(int f, double eta) {  // f = 0, 1, 2: I_{-1/2}, I_{1/2}, I_{3/2}
+  int seg; double t, p[3];
+  fd_locate(eta, seg, t, p[0], p[1], p[2]);
+  double a = FD_COEF[f][seg][FD_NC - 1];
+  for (int i = FD_NC - 2; i >= 0; --i) a = fma(a, t, FD_COEF[f][seg][i]);
+  return a * p[f];
 }
+double fd_half_host(double eta) { return fd_host(1, eta); }
 double fd_half_inverse_host(double y) {
   double lo = log(y / 0.88622692545275801365), hi = pow(1.5 * y, 2.0 / 3.0) + 2.0;
   if (hi < lo + 2.0) hi = lo + 2.0;
@@ -281,6 +282,16 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   C.E_ie0 = C.Ne / G.vol * asum;
   C.xc = p->xc; C.mix_mode = p->mix_mode; C.mix_warmup = p->mix_warmup; C.mix_w_fixed = p->mix_w_fixed;
   C.tol_F = p->scf_tol_F; C.tol_dn = p->scf_tol_dn;
+  C.q_F = 0.0; C.q_dn = 0.0;
+  if (p->xc == 1) {  // reading A13: quanta of a PZ81 branch flip at n* = 3/(4 pi)
+    const double nstar = 0.75 / ARCHE_PI, den = 1.0 + 1.0529 + 0.3334, ec_hi = -0.1423 / den, ec_lo = -0.048 - 0.0116;
+    const double vc_hi = ec_hi * (1.0 + (7.0 / 6.0) * 1.0529 + (4.0 / 3.0) * 0.3334) / den;
+    const double vc_lo = -0.048 - 0.0311 / 3.0 + (2.0 * -0.0116 - 0.0020) / 3.0;
+    const double eta_star = fd_half_inverse_host(nstar / C.cTF);
+    const double chi_star = C.cTF * 0.5 * fd_host(0, eta_star) / p->kT;
+    C.q_F = fabs(ec_hi - ec_lo) * nstar * G.dV;
+    C.q_dn = chi_star * fabs(vc_hi - vc_lo) * sqrt(G.dV);
+  }
   {  // Ewald alpha (reading A18)
     double rc = 0.5 * fmin(G.Lx, fmin(G.Ly, G.Lz));
     double kc = fmin(nx / (2.0 * G.Lx), fmin(ny / (2.0 * G.Ly), nz / (2.0 * G.Lz)));
@@ -534,7 +545,7 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     LAUNCHED(c);
   }
   // reset per-solve scalars (iter, F_total, converged); mu and U_ii persist
-  CK(cudaMemsetAsync(&c->sc->iter, 0, sizeof(int) * 2, c->stream));
+  CK(cudaMemsetAsync(&c->sc->iter, 0, sizeof(int) * 4, c->stream));   // iter, converged, mu_evals_total, flip_seen
   CK(cudaMemsetAsync(&c->sc->F_total, 0, sizeof(double), c->stream));
   CK(cudaMemsetAsync(&c->sc->mu_evals_total, 0, sizeof(int), c->stream));
   c->have_solution = false;

@@ -22,7 +22,7 @@ struct DevScalars {
   double U, EH, Eie;
   // S6/S7
   double w, F_total, F_prev, dn_rel;
-  int iter, converged, mu_evals_total, pad1;
+  int iter, converged, mu_evals_total, flip_seen;   // flip_seen: reading A13, a PZ81 branch flip was detected in this solve
   // per-MD-step
   double U_pp, U_pm_sum, U_pm_fix, U_ii, init_sum, init_scale, K_i;
 };
@@ -31,6 +31,7 @@ struct ScfConst {
   double kT, cTF, Ne, vol, dV, eta0, E_ie0;
   int xc, mix_mode, mix_warmup, pad;
   double mix_w_fixed, tol_F, tol_dn;
+  double q_F, q_dn;   // reading A13: free-energy quantum of one PZ81 branch flip; chi(n*) x V_c jump x sqrt(dV)
 };
 
 // Perdew-Zunger 1981 LDA (unpolarised), Hartree units; restated from the publication (reading D5).
@@ -458,11 +459,20 @@ struct StoreNhatA {
       else w = C.mix_w_fixed;
       const double F = sc->F0 + sc->Exc + EH + Eie + C.E_ie0 + sc->U_ii;
       const double dn_rel = sqrt(sc->dn2 / sc->na2);
-      // reading A13: PZ81's two branches differ by 3.2e-5 Ha in eps_c at r_s = 1 (n* = 3/(4 pi)); a grid point whose
-      // converged density sits on n* flips branch from one iteration to the next and moves F by one such quantum
-      // (eps_c jump x n* x dV) although the density has converged; two quanta are tolerated in the F criterion
-      const double q_branch = C.xc == 1 ? fabs(-0.1423 / (1.0 + 1.0529 + 0.3334) - (-0.048 - 0.0116)) * 0.238732414637843 * C.dV : 0.0;
-      sc->converged = (it >= 2 && fabs(F - sc->F_total) < C.tol_F + 2.0 * q_branch && dn_rel < C.tol_dn) ? 1 : 0;
+      // reading A13: PZ81's two branches differ by 3.2e-5 Ha (eps_c) / 2.7e-5 Ha (V_c) at r_s = 1, n* = 3/(4 pi).  A grid
+      // point whose converged density sits on n* flips branch between iterations: F then moves by whole quanta
+      // q_F = (eps_c jump) n* dV and the density answers the V_c jump with a limit cycle of relative size
+      // q_dn/||n_a|| -- neither criterion can be met below that.  A jump of F by an integer number (1..8) of quanta
+      // right after a change far below one quantum marks the solve; from then on two quanta are tolerated in both criteria.
+      const double dF = fabs(F - sc->F_total);
+      if (C.xc == 1 && it >= 3 && C.q_F > 0.0) {   // a jump: the previous change of F was far below one quantum
+        const double m = dF / C.q_F, r = rint(m), mp = fabs(sc->F_total - sc->F_prev) / C.q_F, rp = rint(mp);
+        const bool near = r >= 1.0 && r <= 8.0 && fabs(m - r) < 0.02, near_prev = rp >= 1.0 && rp <= 8.0 && fabs(mp - rp) < 0.02;
+        if (near && (mp < 0.1 || near_prev)) sc->flip_seen = 1;   // after a quiet change, or twice in a row
+      }
+      const double tolF = C.tol_F + (sc->flip_seen ? 2.02 * C.q_F : 0.0);
+      const double toldn = C.tol_dn + (sc->flip_seen ? 2.0 * C.q_dn / sqrt(sc->na2) : 0.0);
+      sc->converged = (it >= 2 && dF < tolF && dn_rel < toldn) ? 1 : 0;
       sc->F_prev = sc->F_total; sc->F_total = F; sc->w = w; sc->dn_rel = dn_rel; sc->iter = it;
       sc->mu_have_prev = 1;
     }
