@@ -369,7 +369,12 @@ template <bool INVERSE, class LoadOp, class StoreOp>
 cudaError_t pass_x(arche_ctx *c, LoadOp ld, StoreOp st) {
   const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
   FastGeom fg{nx, ny, nz, P, c->tw[0], c->stop};
-  cudaError_t e = c->use_fast ? fft_launch_x_fast<INVERSE>(nx, fg, ld, st, c->stream) : cudaErrorNotSupported;
+  // plain passes of the streamed form run the light configuration (LoadReal / StoreRealPlain / LoadComplex / StoreComplex)
+  constexpr bool plain = (std::is_same<LoadOp, LoadReal>::value || std::is_same<LoadOp, LoadComplex>::value) &&
+                         (std::is_same<StoreOp, StoreComplex>::value || std::is_same<StoreOp, StoreRealPlain>::value);
+  cudaError_t e = cudaErrorNotSupported;
+  if (c->use_fast) e = (plain && nx >= 128) ? fft_launch_x_fast<INVERSE, plain>(nx, fg, ld, st, c->stream)
+                                            : fft_launch_x_fast<INVERSE, false>(nx, fg, ld, st, c->stream);
   if (e == cudaErrorNotSupported) { c->plan[0].stop = c->stop; e = fft_launch_real_x<INVERSE>(c->plan[0], nx, ny, nz, P, ld, st, c->stream); }
   return e;
 }

@@ -10,7 +10,6 @@
 namespace arche {
 
 constexpr int kMaxRed = 8;        // max simultaneous sums per reduction
-constexpr int kRedBlocksMax = 2048;
 
 struct GridGeom {
   int nx, ny, nz;

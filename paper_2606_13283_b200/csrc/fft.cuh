@@ -1,4 +1,7 @@
-// fft.cuh -- hand-written fp64 complex 3D FFT for sm_100a (no cuFFT anywhere on the product path).
+// fft.cuh -- hand-written fp64 3D FFT for sm_100a (no cuFFT anywhere on the product path): the GENERIC passes for any
+// 2^a 3^b length (shared-memory Stockham stages, run-time radix plan) and the functor protocol.  The production
+// sizes 32..384 take the register two-stage passes of fft_fast.cuh; these kernels serve every other length, the
+// stand-alone complex transform arche_fft3d, and the r2c / c2r x passes of odd-sized grids.
 //
 // One kernel launch per axis.  A block owns a tile of L lines of length N of that axis:
 //   axis x: L consecutive x-lines (each line contiguous in memory);

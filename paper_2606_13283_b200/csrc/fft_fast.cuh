@@ -116,7 +116,6 @@ template <> struct FastPlan<128> { static constexpr bool ok = true; static const
 template <> struct FastPlan<192> { static constexpr bool ok = true; static constexpr int R1 = 12, R2 = 16; };
 template <> struct FastPlan<256> { static constexpr bool ok = true; static constexpr int R1 = 16, R2 = 16; };
 template <> struct FastPlan<384> { static constexpr bool ok = true; static constexpr int R1 = 16, R2 = 24; };
-static inline bool fft_fast_size(int n) { return n == 32 || n == 64 || n == 128 || n == 192 || n == 256 || n == 384; }
 
 struct FastGeom {
   int nx, ny, nz, P;        // real grid and half-spectrum pitch
@@ -227,6 +226,11 @@ constexpr int kFastLP = 8;  // line pairs per block
 // 256 threads: the FFT stages need only LP*max(R1,R2) <= 192 of them, the pointwise prologue/epilogue (Fermi-Dirac
 // integrals, XC) uses all
 template <int N> __host__ __device__ constexpr int fast_threads_x() { return 256; }
+// plain x passes (no pointwise functor work): just the butterfly threads, and more resident blocks per SM instead
+template <int N> __host__ __device__ constexpr int fast_threads_x_light() {
+  return kFastLP * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
+}
+template <int N> __host__ __device__ constexpr int fast_blocks_x_light() { return N >= 384 ? 3 : 4; }
 template <int N> __host__ __device__ constexpr int fast_row_x() { return N + N / FastPlan<N>::R1; }   // padded smem row (elements)
 template <int N> __device__ __forceinline__ int fast_pos(int i) { return i + i / FastPlan<N>::R1; }
 
@@ -327,26 +331,30 @@ __device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, Stor
   group_sync(bar, TH);
 }
 
-template <int N, class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(fast_threads_x<N>()) fft_r2c_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+template <int N, bool LIGHT, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>(), LIGHT ? fast_blocks_x_light<N>() : 1)
+    fft_r2c_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
   extern __shared__ double smem_raw[];
   LoadOp ld = ld_in;
   StoreOp st = st_in;
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
-  fft_r2c_tile<N, true>(G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw));
+  fft_r2c_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>()>(G, ld, st, blockIdx.x,
+                                                                               reinterpret_cast<double2 *>(smem_raw));
   ld.finish(smem_raw);
   st.finish(smem_raw);
 }
 
-template <int N, class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(fast_threads_x<N>()) fft_c2r_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+template <int N, bool LIGHT, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>(), LIGHT ? fast_blocks_x_light<N>() : 1)
+    fft_c2r_fast_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
   extern __shared__ double smem_raw[];
   LoadOp ld = ld_in;
   StoreOp st = st_in;
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
-  fft_c2r_tile<N, true>(G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw));
+  fft_c2r_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>()>(G, ld, st, blockIdx.x,
+                                                                               reinterpret_cast<double2 *>(smem_raw));
   ld.finish(smem_raw);
   st.finish(smem_raw);
 }
@@ -381,41 +389,43 @@ static inline cudaError_t fft_launch_yz_fast(int n, const FastGeom &G, LoadOp ld
   }
 }
 
-template <int N, bool INVERSE, class LoadOp, class StoreOp>
+template <int N, bool INVERSE, bool LIGHT, class LoadOp, class StoreOp>
 static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
   size_t smem = sizeof(double2) * kFastLP * fast_row_x<N>();
   if (smem < 4096) smem = 4096;
   const unsigned blocks = (unsigned)((long long)G.ny * G.nz / (2 * kFastLP));
+  constexpr int TH = LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>();
   static bool attr_set = false;
   if constexpr (INVERSE) {
-    auto kern = fft_c2r_fast_kernel<N, LoadOp, StoreOp>;
+    auto kern = fft_c2r_fast_kernel<N, LIGHT, LoadOp, StoreOp>;
     if (!attr_set) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
       if (e != cudaSuccess) return e;
       attr_set = true;
     }
-    kern<<<blocks, fast_threads_x<N>(), smem, stream>>>(G, ld, st);
+    kern<<<blocks, TH, smem, stream>>>(G, ld, st);
   } else {
-    auto kern = fft_r2c_fast_kernel<N, LoadOp, StoreOp>;
+    auto kern = fft_r2c_fast_kernel<N, LIGHT, LoadOp, StoreOp>;
     if (!attr_set) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
       if (e != cudaSuccess) return e;
       attr_set = true;
     }
-    kern<<<blocks, fast_threads_x<N>(), smem, stream>>>(G, ld, st);
+    kern<<<blocks, TH, smem, stream>>>(G, ld, st);
   }
   return cudaGetLastError();
 }
-template <bool INVERSE, class LoadOp, class StoreOp>
+// LIGHT: the functors do no arithmetic worth extra threads (plain loads/stores): butterfly threads only, 3-4 blocks per SM
+template <bool INVERSE, bool LIGHT, class LoadOp, class StoreOp>
 static inline cudaError_t fft_launch_x_fast(int n, const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
   if (((long long)G.ny * G.nz) % (2 * kFastLP) != 0) return cudaErrorNotSupported;
   switch (n) {
-    case 32: return fft_launch_x_fast_n<32, INVERSE>(G, ld, st, stream);
-    case 64: return fft_launch_x_fast_n<64, INVERSE>(G, ld, st, stream);
-    case 128: return fft_launch_x_fast_n<128, INVERSE>(G, ld, st, stream);
-    case 192: return fft_launch_x_fast_n<192, INVERSE>(G, ld, st, stream);
-    case 256: return fft_launch_x_fast_n<256, INVERSE>(G, ld, st, stream);
-    case 384: return fft_launch_x_fast_n<384, INVERSE>(G, ld, st, stream);
+    case 32: return fft_launch_x_fast_n<32, INVERSE, LIGHT>(G, ld, st, stream);
+    case 64: return fft_launch_x_fast_n<64, INVERSE, LIGHT>(G, ld, st, stream);
+    case 128: return fft_launch_x_fast_n<128, INVERSE, LIGHT>(G, ld, st, stream);
+    case 192: return fft_launch_x_fast_n<192, INVERSE, LIGHT>(G, ld, st, stream);
+    case 256: return fft_launch_x_fast_n<256, INVERSE, LIGHT>(G, ld, st, stream);
+    case 384: return fft_launch_x_fast_n<384, INVERSE, LIGHT>(G, ld, st, stream);
     default: return cudaErrorNotSupported;
   }
 }

@@ -1,6 +1,8 @@
-// scf_kernels.cuh -- SCF-iteration kernels and the functors fused into the FFT passes.
-// Steps S1..S7 of DESIGN.md: potential assembly in G-space, real-part + V_xc epilogue,
-// device-side Newton-in-bracket for mu (Eq. 19), density + local reductions, G-space reductions, mixing.
+// scf_kernels.cuh -- SCF-iteration kernels and the pointwise functors of steps S1..S7:
+// potential assembly in G-space, V_i epilogue with XC, device-side secant/Newton-in-bracket for mu (Eq. 19), density
+// and local reductions, G-space reductions, mixing.  The functors run in three hosts: fused into the FFT passes
+// (fft_fast.cuh, fft.cuh), in the streaming kernels below (large grids), and in the persistent kernel
+// (scf_persistent.cuh).
 #pragma once
 #include "common.cuh"
 #include "fd.cuh"
