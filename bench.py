@@ -123,13 +123,13 @@ class ClockSampler:
                 "reasons": sorted(self.reasons)}
 
 
-def oracle_sample(cfg, workload, iters=2, iters_per_step=None):
+def oracle_sample(cfg, workload, iters=2, iters_per_step=None, target_s=15.0):
     """bounded oracle sample: `iters` SCF iterations of the workload from the uniform density + the ion-grid work"""
     import oracle
     o = oracle.Oracle(cfg, **TOL)
     t0 = time.perf_counter(); o.scf_begin(cfg["pos"]); t_ion = time.perf_counter() - t0
     t0 = time.perf_counter(); o.scf_iter(); t_first = time.perf_counter() - t0
-    iters = max(iters, min(40, int(15.0 / max(t_first, 1e-3))))     # about 15 s of CPU work in total
+    iters = max(iters, min(40, int(target_s / max(t_first, 1e-3))))     # about target_s seconds of CPU work in total
     t0 = time.perf_counter()
     for _ in range(iters):
         o.scf_iter()
@@ -149,7 +149,7 @@ def run_reference(args, cfg):
         return
     vals = []
     for _ in range(args.warmup + args.steps):
-        cb = oracle_sample(cfg, args.workload, iters=1)
+        cb = oracle_sample(cfg, args.workload, iters=1, target_s=3.0)   # one bounded sample per "step"
         vals.append(cb)
     use = vals[args.warmup:] or vals
     v = float(np.mean([x["value"] for x in use]))
