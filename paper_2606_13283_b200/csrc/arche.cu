@@ -645,7 +645,7 @@ int compute_forces(arche_ctx *c) {
     force_kernel<1><<<fg, FC_THREADS, fsm, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,
                                                         c->nh_a, c->S, c->S2, c->F_part);
   LAUNCHED(c); }
-  force_finish_kernel<<<(3 * ni + 127) / 128, 128, 0, c->stream>>>(ni, c->force_slabs, c->F_part, c->F_pp, c->Z,
+  force_finish_kernel<<<(3 * ni * 32 + 127) / 128, 128, 0, c->stream>>>(ni, c->force_slabs, c->F_part, c->F_pp, c->Z,
                                                                    -2.0 * ARCHE_PI / G.vol, c->F);
   LAUNCHED(c);
   c->have_forces = true;

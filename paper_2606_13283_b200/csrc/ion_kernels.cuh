@@ -429,13 +429,15 @@ __global__ void __launch_bounds__(FC_THREADS) force_kernel(
   }
 }
 
+// one warp per force component: the lanes stride over the slabs, fixed-order shuffle tree (deterministic)
 __global__ void force_finish_kernel(int nions, int nslabs, const double *__restrict__ F_part, const double *__restrict__ F_pp,
                                     const double *__restrict__ Z, double pref /* -2 pi/|Omega| */, double *__restrict__ F) {
-  const int e = blockIdx.x * blockDim.x + threadIdx.x;
+  const int e = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (e >= 3 * nions) return;
   double a = 0.0;
-  for (int s = 0; s < nslabs; ++s) a += F_part[(size_t)s * nions * 3 + e];
-  F[e] = pref * Z[e / 3] * a + F_pp[e];
+  for (int s = lane; s < nslabs; s += 32) a += F_part[(size_t)s * nions * 3 + e];
+  a = warp_sum(a);
+  if (lane == 0) F[e] = pref * Z[e / 3] * a + F_pp[e];
 }
 
 // velocity Verlet pieces (reading D2)
