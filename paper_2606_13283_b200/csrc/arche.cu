@@ -282,7 +282,7 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   C.E_ie0 = C.Ne / G.vol * asum;
   C.xc = p->xc; C.mix_mode = p->mix_mode; C.mix_warmup = p->mix_warmup; C.mix_w_fixed = p->mix_w_fixed;
   C.tol_F = p->scf_tol_F; C.tol_dn = p->scf_tol_dn;
-  C.q_F = 0.0; C.q_dn = 0.0;
+  C.q_F = 0.0; C.q_dn = 0.0; C.inv_qF = 0.0; C.inv_vol = 1.0 / G.vol;
   if (p->xc == 1) {  // reading A13: quanta of a PZ81 branch flip at n* = 3/(4 pi)
     const double nstar = 0.75 / ARCHE_PI, den = 1.0 + 1.0529 + 0.3334, ec_hi = -0.1423 / den, ec_lo = -0.048 - 0.0116;
     const double vc_hi = ec_hi * (1.0 + (7.0 / 6.0) * 1.0529 + (4.0 / 3.0) * 0.3334) / den;
@@ -291,6 +291,7 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     const double chi_star = C.cTF * 0.5 * fd_host(0, eta_star) / p->kT;
     C.q_F = fabs(ec_hi - ec_lo) * nstar * G.dV;
     C.q_dn = chi_star * fabs(vc_hi - vc_lo) * sqrt(G.dV);
+    C.inv_qF = 1.0 / C.q_F;
   }
   {  // Ewald alpha (reading A18)
     double rc = 0.5 * fmin(G.Lx, fmin(G.Ly, G.Lz));

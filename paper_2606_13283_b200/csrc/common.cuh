@@ -88,11 +88,26 @@ template <int NQ>
 __device__ __forceinline__ void block_totals(const int (&op)[NQ], const double *in /*[gridDim.x][NQ]*/, double *smem,
                                              double (&t)[NQ]) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  for (int q = wid; q < NQ; q += nw) {
-    double a = op[q] == 0 ? 0.0 : (op[q] == 1 ? 1.0e308 : -1.0e308);
-    for (unsigned int b = lane; b < gridDim.x; b += 32) a = red_combine(a, __ldcg(&in[(size_t)b * NQ + q]), op[q]);
-    a = warp_red(a, op[q]);
-    if (lane == 0) smem[q] = a;
+  constexpr int QPW = 2;   // quantities per warp in flight: one L2 round trip for up to 2*warps quantities
+  for (int q0 = wid; q0 < NQ; q0 += QPW * nw) {
+    double a[QPW];
+#pragma unroll
+    for (int u = 0; u < QPW; ++u) {
+      const int q = q0 + u * nw;
+      a[u] = (q < NQ && op[q < NQ ? q : 0] != 0) ? (op[q] == 1 ? 1.0e308 : -1.0e308) : 0.0;
+    }
+    for (unsigned int b = lane; b < gridDim.x; b += 32) {
+#pragma unroll
+      for (int u = 0; u < QPW; ++u) {
+        const int q = q0 + u * nw;
+        if (q < NQ) a[u] = red_combine(a[u], __ldcg(&in[(size_t)b * NQ + q]), op[q]);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < QPW; ++u) {
+      const int q = q0 + u * nw;
+      if (q < NQ) { const double r = warp_red(a[u], op[q]); if (lane == 0) smem[q] = r; }
+    }
   }
   __syncthreads();
 #pragma unroll

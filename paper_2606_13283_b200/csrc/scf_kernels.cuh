@@ -33,6 +33,7 @@ struct ScfConst {
   double kT, cTF, Ne, vol, dV, eta0, E_ie0;
   int xc, mix_mode, mix_warmup, pad;
   double mix_w_fixed, tol_F, tol_dn;
+  double inv_vol, inv_qF;   // reciprocals for the single-thread scalar updates (fp64 divisions cost ~300 cycles each there)
   double q_F, q_dn;   // reading A13: free-energy quantum of one PZ81 branch flip; chi(n*) x V_c jump x sqrt(dV)
 };
 
@@ -452,7 +453,7 @@ struct StoreNhatA {
   // grid totals {U, E_H, E_ie sums} -> energies, w (Eq. 30-31), free energy and the stop flag
   static __device__ __forceinline__ void apply(const double *t, const ScfConst &C, DevScalars *sc) {
     {
-      const double U = t[0] / C.vol, EH = 0.5 * t[1] / C.vol, Eie = t[2] / C.vol;
+      const double U = t[0] * C.inv_vol, EH = 0.5 * t[1] * C.inv_vol, Eie = t[2] * C.inv_vol;
       sc->U = U; sc->EH = EH; sc->Eie = Eie;
       const int it = sc->iter + 1;
       const double K = sc->K;
@@ -468,7 +469,7 @@ struct StoreNhatA {
       // right after a change far below one quantum marks the solve; from then on two quanta are tolerated in both criteria.
       const double dF = fabs(F - sc->F_total);
       if (C.xc == 1 && it >= 3 && C.q_F > 0.0) {   // a jump: the previous change of F was far below one quantum
-        const double m = dF / C.q_F, r = rint(m), mp = fabs(sc->F_total - sc->F_prev) / C.q_F, rp = rint(mp);
+        const double m = dF * C.inv_qF, r = rint(m), mp = fabs(sc->F_total - sc->F_prev) * C.inv_qF, rp = rint(mp);
         const bool near = r >= 1.0 && r <= 8.0 && fabs(m - r) < 0.02, near_prev = rp >= 1.0 && rp <= 8.0 && fabs(mp - rp) < 0.02;
         if (near && (mp < 0.1 || near_prev)) sc->flip_seen = 1;   // after a quiet change, or twice in a row
       }
