@@ -1,0 +1,45 @@
+"""Host-side logic of bench.py that needs no GPU: byte/flop models, roofline selection, workload description."""
+import os
+import sys
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+import arche_inputs as ai  # noqa: E402
+import bench  # noqa: E402
+
+
+def test_bytes_per_point_models():
+    fused = bench.bytes_per_point(64, True)
+    h = 16.0 * 40 / 64                       # nx/2+1 = 33 stored columns padded to 40
+    assert fused["fft_y"] == 2 * h and fused["fft_inv_z_potential"] == 5 * h and fused["density"] == 24 + h
+    streamed = bench.bytes_per_point(384, False)
+    h = 16.0 * 200 / 384
+    assert abs(streamed["potential_g"] - 5 * h) < 1e-12 and streamed["vi_r"] == 40 and streamed["density_r"] == 24
+    assert "density" not in streamed and "potential_g" not in fused
+    # one SCF iteration of the streamed form moves 18 h + 80 (+ 8 per mu evaluation) bytes per point
+    per_iter = sum(streamed[k] * (2 if k == "fft_y" else 1) for k in streamed if k not in ("mix", "mu_pass"))
+    assert abs(per_iter - (18 * h + 80)) < 1e-9
+
+
+def test_roofline_entry_picks_the_binding_bound():
+    bpp = bench.bytes_per_point(384, False)
+    ng = 384 ** 3
+    e = bench.roofline_entry("potential_g", 0.357, ng, bpp, 6547.2, "measured")
+    assert e["bound"] == "hbm" and 0.95 < e["frac"] < 1.05
+    e = bench.roofline_entry("density_r", 0.720, ng, bpp, 6547.2, "measured")
+    assert e["bound"] == "alu" and 0.35 < e["frac"] < 0.5 and e["unit"] == "TFLOP/s"
+    # the plain c2r pass of the streamed form carries no epilogue arithmetic: HBM bound only
+    e = bench.roofline_entry("fft_inv_x_vi", 0.244, ng, bpp, 6547.2, "measured")
+    assert e["bound"] == "hbm"
+    assert abs(bench.FP64_PEAK_TFLOPS - 37.22) < 0.01
+
+
+def test_workload_description_and_configs():
+    for name, ions, grid in (("c1", 16, 32), ("c2", 128, 64), ("c3", 256, 128), ("c4", 1024, 192)):
+        cfg = ai.make_config(name)
+        assert len(cfg["Z"]) == ions and int(cfg["grid"][0]) == grid
+        w = bench.workload_config(cfg, name)
+        assert name in w["workload"] and "stop_rule" in w
+    cfg = ai.make_config("c5", grid=96)
+    assert len(cfg["Z"]) == 2000 and int(cfg["grid"][2]) == 96
