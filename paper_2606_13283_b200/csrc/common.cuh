@@ -71,43 +71,39 @@ __device__ __forceinline__ void block_reduce(double (&v)[NQ], const int (&op)[NQ
 
 // Barrier-based form of the grid reduction for cooperative kernels: every block writes its partials, the caller
 // issues a grid barrier, then every block sums all partials in the same fixed order (no atomics, no last-block
-// serialisation; all blocks end up with identical totals).
+// serialisation; all blocks end up with identical totals).  Partials are stored [quantity][block] so that a warp
+// reads one quantity of 32 blocks as one contiguous 256-byte segment.
 template <int NQ>
 __device__ __forceinline__ void block_partials(double (&v)[NQ], const int (&op)[NQ], double *smem /*[NQ*32]*/,
-                                               double *out /*[gridDim.x][stride]*/, int stride = NQ, int offset = 0) {
+                                               double *out /*[stride][gridDim.x]*/, int stride = NQ, int offset = 0) {
+  (void)stride;
   block_reduce<NQ>(v, op, smem);
   if (threadIdx.x == 0) {
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) out[(size_t)blockIdx.x * stride + offset + q] = v[q];
+    for (int q = 0; q < NQ; ++q) out[(size_t)(offset + q) * gridDim.x + blockIdx.x] = v[q];
   }
 }
-// totals valid in thread 0 (written to t[NQ] there); call after the grid barrier that follows block_partials.
-// Warp q sums quantity q over the blocks (lane-strided, then one shuffle tree): one L2 round trip and no second
-// reduction level; needs NQ <= warps per block.
+// totals valid in every thread (t[NQ]); call after the grid barrier that follows block_partials.  Warp q sums
+// quantity q over the blocks: the loads of up to 160 blocks are issued together (one L2 round trip), then one
+// shuffle tree; needs NQ <= 2 x warps per block.
 template <int NQ>
-__device__ __forceinline__ void block_totals(const int (&op)[NQ], const double *in /*[gridDim.x][NQ]*/, double *smem,
+__device__ __forceinline__ void block_totals(const int (&op)[NQ], const double *in /*[NQ][gridDim.x]*/, double *smem,
                                              double (&t)[NQ]) {
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  constexpr int QPW = 2;   // quantities per warp in flight: one L2 round trip for up to 2*warps quantities
-  for (int q0 = wid; q0 < NQ; q0 += QPW * nw) {
-    double a[QPW];
+  const unsigned int G = gridDim.x;
+  for (int q = wid; q < NQ; q += nw) {
+    const int o = op[q];
+    const double ident = o == 0 ? 0.0 : (o == 1 ? 1.0e308 : -1.0e308);
+    const double *row = in + (size_t)q * G;
+    double v[5];
 #pragma unroll
-    for (int u = 0; u < QPW; ++u) {
-      const int q = q0 + u * nw;
-      a[u] = (q < NQ && op[q < NQ ? q : 0] != 0) ? (op[q] == 1 ? 1.0e308 : -1.0e308) : 0.0;
-    }
-    for (unsigned int b = lane; b < gridDim.x; b += 32) {
+    for (int k = 0; k < 5; ++k) { const unsigned int b = lane + 32 * k; v[k] = b < G ? __ldcg(row + b) : ident; }
+    double a = v[0];
 #pragma unroll
-      for (int u = 0; u < QPW; ++u) {
-        const int q = q0 + u * nw;
-        if (q < NQ) a[u] = red_combine(a[u], __ldcg(&in[(size_t)b * NQ + q]), op[q]);
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < QPW; ++u) {
-      const int q = q0 + u * nw;
-      if (q < NQ) { const double r = warp_red(a[u], op[q]); if (lane == 0) smem[q] = r; }
-    }
+    for (int k = 1; k < 5; ++k) a = red_combine(a, v[k], o);
+    for (unsigned int b = lane + 160; b < G; b += 32) a = red_combine(a, __ldcg(row + b), o);
+    a = warp_red(a, o);
+    if (lane == 0) smem[q] = a;
   }
   __syncthreads();
 #pragma unroll
