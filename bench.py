@@ -361,6 +361,11 @@ def main():
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_source": peak_src,
                 "share_of_step": round(t_scf * 1e3 / tot_prof, 4), "bytes_per_iteration": bpi,
                 "us_per_iteration": round(1e6 * t_scf / n_it, 2)}
+        # DRAM bytes of ONE launch (= one solve) from the committed ncu --set full capture of this workload
+        ncu_traffic = {"c2": (7.526e6 + 0.778e6, "profiles/r01e_c2_ncu_full.csv")}
+        if args.workload in ncu_traffic:
+            roof["traffic"], roof["traffic_source"] = ncu_traffic[args.workload]
+            roof["algorithmic_bytes_per_launch"] = bpi * iters / max(args.steps, 1)
         roof["note"] = ("the 64^3 fields are L2-resident (ncu: 7.5 MB of DRAM reads per 9 ms solve): the kernel is bound by "
                         "dependent latency chains and 9 grid barriers per iteration, not by HBM; the fraction is the "
                         "algorithmic traffic against the HBM peak as the contract asks. Large-grid rooflines: "
