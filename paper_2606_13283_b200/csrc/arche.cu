@@ -594,8 +594,9 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
       conv = fixed <= 0 && c->h_sc->converged;
       goto solved;
     }
-    if (e != cudaErrorNotSupported) return fail(c, ARCHE_ECUDA, "scf_persistent_launch", e);
-    c->persist = false;   // no instantiation for this grid: per-pass form from now on
+    if (e == cudaErrorCooperativeLaunchTooLarge) (void)cudaGetLastError();   // GPU shared with another context: per-pass form
+    else if (e != cudaErrorNotSupported) return fail(c, ARCHE_ECUDA, "scf_persistent_launch", e);
+    c->persist = false;   // no instantiation for this grid (or no room for the resident grid): per-pass form from now on
   }
   // Iterations are launched in batches without a host round trip; once the S5 epilogue has set the stop flag the
   // kernels of the remaining iterations of the batch return at once, so the state stays that of the converged
