@@ -227,22 +227,23 @@ constexpr int kFastLP = 8;  // line pairs per block
 // integrals, XC) uses all
 template <int N> __host__ __device__ constexpr int fast_threads_x() { return 256; }
 // plain x passes (no pointwise functor work): just the butterfly threads, and more resident blocks per SM instead
+constexpr int kFastLPLight = 4;   // line pairs per block of the light configuration: half the tile, twice the blocks
 template <int N> __host__ __device__ constexpr int fast_threads_x_light() {
-  return kFastLP * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
+  return kFastLPLight * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
 }
-template <int N> __host__ __device__ constexpr int fast_blocks_x_light() { return N >= 384 ? 3 : 4; }
+template <int N> __host__ __device__ constexpr int fast_blocks_x_light() { return N >= 384 ? 6 : 8; }
 template <int N> __host__ __device__ constexpr int fast_row_x() { return N + N / FastPlan<N>::R1; }   // padded smem row (elements)
 template <int N> __device__ __forceinline__ int fast_pos(int i) { return i + i / FastPlan<N>::R1; }
 
 // the two stages on the tile's LP complex lines held in shared memory (in place); t = thread index within the group
 // of TH threads that owns the tile, bar = the group's barrier id (0 with the whole block)
-template <int N, int TH>
+template <int N, int TH, int LP = kFastLP>
 __device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *tw, int t, int bar) {
   constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, ROW = fast_row_x<N>();
-  static_assert(TH >= kFastLP * R1 && TH >= kFastLP * R2, "one butterfly per thread");
+  static_assert(TH >= LP * R1 && TH >= LP * R2, "one butterfly per thread");
   {
     const int p = t / R2, j1 = t % R2;
-    const bool act = t < kFastLP * R2;
+    const bool act = t < LP * R2;
     double2 v[R1];
     if (act) {
 #pragma unroll
@@ -256,7 +257,7 @@ __device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *tw, i
     }
   }
   group_sync(bar, TH);
-  if (t < kFastLP * R1) {
+  if (t < LP * R1) {
     const int p = t / R1, j2 = t % R1;
     double2 v[R2];
 #pragma unroll
@@ -271,14 +272,14 @@ __device__ __forceinline__ void fast_stages_x(double2 *buf, const double2 *tw, i
 }
 
 // one x tile (8 pairs of real lines) by the whole block (256 threads); buf = [LP][ROW] shared
-template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), class LoadOp, class StoreOp>
+template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), int LP = kFastLP, class LoadOp, class StoreOp>
 __device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf,
                                              int tg = threadIdx.x, int bar = 0) {
   constexpr int ROW = fast_row_x<N>(), NXH = N / 2 + 1;
-  const long long line0 = (long long)tile * (2 * kFastLP);
+  const long long line0 = (long long)tile * (2 * LP);
   if (PREFETCH)
-    for (int e = tg * 16; e < 2 * kFastLP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
-  for (int e = tg; e < kFastLP * N; e += TH) {
+    for (int e = tg * 16; e < 2 * LP * N; e += TH * 16) ld.prefetch(line0 * N + e);   // contiguous real tile
+  for (int e = tg; e < LP * N; e += TH) {
     const int p = e / N, i = e % N;
     const long long la = line0 + 2 * p, lb = la + 1;
     double a, b;
@@ -286,8 +287,8 @@ __device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, Stor
     buf[p * ROW + fast_pos<N>(i)] = make_double2(a, b);
   }
   group_sync(bar, TH);
-  fast_stages_x<N, TH>(buf, G.tw, tg, bar);
-  for (int e = tg; e < kFastLP * G.P; e += TH) {
+  fast_stages_x<N, TH, LP>(buf, G.tw, tg, bar);
+  for (int e = tg; e < LP * G.P; e += TH) {
     const int p = e / G.P, k = e % G.P;
     const long long la = line0 + 2 * p, lb = la + 1;
     double2 A = make_double2(0.0, 0.0), B = A;
@@ -302,16 +303,16 @@ __device__ __forceinline__ void fft_r2c_tile(const FastGeom &G, LoadOp &ld, Stor
   group_sync(bar, TH);
 }
 
-template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), class LoadOp, class StoreOp>
+template <int N, bool PREFETCH, int TH = fast_threads_x<N>(), int LP = kFastLP, class LoadOp, class StoreOp>
 __device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, StoreOp &st, int tile, double2 *buf,
                                              int tg = threadIdx.x, int bar = 0) {
   constexpr int ROW = fast_row_x<N>(), NXH = N / 2 + 1;
-  const long long line0 = (long long)tile * (2 * kFastLP);
+  const long long line0 = (long long)tile * (2 * LP);
   if (PREFETCH) {
-    for (int e = tg * 8; e < 2 * kFastLP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile
-    for (int e = tg * 16; e < 2 * kFastLP * N; e += TH * 16) st.prefetch(line0 * N + e);    // operands of the epilogue
+    for (int e = tg * 8; e < 2 * LP * G.P; e += TH * 8) ld.prefetch(line0 * G.P + e);  // contiguous half tile
+    for (int e = tg * 16; e < 2 * LP * N; e += TH * 16) st.prefetch(line0 * N + e);    // operands of the epilogue
   }
-  for (int e = tg; e < kFastLP * NXH; e += TH) {
+  for (int e = tg; e < LP * NXH; e += TH) {
     const int p = e / NXH, k = e % NXH;
     const long long la = line0 + 2 * p, lb = la + 1;
     double2 A, B;
@@ -321,8 +322,8 @@ __device__ __forceinline__ void fft_c2r_tile(const FastGeom &G, LoadOp &ld, Stor
     if (k > 0 && 2 * k < N) buf[p * ROW + fast_pos<N>(N - k)] = make_double2(A.x + B.y, A.y - B.x);  // conj(conj A + i conj B)
   }
   group_sync(bar, TH);
-  fast_stages_x<N, TH>(buf, G.tw, tg, bar);
-  for (int e = tg; e < kFastLP * N; e += TH) {
+  fast_stages_x<N, TH, LP>(buf, G.tw, tg, bar);
+  for (int e = tg; e < LP * N; e += TH) {
     const int p = e / N, i = e % N;
     const long long la = line0 + 2 * p, lb = la + 1;
     const double2 z = buf[p * ROW + fast_pos<N>(i)];
@@ -339,8 +340,8 @@ __global__ void __launch_bounds__(LIGHT ? fast_threads_x_light<N>() : fast_threa
   StoreOp st = st_in;
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
-  fft_r2c_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>()>(G, ld, st, blockIdx.x,
-                                                                               reinterpret_cast<double2 *>(smem_raw));
+  fft_r2c_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>(), LIGHT ? kFastLPLight : kFastLP>(
+      G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw));
   ld.finish(smem_raw);
   st.finish(smem_raw);
 }
@@ -353,8 +354,8 @@ __global__ void __launch_bounds__(LIGHT ? fast_threads_x_light<N>() : fast_threa
   StoreOp st = st_in;
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
-  fft_c2r_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>()>(G, ld, st, blockIdx.x,
-                                                                               reinterpret_cast<double2 *>(smem_raw));
+  fft_c2r_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>(), LIGHT ? kFastLPLight : kFastLP>(
+      G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw));
   ld.finish(smem_raw);
   st.finish(smem_raw);
 }
@@ -391,9 +392,10 @@ static inline cudaError_t fft_launch_yz_fast(int n, const FastGeom &G, LoadOp ld
 
 template <int N, bool INVERSE, bool LIGHT, class LoadOp, class StoreOp>
 static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
-  size_t smem = sizeof(double2) * kFastLP * fast_row_x<N>();
+  constexpr int LP = LIGHT ? kFastLPLight : kFastLP;
+  size_t smem = sizeof(double2) * LP * fast_row_x<N>();
   if (smem < 4096) smem = 4096;
-  const unsigned blocks = (unsigned)((long long)G.ny * G.nz / (2 * kFastLP));
+  const unsigned blocks = (unsigned)((long long)G.ny * G.nz / (2 * LP));
   constexpr int TH = LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>();
   static bool attr_set = false;
   if constexpr (INVERSE) {
