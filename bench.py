@@ -232,6 +232,23 @@ def run_iteration_sweep(args):
                      "frac": round(e["frac"], 3)}
         else:
             rl[k] = {"ms": round(ms / n, 4)}
+    # comparison column only (BASELINE.json: cuFFT never on the product path): torch.fft.rfftn = cuFFT D2Z on the same grid
+    cufft_ms = None
+    try:
+        a = torch.randn(args.grid, args.grid, args.grid, dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            torch.fft.rfftn(a)
+        c0 = torch.cuda.Event(enable_timing=True); c1 = torch.cuda.Event(enable_timing=True)
+        c0.record()
+        for _ in range(10):
+            torch.fft.rfftn(a)
+        c1.record(); torch.cuda.synchronize()
+        cufft_ms = c0.elapsed_time(c1) / 10
+        del a
+    except Exception:
+        pass
+    fwd = [k for k in ("fft_fwd_x_real", "fft_y", "fft_fwd_z_reduce") if k in rl]
+    own_r2c_ms = sum(rl[k]["ms"] for k in fwd) if len(fwd) == 3 and not g.is_fused() else None
     hbm_classes = [k for k in rl if rl[k].get("bound") == "hbm"]
     tot_b = sum(bpp[k] * g.ng * prof[k][1] for k in hbm_classes)
     tot_t = sum(prof[k][0] for k in hbm_classes) * 1e-3
@@ -244,6 +261,8 @@ def run_iteration_sweep(args):
                        "fused": g.is_fused()},
             "grid_points_per_s": g.ng / it_ms * 1e3, "mu_evals_per_iter": evals_per_iter, "clocks": cs.summary(),
             "hbm_classes_aggregate_gbs": tot_b / tot_t / 1e9 if tot_t > 0 else None, "hbm_peak_gbs": peak,
+            "fft_comparison": {"own_r2c_3d_ms": own_r2c_ms, "cufft_d2z_3d_ms": cufft_ms,
+                               "note": "own = plain x (r2c) + y + z passes of the streamed form; cuFFT through torch.fft.rfftn, comparison only"},
             "kernels": rl}
     print(json.dumps(line))
 
