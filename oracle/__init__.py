@@ -79,6 +79,7 @@ def lib():
         L.oracle_scf_solve.argtypes = [C.c_void_p, dp, C.POINTER(Result)]
         L.oracle_forces.argtypes = [C.c_void_p, dp]
         L.oracle_md_step.argtypes = [C.c_void_p, C.c_double, dp, dp, C.POINTER(Result)]
+        L.oracle_stress.argtypes = [C.c_void_p, dp, dp]
         L.oracle_get_real.argtypes = [C.c_void_p, C.c_int, dp]
         L.oracle_get_complex.argtypes = [C.c_void_p, C.c_int, dp]
         L.oracle_num_threads.restype = C.c_int
@@ -161,6 +162,9 @@ def force_ie(cell, grid, pos, Z, rc, nhat) -> np.ndarray:
     return F
 
 
+STRESS_ROWS = ("i", "e", "xc", "pp", "pm", "je", "ee", "ie", "total")
+
+
 class Oracle:
     """SCF/MD context (mirrors the C-ABI of the product, with host arrays)."""
 
@@ -221,6 +225,18 @@ class Oracle:
         if rc != 0:
             raise RuntimeError("oracle_forces before a solve")
         return F
+
+    def stress(self, vel=None) -> dict:
+        """Stress tensor of the last solve: {'i','e','xc','pp','pm','je','ee','ie','total'} ->
+        [xx, yy, zz, yz, xz, xy], and 'P' = -tr(total)/3."""
+        out = np.zeros(55)
+        v = None if vel is None else _dp(_f64(vel))
+        rc = lib().oracle_stress(self._h, v, _dp(out))
+        if rc != 0:
+            raise RuntimeError("oracle_stress before a solve")
+        d = {k: out[6 * r:6 * r + 6].copy() for r, k in enumerate(STRESS_ROWS)}
+        d["P"] = float(out[54])
+        return d
 
     def md_step(self, dt, pos, vel) -> dict:
         """pos, vel: float64 C-contiguous arrays, updated in place."""

@@ -670,6 +670,82 @@ int oracle_md_step(oracle_ctx *c, double dt, double *pos, double *vel, oracle_re
   return rc;
 }
 
+/* ======================================================================================== */
+/* f1: stress tensor and pressure.  sigma_mn = (1/|Omega|) dE/d(eps_mn): the cell and every r_j   */
+/* are strained, k_m -> k_m - eps_mn k_n, |Omega| -> |Omega|(1 + tr eps), nhat(k) and S_Z(k) keep  */
+/* their values (fixed scaled coordinates and scaled density), alpha is held fixed.              */
+/* rows: 0 i (Eq. 37), 1 e (Eq. 39), 2 xc (reading A21), 3 pp (Eq. 49), 4 pm (Eq. 50), 5 je       */
+/* (Eq. 51), 6 ee (Eq. 54), 7 ie (PAPER.md:483-487 incl. the k=0 term of Eq. 55), 8 total (35).   */
+/* columns: xx, yy, zz, yz, xz, xy.                                                              */
+/* ======================================================================================== */
+int oracle_stress(oracle_ctx *c, const double *vel, double *out) {
+  if (!c->have_solution) return -1;
+  static const int MU[6] = {0, 1, 2, 1, 0, 0}, NU[6] = {0, 1, 2, 2, 2, 1};
+  const int n = c->p.n_ions;
+  const double vol = c->vol, a = c->alpha, rc = c->p.psp_rc;
+  long double s[9][6];
+  for (int r = 0; r < 9; ++r)
+    for (int q = 0; q < 6; ++q) s[r][q] = 0.0L;
+  /* Eq. 37: sigma^i = -(2/|Omega|) sum_i m_i v_m v_n / 2 */
+  if (vel)
+    for (int j = 0; j < n; ++j)
+      for (int q = 0; q < 6; ++q) s[0][q] -= c->mass[j] * vel[3 * j + MU[q]] * vel[3 * j + NU[q]] / vol;
+  /* Eq. 39: sigma^e = -(2 K_e/(3|Omega|)) delta;  reading A21: sigma^xc = (1/|Omega|) int n (eps_xc - v_xc) delta */
+  long double sxc = 0.0L;
+  for (size_t g = 0; g < c->ng; ++g) {
+    double e, v;
+    oracle_xc(c->p.xc, c->n_a[g], &e, &v);
+    sxc += c->n_a[g] * (e - v);
+  }
+  for (int q = 0; q < 3; ++q) {
+    s[1][q] = -2.0 * c->last.K_e / (3.0 * vol);
+    s[2][q] = (double)sxc * c->dV / vol;
+  }
+  /* Eq. 49: short-range pairs, minimum image as in Eq. 41 */
+  for (int i = 0; i < n; ++i)
+    for (int j = i + 1; j < n; ++j) {
+      double d[3], r2 = 0.0;
+      for (int k = 0; k < 3; ++k) {
+        d[k] = c->pos[3 * i + k] - c->pos[3 * j + k];
+        d[k] -= c->p.cell[k] * rint(d[k] / c->p.cell[k]);
+        r2 += d[k] * d[k];
+      }
+      double r = sqrt(r2);
+      double f = c->Z[i] * c->Z[j] * (erfc(a * r) / r + 2.0 * a / sqrt(PI) * exp(-a * a * r2)) / r2;
+      for (int q = 0; q < 6; ++q) s[3][q] -= f * d[MU[q]] * d[NU[q]] / vol;
+    }
+  /* Eq. 51 */
+  for (int q = 0; q < 3; ++q) s[5][q] = PI * c->Q * c->Q / (2.0 * a * a * vol * vol);
+  /* G-space sums over the literal k set: Eq. 50, Eq. 54 */
+  for (size_t g = 0; g < c->ng; ++g) {
+    double k[3];
+    kvec(c, g, k);
+    double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2];
+    if (k2 == 0.0) continue;
+    double ka = sqrt(k2);
+    double S2 = creal(c->S[g]) * creal(c->S[g]) + cimag(c->S[g]) * cimag(c->S[g]);
+    double va = exp(-PI * PI * k2 / (a * a)) / (PI * k2);
+    double n2 = creal(c->nh_a[g]) * creal(c->nh_a[g]) + cimag(c->nh_a[g]) * cimag(c->nh_a[g]);
+    /* d/dk of the Ashcroft form factor -cos(2 pi k rc)/(pi k^2) */
+    double dv = 2.0 * rc * sin(2.0 * PI * ka * rc) / k2 + 2.0 * cos(2.0 * PI * ka * rc) / (PI * k2 * ka);
+    /* nhat(k) sum_j Z_j dv e^{+2 pi i k.r_j} = nhat conj(S_Z) dv; its real part (the sum is real, reading A6) */
+    double nS = creal(c->nh_a[g] * conj(c->S[g]));
+    for (int q = 0; q < 6; ++q) {
+      double kk = k[MU[q]] * k[NU[q]], dl = q < 3 ? 1.0 : 0.0;
+      s[4][q] += va * S2 * (2.0 * kk * (PI * PI / (a * a) + 1.0 / k2) - dl) / (2.0 * vol * vol);
+      s[6][q] += n2 / (PI * k2) * (2.0 * kk / k2 - dl) / (2.0 * vol * vol);
+      s[7][q] -= nS * dv * kk / ka / (vol * vol);
+    }
+  }
+  for (int q = 0; q < 3; ++q) s[7][q] -= (c->last.E_ie + c->last.E_ie0) / vol;
+  for (int r = 0; r < 8; ++r)
+    for (int q = 0; q < 6; ++q) s[8][q] += s[r][q];
+  for (int r = 0; r < 9; ++r)
+    for (int q = 0; q < 6; ++q) out[6 * r + q] = (double)s[r][q];
+  out[54] = -(double)(s[8][0] + s[8][1] + s[8][2]) / 3.0; /* Eq. 34 */
+  return 0;
+}
+
 int oracle_get_real(oracle_ctx *c, int which, double *dst) {
   const double *src = which == 0 ? c->n_a : which == 1 ? c->n_i : which == 2 ? c->V_i : NULL;
   if (!src) return -1;

@@ -90,6 +90,13 @@ int oracle_get_complex(oracle_ctx *c, int which, double *dst);
 /* F^ie only, for an arbitrary density given in G-space (used by the fixed-density FD pin) */
 void oracle_force_ie(const double cell[3], const int grid[3], int n_ions, const double *pos,
                      const double *Z, double rc, const double *nhat_complex, double *F);
+/* f1: average virial stress tensor and pressure from the last solve (PAPER.md:341-347 Eq. 34-35, :355 Eq. 37,
+ * :372 Eq. 39, :423-440 Eq. 48-51, :458-461 Eq. 54, :483-487; LDA term: DESIGN.md reading A21).
+ * sigma_mn = (1/|Omega|) dE/d(eps_mn) at fixed scaled coordinates and fixed Ewald alpha; P = -tr(Sigma)/3.
+ * out[9*6 + 1]: rows i, e, xc, pp, pm, je, ee, ie, total; columns xx, yy, zz, yz, xz, xy; out[54] = P.
+ * vel[n_ions*3] may be NULL (sigma^i = 0).  Pins: tests/test_oracle_stress_pins.py. */
+#define ORACLE_STRESS_DOUBLES 55
+int oracle_stress(oracle_ctx *c, const double *vel, double *out);
 int oracle_num_threads(void);
 
 #ifdef __cplusplus
