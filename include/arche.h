@@ -89,6 +89,16 @@ int arche_set_input_density(arche_ctx *c, const double *d_n);
  * written to d_F[n_ions*3].  ARCHE_EINVAL before any solve. */
 int arche_forces(arche_ctx *c, double *d_F);
 
+/* Average virial stress tensor and pressure of the last solve (Eq. 34-35; terms Eq. 37
+ * P:355, Eq. 39, Eq. 48-51, Eq. 54, sigma^ie P:483-487; sign convention and the LDA term:
+ * DESIGN.md reading A21): sigma_mn = (1/|Omega|) dE/d(eps_mn) at fixed scaled coordinates and fixed Ewald alpha,
+ * P = -tr(Sigma)/3, Hartree/bohr^3.
+ * h_out: HOST array of ARCHE_STRESS_DOUBLES doubles, owned by the caller: 9 rows (i, e, xc, pp, pm, je, ee, ie,
+ * total) x 6 columns (xx, yy, zz, yz, xz, xy), then P.  d_vel: DEVICE [n_ions*3] ion velocities for sigma^i, or NULL
+ * (sigma^i = 0).  Stream-ordered, synchronises before filling h_out.  ARCHE_EINVAL before any solve. */
+#define ARCHE_STRESS_DOUBLES 55
+int arche_stress(arche_ctx *c, const double *d_vel, double *h_out);
+
 /* One velocity-Verlet step of length dt (a.u.) (reading D2): half kick, drift, SCF solve at the
  * new positions, forces, half kick.  d_pos/d_vel [n_ions*3] are updated in place.  The first call also solves
  * at the starting positions to obtain the initial forces. */
@@ -127,7 +137,7 @@ long long arche_launch_count(const arche_ctx *c);
  * 10 Ewald pair kernel, 11 other.  On grids beyond the L2 the pointwise work runs as streaming kernels around plain
  * passes (arche_is_fused() == 0): 12 G-space potential assembly + mixing (S1/S6), 13 V_i assembly + XC + first mu
  * evaluation (S2), 14 density and local reductions (S4), 15 G-space reductions (S5); classes 0, 2, 5, 6 are then the
- * plain passes and 4 is unused.  arche_profile_get returns the summed milliseconds and launch count of a class. */
+ * plain passes and 4 is unused.  16 field sums of arche_stress (f1).  arche_profile_get returns the summed milliseconds and launch count of a class. */
 int arche_profile_enable(arche_ctx *c, int on);
 int arche_is_fused(const arche_ctx *c);
 /* 1 when arche_scf_solve runs the whole SCF loop in one persistent cooperative launch (fused form on 32^3 / 64^3 grids;

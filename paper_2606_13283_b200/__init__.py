@@ -17,7 +17,7 @@ from .build import LIB, build
 __all__ = ["Arche", "ArcheError", "load", "SYMBOLS", "Params", "Result"]
 
 SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_last_error", "arche_scf_solve",
-           "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_md_step",
+           "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_stress", "arche_md_step",
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
            "arche_rfft3d_forward", "arche_rfft3d_inverse",
            "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused", "arche_is_persistent"]
@@ -71,6 +71,7 @@ def load(rebuild_if_stale: bool = True):
     L.arche_scf_iter.argtypes = [vp, C.POINTER(Result)]
     L.arche_set_input_density.argtypes = [vp, dp]
     L.arche_forces.argtypes = [vp, dp]
+    L.arche_stress.argtypes = [vp, dp, C.POINTER(C.c_double)]
     L.arche_md_step.argtypes = [vp, C.c_double, dp, dp, C.POINTER(Result)]
     L.arche_md_step_host.argtypes = [vp, C.c_double, dp, dp, dp, C.POINTER(Result)]
     L.arche_get_real.argtypes = [vp, C.c_int, dp]
@@ -191,6 +192,19 @@ class Arche:
         self._check(self.lib.arche_forces(self._h, F.data_ptr()))
         return F
 
+    STRESS_ROWS = ("i", "e", "xc", "pp", "pm", "je", "ee", "ie", "total")
+
+    def stress(self, vel=None) -> dict:
+        """Stress tensor of the last solve (include/arche.h: arche_stress): row name -> [xx, yy, zz, yz, xz, xy]
+        (numpy), and 'P' = -tr(total)/3.  vel: CUDA float64 tensor [n_ions,3] or None."""
+        import numpy as np
+        out = (C.c_double * 55)()
+        self._check(self.lib.arche_stress(self._h, None if vel is None else vel.data_ptr(), out))
+        a = np.array(out[:])
+        d = {k: a[6 * r:6 * r + 6].copy() for r, k in enumerate(self.STRESS_ROWS)}
+        d["P"] = float(a[54])
+        return d
+
     def md_step(self, dt, pos, vel) -> dict:
         """pos, vel: CUDA float64 tensors [n_ions,3], updated in place."""
         r = Result()
@@ -251,7 +265,7 @@ class Arche:
 
     PROFILE_CLASSES = ("fft_inv_z_potential", "fft_y", "fft_inv_x_vi", "mu_pass", "density", "fft_fwd_x_real",
                        "fft_fwd_z_reduce", "mix", "structure_factor", "force", "ewald_pp", "other",
-                       "potential_g", "vi_r", "density_r", "reduce_g")
+                       "potential_g", "vi_r", "density_r", "reduce_g", "stress_fields")
 
     def is_fused(self) -> bool:
         return bool(self.lib.arche_is_fused(self._h))

@@ -18,6 +18,7 @@
 #include "ion_kernels.cuh"
 #include "scf_kernels.cuh"
 #include "scf_persistent.cuh"
+#include "stress_kernels.cuh"
 
 using namespace arche;
 
@@ -28,7 +29,7 @@ constexpr int kScfBatch = 6;      // SCF iterations launched between two reads o
 constexpr int kProfPairs = 512;
 // kernel classes for arche_profile_get
 enum ProfClass { PC_FFT_INV_Z = 0, PC_FFT_Y, PC_FFT_INV_X, PC_MU, PC_DENSITY, PC_FFT_FWD_X, PC_FFT_FWD_Z, PC_MIX,
-                 PC_SFAC, PC_FORCE, PC_EWALD, PC_OTHER, PC_POT_G, PC_VI_R, PC_DENS_R, PC_RED_G, kProfClasses };
+                 PC_SFAC, PC_FORCE, PC_EWALD, PC_OTHER, PC_POT_G, PC_VI_R, PC_DENS_R, PC_RED_G, PC_STRESS, kProfClasses };
 constexpr int kEwBlocks = 148 * 8;
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -100,6 +101,8 @@ struct arche_ctx {
   double2 *tw[3];
   double2 *ax_ij, *ax_ji, *by_ij, *cz_ij;
   double *Z, *mass, *pos, *F, *F_pp, *e_pp, *F_part, *vel_tmp;
+  double *pp_part, *stress;   // [nions][6] short-range stress sums; [64] assembled table (device)
+  double *h_stress;           // pinned [64]
   double *fdtab, *partials;
   unsigned int *counter;
   unsigned long long *phase_ns;
@@ -175,6 +178,7 @@ size_t layout(arche_ctx *c, char *base) {
   c->Z = w.take<double>(ni); c->mass = w.take<double>(ni); c->pos = w.take<double>(3 * ni);
   c->F = w.take<double>(3 * ni); c->F_pp = w.take<double>(3 * ni); c->e_pp = w.take<double>(ni);
   c->vel_tmp = w.take<double>(3 * ni);
+  c->pp_part = w.take<double>(6 * ni); c->stress = w.take<double>(64);
   c->F_part = w.take<double>((size_t)c->force_slabs * ni * 3);
   c->fdtab = w.take<double>(kFdTabDoubles);
   c->partials = w.take<double>((size_t)c->red_blocks * kMaxRed);
@@ -234,6 +238,7 @@ extern "C" long long arche_launch_count(const arche_ctx *c) { return c ? c->laun
 extern "C" void arche_destroy(arche_ctx *c) {
   if (!c) return;
   if (c->h_sc) cudaFreeHost(c->h_sc);
+  if (c->h_stress) cudaFreeHost(c->h_stress);
   for (int k = 0; k < 2 * kProfPairs; ++k) if (c->prof_ev[k]) cudaEventDestroy(c->prof_ev[k]);
   delete c;
 }
@@ -262,6 +267,8 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   const int nx = p->grid[0], ny = p->grid[1], nz = p->grid[2];
   cudaError_t e = cudaMallocHost((void **)&c->h_sc, sizeof(DevScalars));
   if (e != cudaSuccess) { delete c; return ARCHE_ECUDA; }
+  e = cudaMallocHost((void **)&c->h_stress, 64 * sizeof(double));
+  if (e != cudaSuccess) { cudaFreeHost(c->h_sc); delete c; return ARCHE_ECUDA; }
   // ---- geometry and constants
   GridGeom &G = c->G;
   G.nx = nx; G.ny = ny; G.nz = nz; G.ng = c->ng; G.nxh = c->nxh; G.P = c->P; G.nh = c->nh;
@@ -654,6 +661,30 @@ int compute_forces(arche_ctx *c) {
   return ARCHE_OK;
 }
 
+// f1: stress tensor and pressure of the last solve (stress_kernels.cuh): 3 launches (2 without ions)
+int compute_stress(arche_ctx *c, const double *d_vel) {
+  if (!c->have_solution) return fail(c, ARCHE_EINVAL, "arche_stress before a solve");
+  const int ni = c->nions;
+  const GridGeom &G = c->G;
+  const long long work = c->nh > c->ng ? c->nh : c->ng;
+  long long nb = (work + kStressThreads - 1) / kStressThreads;
+  const long long cap = (long long)c->red_blocks * kMaxRed / kStressSums, full = (long long)c->sm_count * 8;
+  if (nb > full) nb = full;
+  if (nb > cap) nb = cap;
+  { ProfScope ps(c, PC_STRESS);
+  stress_fields_kernel<<<(unsigned)nb, kStressThreads, 0, c->stream>>>(G, c->nh_a, c->S, c->S2, c->n_a, c->p.xc, c->alpha,
+                                                                     c->p.psp_rc, c->partials);
+  LAUNCHED(c); }
+  if (ni > 0) {
+    stress_pp_kernel<<<ni, 128, 0, c->stream>>>(c->pos, c->Z, ni, G.Lx, G.Ly, G.Lz, c->alpha, c->pp_part);
+    LAUNCHED(c);
+  }
+  const StressConst K{G.vol, G.dV, c->alpha, c->Q, c->C.E_ie0};
+  stress_finish_kernel<<<1, kStressThreads, 0, c->stream>>>((int)nb, c->partials, ni, c->pp_part, d_vel, c->mass, c->sc, K, c->stress);
+  LAUNCHED(c);
+  return ARCHE_OK;
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -696,6 +727,17 @@ extern "C" int arche_forces(arche_ctx *c, double *d_F) {
   int rc = compute_forces(c);
   if (rc) return rc;
   if (d_F && c->nions > 0) CK(cudaMemcpyAsync(d_F, c->F, 3 * c->nions * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  return ARCHE_OK;
+}
+
+extern "C" int arche_stress(arche_ctx *c, const double *d_vel, double *h_out) {
+  if (!c || !h_out) return ARCHE_EINVAL;
+  int rc = compute_stress(c, d_vel);
+  if (rc) return rc;
+  CK(cudaMemcpyAsync(c->h_stress, c->stress, kStressOut * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  if (c->prof) prof_harvest(c);
+  memcpy(h_out, c->h_stress, kStressOut * sizeof(double));
   return ARCHE_OK;
 }
 

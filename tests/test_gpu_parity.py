@@ -32,6 +32,21 @@ def _rel(a, b):
     return float(np.abs(a - b).max() / np.abs(b).max())
 
 
+TOL_STRESS = 1e-10
+
+
+def _check_stress(sg, so):
+    """every row of the 9 x 6 table and P, relative 1e-10 of the largest term entering (the total and the
+    off-diagonal components are sums with cancellation)"""
+    big = max(np.abs(so[k]).max() for k in so if k != "P")
+    for k in so:
+        if k == "P":
+            assert abs(sg[k] - so[k]) < TOL_STRESS * big, (k, sg[k], so[k])
+            continue
+        scale = big if k == "total" else max(np.abs(so[k]).max(), 1e-300)
+        assert np.abs(sg[k] - so[k]).max() <= TOL_STRESS * scale + 1e-16 * big, (k, sg[k], so[k])   # + round-off of rows that vanish
+
+
 def test_fermi_dirac_parity(orc, torch_cuda):
     cfg = ai.make_small()
     g = _gpu(cfg)
@@ -174,6 +189,8 @@ def test_full_size_configs_iterations_and_forces(orc, torch_cuda, name, iters):
     assert _rel(g.get_complex("nhat_a").cpu().numpy(), o.get_complex("nhat_a")) < TOL_N
     Fg = g.forces().cpu().numpy(); Fo = o.forces()
     assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max()
+    import torch
+    _check_stress(g.stress(torch.as_tensor(cfg["vel"], device="cuda")), o.stress(cfg["vel"]))
     dV = float(np.prod(cfg["cell"]) / np.prod(cfg["grid"]))
     assert abs(g.get_real("n_a").sum().item() * dV - cfg["Z"].sum()) < 1e-12 * cfg["Z"].sum()
 
@@ -215,6 +232,39 @@ def test_converged_solve_and_forces(orc, torch_cuda, pointwise_mode):
     r2 = g2.scf_solve(cfg["pos"])
     assert r2["converged"] == 1 and abs(r2["scf_iters"] - ro["scf_iters"]) <= 1
     assert _rel(g.get_complex("ghat").cpu().numpy(), o.get_complex("ghat")) < 1e-8
+
+
+@pytest.mark.parametrize("grid,cell,xc", [((24, 16, 18), [9.0, 7.5, 8.0], 1), ((12, 8, 9), [7.0, 7.6, 8.3], 1),
+                                          ((9, 27, 16), [6.5, 9.0, 8.0], 0), ((32, 32, 32), [9.0, 9.5, 10.0], 1)])
+def test_stress_tensor_and_pressure(orc, torch_cuda, grid, cell, xc):
+    """f1: all nine rows x six components + P against the oracle on a converged density; anisotropic
+    cells so that every off-diagonal component is non-zero; even sizes (Nyquist planes on every axis, where the half
+    spectrum needs S2 and the sign flips), odd sizes, mixed; with and without velocities."""
+    torch = torch_cuda
+    cfg = ai.make_small(n_ions=5, grid=grid, cell=cell, T_eV=10.0, seed=11, dmin=2.0)
+    cfg["xc"] = xc
+    g, o, rg, ro = _solve_pair(orc, cfg, scf_tol_dn=1e-10, init_mode=0)
+    so = o.stress(cfg["vel"])
+    sg = g.stress(torch.as_tensor(cfg["vel"], device="cuda"))
+    _check_stress(sg, so)
+    for row in ("pp", "pm", "ee", "ie", "i"):
+        assert np.abs(so[row][3:]).min() > 0          # the shear components are exercised
+    _check_stress(g.stress(), o.stress())
+    assert abs(sg["P"] + sg["total"][:3].sum() / 3) < 1e-15
+
+
+def test_stress_edge_cases(orc, torch_cuda):
+    from paper_2606_13283_b200 import ArcheError
+    cfg = dict(cell=[5.0, 6.0, 7.0], grid=[8, 12, 16], Z=np.zeros(0), mass=np.zeros(0), kT=0.4)
+    g = _gpu(cfg, n_electrons=9.0); o = orc.Oracle(cfg, n_electrons=9.0)
+    with pytest.raises(ArcheError):
+        g.stress()                                                  # before any solve
+    rg = g.scf_solve(np.zeros((0, 3))); ro = o.scf_solve(np.zeros((0, 3)))
+    sg, so = g.stress(), o.stress()                                 # uniform gas: only sigma^e and sigma^xc
+    _check_stress(sg, so)
+    assert abs(sg["P"] - (2 * rg["K_e"] / (3 * 210.0) - sg["xc"][0])) < 1e-15
+    for row in ("i", "pp", "pm", "je", "ie"):
+        assert np.all(sg[row] == 0), row
 
 
 def test_c1_md_trajectory(orc, torch_cuda):
