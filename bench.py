@@ -43,7 +43,8 @@ def bytes_per_point(nx, fused=True):
                 "mu_pass": 8,                  # per evaluation of N(mu): read V_i (L2/register-cached on small grids)
                 "density": 24 + h,             # read V_i, n_i; write n_a, work (r2c x pass with the density prologue)
                 "fft_fwd_z_reduce": 4 * h,     # read work, nhat_i, Vhat_ie; write nhat_a
-                "mix": 16 + 3 * h}
+                "mix": 16 + 3 * h,
+                "stress_fields": 3 * h + 8}    # f1: read nhat_a, S_Z, S2 and n_a once
     return {"potential_g": 5 * h,              # streaming: read nhat_i, nhat_a, Vhat_ie; write nhat_i, work
             "fft_inv_z_potential": 2 * h, "fft_y": 2 * h, "fft_inv_x_vi": h + 8,      # plain passes
             "vi_r": 40,                        # read V_H, n_i, n_a; write n_i, V_i
@@ -51,7 +52,8 @@ def bytes_per_point(nx, fused=True):
             "density_r": 24,                   # read V_i, n_i; write n_a
             "fft_fwd_x_real": 8 + h, "fft_fwd_z_reduce": 2 * h,                        # plain passes
             "reduce_g": 3 * h,                 # read nhat_a, nhat_i, Vhat_ie
-            "mix": 16 + 3 * h}
+            "mix": 16 + 3 * h,
+            "stress_fields": 3 * h + 8}
 
 
 # fp64 work per grid point of the arithmetic-bound classes, counted from the kernels (an FMA = 2 flops): one
@@ -216,6 +218,8 @@ def run_iteration_sweep(args):
     for _ in range(K):
         r = g.scf_iter()
     g.forces()
+    for _ in range(3):
+        g.stress()                                # f1: three launches of the field-sum kernel (the class time is their mean)
     prof = g.profile_get()
     g.profile_enable(False)
     evals_per_iter = r["mu_evals"] / K
@@ -344,6 +348,17 @@ def main():
     t_prof, iters_prof = timed_steps(args.steps, lambda: g.md_step(dt, pos2, vel2))
     prof = g.profile_get()
     g.profile_enable(False)
+    # ---- f1: stress tensor + pressure of the last step's state (reported beside the step, not inside its timed region)
+    for _ in range(3):
+        g.stress(vel2)
+    s0 = torch.cuda.Event(enable_timing=True); s1 = torch.cuda.Event(enable_timing=True)
+    ls = g.launch_count()
+    s0.record(g.stream)
+    for _ in range(10):
+        st = g.stress(vel2)
+    s1.record(g.stream); torch.cuda.synchronize()
+    stress = {"ms_per_call": s0.elapsed_time(s1) / 10, "launches_per_call": (g.launch_count() - ls) / 10,
+              "pressure_Ha_per_bohr3": st["P"], "note": "arche_stress incl. its D2H of 55 doubles; outside the timed MD step"}
 
     t_dev_max, t_e2e_max = max_over_ranks([t_dev, t_e2e], device=dev)
     if rank != 0:
@@ -404,7 +419,7 @@ def main():
                     "h2d_bytes_per_step": 2 * 3 * g.n_ions * 8, "d2h_bytes_per_step": 3 * 3 * g.n_ions * 8 + 136,
                     "scf_iters_per_step": iters_e2e / args.steps},
             "gpu_launches": int(launches),
-            "mu_evals_per_iter": evals_per_iter, "roofline": roof, "kernels": kernels}
+            "mu_evals_per_iter": evals_per_iter, "roofline": roof, "kernels": kernels, "stress": stress}
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = oracle_sample(cfg, args.workload, iters=2, iters_per_step=iters / args.steps)
     print(json.dumps(line))
