@@ -17,8 +17,10 @@ def test_bytes_per_point_models():
     h = 16.0 * 200 / 384
     assert abs(streamed["potential_g"] - 5 * h) < 1e-12 and streamed["vi_r"] == 40 and streamed["density_r"] == 24
     assert "density" not in streamed and "potential_g" not in fused
+    assert abs(streamed["stress_fields"] - (3 * h + 8)) < 1e-12       # f1: once per stress call, not per iteration
     # one SCF iteration of the streamed form moves 18 h + 80 (+ 8 per mu evaluation) bytes per point
-    per_iter = sum(streamed[k] * (2 if k == "fft_y" else 1) for k in streamed if k not in ("mix", "mu_pass"))
+    per_iter = sum(streamed[k] * (2 if k == "fft_y" else 1) for k in streamed
+                   if k not in ("mix", "mu_pass", "stress_fields"))
     assert abs(per_iter - (18 * h + 80)) < 1e-9
 
 
