@@ -254,10 +254,29 @@ __device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &g
           else mu_accumulate4<false>(s_tab, vv, ok, mu, inv_kT, s1, s0);
         }
       } else {
-        for (long long g0 = tid; g0 < ng; g0 += 4 * nthreads) {
+        // two groups of four loads stay in flight ahead of the evaluation (with 16-24 warps per SM the exposed HBM
+        // latency, not the table reads, bounded this loop)
+        double va[4], vb[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const long long ga = tid + q * nthreads, gb = ga + 4 * nthreads;
+          va[q] = ga < ng ? V_i[ga] : 0.0; vb[q] = gb < ng ? V_i[gb] : 0.0;
+        }
+        for (long long g0 = tid; g0 < ng; g0 += 8 * nthreads) {
           double vv[4]; bool ok[4];
 #pragma unroll
-          for (int q = 0; q < 4; ++q) { const long long g = g0 + q * nthreads; ok[q] = g < ng; vv[q] = ok[q] ? V_i[g] : 0.0; }
+          for (int q = 0; q < 4; ++q) {
+            const long long g = g0 + q * nthreads, gn = g + 8 * nthreads;
+            ok[q] = g < ng; vv[q] = va[q]; va[q] = gn < ng ? V_i[gn] : 0.0;
+          }
+          if (want_slope) mu_accumulate4<true>(s_tab, vv, ok, mu, inv_kT, s1, s0);
+          else mu_accumulate4<false>(s_tab, vv, ok, mu, inv_kT, s1, s0);
+          if (g0 + 4 * nthreads >= ng) break;
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const long long g = g0 + (4 + q) * nthreads, gn = g + 8 * nthreads;
+            ok[q] = g < ng; vv[q] = vb[q]; vb[q] = gn < ng ? V_i[gn] : 0.0;
+          }
           if (want_slope) mu_accumulate4<true>(s_tab, vv, ok, mu, inv_kT, s1, s0);
           else mu_accumulate4<false>(s_tab, vv, ok, mu, inv_kT, s1, s0);
         }
@@ -301,13 +320,13 @@ __device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &g
   return mu;   // identical in every thread of the grid
 }
 
-__global__ void __launch_bounds__(256) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
+__global__ void __launch_bounds__(256, 3) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
                                                        DevScalars *sc, const double *__restrict__ fdtab,
                                                        double *partials, int max_pass, const int *stop) {
   namespace cg = cooperative_groups;
   if (stop && *stop) return;   // uniform over the grid: no block reaches a barrier
   cg::grid_group grid = cg::this_grid();
-  __shared__ double s_tab[kFdTabDoubles];
+  __shared__ __align__(16) double s_tab[kFdTabDoubles];
   __shared__ double s_red[2 * 32 + 2];
   __shared__ double s_bc[2];
   fd_load_tables(s_tab, fdtab);
@@ -683,7 +702,7 @@ __global__ void compress_half_kernel(double2 *__restrict__ dst, const double2 *_
 }
 
 __global__ void fermi_dirac_kernel(int twice_j, const double *eta, double *out, size_t n, const double *fdtab) {
-  __shared__ double s_tab[kFdTabDoubles];
+  __shared__ __align__(16) double s_tab[kFdTabDoubles];
   fd_load_tables(s_tab, fdtab);
   __syncthreads();
   for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < n; g += (size_t)gridDim.x * blockDim.x) {

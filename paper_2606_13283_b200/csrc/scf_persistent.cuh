@@ -62,7 +62,7 @@ template <int NX, int NY, int NZ>
 __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_persistent_kernel(PersistParams p) {
   namespace cg = cooperative_groups;
   cg::grid_group grid = cg::this_grid();
-  extern __shared__ double smem[];
+  extern __shared__ __align__(16) double smem[];
   double *s_tab = smem;
   double *s_red = s_tab + kFdTabDoubles;
   double *s_bc = s_red + 10 * 33;
