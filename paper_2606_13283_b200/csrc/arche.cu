@@ -450,6 +450,8 @@ int scf_iteration(arche_ctx *c) {
   const int pmax = c->ew_grid * 2;
   auto fit = [&](long long work) { long long b = (work + 255) / 256; return (int)(b < c->sm_count ? c->sm_count : (b > pmax ? pmax : b)); };
   const int pg = fit(c->nh / 4), pr = fit(c->ng / 4);
+  // real-space Fermi-Dirac kernels of the streamed form: table in shared memory, co-resident blocks only
+  auto prt = [&](int per_sm) { const int b = c->sm_count * per_sm; return pr < b ? pr : b; };
   // S1 + S2 (+ the pending S6 of the previous iteration, + the first mu evaluation)
   LoadPotentialG lp;
   lp.nh_i = c->nh_i; lp.nh_a = c->nh_a; lp.vh_ie = c->vh_ie; lp.kx2 = c->kx2; lp.ky2 = c->ky2; lp.kz2 = c->kz2;
@@ -467,7 +469,7 @@ int scf_iteration(arche_ctx *c) {
     rc = fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{c->V_i}, PC_FFT_INV_Z, PC_FFT_INV_X);
     if (rc) return rc;
     { ProfScope ps(c, PC_VI_R);
-      pointwise_r_kernel<<<pr, 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop); LAUNCHED(c); }
+      pointwise_r_kernel<LoadReal, StoreVi, true><<<prt(4), 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
   }
   c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
@@ -491,7 +493,7 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_DENS_R);
-      pointwise_r_kernel<<<pr, 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop); LAUNCHED(c); }
+      pointwise_r_kernel<LoadDensity, StoreNull, true><<<prt(3), 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
     rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
     if (rc) return rc;
     { ProfScope ps(c, PC_RED_G);

@@ -133,6 +133,7 @@ struct StoreVi {
   int xc, mix;
   double w, mu0, acc_min, acc_max, acc_sum, acc_n;
   int have_mu;
+  __device__ __forceinline__ void set_table(const double *t) { fdtab = t; }
   __device__ __forceinline__ void begin() {
     w = mix ? sc->w : 1.0;
     have_mu = sc->mu_have_prev; mu0 = sc->mu;
@@ -345,6 +346,7 @@ struct LoadDensity {
   const double *fdtab;
   ScfConst C;
   double mu, inv_kT, sK, sdn2, sna2, sF0, sKe, sExc, sChi;
+  __device__ __forceinline__ void set_table(const double *t) { fdtab = t; }
   __device__ __forceinline__ void begin() {
     mu = sc->mu; inv_kT = 1.0 / C.kT;
     sK = sdn2 = sna2 = sF0 = sKe = sExc = sChi = 0.0;
@@ -405,6 +407,7 @@ struct LoadDensity {
 // ---- S5: forward FFT of the real n_a; the z-pass epilogue scales by dV, stores nhat_a, reduces U, E_H, E_ie ------
 struct LoadReal {
   const double *src;
+  __device__ __forceinline__ void set_table(const double *) {}
   __device__ __forceinline__ void begin() {}
   __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(src + idx); }
   __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) { re = src[idx]; im = 0.0; }
@@ -627,6 +630,7 @@ struct StoreRealPlain {
 // little parallelism for their extra operand streams (z passes) and their Fermi-Dirac/XC arithmetic (x passes).
 // There the same functors run in these grid-stride kernels at full occupancy, around plain FFT passes.
 struct StoreNull {
+  __device__ __forceinline__ void set_table(const double *) {}
   __device__ __forceinline__ void begin() {}
   __device__ __forceinline__ void store_real2(long long, long long, double, double) {}
   __device__ __forceinline__ void finish(double *) {}
@@ -651,13 +655,22 @@ __global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp 
   st.finish(s_red);
 }
 
-// real fields, two elements per thread and step (the functors interleave their two Fermi-Dirac evaluations); ng even
-template <class LoadOp, class StoreOp>
-__global__ void __launch_bounds__(256) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng, const int *stop) {
+// real fields, two elements per thread and step (the functors interleave their two Fermi-Dirac evaluations); ng even.
+// SMEM_TAB: the block first copies the Fermi-Dirac table (g_tab) to shared memory and the functors read it there --
+// for the streamed form, launched with as many blocks as are co-resident (the table copy is paid once per block).
+template <class LoadOp, class StoreOp, bool SMEM_TAB = false>
+__global__ void __launch_bounds__(256) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng, const int *stop,
+                                                          const double *__restrict__ g_tab = nullptr) {
   __shared__ double s_red[kMaxRed * 33];
+  __shared__ __align__(16) double s_tab[SMEM_TAB ? kFdTabDoubles : 2];
   if (stop && *stop) return;
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  if (SMEM_TAB) {
+    fd_load_tables(s_tab, g_tab);
+    __syncthreads();
+    ld.set_table(s_tab); st.set_table(s_tab);
+  }
   ld.begin(); st.begin();
   const long long half = ng / 2;
   for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < half; g += (long long)gridDim.x * blockDim.x) {
