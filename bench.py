@@ -396,7 +396,7 @@ def main():
                 "share_of_step": round(t_scf * 1e3 / tot_prof, 4), "bytes_per_iteration": bpi,
                 "us_per_iteration": round(1e6 * t_scf / n_it, 2)}
         # DRAM bytes of ONE launch (= one solve) from the committed ncu --set full capture of this workload
-        ncu_traffic = {"c2": (7.526e6 + 0.778e6, "profiles/r01e_c2_ncu_full.csv")}
+        ncu_traffic = {"c2": (7.530e6 + 0.969e6, "profiles/r01k_c2_ncu_full.csv")}
         if args.workload in ncu_traffic:
             roof["traffic"], roof["traffic_source"] = ncu_traffic[args.workload]
             roof["algorithmic_bytes_per_launch"] = bpi * iters / max(args.steps, 1)
