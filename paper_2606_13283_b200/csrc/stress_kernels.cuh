@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(kStressThreads) stress_fields_kernel(
   for (int q = 0; q < kStressSums; ++q) acc[q] = 0.0;
   const unsigned int P = (unsigned int)G.P, ny = (unsigned int)G.ny;
   const int nyq_x = (G.nx % 2 == 0) ? G.nx / 2 : -1, nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
-  const double pi2_a2 = ARCHE_PI * ARCHE_PI / (alpha * alpha), inv_pi = 1.0 / ARCHE_PI, two_pi_rc = 2.0 * ARCHE_PI * rc;
+  const double pi2_a2 = ARCHE_PI * ARCHE_PI / (alpha * alpha), inv_pi = 1.0 / ARCHE_PI, two_rc = 2.0 * rc;
   const long long stride = (long long)gridDim.x * blockDim.x;
   for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < G.nh; g += stride) {
     const unsigned int ug = (unsigned int)g, ix = ug % P, row = ug / P, iy = row % ny, iz = row / ny;
@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(kStressThreads) stress_fields_kernel(
     const double k2 = kx * kx + ky * ky + kz * kz;
     if (k2 == 0.0) continue;
     const double2 n = nh_a[g], s1 = S[g], s2 = S2[g];
-    const double ik2 = 1.0 / k2, ka = sqrt(k2);
+    const double ik = rsqrt(k2), ik2 = ik * ik, ka = k2 * ik;   // one reciprocal square root instead of sqrt + three divisions
     const double hw = ((int)ix == 0 || (int)ix == nyq_x) ? 0.5 : 1.0;   // wt(ix)/2
     const bool fx = (int)ix == nyq_x, fy = (int)iy == nyq_y, fz = (int)iz == nyq_z;
     const double sg[3] = {(fy != fz) ? -1.0 : 1.0, (fx != fz) ? -1.0 : 1.0, (fx != fy) ? -1.0 : 1.0};   // yz, xz, xy
@@ -52,8 +52,8 @@ __global__ void __launch_bounds__(kStressThreads) stress_fields_kernel(
     const double e = (n.x * n.x + n.y * n.y) * inv_pi * ik2;
     // Re(nhat conj(S_Z)) v'(k) k_m k_n/|k|, v(k) = -cos(2 pi k rc)/(pi k^2)
     double sn, cs;
-    sincos(two_pi_rc * ka, &sn, &cs);
-    const double dv_k = (2.0 * rc * sn * ik2 + 2.0 * cs * inv_pi * ik2 / ka) / ka;
+    sincospi(two_rc * ka, &sn, &cs);
+    const double dv_k = (2.0 * rc * sn * ik2 + 2.0 * cs * inv_pi * ik2 * ik) * ik;
     const double b1 = dv_k * (n.x * s1.x + n.y * s1.y), b2 = dv_k * (n.x * s2.x + n.y * s2.y);
     acc[0] += hw * (a1 + a2);
     acc[7] += 2.0 * hw * e;
