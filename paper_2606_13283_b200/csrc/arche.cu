@@ -469,7 +469,7 @@ int scf_iteration(arche_ctx *c) {
     rc = fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{c->V_i}, PC_FFT_INV_Z, PC_FFT_INV_X);
     if (rc) return rc;
     { ProfScope ps(c, PC_VI_R);
-      pointwise_r_kernel<LoadReal, StoreVi, true><<<prt(4), 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
+      pointwise_r_kernel<LoadReal, StoreVi, true, 4><<<prt(4), 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
   }
   c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
@@ -493,7 +493,7 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_DENS_R);
-      pointwise_r_kernel<LoadDensity, StoreNull, true><<<prt(3), 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
+      pointwise_r_kernel<LoadDensity, StoreNull, true, 4><<<prt(4), 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
     rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
     if (rc) return rc;
     { ProfScope ps(c, PC_RED_G);

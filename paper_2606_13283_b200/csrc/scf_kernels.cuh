@@ -658,8 +658,8 @@ __global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp 
 // real fields, two elements per thread and step (the functors interleave their two Fermi-Dirac evaluations); ng even.
 // SMEM_TAB: the block first copies the Fermi-Dirac table (g_tab) to shared memory and the functors read it there --
 // for the streamed form, launched with as many blocks as are co-resident (the table copy is paid once per block).
-template <class LoadOp, class StoreOp, bool SMEM_TAB = false>
-__global__ void __launch_bounds__(256) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng, const int *stop,
+template <class LoadOp, class StoreOp, bool SMEM_TAB = false, int MIN_BLOCKS = 1>
+__global__ void __launch_bounds__(256, MIN_BLOCKS) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng, const int *stop,
                                                           const double *__restrict__ g_tab = nullptr) {
   __shared__ double s_red[kMaxRed * 33];
   __shared__ __align__(16) double s_tab[SMEM_TAB ? kFdTabDoubles : 2];
