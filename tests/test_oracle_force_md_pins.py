@@ -106,3 +106,25 @@ def test_one_center_init_reduces_iterations(orc):
         pos[:, 0] += 0.05
         its[mode] = o.scf_solve(pos)["scf_iters"]
     assert its[1] < its[0]
+
+
+def test_structure_factor_and_ionic_potential_do_not_depend_on_the_grid(orc):
+    """S_Z(k) = sum_j Z_j exp(-2 pi i k.R_j) and Vhat_ie(k) = v(k) S_Z(k) are functions of the
+    integer wave vector m (k = m/L) and the ions only: the same cell on an 8^3 and a 12 x 10 x 14 grid must give the
+    same values at every |m_i| <= 3 (off both grids' Nyquist planes).  This is what the sampled full-size GPU test of
+    the c5 sweep relies on."""
+    cfg = ai.make_config("c1")
+    a = dict(cfg); a["grid"] = np.array([8, 8, 8])
+    b = dict(cfg); b["grid"] = np.array([12, 10, 14])
+    oa = orc.Oracle(a); ob = orc.Oracle(b)
+    oa.scf_begin(cfg["pos"]); ob.scf_begin(cfg["pos"])
+    m = np.arange(-3, 4)
+    for name in ("S_Z", "Vhat_ie"):
+        fa = oa.get_complex(name)[np.ix_(m % 8, m % 8, m % 8)]          # [iz][iy][ix]
+        fb = ob.get_complex(name)[np.ix_(m % 14, m % 10, m % 12)]
+        assert np.abs(fa - fb).max() <= 1e-13 * np.abs(fb).max(), name
+    # and the definition itself at one wave vector, written out
+    mz, my, mx = 2, -1, 3
+    k = np.array([mx, my, mz]) / np.asarray(cfg["cell"])
+    direct = np.sum(cfg["Z"] * np.exp(-2j * np.pi * (cfg["pos"] @ k)))
+    assert abs(oa.get_complex("S_Z")[mz % 8, my % 8, mx % 8] - direct) < 1e-12 * abs(cfg["Z"].sum())
