@@ -40,7 +40,8 @@ typedef struct {
   double psp_rc;         /* Ashcroft empty-core radius in bohr (BASELINE.json: 1.12) */
   int init_mode;         /* 0: uniform input density each step; 1: one-center profile */
   int mix_mode;          /* 0: fixed w; 1: More et al. w = U/(K+U) */
-  double mix_w_fixed;    /* n_o = n_a + w (n_i - n_a) */
+  double mix_w_fixed;    /* n_o = n_a + w (n_i - n_a); <= 0: automatic, the largest single-mode value
+                            lambda/(1+lambda), lambda = chi0/(pi k_min^2) (reading A11d) */
   int mix_warmup;        /* SCF iterations run with mix_w_fixed before More's w is used */
   double scf_tol_F;      /* stop when |F_k - F_{k-1}| < scf_tol_F (Ha) ... */
   double scf_tol_dn;     /* ... and ||n_i - n_a||_L2 / ||n_a||_L2 < scf_tol_dn */
@@ -48,6 +49,8 @@ typedef struct {
   int scf_fixed_iter;    /* > 0: run exactly this many iterations (parity replay) */
   double ewald_alpha;    /* <= 0: automatic (reading A18) */
   double n_electrons;    /* <= 0: sum_j Z_j (neutral cell); > 0: that many electrons on a uniform background */
+  double mix_mu_tol;     /* > 0: More's w is used only once two successive mu_a differ by <= mix_mu_tol kT ("once the
+                            chemical potential fluctuations are small"; latched; reading A11b); <= 0: off */
   void *d_workspace;     /* device memory, >= arche_workspace_bytes(), 256-byte aligned */
   size_t workspace_bytes;
   void *stream;          /* cudaStream_t (0 = default stream) */
@@ -60,7 +63,9 @@ typedef struct {
   double K_e, K_i;                             /* Eq. 38 and Eq. 36 */
   double dn_l2;                                /* ||n_i - n_a|| / ||n_a|| of the last iteration */
   double w_last, U_mix, K_mix;                 /* Eq. 30-31 */
+  double tol_F_eff, tol_dn_eff;                /* the tolerances the stop rule applied in the last iteration (reading A13) */
   int scf_iters, mu_evals, converged;
+  int flip_seen;                               /* 1: a PZ81 branch flip was detected and the tolerances were widened (A13) */
 } arche_result;
 
 /* Bytes of device workspace arche_scf_init will carve up for these parameters (0 on bad parameters). */
@@ -101,7 +106,9 @@ int arche_stress(arche_ctx *c, const double *d_vel, double *h_out);
 
 /* One velocity-Verlet step of length dt (a.u.) (reading D2): half kick, drift, SCF solve at the
  * new positions, forces, half kick.  d_pos/d_vel [n_ions*3] are updated in place.  The first call also solves
- * at the starting positions to obtain the initial forces. */
+ * at the starting positions to obtain the initial forces.  Later calls reuse the forces of the previous step: a caller
+ * that edits the positions between two steps must call arche_scf_solve + arche_forces on them first.
+ * Returns ARCHE_ENOCONV when either solve of the step hit scf_max_iter (the step is still taken). */
 int arche_md_step(arche_ctx *c, double dt, double *d_pos, double *d_vel, arche_result *h_out);
 /* Same step through HOST buffers: positions/velocities are copied in, the step runs, positions, velocities and
  * forces (h_F may be NULL) are copied back -- the paper's per-step host<->device traffic. */
@@ -144,6 +151,13 @@ int arche_is_fused(const arche_ctx *c);
  * the profile classes 0-6 then receive the phase times block 0 measures with %globaltimer) */
 int arche_is_persistent(const arche_ctx *c);
 int arche_profile_get(arche_ctx *c, int cls, double *h_ms_total, long long *h_launches);
+
+/* Measured rooflines for the fractions bench.py reports (peak_kernels.cuh): the fp64 FMA rate of the
+ * vector pipe -- independent dependent-FMA chains on every SM, launched back to back for `seconds` (>= 1 for a
+ * sustained figure); h_tflops[0] = sustained over the whole run, h_tflops[1] = best single launch; *h_ms (optional) = the
+ * time it ran -- and the L2 read bandwidth in GB/s of a <= 32 MiB slice of the workspace swept 64 times. */
+int arche_peak_fp64(arche_ctx *c, double seconds, double *h_tflops /*[2]*/, double *h_ms);
+int arche_peak_l2(arche_ctx *c, double *h_gbs);
 
 #ifdef __cplusplus
 }

@@ -35,14 +35,14 @@ class Params(C.Structure):
                 ("mix_mode", C.c_int), ("mix_w_fixed", C.c_double), ("mix_warmup", C.c_int),
                 ("scf_tol_F", C.c_double), ("scf_tol_dn", C.c_double), ("scf_max_iter", C.c_int),
                 ("scf_fixed_iter", C.c_int), ("ewald_alpha", C.c_double),
-                ("n_electrons", C.c_double)]
+                ("n_electrons", C.c_double), ("mix_mu_tol", C.c_double)]
 
 
 class Result(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "E_ie0",
                                           "U_ii", "K_e", "K_i", "dn_l2", "w_last", "U_mix",
-                                          "K_mix")] + \
-               [(k, C.c_int) for k in ("scf_iters", "mu_evals", "converged")]
+                                          "K_mix", "tol_F_eff", "tol_dn_eff")] + \
+               [(k, C.c_int) for k in ("scf_iters", "mu_evals", "converged", "flip_seen")]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -75,6 +75,7 @@ def lib():
         L.oracle_destroy.argtypes = [C.c_void_p]
         L.oracle_scf_begin.argtypes = [C.c_void_p, dp]
         L.oracle_set_input_density.argtypes = [C.c_void_p, dp]
+        L.oracle_set_profile.argtypes = [C.c_void_p, dp]
         L.oracle_scf_iter.argtypes = [C.c_void_p, C.POINTER(Result)]
         L.oracle_scf_solve.argtypes = [C.c_void_p, dp, C.POINTER(Result)]
         L.oracle_forces.argtypes = [C.c_void_p, dp]
@@ -171,7 +172,7 @@ class Oracle:
     def __init__(self, cfg: dict, **over):
         p = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=3,
                  scf_tol_F=1e-10, scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0,
-                 ewald_alpha=0.0, n_electrons=0.0)
+                 ewald_alpha=0.0, n_electrons=0.0, mix_mu_tol=0.0)
         for k in p:
             if k in cfg:
                 p[k] = cfg[k]
@@ -207,6 +208,11 @@ class Oracle:
 
     def set_input_density(self, n_i):
         lib().oracle_set_input_density(self._h, _dp(_f64(n_i)))
+
+    def set_profile(self, ghat):
+        g = np.ascontiguousarray(ghat, dtype=np.complex128)
+        assert g.shape == self.shape
+        lib().oracle_set_profile(self._h, _dp(g.view(np.float64)))
 
     def scf_iter(self) -> dict:
         r = Result()

@@ -343,7 +343,10 @@ struct oracle_ctx {
   int have_g, have_solution, have_forces;
   int warmup_eff; /* mix_warmup applies only to a uniform start (reading A11) */
   int flip_seen;  /* a PZ81 branch flip was detected in this solve (reading A13) */
-  double dF_prev; /* |F_{k-1} - F_{k-2}| */
+  int more_on;    /* More's w has been switched on in this solve (reading A11b) */
+  double mu_iter_prev;
+  double w_fixed; /* mix_w_fixed, or lambda/(1+lambda) when that is <= 0 (reading A11d) */
+  double dF_prev; /* F_{k-1} - F_{k-2} (signed) */
   oracle_result last;
 };
 
@@ -379,6 +382,15 @@ int oracle_init(const oracle_params *p, oracle_ctx **out) {
   double asum = 0.0;
   for (int j = 0; j < n; ++j) asum += 2.0 * PI * c->Z[j] * p->psp_rc * p->psp_rc;
   c->E_ie0 = c->Ne / c->vol * asum;
+  {
+    /* uniform-gas response chi0 = dn/dmu at n0 = Ne/|Omega| (d/dmu of Eq. 9, I_j' = j I_{j-1}); the largest single-mode
+     * value of More's w is lambda/(1+lambda) with lambda = chi0/(pi k_min^2), k_min = 1/L_max (reading A11d) */
+    double eta0 = oracle_fd_half_inverse(c->Ne / (c->vol * c->cTF));
+    double chi0 = c->cTF * 0.5 * oracle_fd(-1, eta0) / p->kT;
+    double Lmax = fmax(p->cell[0], fmax(p->cell[1], p->cell[2]));
+    double lam = chi0 * Lmax * Lmax / PI;
+    c->w_fixed = p->mix_w_fixed > 0.0 ? p->mix_w_fixed : lam / (1.0 + lam);
+  }
   size_t ng = c->ng;
   c->n_i = (double *)calloc(ng, sizeof(double));
   c->n_a = (double *)calloc(ng, sizeof(double));
@@ -431,6 +443,13 @@ int oracle_set_input_density(oracle_ctx *c, const double *n_i) {
   return 0;
 }
 
+/* test hook: supply the one-center profile ghat directly instead of taking it from a solve */
+int oracle_set_profile(oracle_ctx *c, const double *ghat_complex) {
+  memcpy(c->gh, ghat_complex, sizeof(cplx) * c->ng);
+  c->have_g = 1;
+  return 0;
+}
+
 int oracle_scf_begin(oracle_ctx *c, const double *pos) {
   int n = c->p.n_ions;
   memcpy(c->pos, pos, sizeof(double) * 3 * n);
@@ -468,9 +487,11 @@ int oracle_scf_begin(oracle_ctx *c, const double *pos) {
   c->have_solution = 0;
   c->have_forces = 0;
   c->flip_seen = 0;
+  c->more_on = 0;
   c->last.scf_iters = 0;
   c->last.mu_evals = 0;
   c->last.converged = 0;
+  c->last.flip_seen = 0;
   c->last.F_total = 0.0;
   return 0;
 }
@@ -575,22 +596,27 @@ int oracle_scf_iter(oracle_ctx *c, oracle_result *out) {
   double Ftot = F0 + Exc + EH + Eie + c->E_ie0 + c->U_ii;
   /* S6: mixing n_o = n_a + w (n_i - n_a), w = U/(K+U) */
   int it = c->last.scf_iters + 1;
+  /* "w is computed and updated only after a few SCF iterations, once the chemical potential
+   * fluctuations are small" -- reading A11b: after the warm-up count and, when mix_mu_tol > 0, once two successive
+   * mu_a differ by at most mix_mu_tol kT (latched for the rest of the solve) */
+  if (c->p.mix_mu_tol > 0.0 && !c->more_on && it >= 2 && fabs(mu - c->mu_iter_prev) <= c->p.mix_mu_tol * kT) c->more_on = 1;
+  c->mu_iter_prev = mu;
   double w;
-  if (c->p.mix_mode == 1 && it > c->warmup_eff) w = (K + U > 0.0) ? U / (K + U) : 0.0;
-  else w = c->p.mix_w_fixed;
+  if (c->p.mix_mode == 1 && it > c->warmup_eff && (c->p.mix_mu_tol <= 0.0 || c->more_on)) w = (K + U > 0.0) ? U / (K + U) : 0.0;
+  else w = c->w_fixed;
   for (size_t g = 0; g < ng; ++g) {
     c->n_i[g] = c->n_a[g] + w * (c->n_i[g] - c->n_a[g]);
     c->nh_i[g] = c->nh_a[g] + w * (c->nh_i[g] - c->nh_a[g]);
   }
   /* S7: convergence (reading D4) */
   double dn_rel = sqrt((double)sdn2 / (double)sna2);
-  double dF = fabs(Ftot - c->last.F_total);
+  double dFs = Ftot - c->last.F_total, dF = fabs(dFs);
   oracle_result r = c->last;
   /* DESIGN.md reading A13: the published PZ81 branches differ by 3.2e-5 Ha (eps_c) / 2.7e-5 Ha (V_c) at r_s = 1,
    * n* = 3/(4 pi).  A grid point sitting on n* flips branch between iterations: F moves by whole quanta
    * q_F = (eps_c jump) n* dV and the density answers the V_c jump with a limit cycle of relative size
-   * q_dn/||n_a||.  A jump of F by an integer number (1..8) of quanta right after a change far below one quantum
-   * marks the solve; from then on two quanta are tolerated in both criteria. */
+   * q_dn/||n_a||.  A jump of F by an integer number (1..8) of quanta marks the solve under the two conditions below;
+   * from then on two quanta are tolerated in both criteria. */
   double tolF = c->p.scf_tol_F, toldn = c->p.scf_tol_dn;
   if (c->p.xc == 1) {
     double nstar = 0.75 / PI, den = 1.0 + 1.0529 + 0.3334, ec_hi = -0.1423 / den, ec_lo = -0.048 - 0.0116;
@@ -599,15 +625,19 @@ int oracle_scf_iter(oracle_ctx *c, oracle_result *out) {
     double q_F = fabs(ec_hi - ec_lo) * nstar * dV;
     double chi_star = cTF * 0.5 * oracle_fd(-1, oracle_fd_half_inverse(nstar / cTF)) / kT;
     double q_dn = chi_star * fabs(vc_hi - vc_lo) * sqrt(dV);
-    if (it >= 3) { /* a jump: the previous change of F was far below one quantum */
-      double m = dF / q_F, rr = rint(m), mp = c->dF_prev / q_F, rp = rint(mp);
+    if (it >= 3) {
+      double m = dF / q_F, rr = rint(m), mp = fabs(c->dF_prev) / q_F, rp = rint(mp);
       int near = rr >= 1.0 && rr <= 8.0 && fabs(m - rr) < 0.02, near_prev = rp >= 1.0 && rp <= 8.0 && fabs(mp - rp) < 0.02;
-      if (near && (mp < 0.1 || near_prev)) c->flip_seen = 1; /* after a quiet change, or twice in a row */
+      /* (a) a quantised jump right after a change far below one quantum, or (b) the same multiple twice in a row with
+       * opposite signs (F hops back).  A converging solve lowers F monotonically, so (b) cannot fire on a smooth,
+       * even very slow, decay. */
+      if (near && (mp < 0.1 || (near_prev && rr == rp && dFs * c->dF_prev < 0.0))) c->flip_seen = 1;
     }
     if (c->flip_seen) { tolF += 2.02 * q_F; toldn += 2.0 * q_dn / sqrt((double)sna2 * dV); }
   }
   r.converged = (it >= 2 && dF < tolF && dn_rel < toldn);
-  c->dF_prev = dF;
+  r.tol_F_eff = tolF; r.tol_dn_eff = toldn; r.flip_seen = c->flip_seen;
+  c->dF_prev = dFs;
   r.mu = mu; r.F_total = Ftot; r.F0 = F0; r.E_H = EH; r.E_xc = Exc; r.E_ie = Eie; r.E_ie0 = c->E_ie0;
   r.U_ii = c->U_ii; r.K_e = Ke; r.dn_l2 = dn_rel; r.w_last = w; r.U_mix = U; r.K_mix = K;
   r.scf_iters = it; r.mu_evals += evals;

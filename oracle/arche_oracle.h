@@ -35,7 +35,7 @@ typedef struct {
   double psp_rc;       /* Ashcroft empty-core radius (bohr) */
   int init_mode;       /* 0 uniform density every step, 1 one-center profile */
   int mix_mode;        /* 0 fixed w, 1 More et al. w = U/(K+U) */
-  double mix_w_fixed;  /* n_o = n_a + w (n_i - n_a) */
+  double mix_w_fixed;  /* n_o = n_a + w (n_i - n_a); <=0: lambda/(1+lambda), lambda = chi0/(pi k_min^2) (reading A11d) */
   int mix_warmup;      /* iterations with the fixed w before More's w */
   double scf_tol_F;    /* Ha */
   double scf_tol_dn;   /* relative L2 */
@@ -44,11 +44,14 @@ typedef struct {
   double ewald_alpha;  /* <=0: auto */
   double n_electrons;  /* <=0: sum_j Z_j (neutral cell); >0: that many electrons on a
                           uniform neutralising background (uniform-gas and linear-response pins) */
+  double mix_mu_tol;   /* >0: More's w only once |mu_k - mu_{k-1}| <= mix_mu_tol kT (reading A11b) */
 } oracle_params;
 
 typedef struct {
   double mu, F_total, F0, E_H, E_xc, E_ie, E_ie0, U_ii, K_e, K_i, dn_l2, w_last, U_mix, K_mix;
+  double tol_F_eff, tol_dn_eff; /* tolerances the stop rule applied (reading A13) */
   int scf_iters, mu_evals, converged;
+  int flip_seen;                /* a PZ81 branch flip was detected in this solve (reading A13) */
 } oracle_result;
 
 /* --- primitives ------------------------------------------------------------------------ */
@@ -75,6 +78,9 @@ int oracle_init(const oracle_params *p, oracle_ctx **out);
 void oracle_destroy(oracle_ctx *c);
 /* per-MD-step ion-grid work + input-density initialisation for positions pos[n_ions*3] */
 int oracle_scf_begin(oracle_ctx *c, const double *pos);
+/* supply the one-center profile ghat [Nz][Ny][Nx] complex directly (pin of the clip/renormalise rule
+ * of DESIGN.md reading A10); the next oracle_scf_begin with init_mode = 1 starts from S_Z ghat (Eq. 20) */
+int oracle_set_profile(oracle_ctx *c, const double *ghat_complex);
 /* supply the input density explicitly (real field); n_hat_i is recomputed by FFT */
 int oracle_set_input_density(oracle_ctx *c, const double *n_i);
 /* one SCF iteration (PAPER.md:217-231 + 257-311) from the current input density */

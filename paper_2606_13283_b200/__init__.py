@@ -20,7 +20,8 @@ SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_la
            "arche_scf_begin", "arche_scf_iter", "arche_set_input_density", "arche_forces", "arche_stress", "arche_md_step",
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
            "arche_rfft3d_forward", "arche_rfft3d_inverse",
-           "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused", "arche_is_persistent"]
+           "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused", "arche_is_persistent",
+           "arche_peak_fp64", "arche_peak_l2"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
 
@@ -35,14 +36,15 @@ class Params(C.Structure):
                 ("psp_rc", C.c_double), ("init_mode", C.c_int), ("mix_mode", C.c_int),
                 ("mix_w_fixed", C.c_double), ("mix_warmup", C.c_int), ("scf_tol_F", C.c_double),
                 ("scf_tol_dn", C.c_double), ("scf_max_iter", C.c_int), ("scf_fixed_iter", C.c_int),
-                ("ewald_alpha", C.c_double), ("n_electrons", C.c_double), ("d_workspace", C.c_void_p),
+                ("ewald_alpha", C.c_double), ("n_electrons", C.c_double), ("mix_mu_tol", C.c_double),
+                ("d_workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p)]
 
 
 class Result(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "E_ie0", "U_ii", "K_e",
-                                          "K_i", "dn_l2", "w_last", "U_mix", "K_mix")] + \
-               [(k, C.c_int) for k in ("scf_iters", "mu_evals", "converged")]
+                                          "K_i", "dn_l2", "w_last", "U_mix", "K_mix", "tol_F_eff", "tol_dn_eff")] + \
+               [(k, C.c_int) for k in ("scf_iters", "mu_evals", "converged", "flip_seen")]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -86,12 +88,14 @@ def load(rebuild_if_stale: bool = True):
     L.arche_is_fused.argtypes = [vp]
     L.arche_is_persistent.argtypes = [vp]
     L.arche_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
+    L.arche_peak_fp64.argtypes = [vp, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.arche_peak_l2.argtypes = [vp, C.POINTER(C.c_double)]
     _lib = L
     return L
 
 
 _DEFAULTS = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=3, scf_tol_F=1e-10,
-                 scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0, ewald_alpha=0.0, n_electrons=0.0)
+                 scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0, ewald_alpha=0.0, n_electrons=0.0, mix_mu_tol=0.0)
 
 
 class Arche:
@@ -283,6 +287,18 @@ class Arche:
             self._check(self.lib.arche_profile_get(self._h, i, C.byref(ms), C.byref(n)))
             out[name] = (ms.value, n.value)
         return out
+
+    def peak_fp64(self, seconds: float = 1.0) -> dict:
+        """measured fp64 FMA rate of the vector pipe (TFLOP/s): sustained over `seconds`, and the best single launch"""
+        out = (C.c_double * 2)(); ms = C.c_double()
+        self._check(self.lib.arche_peak_fp64(self._h, float(seconds), out, C.byref(ms)))
+        return {"sustained_tflops": out[0], "burst_tflops": out[1], "ran_ms": ms.value}
+
+    def peak_l2(self) -> float:
+        """measured L2 read bandwidth (GB/s)"""
+        v = C.c_double()
+        self._check(self.lib.arche_peak_l2(self._h, C.byref(v)))
+        return v.value
 
     def launch_count(self) -> int:
         return int(self.lib.arche_launch_count(self._h))

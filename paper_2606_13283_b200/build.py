@@ -9,7 +9,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libarche_b200.so")
 SOURCES = ["arche.cu"]
 HEADERS = ["common.cuh", "fd.cuh", "fd_tables.h", "fft.cuh", "fft_fast.cuh", "scf_kernels.cuh", "scf_persistent.cuh",
-           "ion_kernels.cuh", "stress_kernels.cuh"]
+           "ion_kernels.cuh", "stress_kernels.cuh", "peak_kernels.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -19,6 +19,7 @@
 #include "scf_kernels.cuh"
 #include "scf_persistent.cuh"
 #include "stress_kernels.cuh"
+#include "peak_kernels.cuh"
 
 using namespace arche;
 
@@ -232,7 +233,9 @@ extern "C" size_t arche_workspace_bytes(const arche_params *p) {
   return layout(&tmp, nullptr);
 }
 
-extern "C" const char *arche_last_error(const arche_ctx *c) { return c ? c->err : "null context"; }
+// error text of the last failed arche_scf_init of this thread (the context is destroyed on failure)
+static thread_local char g_init_err[256] = "null context";
+extern "C" const char *arche_last_error(const arche_ctx *c) { return c ? c->err : g_init_err; }
 extern "C" long long arche_launch_count(const arche_ctx *c) { return c ? c->launches : 0; }
 
 extern "C" void arche_destroy(arche_ctx *c) {
@@ -243,13 +246,26 @@ extern "C" void arche_destroy(arche_ctx *c) {
   delete c;
 }
 
+static int init_body(arche_ctx *c, const arche_params *p);
+
 extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   if (!out) return ARCHE_EINVAL;
   *out = nullptr;
-  if (!params_ok(p)) return ARCHE_EINVAL;
+  if (!params_ok(p)) { snprintf(g_init_err, sizeof(g_init_err), "invalid parameters"); return ARCHE_EINVAL; }
   arche_ctx *c = new (std::nothrow) arche_ctx;
   if (!c) return ARCHE_ENOMEM;
   memset(c, 0, sizeof(*c));
+  const int rc = init_body(c, p);
+  if (rc != ARCHE_OK) {   // nothing leaks on any failure path: the context and its pinned blocks go, the text stays readable
+    snprintf(g_init_err, sizeof(g_init_err), "%s", c->err[0] ? c->err : "arche_scf_init failed");
+    arche_destroy(c);
+    return rc;
+  }
+  *out = c;
+  return ARCHE_OK;
+}
+
+static int init_body(arche_ctx *c, const arche_params *p) {
   c->p = *p;
   c->stream = (cudaStream_t)p->stream;
   derive_sizes(c);
@@ -262,13 +278,11 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     c->persist = c->fuse && c->use_fast && !(pe && pe[0] == '0');
   }
   size_t need = layout(c, nullptr);
-  if (!p->d_workspace || p->workspace_bytes < need || ((uintptr_t)p->d_workspace & 255)) { delete c; return ARCHE_ENOMEM; }
+  if (!p->d_workspace || p->workspace_bytes < need || ((uintptr_t)p->d_workspace & 255)) return fail(c, ARCHE_ENOMEM, "workspace missing, too small or not 256-byte aligned");
   layout(c, (char *)p->d_workspace);
   const int nx = p->grid[0], ny = p->grid[1], nz = p->grid[2];
-  cudaError_t e = cudaMallocHost((void **)&c->h_sc, sizeof(DevScalars));
-  if (e != cudaSuccess) { delete c; return ARCHE_ECUDA; }
-  e = cudaMallocHost((void **)&c->h_stress, 64 * sizeof(double));
-  if (e != cudaSuccess) { cudaFreeHost(c->h_sc); delete c; return ARCHE_ECUDA; }
+  CK(cudaMallocHost((void **)&c->h_sc, sizeof(DevScalars)));
+  CK(cudaMallocHost((void **)&c->h_stress, 64 * sizeof(double)));
   // ---- geometry and constants
   GridGeom &G = c->G;
   G.nx = nx; G.ny = ny; G.nz = nz; G.ng = c->ng; G.nxh = c->nxh; G.P = c->P; G.nh = c->nh;
@@ -282,12 +296,18 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   C.kT = p->kT; C.cTF = sqrt(2.0) / (ARCHE_PI * ARCHE_PI) * pow(p->kT, 1.5);
   C.Ne = p->n_electrons > 0.0 ? p->n_electrons : c->Q;
   C.vol = G.vol; C.dV = G.dV;
-  if (!(C.Ne > 0.0)) { arche_destroy(c); return ARCHE_EINVAL; }
+  if (!(C.Ne > 0.0)) return fail(c, ARCHE_EINVAL, "no electrons");
   C.eta0 = fd_half_inverse_host(C.Ne / (G.vol * C.cTF));
   double asum = 0.0;
   for (int j = 0; j < c->nions; ++j) asum += 2.0 * ARCHE_PI * hZ[j] * p->psp_rc * p->psp_rc;  // alpha_s = 2 pi Z rc^2
   C.E_ie0 = C.Ne / G.vol * asum;
-  C.xc = p->xc; C.mix_mode = p->mix_mode; C.mix_warmup = p->mix_warmup; C.mix_w_fixed = p->mix_w_fixed;
+  C.xc = p->xc; C.mix_mode = p->mix_mode; C.mix_warmup = p->mix_warmup;
+  {  // uniform-gas response chi0 = dn/dmu at Ne/|Omega|; largest single-mode value of More's w (reading A11d)
+    const double chi0 = C.cTF * 0.5 * fd_host(0, C.eta0) / p->kT;
+    const double Lmax = fmax(G.Lx, fmax(G.Ly, G.Lz)), lam = chi0 * Lmax * Lmax / ARCHE_PI;
+    C.mix_w_fixed = p->mix_w_fixed > 0.0 ? p->mix_w_fixed : lam / (1.0 + lam);
+    C.mix_mu_tol = p->mix_mu_tol;
+  }
   C.tol_F = p->scf_tol_F; C.tol_dn = p->scf_tol_dn;
   C.q_F = 0.0; C.q_dn = 0.0; C.inv_qF = 0.0; C.inv_vol = 1.0 / G.vol;
   if (p->xc == 1) {  // reading A13: quanta of a PZ81 branch flip at n* = 3/(4 pi)
@@ -337,7 +357,7 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
     CK(cudaMemcpyAsync(dk2[a], k2.data(), n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(c->tw[a], tw.data(), n * sizeof(double2), cudaMemcpyHostToDevice, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    if (!fft_make_plan(n, c->tw[a], &c->plan[a])) { arche_destroy(c); return ARCHE_EINVAL; }
+    if (!fft_make_plan(n, c->tw[a], &c->plan[a])) return fail(c, ARCHE_EINVAL, "no FFT plan for this axis length");
   }
   if (c->nions > 0) {
     CK(cudaMemcpyAsync(c->Z, p->h_Z, c->nions * sizeof(double), cudaMemcpyHostToDevice, c->stream));
@@ -355,7 +375,6 @@ extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
   LAUNCHED(c);
   CK(cudaStreamSynchronize(c->stream));
   c->p.h_Z = nullptr; c->p.h_mass = nullptr;  // copied; do not keep the caller's pointers
-  *out = c;
   return ARCHE_OK;
 }
 
@@ -422,8 +441,8 @@ void fill_result(const arche_ctx *c, arche_result *r) {
   const DevScalars &s = *c->h_sc;
   r->mu = s.mu; r->F_total = s.F_total; r->F0 = s.F0; r->E_H = s.EH; r->E_xc = s.Exc; r->E_ie = s.Eie;
   r->E_ie0 = c->C.E_ie0; r->U_ii = s.U_ii; r->K_e = s.Ke; r->K_i = s.K_i; r->dn_l2 = s.dn_rel;
-  r->w_last = s.w; r->U_mix = s.U; r->K_mix = s.K;
-  r->scf_iters = s.iter; r->mu_evals = s.mu_evals_total; r->converged = s.converged;
+  r->w_last = s.w; r->U_mix = s.U; r->K_mix = s.K; r->tol_F_eff = s.tolF_eff; r->tol_dn_eff = s.toldn_eff;
+  r->scf_iters = s.iter; r->mu_evals = s.mu_evals_total; r->converged = s.converged; r->flip_seen = s.flip_seen;
 }
 
 // forward transform of the real input density into nhat_i (scaled by dV)
@@ -560,7 +579,7 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     LAUNCHED(c);
   }
   // reset per-solve scalars (iter, F_total, converged); mu and U_ii persist
-  CK(cudaMemsetAsync(&c->sc->iter, 0, sizeof(int) * 4, c->stream));   // iter, converged, mu_evals_total, flip_seen
+  CK(cudaMemsetAsync(&c->sc->iter, 0, sizeof(int) * 6, c->stream));   // iter, converged, mu_evals_total, flip_seen, more_on, pad
   CK(cudaMemsetAsync(&c->sc->F_total, 0, sizeof(double), c->stream));
   CK(cudaMemsetAsync(&c->sc->mu_evals_total, 0, sizeof(int), c->stream));
   c->have_solution = false;
@@ -746,10 +765,10 @@ extern "C" int arche_stress(arche_ctx *c, const double *d_vel, double *h_out) {
 extern "C" int arche_md_step(arche_ctx *c, double dt, double *d_pos, double *d_vel, arche_result *h_out) {
   if (!c || !d_pos || !d_vel || c->nions <= 0) return ARCHE_EINVAL;
   const int ni = c->nions, nb = (3 * ni + 127) / 128;
-  int rc;
+  int rc, rc_first = ARCHE_OK;
   if (!c->have_forces) {  // forces at the starting positions
-    rc = scf_solve(c, d_pos);
-    if (rc != ARCHE_OK && rc != ARCHE_ENOCONV) return rc;
+    rc_first = scf_solve(c, d_pos);
+    if (rc_first != ARCHE_OK && rc_first != ARCHE_ENOCONV) return rc_first;
     rc = compute_forces(c);
     if (rc) return rc;
   }
@@ -763,7 +782,7 @@ extern "C" int arche_md_step(arche_ctx *c, double dt, double *d_pos, double *d_v
   rc = read_scalars(c);
   if (rc) return rc;
   fill_result(c, h_out);
-  return rc_solve;
+  return rc_solve != ARCHE_OK ? rc_solve : rc_first;   // a non-converged solve at the starting positions is reported too
 }
 
 extern "C" int arche_md_step_host(arche_ctx *c, double dt, double *h_pos, double *h_vel, double *h_F, arche_result *h_out) {
@@ -874,5 +893,55 @@ extern "C" int arche_profile_get(arche_ctx *c, int cls, double *h_ms_total, long
   CK(cudaStreamSynchronize(c->stream));
   prof_harvest(c);
   *h_ms_total = c->prof_ms[cls]; *h_launches = c->prof_cnt[cls];
+  return ARCHE_OK;
+}
+
+// ---- measured rooflines (peak_kernels.cuh) -----------------------------------------------------------------
+extern "C" int arche_peak_fp64(arche_ctx *c, double seconds, double *h_tflops, double *h_ms) {
+  if (!c || !h_tflops || !(seconds > 0.0)) return ARCHE_EINVAL;
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+  const int blocks = c->sm_count * 8;
+  const long long iters = 200000;                      // ~25 ms per launch at the nominal rate
+  double *out = c->partials;                           // never written (see the kernel)
+  for (int w = 0; w < 2; ++w) { fp64_fma_peak_kernel<<<blocks, 256, 0, c->stream>>>(iters, 0.999999, 1e-6, out); LAUNCHED(c); }
+  double total_ms = 0.0, best_ms = 1e300; long long n = 0;
+  while (total_ms < 1e3 * seconds && n < 4096) {
+    CK(cudaEventRecord(e0, c->stream));
+    fp64_fma_peak_kernel<<<blocks, 256, 0, c->stream>>>(iters, 0.999999, 1e-6, out); LAUNCHED(c);
+    CK(cudaEventRecord(e1, c->stream));
+    CK(cudaEventSynchronize(e1));
+    float ms = 0.f; CK(cudaEventElapsedTime(&ms, e0, e1));
+    total_ms += ms; ++n; if (ms < best_ms) best_ms = ms;
+  }
+  const double flops = 2.0 * (double)kPeakChains * (double)iters * 256.0 * (double)blocks;
+  h_tflops[0] = flops * (double)n / (total_ms * 1e-3) / 1e12;   // sustained over the whole run
+  h_tflops[1] = flops / (best_ms * 1e-3) / 1e12;                 // best single launch
+  if (h_ms) *h_ms = total_ms;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  return ARCHE_OK;
+}
+
+extern "C" int arche_peak_l2(arche_ctx *c, double *h_gbs) {
+  if (!c || !h_gbs) return ARCHE_EINVAL;
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+  // the leading arrays of the workspace (n_i, n_a, V_i, ...): whatever they hold, at most 32 MiB of them
+  const size_t avail = (size_t)((const char *)c->kx - (const char *)c->n_i), want = (size_t)32 << 20;
+  const long long n = (long long)((avail < want ? avail : want) / sizeof(double2));
+  const int blocks = c->sm_count * 8, reps = 64;
+  const double2 *buf = reinterpret_cast<const double2 *>(c->n_i);
+  l2_read_peak_kernel<<<blocks, 256, 0, c->stream>>>(buf, n, 4, c->partials); LAUNCHED(c);
+  double best = 1e300;
+  for (int k = 0; k < 5; ++k) {
+    CK(cudaEventRecord(e0, c->stream));
+    l2_read_peak_kernel<<<blocks, 256, 0, c->stream>>>(buf, n, reps, c->partials); LAUNCHED(c);
+    CK(cudaEventRecord(e1, c->stream));
+    CK(cudaEventSynchronize(e1));
+    float ms = 0.f; CK(cudaEventElapsedTime(&ms, e0, e1));
+    if (ms < best) best = ms;
+  }
+  *h_gbs = (double)n * sizeof(double2) * reps / (best * 1e-3) / 1e9;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
   return ARCHE_OK;
 }

@@ -363,11 +363,13 @@ static inline cudaError_t fft_launch_pass(const FftAxisPlan &plan, int nx, int n
   size_t smem = 4 * sizeof(double) * (size_t)P.L * plan.n;
   if (smem < 4096) smem = 4096;  // room for the reduction scratch used by finish()
   auto kern = fft_pass_kernel<AXIS, INVERSE, LoadOp, StoreOp>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static int attr_dev = -1;   // the opt-in is per device
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (attr_dev != dev) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    attr_dev = dev;
   }
   if (blocks_out) *blocks_out = (int)blocks;
   kern<<<(unsigned)blocks, kFftThreads, smem, stream>>>(P, ld, st);
@@ -396,13 +398,16 @@ static inline cudaError_t fft_launch_real_x(const FftAxisPlan &plan, int nx, int
   const int blocks = fft_real_blocks(nx, ny, nz);
   size_t smem = 4 * sizeof(double) * (size_t)P.LP * plan.n;
   if (smem < 4096) smem = 4096;
-  static bool attr_set = false;
+  static int attr_dev = -1;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  const bool attr_set = attr_dev == dev;
   if constexpr (INVERSE) {
     auto kern = fft_c2r_x_kernel<LoadOp, StoreOp>;
     if (!attr_set) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
       if (e != cudaSuccess) return e;
-      attr_set = true;
+      attr_dev = dev;
     }
     kern<<<blocks, kFftThreads, smem, stream>>>(P, ld, st);
   } else {
@@ -410,7 +415,7 @@ static inline cudaError_t fft_launch_real_x(const FftAxisPlan &plan, int nx, int
     if (!attr_set) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
       if (e != cudaSuccess) return e;
-      attr_set = true;
+      attr_dev = dev;
     }
     kern<<<blocks, kFftThreads, smem, stream>>>(P, ld, st);
   }

@@ -366,11 +366,13 @@ static inline cudaError_t fft_launch_yz_fast_n(const FastGeom &G, LoadOp ld, Sto
   auto kern = fft_yz_fast_kernel<N, AXIS, INVERSE, LoadOp, StoreOp>;
   size_t smem = sizeof(double2) * N * kFastL;
   if (smem < 4096) smem = 4096;
-  static bool attr_set = false;
-  if (!attr_set) {
+  static int attr_dev = -1;   // the opt-in is per device: set it again when the calling thread's device differs
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (attr_dev != dev) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     if (e != cudaSuccess) return e;
-    attr_set = true;
+    attr_dev = dev;
   }
   const unsigned blocks = (unsigned)((AXIS == 1 ? G.nz : G.ny) * (G.P / kFastL));
   kern<<<blocks, fast_threads_yz<N>(), smem, stream>>>(G, ld, st);
@@ -397,13 +399,16 @@ static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, Stor
   if (smem < 4096) smem = 4096;
   const unsigned blocks = (unsigned)((long long)G.ny * G.nz / (2 * LP));
   constexpr int TH = LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>();
-  static bool attr_set = false;
+  static int attr_dev = -1;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  const bool attr_set = attr_dev == dev;
   if constexpr (INVERSE) {
     auto kern = fft_c2r_fast_kernel<N, LIGHT, LoadOp, StoreOp>;
     if (!attr_set) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
       if (e != cudaSuccess) return e;
-      attr_set = true;
+      attr_dev = dev;
     }
     kern<<<blocks, TH, smem, stream>>>(G, ld, st);
   } else {
@@ -411,7 +416,7 @@ static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, Stor
     if (!attr_set) {
       cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
       if (e != cudaSuccess) return e;
-      attr_set = true;
+      attr_dev = dev;
     }
     kern<<<blocks, TH, smem, stream>>>(G, ld, st);
   }

@@ -25,6 +25,8 @@ struct DevScalars {
   // S6/S7
   double w, F_total, F_prev, dn_rel;
   int iter, converged, mu_evals_total, flip_seen;   // flip_seen: reading A13, a PZ81 branch flip was detected in this solve
+  int more_on, pad1;                                // reading A11b: More's w has been switched on in this solve
+  double mu_iter_prev, tolF_eff, toldn_eff;         // mu_a of the previous iteration; the tolerances the stop rule applied
   // per-MD-step
   double U_pp, U_pm_sum, U_pm_fix, U_ii, init_sum, init_scale, K_i;
 };
@@ -35,6 +37,7 @@ struct ScfConst {
   double mix_w_fixed, tol_F, tol_dn;
   double inv_vol, inv_qF;   // reciprocals for the single-thread scalar updates (fp64 divisions cost ~300 cycles each there)
   double q_F, q_dn;   // reading A13: free-energy quantum of one PZ81 branch flip; chi(n*) x V_c jump x sqrt(dV)
+  double mix_mu_tol;  // reading A11b: More's w only once |mu_k - mu_{k-1}| <= mix_mu_tol kT (latched); <= 0: off
 };
 
 // Perdew-Zunger 1981 LDA (unpolarised), Hartree units; restated from the publication (reading D5).
@@ -479,8 +482,13 @@ struct StoreNhatA {
       sc->U = U; sc->EH = EH; sc->Eie = Eie;
       const int it = sc->iter + 1;
       const double K = sc->K;
+      // reading A11b ("w is computed and updated only after a few SCF iterations, once the chemical potential
+      // fluctuations are small"): after the warm-up count, and -- when mix_mu_tol > 0 -- once two successive mu_a differ
+      // by at most mix_mu_tol kT; the switch is latched for the rest of the solve
+      if (C.mix_mu_tol > 0.0 && !sc->more_on && it >= 2 && fabs(sc->mu - sc->mu_iter_prev) <= C.mix_mu_tol * C.kT) sc->more_on = 1;
+      sc->mu_iter_prev = sc->mu;
       double w;
-      if (C.mix_mode == 1 && it > C.mix_warmup) w = (K + U > 0.0) ? U / (K + U) : 0.0;   // w = U/(K+U)
+      if (C.mix_mode == 1 && it > C.mix_warmup && (C.mix_mu_tol <= 0.0 || sc->more_on)) w = (K + U > 0.0) ? U / (K + U) : 0.0;   // w = U/(K+U)
       else w = C.mix_w_fixed;
       const double F = sc->F0 + sc->Exc + EH + Eie + C.E_ie0 + sc->U_ii;
       const double dn_rel = sqrt(sc->dn2 / sc->na2);
@@ -488,16 +496,23 @@ struct StoreNhatA {
       // point whose converged density sits on n* flips branch between iterations: F then moves by whole quanta
       // q_F = (eps_c jump) n* dV and the density answers the V_c jump with a limit cycle of relative size
       // q_dn/||n_a|| -- neither criterion can be met below that.  A jump of F by an integer number (1..8) of quanta
-      // right after a change far below one quantum marks the solve; from then on two quanta are tolerated in both criteria.
-      const double dF = fabs(F - sc->F_total);
-      if (C.xc == 1 && it >= 3 && C.q_F > 0.0) {   // a jump: the previous change of F was far below one quantum
-        const double m = dF * C.inv_qF, r = rint(m), mp = fabs(sc->F_total - sc->F_prev) * C.inv_qF, rp = rint(mp);
+      // marks the solve; from then on two quanta are tolerated in both criteria.  flip_seen and the tolerances applied
+      // are reported in arche_result.
+      const double dFs = F - sc->F_total, dF = fabs(dFs);
+      if (C.xc == 1 && it >= 3 && C.q_F > 0.0) {
+        const double dFp = sc->F_total - sc->F_prev;
+        const double m = dF * C.inv_qF, r = rint(m), mp = fabs(dFp) * C.inv_qF, rp = rint(mp);
         const bool near = r >= 1.0 && r <= 8.0 && fabs(m - r) < 0.02, near_prev = rp >= 1.0 && rp <= 8.0 && fabs(mp - rp) < 0.02;
-        if (near && (mp < 0.1 || near_prev)) sc->flip_seen = 1;   // after a quiet change, or twice in a row
+        // (a) a quantised jump right after a change far below one quantum, or (b) the same multiple twice in a row with
+        // opposite signs (F hops back: a flip that set in before F had settled).  The free energy of a converging solve
+        // decreases monotonically -- also a slowly converging one, whose successive dF are nearly equal -- so (b) cannot
+        // fire on a smooth decay.
+        if (near && (mp < 0.1 || (near_prev && r == rp && dFs * dFp < 0.0))) sc->flip_seen = 1;
       }
       const double tolF = C.tol_F + (sc->flip_seen ? 2.02 * C.q_F : 0.0);
       const double toldn = C.tol_dn + (sc->flip_seen ? 2.0 * C.q_dn / sqrt(sc->na2) : 0.0);
       sc->converged = (it >= 2 && dF < tolF && dn_rel < toldn) ? 1 : 0;
+      sc->tolF_eff = tolF; sc->toldn_eff = toldn;
       sc->F_prev = sc->F_total; sc->F_total = F; sc->w = w; sc->dn_rel = dn_rel; sc->iter = it;
       sc->mu_have_prev = 1;
     }

@@ -1,0 +1,217 @@
+"""Pins added in round 2 for the parts of the oracle VERDICT r01 listed as unpinned (no GPU):
+the PZ81 branch-flip stop rule (reading A13), the clip / renormalise rule of the one-center start (reading A10),
+the PZ81 constants on both branches, brute-force image sums of pair forces, and the egg-box residual |sum F|
+falling with grid refinement (reading A17-iii).  P:NNN = PAPER.md line."""
+import numpy as np
+import pytest
+
+import arche_inputs as ai
+from flip_case import KW as FLIP_KW, NSTAR, find_flip_case
+
+PI = np.pi
+
+
+# ---------------------------------------------------------------- PZ81 (reading D5): constants of both branches
+def test_pz81_values_written_out_by_hand(orc):
+    """eps_c and V_c at r_s = 0.5 (log branch) and r_s = 2 (Pade branch) evaluated BY HAND from the constants printed in
+    the 1981 article (gamma = -0.1423, beta1 = 1.0529, beta2 = 0.3334; A = 0.0311, B = -0.048, C = 0.0020, D = -0.0116):
+      r_s = 0.5: ln r_s = -0.693147181
+        eps_c = 0.0311(-0.693147181) - 0.048 + 0.0020(0.5)(-0.693147181) - 0.0116(0.5)
+              = -0.021556877 - 0.048 - 0.000693147 - 0.0058                       = -0.076050024
+        V_c   = A ln r_s + (B - A/3) + (2/3) C r_s ln r_s + ((2D - C)/3) r_s
+              = -0.021556877 - 0.058366667 - 0.000462098 - 0.0042                 = -0.084585642
+      r_s = 2:  sqrt r_s = 1.414213562, den = 1 + 1.0529(1.414213562) + 0.3334(2) = 3.155825460
+        eps_c = -0.1423/3.155825460                                               = -0.045091214
+        V_c   = eps_c (1 + (7/6)(1.0529)(1.414213562) + (4/3)(0.3334)(2))/den
+              = -0.045091214 (3.626263743)/3.155825460                            = -0.051812942
+    A wrong or transposed digit in any of the seven constants moves at least one of the four numbers by > 1e-6."""
+    for rs, ec, vc in ((0.5, -0.076050024, -0.084585642), (2.0, -0.045091214, -0.051812942)):
+        n = 3.0 / (4.0 * PI * rs ** 3)
+        ex = -0.75 * (3.0 * n / PI) ** (1.0 / 3.0)
+        e, v = orc.xc(n)
+        assert abs((e - ex) - ec) < 1e-8, (rs, e - ex)
+        assert abs((v - 4.0 / 3.0 * ex) - vc) < 1e-8, (rs, v - 4.0 / 3.0 * ex)
+
+
+def test_pz81_C_and_D_follow_from_continuity_at_rs_1(orc):
+    """Perdew and Zunger fix C and D by making eps_c and its r_s-derivative (hence V_c) continuous at r_s = 1 and print
+    them with four decimals.  Solving the two matching conditions with the OTHER five constants gives C = 0.00201...,
+    D = -0.01165..., which round to the printed 0.0020 and -0.0116; the residual jumps of the oracle at r_s = 1 are then
+    the rounding of C and D and nothing else."""
+    g, b1, b2, A, B = -0.1423, 1.0529, 0.3334, 0.0311, -0.048
+    den = 1.0 + b1 + b2
+    ec1 = g / den                                         # Pade branch at r_s = 1
+    dec1 = -g * (0.5 * b1 + b2) / den ** 2                # d eps_c / d r_s at r_s = 1
+    # log branch at r_s = 1: eps_c = B + D, d eps_c/d r_s = A + C + D
+    D = ec1 - B
+    C = dec1 - A - D
+    assert round(C, 4) == 0.0020 and round(D, 4) == -0.0116
+    lo, hi = orc.xc(NSTAR * (1 + 1e-12)), orc.xc(NSTAR * (1 - 1e-12))     # r_s just below / above 1
+    # jump of eps_c = (D_printed - D); jump of V_c = eps_c - (r_s/3) d eps_c/d r_s difference
+    assert abs((lo[0] - hi[0]) - (-0.0116 - D)) < 1e-9
+    dlo = A + 0.0020 + (-0.0116)
+    assert abs((lo[1] - hi[1]) - ((-0.0116 - D) - (dlo - dec1) / 3.0)) < 1e-9
+    assert 2e-5 < abs(lo[0] - hi[0]) < 5e-5 and 2e-5 < abs(lo[1] - hi[1]) < 5e-5
+
+
+# ---------------------------------------------------------------- stop rule with a PZ81 branch flip (reading A13)
+@pytest.fixture(scope="module")
+def flip(orc):
+    return find_flip_case(orc)
+
+
+def test_stop_rule_branch_flip_constructed(orc, flip):
+    """One grid point driven across n* = 3/(4 pi): the SCF then has no fixed point (V_c jumps UP by 2.6e-5 Ha when the
+    density rises through n*, which pushes the density back down), F hops by whole quanta
+    q_F = |eps_c(n*+) - eps_c(n*-)| n* dV and the strict criteria can never be met.  Checks, against evaluations that do
+    not go through the oracle's stop rule: the quanta seen in the iteration history, flip_seen, the widened tolerances,
+    and that smooth solves on either side keep the strict rule."""
+    cfg, Ne, Ne_lo, Ne_hi, g0 = flip
+    dV = float(np.prod(cfg["cell"])) / 64
+    ep, vp = orc.xc(NSTAR * (1 + 1e-12)); em, vm = orc.xc(NSTAR * (1 - 1e-12))
+    q_F = abs(ep - em) * NSTAR * dV                                    # independent of the rule's own constants
+    o = orc.Oracle(cfg, n_electrons=Ne, **FLIP_KW)
+    o.scf_begin(cfg["pos"])
+    hist = [o.scf_iter() for _ in range(70)]
+    late = hist[30:]
+    dF = np.diff([h["F_total"] for h in hist])[29:]
+    m = np.abs(dF) / q_F
+    assert np.all(np.abs(m - np.rint(m)) < 0.02), m                    # every late change is a whole number of quanta
+    assert np.rint(m).max() >= 1 and np.rint(m).max() <= 8             # ... and some are not zero: F never settles
+    side = np.array([o.get_real("n_a").ravel()[g0] > NSTAR for _ in (0,)])   # the point sits within the cycle's reach
+    assert min(h["dn_l2"] for h in late) > 1e-9 > FLIP_KW["scf_tol_dn"]      # strict density criterion unreachable
+    assert all(h["flip_seen"] == 1 for h in late)
+    assert late[-1]["converged"] == 1
+    # widened tolerances: + 2.02 q_F and + 2 q_dn/||n_a||, q_dn = chi(n*) |V_c jump| sqrt(dV)
+    assert abs(late[-1]["tol_F_eff"] - (FLIP_KW["scf_tol_F"] + 2.02 * q_F)) < 1e-6 * q_F
+    kT = cfg["kT"]; cTF = np.sqrt(2.0) / PI ** 2 * kT ** 1.5
+    eta = orc.fd_half_inverse(NSTAR / cTF); h_ = 1e-4
+    chi = cTF * (orc.fd(1, eta + h_)[0] - orc.fd(1, eta - h_)[0]) / (2 * h_ * kT)    # dn/dmu by central difference
+    na = o.get_real("n_a"); norm = np.sqrt((na ** 2).sum() * dV)
+    want = FLIP_KW["scf_tol_dn"] + 2.0 * chi * abs(vp - vm) * np.sqrt(dV) / norm
+    assert abs(late[-1]["tol_dn_eff"] / want - 1) < 1e-6
+    assert max(h["dn_l2"] for h in late) < want                        # the limit cycle fits inside the widened bound
+    # smooth solves on either side: strict rule, no flag
+    for Ne_s in (Ne_lo, Ne_hi):
+        os_ = orc.Oracle(cfg, n_electrons=Ne_s, **FLIP_KW)
+        r = os_.scf_solve(cfg["pos"])
+        assert r["converged"] == 1 and r["flip_seen"] == 0
+        assert r["tol_F_eff"] == FLIP_KW["scf_tol_F"] and r["tol_dn_eff"] == FLIP_KW["scf_tol_dn"]
+        assert r["dn_l2"] < FLIP_KW["scf_tol_dn"]
+
+
+def test_stop_rule_not_fooled_by_slow_smooth_convergence(orc):
+    """A solve that converges slowly (fixed w = 0.9: dF shrinks by ~0.8 per iteration, successive dF nearly equal while
+    they pass through the 1..8 quanta window) must keep the strict rule: F decreases monotonically, so the
+    same-multiple-with-opposite-sign trigger cannot fire."""
+    cfg = ai.make_small(n_ions=2, L=6.0, grid=(8, 8, 8), T_eV=10.0, seed=5)
+    o = orc.Oracle(cfg, mix_mode=0, mix_w_fixed=0.9, init_mode=0, scf_tol_F=1e-12, scf_tol_dn=1e-9, scf_max_iter=400)
+    r = o.scf_solve(cfg["pos"])
+    assert r["converged"] == 1 and r["flip_seen"] == 0 and r["scf_iters"] > 100
+    assert r["tol_F_eff"] == 1e-12 and r["dn_l2"] < 1e-9
+
+
+# ---------------------------------------------------------------- one-center start: clip / renormalise (reading A10)
+def test_one_center_clip_and_renormalise(orc):
+    """Hand-built profile ghat with a negative lobe in real space (a Mexican-hat form factor): n_i = S_Z ghat (Eq. 20,
+    P:253) -> inverse transform, real part, clip at 1e-3 N_e/|Omega|, rescale to N_e.  Properties that fix the rule:
+    the raw field does go negative; afterwards the integral is N_e to round-off, the minimum is floor x scale with
+    scale < 1 (clipping only adds charge), and every unclipped point is the raw value times the same scale."""
+    cfg = ai.make_small(n_ions=3, L=7.0, grid=(12, 10, 8), cell=[7.0, 6.0, 5.0], seed=13)
+    o = orc.Oracle(cfg, init_mode=1)
+    cell, grid = cfg["cell"], cfg["grid"]
+    nx, ny, nz = (int(g) for g in grid)
+    vol = float(cell.prod()); Ne = float(cfg["Z"].sum()); Q = Ne
+
+    def m(N):
+        i = np.arange(N); return np.where(i <= N // 2, i, i - N)
+    kz, ky, kx = np.meshgrid(m(nz) / cell[2], m(ny) / cell[1], m(nx) / cell[0], indexing="ij")
+    k2 = kx ** 2 + ky ** 2 + kz ** 2
+    ghat = (Ne / Q) * (1.0 - 40.0 * k2) * np.exp(-6.0 * k2)            # ghat(0) = N_e/Q: charge preserved before clipping
+    o.set_profile(ghat.astype(np.complex128))
+    o.scf_begin(cfg["pos"])
+    n_i = o.get_real("n_i")
+    S = orc.structure_factor(cell, grid, cfg["pos"], cfg["Z"])         # pinned separately (test_oracle_pins.py)
+    raw = np.fft.ifftn(S * ghat).real * (nx * ny * nz) / vol           # f(r) = (1/|Omega|) sum_k fhat e^{+2 pi i k.r}
+    floor = 1e-3 * Ne / vol
+    assert raw.min() < -10 * floor                                     # the negative lobe is really there
+    dV = vol / (nx * ny * nz)
+    assert abs(n_i.sum() * dV - Ne) < 1e-13 * Ne
+    clipped = raw < floor
+    assert clipped.sum() > 10 and (~clipped).sum() > 10
+    scale = n_i[~clipped] / raw[~clipped]
+    assert np.ptp(scale) < 1e-12 and 0 < scale.mean() < 1.0
+    assert np.abs(n_i[clipped] - floor * scale.mean()).max() < 1e-15
+    assert abs(n_i.min() - floor * scale.mean()) < 1e-15
+    # nhat_i is the transform of the fixed-up density, not S ghat
+    nh = o.get_complex("nhat_i")
+    assert abs(nh[0, 0, 0] - Ne) < 1e-12 * Ne
+    assert np.abs(nh - np.fft.fftn(n_i) * dV).max() < 1e-12 * Ne
+
+
+# ---------------------------------------------------------------- Ewald forces vs brute-force image sums (pin P6)
+def _image_sum_force(cell, pos, Z, N):
+    """Z_j [ sum_k sum_{R in (-N..N)^3}' Z_k (r_jk + R)/|r_jk + R|^3 - (4 pi/(3|Omega|)) sum_k Z_k (r_j - r_k) ]:
+    the direct Coulomb sum over a cube of periodic images plus, for the neutralising background and the conditional
+    convergence of the cubic summation order, the field of the uniformly charged cube and the surface (dipole) term,
+    which combine into the last, translation-invariant, term."""
+    r = np.arange(-N, N + 1)
+    R = np.stack(np.meshgrid(r, r, r, indexing="ij"), -1).reshape(-1, 3) * cell
+    vol = cell.prod()
+    F = np.zeros_like(pos)
+    for j in range(len(Z)):
+        for k in range(len(Z)):
+            d = pos[j] - pos[k] + R
+            if j == k:
+                d = d[np.abs(R).sum(1) > 0]
+            F[j] += Z[j] * Z[k] * (d / (np.einsum("ij,ij->i", d, d) ** 1.5)[:, None]).sum(0)
+            F[j] -= Z[j] * Z[k] * 4 * PI / (3 * vol) * (pos[j] - pos[k])
+    return F
+
+
+@pytest.mark.parametrize("Z", [[3.0, 1.0, 2.0], [1.0, -1.0, 2.0, -2.0]])
+def test_ewald_forces_equal_brute_force_image_sums(orc, Z):
+    """F^ii of Eq. 45-47 against direct sums of pair forces over (2N+1)^3 periodic images of a 3-4 ion cubic
+    cell (positive ions on a background, and a neutral mixed-sign cell).  The cube of images has side a = (2N+1)L and
+    the remainder of the sum falls like 1/a^2 (the next term of the field inside a uniformly charged cube); one
+    Richardson step in 1/a^2 on N = 10, 20 leaves ~1e-6 of the largest force."""
+    Z = np.array(Z); n = len(Z)
+    L = 5.0; cell = np.array([L, L, L])
+    rng = np.random.default_rng(17 + n)
+    pos = np.array([[0.7, 1.1, 3.9], [3.6, 4.2, 0.9], [2.2, 2.9, 2.4], [4.4, 0.6, 3.1]])[:n] + 0.1 * rng.random((n, 3))
+    _, F = orc.ewald(cell, np.array([24, 24, 24], dtype=np.int32), pos, Z)
+    f10, f20 = _image_sum_force(cell, pos, Z, 10), _image_sum_force(cell, pos, Z, 20)
+    h10, h20 = 1.0 / 21.0 ** 2, 1.0 / 41.0 ** 2
+    brute = (f20 * h10 - f10 * h20) / (h10 - h20)
+    assert np.abs(F - brute).max() < 3e-6 * np.abs(F).max(), (np.abs(F - brute).max(), np.abs(F).max())
+    assert np.abs(f20 - F).max() < 3e-3 * np.abs(F).max()              # the unextrapolated sum is already close
+
+
+# ---------------------------------------------------------------- egg-box residual (reading A17-iii)
+def test_total_force_sum_is_the_egg_box_derivative(orc):
+    """"Forces summing to zero" (BASELINE.json north_star) holds for F^ii to round-off.  For F^ie it cannot hold on a grid:
+    the pointwise non-linear terms (F_0, XC) alias, so F_grid is invariant only under translations by grid vectors and
+    sum_j F_j = -dF_grid/dt for a rigid translation t of all ions (Hellmann-Feynman on the grid) -- NOT zero.  With the
+    Ashcroft empty core (a jump of the potential at r_c, form factor ~ cos(2 pi k r_c)/k^2) that residual does not even
+    fall monotonically with the grid in the affordable range (measured: DESIGN.md reading A17), so what is pinned is
+    the identity itself: the sum of the forces against the central difference of the re-converged free energy."""
+    cfg = ai.make_small(n_ions=3, L=7.0, grid=(12, 12, 12), T_eV=10.0, seed=6)
+    o = orc.Oracle(cfg, init_mode=0, scf_tol_F=1e-12, scf_tol_dn=1e-12, scf_max_iter=400)
+    pos = cfg["pos"]
+    r = o.scf_solve(pos); assert r["converged"] == 1
+    F = o.forces()
+    _, Fii = orc.ewald(cfg["cell"], cfg["grid"], pos, cfg["Z"])
+    assert np.abs(Fii.sum(0)).max() < 1e-11 * np.abs(Fii).max()                 # Newton's third law, exact
+    tot = F.sum(0)
+    assert np.linalg.norm(tot) > 1e-3 * np.abs(F).max()                         # the egg-box residual is not small here
+    for c in range(3):
+        def Ft(h):
+            p = pos.copy(); p[:, c] += h
+            return o.scf_solve(p)["F_total"]
+        fd = lambda h: -(Ft(h) - Ft(-h)) / (2 * h)
+        rich = (4 * fd(1e-3) - fd(2e-3)) / 3
+        assert abs(rich - tot[c]) < 2e-7 * np.abs(F).max(), (c, rich, tot[c])
+    # a translation by one grid spacing changes nothing (exact invariance)
+    d = cfg["cell"] / cfg["grid"]
+    r2 = o.scf_solve(pos + d)
+    assert abs(r2["F_total"] - r["F_total"]) < 1e-11 * abs(r["F_total"])
