@@ -104,6 +104,10 @@ int arche_forces(arche_ctx *c, double *d_F);
 #define ARCHE_STRESS_DOUBLES 55
 int arche_stress(arche_ctx *c, const double *d_vel, double *h_out);
 
+/* Change the iteration control of the following solves: scf_max_iter (0 keeps the current value) and scf_fixed_iter
+ * (> 0: run exactly that many iterations -- parity replay of an oracle run solve by solve; 0: stop rule). */
+int arche_set_scf_iterations(arche_ctx *c, int scf_max_iter, int scf_fixed_iter);
+
 /* One velocity-Verlet step of length dt (a.u.) (reading D2): half kick, drift, SCF solve at the
  * new positions, forces, half kick.  d_pos/d_vel [n_ions*3] are updated in place.  The first call also solves
  * at the starting positions to obtain the initial forces.  Later calls reuse the forces of the previous step: a caller

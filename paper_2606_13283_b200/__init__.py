@@ -21,7 +21,7 @@ SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_la
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
            "arche_rfft3d_forward", "arche_rfft3d_inverse",
            "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused", "arche_is_persistent",
-           "arche_peak_fp64", "arche_peak_l2"]
+           "arche_peak_fp64", "arche_peak_l2", "arche_set_scf_iterations"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
 
@@ -90,6 +90,7 @@ def load(rebuild_if_stale: bool = True):
     L.arche_profile_get.argtypes = [vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_longlong)]
     L.arche_peak_fp64.argtypes = [vp, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.arche_peak_l2.argtypes = [vp, C.POINTER(C.c_double)]
+    L.arche_set_scf_iterations.argtypes = [vp, C.c_int, C.c_int]
     _lib = L
     return L
 
@@ -185,6 +186,9 @@ class Arche:
         r = Result()
         self._check(self.lib.arche_scf_iter(self._h, C.byref(r)))
         return r.asdict()
+
+    def set_scf_iterations(self, max_iter: int = 0, fixed_iter: int = 0):
+        self._check(self.lib.arche_set_scf_iterations(self._h, int(max_iter), int(fixed_iter)))
 
     def set_input_density(self, n):
         d = self._dev(n)

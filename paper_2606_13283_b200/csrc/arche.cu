@@ -869,6 +869,13 @@ extern "C" int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta,
   return ARCHE_OK;
 }
 
+extern "C" int arche_set_scf_iterations(arche_ctx *c, int scf_max_iter, int scf_fixed_iter) {
+  if (!c || scf_max_iter < 0 || scf_fixed_iter < 0) return ARCHE_EINVAL;
+  if (scf_max_iter > 0) c->p.scf_max_iter = scf_max_iter;
+  c->p.scf_fixed_iter = scf_fixed_iter;
+  return ARCHE_OK;
+}
+
 extern "C" int arche_is_fused(const arche_ctx *c) { return c && c->fuse ? 1 : 0; }
 
 extern "C" int arche_is_persistent(const arche_ctx *c) {
