@@ -29,11 +29,15 @@ import arche_inputs as ai  # noqa: E402
 
 # Stop rule of the throughput runs: BASELINE.json's 1e-10 Ha on the free energy and 1e-8 on the relative density
 # residual (reading D4).  Mixing: More's w after a warm-up with the fixed w.
-TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000, mix_warmup=3, mix_w_fixed=0.95)
+TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000, mix_warmup=3, mix_w_fixed=0.95, xc=2)
 # c4 (T = 1 eV, 61-bohr cell): the longest wave has lambda = chi0/(pi k_min^2) ~ 110, so the fixed w of the warm-up must
 # exceed (lambda-1)/(lambda+1): automatic w = lambda/(1+lambda), More's w once |mu_k - mu_{k-1}| < 1e-3 kT (reading A11b)
 TOL_BY_WORKLOAD = {"c4": dict(scf_max_iter=12000, mix_w_fixed=0.0, mix_mu_tol=1e-3)}
 NCU_TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_c5_384_ncu_full.csv")
+
+
+XC_NAME = {1: "PZ81 LDA (constants as printed; eps_c, V_c jump 3e-5 Ha at r_s=1)",
+           2: "PZ81 LDA (C, D at full precision from PZ's continuity conditions at r_s=1: reading A13b)"}
 
 
 def tol_for(workload):
@@ -70,9 +74,10 @@ def bytes_per_point(nx, fused=True):
 # ~ 90 flops; the reductions ~ 20.
 FLOPS_PER_POINT = {"mu_pass": 32, "density": 3 * 30 + 90 + 20, "density_r": 3 * 30 + 90 + 20, "vi_r": 30 + 90 + 10,
                    "fft_inv_x_vi": 30 + 90 + 10}     # fft_inv_x_vi carries the V_i epilogue only in the fused form
-# fp64 flops per (ion, stored half-spectrum point) of the ion-grid sums: one complex FMA pair (8 flops) for S_Z,
-# t = W a_j, P += t, Q += kx t (12 flops) for the forces (ion_kernels.cuh)
-FLOPS_PER_PAIR = {"structure_factor": 8.0, "force": 12.0}
+# fp64 work per (ion, stored half-spectrum point) of the ion-grid sums in FMA-slot units (2 x fp64 pipe instructions:
+# a lone multiply or add occupies the same issue slot as an FMA, and the measured peak counts an FMA as 2): S_Z one
+# complex multiply-add = 4 FMAs; forces t = W a_j (2 mul + 2 FMA), P += t (2 add), Q += kx t (2 FMA) = 8 instructions
+FLOPS_PER_PAIR = {"structure_factor": 8.0, "force": 16.0}
 FP64_DERIVED_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # unit count x clock (B200_PROFILING.md), used only if not measured
 
 
@@ -224,10 +229,11 @@ def workload_config(cfg, name):
            f"warm-up at the automatic w = lambda/(1+lambda), More w = U/(K+U) once |d mu| < {tol['mix_mu_tol']:g} kT (P:311)")
     return {"workload": f"{name}: {len(cfg['Z'])} Al ions (Z=3), cell {[round(float(x), 4) for x in cfg['cell']]} bohr, "
                         f"grid {[int(g) for g in cfg['grid']]} ({ng / 1e6:.2f} M points), T={cfg['T_eV']} eV, "
-                        f"dt={cfg['dt'] / ai.FS_AU:.2f} fs, TF + PZ81 + Ashcroft rc=1.12, one-center init; one step = one "
+                        f"dt={cfg['dt'] / ai.FS_AU:.2f} fs, TF + {XC_NAME[tol['xc']]} + Ashcroft rc=1.12, one-center init; one step = one "
                         f"velocity-Verlet MD step with the SCF run to its stop rule",
-            "stop_rule": f"|dF|<{tol['scf_tol_F']:g} Ha and ||n_i-n_a||/||n_a||<{tol['scf_tol_dn']:g} (widened by two "
-                         f"PZ81 branch-flip quanta when a flip is detected: DESIGN.md reading A13; flagged per run)",
+            "stop_rule": f"|dF|<{tol['scf_tol_F']:g} Ha and ||n_i-n_a||/||n_a||<{tol['scf_tol_dn']:g}" +
+                         (" (widened by two PZ81 branch-flip quanta when a flip is detected: DESIGN.md reading A13; "
+                          "flagged per run as flip_steps)" if tol["xc"] == 1 else " (strict: the XC potential is continuous)"),
             "mixing": mix,
             "l2": ("L2 flushed between timed steps (256 MiB write); fields of %.1f GB per step exceed the 126 MB L2"
                    % (99.0 * ng / 1e9) if ng >= 192 ** 3 else
@@ -397,7 +403,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short c1..c4 runs of the 'configs' block")
     ap.add_argument("--grid", type=int, default=0, help="with --workload c5: grid size (default 384)")
+    ap.add_argument("--xc", type=int, default=2, choices=[1, 2],
+                    help="2 (default): PZ81 with C, D at full precision (continuous at r_s = 1, strict stop rule); 1: as printed")
     args = ap.parse_args()
+    TOL["xc"] = args.xc
     cfg = ai.make_config(args.workload, grid=(args.grid or None) if args.workload == "c5" else None)
     if args.impl == "reference":
         return run_reference(args, cfg)

@@ -36,7 +36,10 @@ typedef struct {
   const double *h_Z;     /* [n_ions] valence charges, host, copied at init */
   const double *h_mass;  /* [n_ions] ion masses in electron masses, host, copied at init */
   double kT;             /* electron (= ion) temperature in Hartree */
-  int xc;                /* 0: none (the paper's own TF derivations); 1: Perdew-Zunger 1981 LDA */
+  int xc;                /* 0: none (the paper's own TF derivations); 1: Perdew-Zunger 1981 LDA, constants as
+                            printed (eps_c, V_c jump by ~3e-5 Ha at r_s = 1: stop rule of DESIGN.md reading A13);
+                            2: the same with C, D at full precision from PZ's own continuity conditions at r_s = 1
+                            (continuous eps_c and V_c, strict stop rule; reading A13b) */
   double psp_rc;         /* Ashcroft empty-core radius in bohr (BASELINE.json: 1.12) */
   int init_mode;         /* 0: uniform input density each step; 1: one-center profile */
   int mix_mode;          /* 0: fixed w; 1: More et al. w = U/(K+U) */

@@ -190,13 +190,22 @@ void oracle_xc(int xc, double n, double *eps, double *v) {
   double vx = (4.0 / 3.0) * ex;
   double rs = cbrt(3.0 / (4.0 * PI * n));
   double ec, vc;
+  const double gam = -0.1423, b1 = 1.0529, b2 = 0.3334, A = 0.0311, B = -0.048;
   if (rs >= 1.0) {
-    const double gam = -0.1423, b1 = 1.0529, b2 = 0.3334;
     double sq = sqrt(rs), den = 1.0 + b1 * sq + b2 * rs;
     ec = gam / den;
     vc = ec * (1.0 + (7.0 / 6.0) * b1 * sq + (4.0 / 3.0) * b2 * rs) / den;
   } else {
-    const double A = 0.0311, B = -0.048, C = 0.0020, D = -0.0116;
+    double C = 0.0020, D = -0.0116; /* xc = 1: as printed in the 1981 article */
+    if (xc == 2) {
+      /* reading A13b: C and D from the matching conditions Perdew and Zunger imposed at r_s = 1 -- eps_c and
+       * d eps_c/d r_s of the two branches equal -- solved with the other five printed constants:
+       *   B + D = gam/den1,   A + C + D = -gam (b1/2 + b2)/den1^2,   den1 = 1 + b1 + b2.
+       * They round to the printed 0.0020 and -0.0116; eps_c and V_c are then continuous. */
+      double den1 = 1.0 + b1 + b2;
+      D = gam / den1 - B;
+      C = -gam * (0.5 * b1 + b2) / (den1 * den1) - A - D;
+    }
     double l = log(rs);
     ec = A * l + B + C * rs * l + D * rs;
     vc = A * l + (B - A / 3.0) + (2.0 / 3.0) * C * rs * l + (2.0 * D - C) / 3.0 * rs;

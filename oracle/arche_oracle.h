@@ -31,7 +31,8 @@ typedef struct {
   const double *Z;     /* [n_ions] valence charges */
   const double *mass;  /* [n_ions] electron masses */
   double kT;           /* Hartree */
-  int xc;              /* 0 none (paper's TF-only derivations), 1 PZ81 LDA */
+  int xc;              /* 0 none (paper's TF-only derivations), 1 PZ81 LDA as printed, 2 PZ81 with C, D
+                          at full precision from its own continuity conditions at r_s = 1 (reading A13b) */
   double psp_rc;       /* Ashcroft empty-core radius (bohr) */
   int init_mode;       /* 0 uniform density every step, 1 one-center profile */
   int mix_mode;        /* 0 fixed w, 1 More et al. w = U/(K+U) */
@@ -61,7 +62,7 @@ double oracle_fd_half_inverse(double y);             /* eta with I_{1/2}(eta) = 
 /* unnormalised DFT along all three axes, in place; sign=-1: exp(-2 pi i mn/N), +1: exp(+...) */
 void oracle_fft3d(int nx, int ny, int nz, double *a_complex, int sign);
 void oracle_dft3d_naive(int nx, int ny, int nz, double *a_complex, int sign);
-/* xc=1: Perdew-Zunger 1981 LDA, unpolarised: energy per electron and potential */
+/* xc=1: Perdew-Zunger 1981 LDA, unpolarised: energy per electron and potential; xc=2: continuous variant (A13b) */
 void oracle_xc(int xc, double n, double *eps_xc, double *v_xc);
 /* S_Z(k) = sum_j Z_j exp(-2 pi i k.r_j) on the grid */
 void oracle_structure_factor(const double cell[3], const int grid[3], int n_ions,

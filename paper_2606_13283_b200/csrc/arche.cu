@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  int r_blocks;    // resident blocks per SM of the streamed real-space Fermi-Dirac kernels
   int force_slabs, force_rows_per_slab, force_ipt;   // ions per thread of the force kernel's register tile
   // device arrays (all inside the caller's workspace)
   double *n_i, *n_a, *V_i, *vps, *va;
@@ -218,7 +219,7 @@ bool params_ok(const arche_params *p) {
   for (int a = 0; a < 3; ++a)
     if (!grid_ok(p->grid[a]) || !(p->cell[a] > 0.0)) return false;
   if (p->n_ions > 0 && (!p->h_Z || !p->h_mass)) return false;
-  if (p->xc != 0 && p->xc != 1) return false;
+  if (p->xc < 0 || p->xc > 2) return false;
   return true;
 }
 
@@ -329,7 +330,15 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     int dev = 0, sms = 0, per_sm = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, 0));
+    // kernels that keep the Fermi-Dirac table (49.5 KB) in dynamic shared memory: opt in on this device
+    CK(cudaFuncSetAttribute(mu_solve_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
+    CK(cudaFuncSetAttribute(fermi_dirac_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
+    CK(cudaFuncSetAttribute(pointwise_r_kernel<LoadReal, StoreVi, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
+    CK(cudaFuncSetAttribute(pointwise_r_kernel<LoadDensity, StoreNull, true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
+    CK(cudaFuncSetAttribute(pointwise_r_kernel<LoadReal, StoreVi, true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
+    CK(cudaFuncSetAttribute(pointwise_r_kernel<LoadDensity, StoreNull, true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
+    { const char *e = getenv("ARCHE_RBLOCKS"); c->r_blocks = (e && e[0] == '4') ? 4 : 3; }
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, kFdTabBytes));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
     c->sm_count = sms;
@@ -488,7 +497,9 @@ int scf_iteration(arche_ctx *c) {
     rc = fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{c->V_i}, PC_FFT_INV_Z, PC_FFT_INV_X);
     if (rc) return rc;
     { ProfScope ps(c, PC_VI_R);
-      pointwise_r_kernel<LoadReal, StoreVi, true, 4><<<prt(4), 256, 0, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
+      if (c->r_blocks == 4) pointwise_r_kernel<LoadReal, StoreVi, true, 4><<<prt(4), 256, kFdTabBytes, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab);
+      else pointwise_r_kernel<LoadReal, StoreVi, true, 3><<<prt(3), 256, kFdTabBytes, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab);
+      LAUNCHED(c); }
   }
   c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
@@ -497,7 +508,7 @@ int scf_iteration(arche_ctx *c) {
     DevScalars *asc = c->sc; const double *atab = c->fdtab; double *apart = c->partials;
     int amax = kMuMaxPasses; const int *astop = c->stop;
     void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax, &astop};
-    CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, 0, c->stream));
+    CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, kFdTabBytes, c->stream));
     ++c->launches; }
   // S4 + S5 (+ w, F, stop flags in the last block of the G-space reduction)
   LoadDensity ldn;
@@ -512,7 +523,9 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_DENS_R);
-      pointwise_r_kernel<LoadDensity, StoreNull, true, 4><<<prt(4), 256, 0, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab); LAUNCHED(c); }
+      if (c->r_blocks == 4) pointwise_r_kernel<LoadDensity, StoreNull, true, 4><<<prt(4), 256, kFdTabBytes, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab);
+      else pointwise_r_kernel<LoadDensity, StoreNull, true, 3><<<prt(3), 256, kFdTabBytes, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab);
+      LAUNCHED(c); }
     rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
     if (rc) return rc;
     { ProfScope ps(c, PC_RED_G);
@@ -864,7 +877,7 @@ extern "C" int arche_fermi_dirac(arche_ctx *c, int twice_j, const double *d_eta,
   if (!c || !d_eta || !d_out || (twice_j != -1 && twice_j != 1 && twice_j != 3)) return ARCHE_EINVAL;
   if (n == 0) return ARCHE_OK;
   int blocks = (int)((n + 255) / 256 < (size_t)kEwBlocks ? (n + 255) / 256 : kEwBlocks);
-  fermi_dirac_kernel<<<blocks, 256, 0, c->stream>>>(twice_j, d_eta, d_out, n, c->fdtab);
+  fermi_dirac_kernel<<<blocks, 256, kFdTabBytes, c->stream>>>(twice_j, d_eta, d_out, n, c->fdtab);
   LAUNCHED(c);
   return ARCHE_OK;
 }

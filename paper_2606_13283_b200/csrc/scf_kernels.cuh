@@ -43,21 +43,57 @@ struct ScfConst {
 // Perdew-Zunger 1981 LDA (unpolarised), Hartree units; restated from the publication (reading D5).
 // One reciprocal cube root gives r_s and n^(1/3) (no division), one reciprocal serves eps_c and V_c on the r_s >= 1
 // branch; the branch is decided on r_s in fp64 exactly as in the oracle (reading A13).
-__device__ __forceinline__ void xc_pz81(double n, double &eps, double &v) {
+// xc = 1: the constants as printed (C = 0.0020, D = -0.0116: eps_c and V_c jump by ~3e-5 Ha at r_s = 1);
+// xc = 2: C and D at full precision from the two matching conditions Perdew and Zunger imposed at r_s = 1 (eps_c and
+//         d eps_c/d r_s continuous) with the other five printed constants -- they round to the printed values; eps_c and
+//         V_c are then continuous and the SCF has a fixed point on every grid (reading A13b).
+namespace pz81 {
+constexpr double g = -0.1423, b1 = 1.0529, b2 = 0.3334, A = 0.0311, B = -0.048;
+constexpr double den1 = 1.0 + b1 + b2, ec1 = g / den1, dec1 = -g * (0.5 * b1 + b2) / (den1 * den1);
+constexpr double D_mod = ec1 - B, C_mod = dec1 - A - D_mod;   // 0.0020191519..., -0.0116320663...
+}  // namespace pz81
+// 1/x for normal x: MUFU.RCP64H seed (20 bits) + two Newton steps (4 DFMA), branch-free.  The compiler's fp64 division
+// and __drcp_rn carry a slow-path branch and ~2x the instructions; the result here is within 1 ulp.
+__device__ __forceinline__ double rcp_fast(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+// u = n^(-1/6) for n > 0: every power PZ81 needs is a product of u (r_s = c u^2, sqrt r_s = sqrt(c) u, n^(1/3) = n u^4),
+// so one Newton iteration chain replaces a cube root and a square root.  fp32 seed exp2(-log2(n)/6) (two MUFU), two
+// steps of u <- u + u (1 - n u^6)/6 (quadratic: 1e-6 -> 4e-12 -> round-off).  Densities below the fp32 range (the
+// empty cores at T = 1 eV) are scaled by 2^96 first: u(n) = 2^16 u(2^96 n).
+__device__ __forceinline__ double inv_sixth_root(double n) {
+  const bool tiny = n < 1.0e-30;
+  const double ns = tiny ? n * 79228162514264337593543950336.0 : n;   // 2^96
+  float seed = exp2f(__log2f((float)ns) * (-1.0f / 6.0f));
+  double u = (double)seed;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    const double u2 = u * u, u6 = u2 * u2 * u2;
+    u = fma(u * (1.0 / 6.0), fma(-ns, u6, 1.0), u);
+  }
+  return tiny ? u * 65536.0 : u;
+}
+__device__ __forceinline__ void xc_pz81(double n, double &eps, double &v, int xc = 1) {
   if (!(n > 0.0)) { eps = 0.0; v = 0.0; return; }
-  const double cx = 0.73855876638202240588;  // (3/4) (3/pi)^(1/3)
-  const double r = rcbrt(n);
-  const double n13 = n * r * r;
-  const double ex = -cx * n13;
-  const double rs = 0.62035049089940001667 * r;  // (3/(4 pi))^(1/3) n^(-1/3)
+  const double cx = 0.73855876638202240588;   // (3/4) (3/pi)^(1/3)
+  const double c0 = 0.62035049089940001667;   // (3/(4 pi))^(1/3): r_s = c0 n^(-1/3)
+  const double sc0 = 0.78762331789974325053;  // sqrt(c0)
+  const double u = inv_sixth_root(n), u2 = u * u;
+  const double ex = -cx * (n * (u2 * u2));
+  const double rs = c0 * u2;
   double ec, vc;
   if (rs >= 1.0) {
-    const double g = -0.1423, b1 = 1.0529, b2 = 0.3334;
-    const double sq = sqrt(rs), inv = __drcp_rn(1.0 + b1 * sq + b2 * rs);
-    ec = g * inv;
-    vc = ec * (1.0 + (7.0 / 6.0) * b1 * sq + (4.0 / 3.0) * b2 * rs) * inv;
+    const double a1 = pz81::b1 * sc0, a2 = pz81::b2 * c0;     // beta1 sqrt(r_s) = a1 u, beta2 r_s = a2 u^2
+    const double inv = rcp_fast(fma(a2, u2, fma(a1, u, 1.0)));
+    ec = pz81::g * inv;
+    vc = ec * fma((4.0 / 3.0) * a2, u2, fma((7.0 / 6.0) * a1, u, 1.0)) * inv;
   } else {
-    const double A = 0.0311, B = -0.048, C = 0.0020, D = -0.0116;
+    const double A = pz81::A, B = pz81::B, C = xc == 2 ? pz81::C_mod : 0.0020, D = xc == 2 ? pz81::D_mod : -0.0116;
     const double l = log(rs);
     ec = A * l + B + C * rs * l + D * rs;
     vc = A * l + (B - A / 3.0) + (2.0 / 3.0) * C * rs * l + (2.0 * D - C) / 3.0 * rs;
@@ -150,24 +186,30 @@ struct StoreVi {
     double v = re * inv_vol;
     double ni = n_i[idx];
     if (mix) { const double na = n_a[idx]; ni = fma(w, ni - na, na); n_i[idx] = ni; }
-    if (xc) { double e, vx; xc_pz81(ni, e, vx); v += vx; }
+    if (xc) { double e, vx; xc_pz81(ni, e, vx, xc); v += vx; }
     V_i[idx] = v;
     acc_min = fmin(acc_min, v); acc_max = fmax(acc_max, v); acc_sum += v;
     if (have_mu) { double a, b, c; fd_eval<2>(fdtab, (mu0 - v) * inv_kT, a, b, c); acc_n += b; }
   }
-  // two elements at once (the two lines of an x-pass pair): interleaves the two Fermi-Dirac evaluations
-  __device__ __forceinline__ void store_real2(long long ia, long long ib, double ra, double rb) {
+  // two elements at once (the two lines of an x-pass pair): interleaves the two Fermi-Dirac evaluations.  Split into
+  // fetch (the global loads) and compute so that the streaming kernel can issue the next pair's loads before it works
+  // on the current pair.
+  struct Pre { double ni0, ni1, na0, na1; };
+  __device__ __forceinline__ void fetch(long long ia, long long ib, Pre &p) const {
+    p.ni0 = n_i[ia]; p.ni1 = n_i[ib];
+    if (mix) { p.na0 = n_a[ia]; p.na1 = n_a[ib]; }
+  }
+  __device__ __forceinline__ void compute(long long ia, long long ib, const Pre &p, double ra, double rb) {
     double v[2] = {ra * inv_vol, rb * inv_vol};
-    double ni[2] = {n_i[ia], n_i[ib]};
+    double ni[2] = {p.ni0, p.ni1};
     if (mix) {
-      const double na0 = n_a[ia], na1 = n_a[ib];
-      ni[0] = fma(w, ni[0] - na0, na0); ni[1] = fma(w, ni[1] - na1, na1);
+      ni[0] = fma(w, ni[0] - p.na0, p.na0); ni[1] = fma(w, ni[1] - p.na1, p.na1);
       n_i[ia] = ni[0]; n_i[ib] = ni[1];
     }
     if (xc) {
       double e, vx;
-      xc_pz81(ni[0], e, vx); v[0] += vx;
-      xc_pz81(ni[1], e, vx); v[1] += vx;
+      xc_pz81(ni[0], e, vx, xc); v[0] += vx;
+      xc_pz81(ni[1], e, vx, xc); v[1] += vx;
     }
     V_i[ia] = v[0]; V_i[ib] = v[1];
     acc_min = fmin(acc_min, fmin(v[0], v[1])); acc_max = fmax(acc_max, fmax(v[0], v[1])); acc_sum += v[0]; acc_sum += v[1];
@@ -176,6 +218,9 @@ struct StoreVi {
       fd_eval_multi<2, 2>(fdtab, eta, a, b, c);
       acc_n += b[0]; acc_n += b[1];
     }
+  }
+  __device__ __forceinline__ void store_real2(long long ia, long long ib, double ra, double rb) {
+    Pre p; fetch(ia, ib, p); compute(ia, ib, p, ra, rb);
   }
   __device__ __forceinline__ void finish(double *smem) {
     double v[4] = {acc_min, acc_max, acc_sum, acc_n};
@@ -216,6 +261,7 @@ __device__ __forceinline__ void mu_accumulate4(const double *tab, const double (
   for (int q = 0; q < 4; ++q) if (ok[q]) { s1 += i12[q]; s0 += im12[q]; }
 }
 
+constexpr size_t kFdTabBytes = sizeof(double) * kFdTabDoubles;
 // s_tab: the Fermi-Dirac table in shared memory (already loaded and synchronised); s_red: [2*32+2]; s_bc: [2];
 // partials: [2][gridDim.x][2], not shared with any other reduction that may run concurrently; sc may be the global
 // scalar block (block 0 writes the result) or a per-block shared copy (sc_is_block_local: every block writes its own)
@@ -257,9 +303,39 @@ __device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &g
           if (want_slope) mu_accumulate4<true>(s_tab, vv, ok, mu, inv_kT, s1, s0);
           else mu_accumulate4<false>(s_tab, vv, ok, mu, inv_kT, s1, s0);
         }
+      } else if (!(ng & 1)) {
+        // streaming pass, lean form (ncu, round 2: this loop issued 74 instructions per point, 55 of them integer/select
+        // bookkeeping on the ALU pipe): 32-bit indices, 16-byte loads of two potentials, no per-element predicates in
+        // the body, the Fermi-Dirac argument from one FMA, the next group's loads in flight during the evaluation
+        const double sA = inv_kT * FD_INV_W, sB = (mu * inv_kT - FD_ETA_A) * FD_INV_W;   // s = sB - v sA
+        const double2 *V2 = reinterpret_cast<const double2 *>(V_i);
+        const int n2 = (int)(ng >> 1), nth = (int)nthreads;
+        int i = (int)tid;
+        const double2 zero2 = make_double2(0.0, 0.0);
+        double2 a = i < n2 ? V2[i] : zero2, b = i + nth < n2 ? V2[i + nth] : zero2;
+        for (; i < n2; i += 2 * nth) {
+          const int in = i + 2 * nth;
+          const double2 an = in < n2 ? V2[in] : zero2, bn = in + nth < n2 ? V2[in + nth] : zero2;
+          if (i + nth < n2) {
+            const double sg[4] = {fma(-a.x, sA, sB), fma(-a.y, sA, sB), fma(-b.x, sA, sB), fma(-b.y, sA, sB)};
+            double im12[4], i12[4], d[4];
+            fd_eval_multi_s<2, 4>(s_tab, sg, im12, i12, d);
+            s1 += (i12[0] + i12[1]) + (i12[2] + i12[3]);
+            if (want_slope) {   // rare (first pass without a previous slope): a second sweep over the same arguments
+              fd_eval_multi_s<1, 4>(s_tab, sg, im12, i12, d);
+              s0 += (im12[0] + im12[1]) + (im12[2] + im12[3]);
+            }
+          } else {
+            const double sg[2] = {fma(-a.x, sA, sB), fma(-a.y, sA, sB)};
+            double im12[2] = {0.0, 0.0}, i12[2], d[2];
+            if (want_slope) fd_eval_multi_s<3, 2>(s_tab, sg, im12, i12, d);
+            else fd_eval_multi_s<2, 2>(s_tab, sg, im12, i12, d);
+            s1 += i12[0] + i12[1]; s0 += im12[0] + im12[1];
+          }
+          a = an; b = bn;
+        }
       } else {
-        // two groups of four loads stay in flight ahead of the evaluation (with 16-24 warps per SM the exposed HBM
-        // latency, not the table reads, bounded this loop)
+        // odd point count (all three axes powers of 3): element-wise form
         double va[4], vb[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
@@ -330,7 +406,7 @@ __global__ void __launch_bounds__(256, 3) mu_solve_kernel(const double *__restri
   namespace cg = cooperative_groups;
   if (stop && *stop) return;   // uniform over the grid: no block reaches a barrier
   cg::grid_group grid = cg::this_grid();
-  __shared__ __align__(16) double s_tab[kFdTabDoubles];
+  extern __shared__ __align__(16) double s_tab[];   // kFdTabDoubles (49.5 KB: dynamic, beyond the 48 KB static limit)
   __shared__ double s_red[2 * 32 + 2];
   __shared__ double s_bc[2];
   fd_load_tables(s_tab, fdtab);
@@ -363,17 +439,21 @@ struct LoadDensity {
     const double chi = C.cTF * 0.5 * im12 * inv_kT;   // dn_a/dmu
     const double dn = n_i[g] - na;
     n_a[g] = na;
-    if (chi > 0.0) sK += dn * dn / chi;               // Eq. 31
+    if (chi > 1.0e-290) sK += dn * dn * rcp_fast(chi);   // Eq. 31
     sdn2 += dn * dn; sna2 += na * na; sChi += chi;
     sF0 += eta * i12 - (2.0 / 3.0) * i32;             // f_0/(kT cTF), from Eq. 38-39
     sKe += i32;                                       // Eq. 38
-    if (C.xc) { double e, vx; xc_pz81(na, e, vx); sExc += na * e; }
+    if (C.xc) { double e, vx; xc_pz81(na, e, vx, C.xc); sExc += na * e; }
     return na;
   }
-  __device__ __forceinline__ void load_real2(long long ia, long long ib, double &ra, double &rb) {
+  struct Pre { double v0, v1, n0, n1; };
+  __device__ __forceinline__ void fetch(long long ia, long long ib, Pre &p) const {
+    p.v0 = V_i[ia]; p.v1 = V_i[ib]; p.n0 = n_i[ia]; p.n1 = n_i[ib];
+  }
+  __device__ __forceinline__ void compute(long long ia, long long ib, const Pre &p, double &ra, double &rb) {
     const long long g[2] = {ia, ib};
-    double eta[2] = {(mu - V_i[ia]) * inv_kT, (mu - V_i[ib]) * inv_kT}, im12[2], i12[2], i32[2];
-    const double ni[2] = {n_i[ia], n_i[ib]};
+    double eta[2] = {(mu - p.v0) * inv_kT, (mu - p.v1) * inv_kT}, im12[2], i12[2], i32[2];
+    const double ni[2] = {p.n0, p.n1};
     fd_eval_multi<7, 2>(fdtab, eta, im12, i12, i32);
     double na[2];
 #pragma unroll
@@ -382,13 +462,16 @@ struct LoadDensity {
       const double chi = C.cTF * 0.5 * im12[m] * inv_kT;
       const double dn = ni[m] - na[m];
       n_a[g[m]] = na[m];
-      if (chi > 0.0) sK += dn * dn / chi;
+      if (chi > 1.0e-290) sK += dn * dn * rcp_fast(chi);   // Eq. 31 (chi underflows only where n_a does: no weight)
       sdn2 += dn * dn; sna2 += na[m] * na[m]; sChi += chi;
       sF0 += eta[m] * i12[m] - (2.0 / 3.0) * i32[m];
       sKe += i32[m];
-      if (C.xc) { double e, vx; xc_pz81(na[m], e, vx); sExc += na[m] * e; }
+      if (C.xc) { double e, vx; xc_pz81(na[m], e, vx, C.xc); sExc += na[m] * e; }
     }
     ra = na[0]; rb = na[1];
+  }
+  __device__ __forceinline__ void load_real2(long long ia, long long ib, double &ra, double &rb) {
+    Pre p; fetch(ia, ib, p); compute(ia, ib, p, ra, rb);
   }
   __device__ __forceinline__ void finish(double *smem) {
     double v[7] = {sK, sdn2, sna2, sF0, sKe, sExc, sChi};
@@ -416,6 +499,9 @@ struct LoadReal {
   __device__ __forceinline__ void operator()(long long idx, int, int, int, double &re, double &im) { re = src[idx]; im = 0.0; }
   __device__ __forceinline__ double load_real(long long idx, int, int, int) { return src[idx]; }
   __device__ __forceinline__ void load_real2(long long ia, long long ib, double &ra, double &rb) { ra = src[ia]; rb = src[ib]; }
+  struct Pre { double a, b; };
+  __device__ __forceinline__ void fetch(long long ia, long long ib, Pre &p) const { p.a = src[ia]; p.b = src[ib]; }
+  __device__ __forceinline__ void compute(long long, long long, const Pre &p, double &ra, double &rb) { ra = p.a; rb = p.b; }
   __device__ __forceinline__ void finish(double *) {}
 };
 
@@ -647,7 +733,11 @@ struct StoreRealPlain {
 struct StoreNull {
   __device__ __forceinline__ void set_table(const double *) {}
   __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long) const {}
   __device__ __forceinline__ void store_real2(long long, long long, double, double) {}
+  struct Pre {};
+  __device__ __forceinline__ void fetch(long long, long long, Pre &) const {}
+  __device__ __forceinline__ void compute(long long, long long, const Pre &, double, double) {}
   __device__ __forceinline__ void finish(double *) {}
 };
 
@@ -677,7 +767,7 @@ template <class LoadOp, class StoreOp, bool SMEM_TAB = false, int MIN_BLOCKS = 1
 __global__ void __launch_bounds__(256, MIN_BLOCKS) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng, const int *stop,
                                                           const double *__restrict__ g_tab = nullptr) {
   __shared__ double s_red[kMaxRed * 33];
-  __shared__ __align__(16) double s_tab[SMEM_TAB ? kFdTabDoubles : 2];
+  extern __shared__ __align__(16) double s_tab[];   // SMEM_TAB: kFdTabDoubles doubles of dynamic shared memory
   if (stop && *stop) return;
   LoadOp ld = ld_in;
   StoreOp st = st_in;
@@ -687,11 +777,21 @@ __global__ void __launch_bounds__(256, MIN_BLOCKS) pointwise_r_kernel(LoadOp ld_
     ld.set_table(s_tab); st.set_table(s_tab);
   }
   ld.begin(); st.begin();
-  const long long half = ng / 2;
-  for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < half; g += (long long)gridDim.x * blockDim.x) {
+  // software pipeline: the operands of the thread's next pair are loaded before it evaluates the current pair (ncu, round
+  // 2: the first use of the loaded potentials was the hottest instruction of these kernels -- nothing else covered the
+  // HBM latency at 24-32 warps per SM; an L2 prefetch hint instead of register loads made them slower)
+  const long long half = ng / 2, stride = (long long)gridDim.x * blockDim.x;
+  long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  typename LoadOp::Pre pl, pln;
+  typename StoreOp::Pre ps, psn;
+  if (g < half) { ld.fetch(g, g + half, pl); st.fetch(g, g + half, ps); }
+  for (; g < half; g += stride) {
+    const long long gn = g + stride;
+    if (gn < half) { ld.fetch(gn, gn + half, pln); st.fetch(gn, gn + half, psn); }
     double a, b;
-    ld.load_real2(g, g + half, a, b);
-    st.store_real2(g, g + half, a, b);
+    ld.compute(g, g + half, pl, a, b);
+    st.compute(g, g + half, ps, a, b);
+    pl = pln; ps = psn;
   }
   ld.finish(s_red);
   st.finish(s_red);
@@ -730,7 +830,7 @@ __global__ void compress_half_kernel(double2 *__restrict__ dst, const double2 *_
 }
 
 __global__ void fermi_dirac_kernel(int twice_j, const double *eta, double *out, size_t n, const double *fdtab) {
-  __shared__ __align__(16) double s_tab[kFdTabDoubles];
+  extern __shared__ __align__(16) double s_tab[];   // kFdTabDoubles
   fd_load_tables(s_tab, fdtab);
   __syncthreads();
   for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < n; g += (size_t)gridDim.x * blockDim.x) {

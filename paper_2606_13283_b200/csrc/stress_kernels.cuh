@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(kStressThreads) stress_fields_kernel(
     for (long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x; r < G.ng; r += stride) {
       const double n = n_a[r];
       double ex, vx;
-      xc_pz81(n, ex, vx);
+      xc_pz81(n, ex, vx, xc);
       acc[20] += n * (ex - vx);
     }
   int op[kStressSums];

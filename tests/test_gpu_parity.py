@@ -124,7 +124,7 @@ def pointwise_mode(request, monkeypatch):
     return request.param
 
 
-@pytest.mark.parametrize("xc", [0, 1])
+@pytest.mark.parametrize("xc", [0, 1, 2])
 def test_single_scf_iteration(orc, torch_cuda, xc, pointwise_mode):
     cfg = ai.make_small(n_ions=4, L=8.0, grid=(16, 12, 24), T_eV=10.0, seed=8)
     g = _gpu(cfg, xc=xc); o = orc.Oracle(cfg, xc=xc)

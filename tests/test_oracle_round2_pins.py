@@ -11,6 +11,11 @@ from flip_case import KW as FLIP_KW, NSTAR, find_flip_case
 PI = np.pi
 
 
+@pytest.fixture(scope="module")
+def flip(orc):
+    return find_flip_case(orc)
+
+
 # ---------------------------------------------------------------- PZ81 (reading D5): constants of both branches
 def test_pz81_values_written_out_by_hand(orc):
     """eps_c and V_c at r_s = 0.5 (log branch) and r_s = 2 (Pade branch) evaluated BY HAND from the constants printed in
@@ -54,12 +59,45 @@ def test_pz81_C_and_D_follow_from_continuity_at_rs_1(orc):
     assert 2e-5 < abs(lo[0] - hi[0]) < 5e-5 and 2e-5 < abs(lo[1] - hi[1]) < 5e-5
 
 
+def test_pz81_continuous_variant(orc):
+    """xc = 2 (reading A13b): C and D at full precision from the continuity conditions.  Pins: the constants (derived here
+    again, independently, and by hand: C = 0.00201915, D = -0.01163207), continuity of eps_c and V_c at r_s = 1 to
+    round-off, identity with xc = 1 on the Pade branch, the size of the difference on the log branch, a hand value at
+    r_s = 0.5, and V_xc = d(n eps_xc)/dn across the branch point."""
+    g, b1, b2, A, B = -0.1423, 1.0529, 0.3334, 0.0311, -0.048
+    den = 1.0 + b1 + b2                                   # 2.3863
+    D = g / den - B                                       # -0.059632066 + 0.048      = -0.011632066
+    C = -g * (0.5 * b1 + b2) / den ** 2 - A - D           # 0.021487085 - 0.0311 + 0.011632066 = 0.002019152
+    assert abs(D - (-0.011632066)) < 1e-9 and abs(C - 0.002019152) < 1e-9
+    lo, hi = orc.xc(NSTAR * (1 + 1e-13), 2), orc.xc(NSTAR * (1 - 1e-13), 2)
+    assert abs(lo[0] - hi[0]) < 1e-12 and abs(lo[1] - hi[1]) < 1e-12   # continuous: only the 2e-13 step in n (xc = 1: 3e-5)
+    for n in (1e-4, 0.01, 0.2, NSTAR * 0.999):
+        assert orc.xc(n, 2) == orc.xc(n, 1)                                       # r_s >= 1: the same branch
+    for rs in (0.9, 0.5, 0.1):
+        n = 3.0 / (4.0 * PI * rs ** 3)
+        d = orc.xc(n, 2)[0] - orc.xc(n, 1)[0]
+        assert abs(d - ((C - 0.0020) * rs * np.log(rs) + (D + 0.0116) * rs)) < 1e-15 and abs(d) < 4e-5
+    # r_s = 0.5 by hand: 0.0311(-0.693147181) - 0.048 + 0.002019152(0.5)(-0.693147181) - 0.011632066(0.5)
+    #                  = -0.021556877 - 0.048 - 0.000699785 - 0.005816033 = -0.076072695
+    n = 3.0 / (4.0 * PI * 0.5 ** 3)
+    assert abs(orc.xc(n, 2)[0] + 0.75 * (3.0 * n / PI) ** (1.0 / 3.0) - (-0.076072695)) < 2e-9
+    for n in (0.05, NSTAR, 0.3, 1.7):                                             # derivative identity, also AT n*
+        h = 1e-5 * n
+        dfdn = ((n + h) * orc.xc(n + h, 2)[0] - (n - h) * orc.xc(n - h, 2)[0]) / (2 * h)
+        assert abs(dfdn / orc.xc(n, 2)[1] - 1) < 1e-8, n
+
+
+def test_continuous_variant_has_a_fixed_point_where_pz81_as_printed_flips(orc, flip):
+    """the constructed branch-flip case (one grid point on n*) with xc = 2: the SCF converges under the STRICT rule"""
+    cfg, Ne, _, _, g0 = flip
+    o = orc.Oracle(cfg, n_electrons=Ne, xc=2, **FLIP_KW)
+    r = o.scf_solve(cfg["pos"])
+    assert r["converged"] == 1 and r["flip_seen"] == 0
+    assert r["tol_F_eff"] == FLIP_KW["scf_tol_F"] and r["dn_l2"] < FLIP_KW["scf_tol_dn"]
+    assert abs(o.get_real("n_a").ravel()[g0] / NSTAR - 1) < 1e-4                  # the point still sits on the branch point
+
+
 # ---------------------------------------------------------------- stop rule with a PZ81 branch flip (reading A13)
-@pytest.fixture(scope="module")
-def flip(orc):
-    return find_flip_case(orc)
-
-
 def test_stop_rule_branch_flip_constructed(orc, flip):
     """One grid point driven across n* = 3/(4 pi): the SCF then has no fixed point (V_c jumps UP by 2.6e-5 Ha when the
     density rises through n*, which pushes the density back down), F hops by whole quanta
