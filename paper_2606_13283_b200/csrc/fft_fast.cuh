@@ -360,6 +360,139 @@ __global__ void __launch_bounds__(LIGHT ? fast_threads_x_light<N>() : fast_threa
   st.finish(smem_raw);
 }
 
+// ---- register-centric x passes (plain passes of the streamed form) -----------------------------------------------
+// The tile kernels above move every element through shared memory seven times (load, two in-place stages, Hermitian
+// split: 112 bytes of shared-memory traffic per packed complex element against 16 bytes of HBM traffic) and were bound
+// by the shared-memory data pipe (ncu, round 1: LSU data pipe 75%, x passes at 0.55-0.61 of the HBM peak while the y/z
+// passes reach 0.75-0.9).  Here both stages live in registers like in the y/z kernels: stage 1 loads global memory
+// straight into registers, one exchange through shared memory between the stages, stage 2 stores straight from
+// registers -- and the Hermitian pairing z[k] <-> z[N-k] exchanges only the upper half of the spectrum (k >= N/2 is
+// written, k <= N/2 reads its partner): 48 bytes of shared-memory traffic per element.
+//   r2c: z = a + i b of two real lines;  A[k] = (z[k] + conj z[N-k])/2,  B[k] = (z[k] - conj z[N-k])/(2i),  k <= N/2.
+//   c2r: z[k] = conj(A[k] + i B[k]), z[N-k] = conj(conj A[k] + i conj B[k]); forward stages; a = Re z, b = -Im z.
+template <int N> __host__ __device__ constexpr int reg_threads_x() {
+  return kFastLPLight * (FastPlan<N>::R1 > FastPlan<N>::R2 ? FastPlan<N>::R1 : FastPlan<N>::R2);
+}
+template <int N> __host__ __device__ constexpr int reg_blocks_x() { return N >= 384 ? 5 : (N >= 256 ? 6 : 8); }
+// the r2c kernel needs all 2 R1 stage-1 loads of a thread in flight at once (168 registers at N = 384: with 126 ptxas
+// consumed the first loads before it issued the last and the HBM latency was paid three to four times per tile)
+template <int N> __host__ __device__ constexpr int reg_blocks_r2c() { return N >= 384 ? 4 : (N >= 192 ? 5 : 8); }
+
+template <int N, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(reg_threads_x<N>(), reg_blocks_r2c<N>()) fft_r2c_reg_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, ROW = fast_row_x<N>(), LP = kFastLPLight;
+  static_assert(R2 % 2 == 0, "the Hermitian exchange splits stage-2 outputs at q = R2/2");
+  extern __shared__ double smem_raw[];
+  double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
+  ld.begin(); st.begin();
+  const int t = threadIdx.x;
+  const long long line0 = (long long)blockIdx.x * (2 * LP);
+  if (t < LP * R2) {   // stage 1: global -> registers -> shared
+    const int p = t / R2, j1 = t % R2;
+    const long long la = (line0 + 2 * p) * N, lb = la + N;
+    double2 v[R1];
+#pragma unroll
+    for (int q = 0; q < R1; ++q) ld.load_real2(la + j1 + q * R2, lb + j1 + q * R2, v[q].x, v[q].y);
+    Dft<R1>::run(v);
+#pragma unroll
+    for (int q = 0; q < R1; ++q) buf[p * ROW + j1 * (R1 + 1) + q] = v[q];
+  }
+  __syncthreads();
+  const bool act = t < LP * R1;
+  const int p = t / R1, j2 = t % R1;
+  double2 v[R2];
+  if (act) {           // stage 2: shared -> registers; v[q] = z[j2 + q R1]
+#pragma unroll
+    for (int q = 0; q < R2; ++q) v[q] = buf[p * ROW + j2 + q * (R1 + 1)];
+#pragma unroll
+    for (int q = 1; q < R2; ++q) v[q] = cmul(v[q], G.tw[q * j2]);
+    Dft<R2>::run(v);
+  }
+  __syncthreads();
+  if (act) {           // upper half of the spectrum (k >= N/2) to shared memory, natural order
+#pragma unroll
+    for (int q = R2 / 2; q < R2; ++q) buf[p * ROW + j2 + q * R1] = v[q];
+  }
+  __syncthreads();
+  if (act) {           // k <= N/2 takes its partner z[N-k] and stores A[k], B[k] straight from registers
+    const long long la = line0 + 2 * p, lb = la + 1;
+    const int iya = (int)(la % G.ny), iza = (int)(la / G.ny), iyb = (int)(lb % G.ny), izb = (int)(lb / G.ny);
+#pragma unroll
+    for (int q = 0; q <= R2 / 2; ++q) {
+      if (q == R2 / 2 && j2 != 0) break;          // k = N/2 belongs to j2 = 0 only
+      const int k = j2 + q * R1;
+      const double2 z = v[q], m = k == 0 ? v[0] : buf[p * ROW + (N - k)];
+      st.store(la * G.P + k, k, iya, iza, 0.5 * (z.x + m.x), 0.5 * (z.y - m.y));
+      st.store(lb * G.P + k, k, iyb, izb, 0.5 * (z.y + m.y), -0.5 * (z.x - m.x));
+    }
+  }
+  ld.finish(smem_raw);
+  st.finish(smem_raw);
+}
+
+template <int N, class LoadOp, class StoreOp>
+__global__ void __launch_bounds__(reg_threads_x<N>(), reg_blocks_x<N>()) fft_c2r_reg_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
+  constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, ROW = fast_row_x<N>(), LP = kFastLPLight;
+  static_assert(R1 % 2 == 0, "the Hermitian exchange splits stage-1 inputs at q = R1/2");
+  extern __shared__ double smem_raw[];
+  double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
+  LoadOp ld = ld_in;
+  StoreOp st = st_in;
+  if (G.stop && *G.stop) return;
+  ld.begin(); st.begin();
+  const int t = threadIdx.x;
+  const long long line0 = (long long)blockIdx.x * (2 * LP);
+  const bool act1 = t < LP * R2;
+  const int p1 = t / R2, j1 = t % R2;
+  double2 v1[R1];
+  if (act1) {          // i = j1 + q R2 <= N/2: load A[i], B[i]; keep z[i], hand z[N-i] to its owner through shared memory
+    const long long la = line0 + 2 * p1, lb = la + 1;
+    const int iya = (int)(la % G.ny), iza = (int)(la / G.ny), iyb = (int)(lb % G.ny), izb = (int)(lb / G.ny);
+#pragma unroll
+    for (int q = 0; q <= R1 / 2; ++q) {
+      if (q == R1 / 2 && j1 != 0) break;          // i = N/2 belongs to j1 = 0 only
+      const int i = j1 + q * R2;
+      double2 A, B;
+      ld(la * G.P + i, i, iya, iza, A.x, A.y);
+      ld(lb * G.P + i, i, iyb, izb, B.x, B.y);
+      v1[q] = make_double2(A.x - B.y, -(A.y + B.x));                                         // conj(A + i B)
+      if (i > 0 && 2 * i < N) buf[p1 * ROW + (N - i)] = make_double2(A.x + B.y, A.y - B.x);   // conj(conj A + i conj B)
+    }
+  }
+  __syncthreads();
+  if (act1) {
+#pragma unroll
+    for (int q = R1 / 2; q < R1; ++q) {
+      if (q == R1 / 2 && j1 == 0) continue;       // loaded above
+      v1[q] = buf[p1 * ROW + j1 + q * R2];
+    }
+    Dft<R1>::run(v1);
+  }
+  __syncthreads();
+  if (act1) {
+#pragma unroll
+    for (int q = 0; q < R1; ++q) buf[p1 * ROW + j1 * (R1 + 1) + q] = v1[q];
+  }
+  __syncthreads();
+  if (t < LP * R1) {   // stage 2: shared -> registers -> global (real lines)
+    const int p = t / R1, j2 = t % R1;
+    const long long la = (line0 + 2 * p) * N, lb = la + N;
+    double2 v[R2];
+#pragma unroll
+    for (int q = 0; q < R2; ++q) v[q] = buf[p * ROW + j2 + q * (R1 + 1)];
+#pragma unroll
+    for (int q = 1; q < R2; ++q) v[q] = cmul(v[q], G.tw[q * j2]);
+    Dft<R2>::run(v);
+#pragma unroll
+    for (int q = 0; q < R2; ++q) st.store_real2(la + j2 + q * R1, lb + j2 + q * R1, v[q].x, -v[q].y);
+  }
+  ld.finish(smem_raw);
+  st.finish(smem_raw);
+}
+
 // ---- host dispatch ------------------------------------------------------------------------------------------
 template <int N, int AXIS, bool INVERSE, class LoadOp, class StoreOp>
 static inline cudaError_t fft_launch_yz_fast_n(const FastGeom &G, LoadOp ld, StoreOp st, cudaStream_t stream) {
@@ -398,29 +531,26 @@ static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, Stor
   size_t smem = sizeof(double2) * LP * fast_row_x<N>();
   if (smem < 4096) smem = 4096;
   const unsigned blocks = (unsigned)((long long)G.ny * G.nz / (2 * LP));
-  constexpr int TH = LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>();
+  constexpr int TH = LIGHT ? reg_threads_x<N>() : fast_threads_x<N>();
   static int attr_dev = -1;
   int dev = 0;
   cudaGetDevice(&dev);
   const bool attr_set = attr_dev == dev;
+  const void *kern;
   if constexpr (INVERSE) {
-    auto kern = fft_c2r_fast_kernel<N, LIGHT, LoadOp, StoreOp>;
-    if (!attr_set) {
-      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-      if (e != cudaSuccess) return e;
-      attr_dev = dev;
-    }
-    kern<<<blocks, TH, smem, stream>>>(G, ld, st);
+    if constexpr (LIGHT) kern = (const void *)fft_c2r_reg_kernel<N, LoadOp, StoreOp>;
+    else kern = (const void *)fft_c2r_fast_kernel<N, false, LoadOp, StoreOp>;
   } else {
-    auto kern = fft_r2c_fast_kernel<N, LIGHT, LoadOp, StoreOp>;
-    if (!attr_set) {
-      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-      if (e != cudaSuccess) return e;
-      attr_dev = dev;
-    }
-    kern<<<blocks, TH, smem, stream>>>(G, ld, st);
+    if constexpr (LIGHT) kern = (const void *)fft_r2c_reg_kernel<N, LoadOp, StoreOp>;
+    else kern = (const void *)fft_r2c_fast_kernel<N, false, LoadOp, StoreOp>;
   }
-  return cudaGetLastError();
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (e != cudaSuccess) return e;
+    attr_dev = dev;
+  }
+  void *args[] = {(void *)&G, (void *)&ld, (void *)&st};
+  return cudaLaunchKernel(kern, dim3(blocks), dim3(TH), args, smem, stream);
 }
 // LIGHT: the functors do no arithmetic worth extra threads (plain loads/stores): butterfly threads only, 3-4 blocks per SM
 template <bool INVERSE, bool LIGHT, class LoadOp, class StoreOp>
