@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  bool pdl;        // programmatic dependent launch between the kernels of an SCF iteration (ARCHE_PDL=0 disables)
   int r_blocks;    // resident blocks per SM of the streamed real-space Fermi-Dirac kernels
   int force_slabs, force_rows_per_slab, force_ipt;   // ions per thread of the force kernel's register tile
   // device arrays (all inside the caller's workspace)
@@ -155,6 +156,18 @@ struct ProfScope {  // records an event pair around the launches issued in its l
   }
   ~ProfScope() { if (k >= 0) cudaEventRecord(c->prof_ev[2 * k + 1], c->stream); }
 };
+
+// launch on the context's stream, with programmatic stream serialization when enabled (kernels call pdl_wait())
+template <class... KArgs, class... Args>
+cudaError_t launch_k(arche_ctx *c, void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = c->pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, args...);
+}
 
 int fft_tile_blocks(int axis, int n, int nx, int ny, int nz) {
   int L = fft_pick_L(axis, n, nx, ny, nz);
@@ -338,6 +351,10 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     CK(cudaFuncSetAttribute(pointwise_r_kernel<LoadReal, StoreVi, true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
     CK(cudaFuncSetAttribute(pointwise_r_kernel<LoadDensity, StoreNull, true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
     { const char *e = getenv("ARCHE_RBLOCKS"); c->r_blocks = (e && e[0] == '4') ? 4 : 3; }
+    // programmatic dependent launch pays where launches are short (measured: 128^3 0.209 -> 0.185 ms per iteration, c3
+    // 155 -> 177 MD steps/s, 192^3 +1.4%) and costs ~2% at 384^3, where early-resident blocks of the next kernel take
+    // shared memory from the tail of the running one: on by default up to 8 M grid points
+    { const char *e = getenv("ARCHE_PDL"); c->pdl = e ? e[0] != '0' : c->ng <= 8000000LL; }
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, kFdTabBytes));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
@@ -396,7 +413,7 @@ namespace {
 template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
 cudaError_t pass_yz(arche_ctx *c, LoadOp ld, StoreOp st) {
   const int ny = c->G.ny, nz = c->G.nz, P = c->P, n = AXIS == 1 ? ny : nz;
-  FastGeom fg{c->G.nx, ny, nz, P, c->tw[AXIS], c->stop};
+  FastGeom fg{c->G.nx, ny, nz, P, c->tw[AXIS], c->stop, c->pdl ? 1 : 0};
   cudaError_t e = c->use_fast ? fft_launch_yz_fast<AXIS, INVERSE>(n, fg, ld, st, c->stream) : cudaErrorNotSupported;
   if (e == cudaErrorNotSupported) { c->plan[AXIS].stop = c->stop; e = fft_launch_pass<AXIS, INVERSE>(c->plan[AXIS], P, ny, nz, ld, st, c->stream); }
   return e;
@@ -404,7 +421,7 @@ cudaError_t pass_yz(arche_ctx *c, LoadOp ld, StoreOp st) {
 template <bool INVERSE, class LoadOp, class StoreOp>
 cudaError_t pass_x(arche_ctx *c, LoadOp ld, StoreOp st) {
   const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
-  FastGeom fg{nx, ny, nz, P, c->tw[0], c->stop};
+  FastGeom fg{nx, ny, nz, P, c->tw[0], c->stop, c->pdl ? 1 : 0};
   // plain passes of the streamed form run the light configuration (LoadReal / StoreRealPlain / LoadComplex / StoreComplex)
   constexpr bool plain = (std::is_same<LoadOp, LoadReal>::value || std::is_same<LoadOp, LoadComplex>::value) &&
                          (std::is_same<StoreOp, StoreComplex>::value || std::is_same<StoreOp, StoreRealPlain>::value);
@@ -493,13 +510,13 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_POT_G);
-      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(lp, StoreComplex{c->work}, c->P, G.ny, c->nh, c->stop); LAUNCHED(c); }
+      CK(launch_k(c, pointwise_g_kernel<LoadPotentialG, StoreComplex>, pg, 256, 0, lp, StoreComplex{c->work}, c->P, G.ny, c->nh, c->stop)); ++c->launches; }
     rc = fft3d_inverse(c, LoadComplex{c->work}, StoreRealPlain{c->V_i}, PC_FFT_INV_Z, PC_FFT_INV_X);
     if (rc) return rc;
     { ProfScope ps(c, PC_VI_R);
-      if (c->r_blocks == 4) pointwise_r_kernel<LoadReal, StoreVi, true, 4><<<prt(4), 256, kFdTabBytes, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab);
-      else pointwise_r_kernel<LoadReal, StoreVi, true, 3><<<prt(3), 256, kFdTabBytes, c->stream>>>(LoadReal{c->V_i}, sv, c->ng, c->stop, c->fdtab);
-      LAUNCHED(c); }
+      if (c->r_blocks == 4) CK(launch_k(c, pointwise_r_kernel<LoadReal, StoreVi, true, 4>, prt(4), 256, kFdTabBytes, LoadReal{c->V_i}, sv, c->ng, c->stop, (const double *)c->fdtab));
+      else CK(launch_k(c, pointwise_r_kernel<LoadReal, StoreVi, true, 3>, prt(3), 256, kFdTabBytes, LoadReal{c->V_i}, sv, c->ng, c->stop, (const double *)c->fdtab));
+      ++c->launches; }
   }
   c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
@@ -523,13 +540,13 @@ int scf_iteration(arche_ctx *c) {
     if (rc) return rc;
   } else {
     { ProfScope ps(c, PC_DENS_R);
-      if (c->r_blocks == 4) pointwise_r_kernel<LoadDensity, StoreNull, true, 4><<<prt(4), 256, kFdTabBytes, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab);
-      else pointwise_r_kernel<LoadDensity, StoreNull, true, 3><<<prt(3), 256, kFdTabBytes, c->stream>>>(ldn, StoreNull{}, c->ng, c->stop, c->fdtab);
-      LAUNCHED(c); }
+      if (c->r_blocks == 4) CK(launch_k(c, pointwise_r_kernel<LoadDensity, StoreNull, true, 4>, prt(4), 256, kFdTabBytes, ldn, StoreNull{}, c->ng, c->stop, (const double *)c->fdtab));
+      else CK(launch_k(c, pointwise_r_kernel<LoadDensity, StoreNull, true, 3>, prt(3), 256, kFdTabBytes, ldn, StoreNull{}, c->ng, c->stop, (const double *)c->fdtab));
+      ++c->launches; }
     rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
     if (rc) return rc;
     { ProfScope ps(c, PC_RED_G);
-      pointwise_g_kernel<<<pg, 256, 0, c->stream>>>(LoadComplex{c->nh_a}, sn, c->P, G.ny, c->nh, c->stop); LAUNCHED(c); }
+      CK(launch_k(c, pointwise_g_kernel<LoadComplex, StoreNhatA>, pg, 256, 0, LoadComplex{c->nh_a}, sn, c->P, G.ny, c->nh, c->stop)); ++c->launches; }
   }
   c->mix_pending = true;   // S6 is applied by the next iteration's S1/S2 passes, or by flush_mix()
   c->have_solution = true;

@@ -24,6 +24,46 @@ struct GridGeom {
 // the later (register-limited, partly serialised) loads find their data in L2 instead of paying HBM latency each
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
+// ---- sm_90+/sm_100a launch and copy primitives (inline PTX) --------------------------------------------------------
+// Programmatic dependent launch: a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start
+// while its predecessor in the stream is still draining.  Every such kernel calls pdl_launch_dependents() first (its own
+// successor may be scheduled as soon as all of its blocks are resident), does the work that does not depend on the
+// predecessor (index arithmetic, the Fermi-Dirac table copy), and calls pdl_wait() before it touches anything an earlier
+// kernel wrote -- the wait returns when the predecessor grid has completed and its writes are visible.  Both are
+// no-ops in a kernel launched without the attribute.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// Bulk asynchronous copy global -> shared (the 1D form of the tensor memory accelerator, cp.async.bulk) completing on
+// an mbarrier: one thread issues the copy, the copy engine moves the bytes without passing through registers or the
+// LSU, every thread waits on the barrier's phase.  Sizes and addresses are multiples of 16 bytes.
+__device__ __forceinline__ unsigned smem_addr_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned arrivals) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(arrivals) : "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // make the initialised barrier visible to the copy engine
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(void *smem_dst, const void *gmem_src, unsigned bytes, unsigned long long *bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_addr_u32(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"(smem_addr_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "MBAR_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra MBAR_DONE;\n"
+      "bra MBAR_WAIT;\n"
+      "MBAR_DONE:\n"
+      "}\n" ::"r"(smem_addr_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);

@@ -121,7 +121,20 @@ struct FastGeom {
   int nx, ny, nz, P;        // real grid and half-spectrum pitch
   const double2 *tw;        // exp(-2 pi i a/N) of the transformed axis
   const int *stop;          // optional device flag: non-zero skips the pass
+  int pdl;                  // host side: launch with programmatic stream serialization (common.cuh)
 };
+
+// kernel launch with optional programmatic dependent launch
+static inline cudaError_t launch_maybe_pdl(const void *kern, dim3 grid, dim3 block, void **args, size_t smem, cudaStream_t stream, bool pdl) {
+  if (!pdl) return cudaLaunchKernel(kern, grid, block, args, smem, stream);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelExC(&cfg, kern, args);
+}
 
 constexpr int kFastL = 8;   // columns per y/z tile (128-byte rows)
 template <int N> __host__ __device__ constexpr int fast_threads_yz() {
@@ -214,6 +227,8 @@ __global__ void __launch_bounds__(fast_threads_yz<N>()) fft_yz_fast_kernel(FastG
   extern __shared__ double smem_raw[];
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  pdl_launch_dependents();
+  pdl_wait();
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   fft_yz_tile<N, AXIS, INVERSE, true>(G, ld, st, blockIdx.x, reinterpret_cast<double2 *>(smem_raw), threadIdx.x, 0);
@@ -338,6 +353,8 @@ __global__ void __launch_bounds__(LIGHT ? fast_threads_x_light<N>() : fast_threa
   extern __shared__ double smem_raw[];
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  pdl_launch_dependents();
+  pdl_wait();
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   fft_r2c_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>(), LIGHT ? kFastLPLight : kFastLP>(
@@ -352,6 +369,8 @@ __global__ void __launch_bounds__(LIGHT ? fast_threads_x_light<N>() : fast_threa
   extern __shared__ double smem_raw[];
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  pdl_launch_dependents();
+  pdl_wait();
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   fft_c2r_tile<N, true, LIGHT ? fast_threads_x_light<N>() : fast_threads_x<N>(), LIGHT ? kFastLPLight : kFastLP>(
@@ -386,6 +405,8 @@ __global__ void __launch_bounds__(reg_threads_x<N>(), reg_blocks_r2c<N>()) fft_r
   double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  pdl_launch_dependents();
+  pdl_wait();
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   const int t = threadIdx.x;
@@ -441,6 +462,8 @@ __global__ void __launch_bounds__(reg_threads_x<N>(), reg_blocks_x<N>()) fft_c2r
   double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
   LoadOp ld = ld_in;
   StoreOp st = st_in;
+  pdl_launch_dependents();
+  pdl_wait();
   if (G.stop && *G.stop) return;
   ld.begin(); st.begin();
   const int t = threadIdx.x;
@@ -508,8 +531,8 @@ static inline cudaError_t fft_launch_yz_fast_n(const FastGeom &G, LoadOp ld, Sto
     attr_dev = dev;
   }
   const unsigned blocks = (unsigned)((AXIS == 1 ? G.nz : G.ny) * (G.P / kFastL));
-  kern<<<blocks, fast_threads_yz<N>(), smem, stream>>>(G, ld, st);
-  return cudaGetLastError();
+  void *args[] = {(void *)&G, (void *)&ld, (void *)&st};
+  return launch_maybe_pdl((const void *)kern, dim3(blocks), dim3(fast_threads_yz<N>()), args, smem, stream, G.pdl != 0);
 }
 // returns cudaErrorNotSupported when the axis length has no fast plan (caller falls back to the generic pass)
 template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
@@ -550,7 +573,7 @@ static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, Stor
     attr_dev = dev;
   }
   void *args[] = {(void *)&G, (void *)&ld, (void *)&st};
-  return cudaLaunchKernel(kern, dim3(blocks), dim3(TH), args, smem, stream);
+  return launch_maybe_pdl(kern, dim3(blocks), dim3(TH), args, smem, stream, G.pdl != 0);
 }
 // LIGHT: the functors do no arithmetic worth extra threads (plain loads/stores): butterfly threads only, 3-4 blocks per SM
 template <bool INVERSE, bool LIGHT, class LoadOp, class StoreOp>

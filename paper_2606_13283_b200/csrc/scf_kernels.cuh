@@ -409,8 +409,8 @@ __global__ void __launch_bounds__(256, 3) mu_solve_kernel(const double *__restri
   extern __shared__ __align__(16) double s_tab[];   // kFdTabDoubles (49.5 KB: dynamic, beyond the 48 KB static limit)
   __shared__ double s_red[2 * 32 + 2];
   __shared__ double s_bc[2];
-  fd_load_tables(s_tab, fdtab);
-  __syncthreads();
+  __shared__ unsigned long long s_bar;
+  fd_load_tables(s_tab, fdtab, &s_bar);
   mu_solve_dev(grid, V_i, ng, C, sc, s_tab, s_red, s_bc, partials, max_pass);
 }
 
@@ -745,6 +745,8 @@ template <class LoadOp, class StoreOp>
 __global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp st_in, int P, int ny, long long nh,
                                                           const int *stop) {
   __shared__ double s_red[kMaxRed * 33];
+  pdl_launch_dependents();
+  pdl_wait();
   if (stop && *stop) return;
   LoadOp ld = ld_in;
   StoreOp st = st_in;
@@ -767,13 +769,19 @@ template <class LoadOp, class StoreOp, bool SMEM_TAB = false, int MIN_BLOCKS = 1
 __global__ void __launch_bounds__(256, MIN_BLOCKS) pointwise_r_kernel(LoadOp ld_in, StoreOp st_in, long long ng, const int *stop,
                                                           const double *__restrict__ g_tab = nullptr) {
   __shared__ double s_red[kMaxRed * 33];
+  __shared__ unsigned long long s_bar;
   extern __shared__ __align__(16) double s_tab[];   // SMEM_TAB: kFdTabDoubles doubles of dynamic shared memory
-  if (stop && *stop) return;
+  pdl_launch_dependents();
+  if (SMEM_TAB) fd_load_tables_async(s_tab, g_tab, &s_bar);   // constant data: the copy runs while the predecessor drains
+  pdl_wait();
+  if (stop && *stop) {             // (the bulk copy must have landed before the block may exit)
+    if (SMEM_TAB) fd_tables_wait(&s_bar);
+    return;
+  }
   LoadOp ld = ld_in;
   StoreOp st = st_in;
   if (SMEM_TAB) {
-    fd_load_tables(s_tab, g_tab);
-    __syncthreads();
+    fd_tables_wait(&s_bar);
     ld.set_table(s_tab); st.set_table(s_tab);
   }
   ld.begin(); st.begin();
@@ -831,8 +839,8 @@ __global__ void compress_half_kernel(double2 *__restrict__ dst, const double2 *_
 
 __global__ void fermi_dirac_kernel(int twice_j, const double *eta, double *out, size_t n, const double *fdtab) {
   extern __shared__ __align__(16) double s_tab[];   // kFdTabDoubles
-  fd_load_tables(s_tab, fdtab);
-  __syncthreads();
+  __shared__ unsigned long long s_bar;
+  fd_load_tables(s_tab, fdtab, &s_bar);
   for (size_t g = (size_t)blockIdx.x * blockDim.x + threadIdx.x; g < n; g += (size_t)gridDim.x * blockDim.x) {
     double a, b, c;
     fd_eval<7>(s_tab, eta[g], a, b, c);

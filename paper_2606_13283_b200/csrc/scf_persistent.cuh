@@ -77,7 +77,8 @@ __global__ void __launch_bounds__(kPersistThreads, kPersistBlocksPerSM) scf_pers
   // block ever waits for another one's scalar result; block 0 writes the copy back at the end
   __shared__ DevScalars s_sc;
   if (threadIdx.x == 0) s_sc = *p.sc;
-  fd_load_tables(s_tab, p.fdtab);
+  __shared__ unsigned long long s_bar;
+  fd_load_tables(s_tab, p.fdtab, &s_bar);
   __syncthreads();
   DevScalars *const sc = &s_sc;
   double *const part_vi = p.partials, *const part_dg = part_vi + (size_t)gridDim.x * 4,   // density 7 + G-space 3 per block
