@@ -52,6 +52,15 @@ typedef struct {
   int scf_fixed_iter;    /* > 0: run exactly this many iterations (parity replay) */
   double ewald_alpha;    /* <= 0: automatic (reading A18) */
   double n_electrons;    /* <= 0: sum_j Z_j (neutral cell); > 0: that many electrons on a uniform background */
+  int psp;               /* 0: Ashcroft empty core with psp_rc (BASELINE.json); 1: tabulated form factor (f2: the paper's
+                            average-atom norm-conserving pseudopotential, or any other local potential) */
+  int psp_nk;            /* psp = 1: table length (>= 4) */
+  double psp_dk;         /* psp = 1: table spacing in k (1/bohr, ordinary frequency); (psp_nk-1) psp_dk must cover every
+                            |k| of the grid, else ARCHE_EINVAL */
+  const double *h_psp_table; /* psp = 1: HOST [psp_nk], copied at init: Du(k_m), k_m = m psp_dk -- the non-Coulomb part of the
+                            form factor per unit charge, V_s(k) = Z_s (-1/(pi k^2) + Du(k)), interpolated by the cubic
+                            Lagrange polynomial through the four nearest nodes (reading A22); Du(0) is the
+                            k = 0 constant alpha_s/Z_s of Eq. 55 */
   double mix_mu_tol;     /* > 0: More's w is used only once two successive mu_a differ by <= mix_mu_tol kT ("once the
                             chemical potential fluctuations are small"; latched; reading A11b); <= 0: off */
   void *d_workspace;     /* device memory, >= arche_workspace_bytes(), 256-byte aligned */

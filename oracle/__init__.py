@@ -15,16 +15,17 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "liboracle.so")
 _SRC = os.path.join(_HERE, "arche_oracle.c")
+_SRC_AA = os.path.join(_HERE, "aa_pseudopotential.c")
 
 
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (-O2 -fopenmp). Building the checker is not using it."""
     hdr = os.path.join(_HERE, "arche_oracle.h")
     stale = (not os.path.exists(_SO)) or any(
-        os.path.getmtime(f) > os.path.getmtime(_SO) for f in (_SRC, hdr))
+        os.path.getmtime(f) > os.path.getmtime(_SO) for f in (_SRC, _SRC_AA, hdr))
     if force or stale:
         subprocess.check_call(["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-std=gnu11",
-                               "-o", _SO, _SRC, "-lm"])
+                               "-o", _SO, _SRC, _SRC_AA, "-lm"])
     return _SO
 
 
@@ -35,7 +36,8 @@ class Params(C.Structure):
                 ("mix_mode", C.c_int), ("mix_w_fixed", C.c_double), ("mix_warmup", C.c_int),
                 ("scf_tol_F", C.c_double), ("scf_tol_dn", C.c_double), ("scf_max_iter", C.c_int),
                 ("scf_fixed_iter", C.c_int), ("ewald_alpha", C.c_double),
-                ("n_electrons", C.c_double), ("mix_mu_tol", C.c_double)]
+                ("n_electrons", C.c_double), ("mix_mu_tol", C.c_double), ("psp", C.c_int), ("psp_nk", C.c_int),
+                ("psp_dk", C.c_double), ("psp_table", C.POINTER(C.c_double))]
 
 
 class Result(C.Structure):
@@ -65,6 +67,8 @@ def lib():
         L.oracle_dft3d_naive.argtypes = [C.c_int, C.c_int, C.c_int, dp, C.c_int]
         L.oracle_xc.argtypes = [C.c_int, C.c_double, dp, dp]
         L.oracle_structure_factor.argtypes = [dp, ip, C.c_int, dp, dp, dp]
+        L.oracle_table_interp.restype = C.c_double
+        L.oracle_table_interp.argtypes = [C.c_int, C.c_double, dp, C.c_double, dp]
         L.oracle_vps_unit.restype = C.c_double
         L.oracle_vps_unit.argtypes = [C.c_double, C.c_double]
         L.oracle_ewald_alpha.restype = C.c_double
@@ -84,6 +88,15 @@ def lib():
         L.oracle_get_real.argtypes = [C.c_void_p, C.c_int, dp]
         L.oracle_get_complex.argtypes = [C.c_void_p, C.c_int, dp]
         L.oracle_num_threads.restype = C.c_int
+        L.oracle_fd_wide.restype = C.c_double
+        L.oracle_fd_wide.argtypes = [C.c_int, C.c_double]
+        L.oracle_fd_half_inverse_wide.restype = C.c_double
+        L.oracle_fd_half_inverse_wide.argtypes = [C.c_double]
+        L.oracle_aa_solve.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int, C.c_int, dp, dp, dp, ip]
+        L.oracle_aa_pseudize.argtypes = [C.c_int, dp, dp, C.c_int, dp, dp]
+        L.oracle_aa_invert.argtypes = [C.c_double, C.c_int, C.c_int, dp, dp, C.c_double, C.c_double, dp]
+        L.oracle_radial_ft.argtypes = [C.c_int, dp, dp, C.c_int, C.c_int, dp, dp]
+        L.oracle_aa_energy.argtypes = [C.c_double, C.c_int, C.c_int, dp, dp, C.c_double, dp, C.c_double, dp]
         _lib = L
     return _lib
 
@@ -163,6 +176,46 @@ def force_ie(cell, grid, pos, Z, rc, nhat) -> np.ndarray:
     return F
 
 
+# ---- f2: average-atom pseudopotential (aa_pseudopotential.c)
+def fd_wide(twice_j, eta):
+    return lib().oracle_fd_wide(int(twice_j), float(eta))
+
+
+def aa_solve(Z, r_ws, kT, xc=0, n=1201):
+    r = np.zeros(n); dens = np.zeros(n); mu = C.c_double(); it = C.c_int()
+    rc = lib().oracle_aa_solve(float(Z), float(r_ws), float(kT), int(xc), n, _dp(r), _dp(dens), C.byref(mu), C.byref(it))
+    if rc != 0:
+        raise RuntimeError(f"oracle_aa_solve: {rc} after {it.value} iterations")
+    return r, dens, mu.value, it.value
+
+
+def aa_pseudize(r, n_aa, ic):
+    n_ps = np.zeros_like(r); abc = np.zeros(3)
+    rc = lib().oracle_aa_pseudize(len(r), _dp(_f64(r)), _dp(_f64(n_aa)), int(ic), _dp(n_ps), _dp(abc))
+    if rc != 0:
+        raise RuntimeError(f"oracle_aa_pseudize: {rc}")
+    return n_ps, abc
+
+
+def aa_invert(kT, xc, r, dens, n0lim, mu):
+    V = np.zeros_like(r)
+    lib().oracle_aa_invert(float(kT), int(xc), len(r), _dp(_f64(r)), _dp(_f64(dens)), float(n0lim), float(mu), _dp(V))
+    return V
+
+
+def radial_ft(r, f, ic, k):
+    k = _f64(np.atleast_1d(k)); out = np.zeros_like(k)
+    lib().oracle_radial_ft(len(r), _dp(_f64(r)), _dp(_f64(f)), int(ic), len(k), _dp(k), _dp(out))
+    return out
+
+
+def aa_energy(kT, xc, r, dens, n0lim, V_ext, Z):
+    out = np.zeros(4)
+    v = None if V_ext is None else _dp(_f64(V_ext))
+    lib().oracle_aa_energy(float(kT), int(xc), len(r), _dp(_f64(r)), _dp(_f64(dens)), float(n0lim), v, float(Z), _dp(out))
+    return out
+
+
 STRESS_ROWS = ("i", "e", "xc", "pp", "pm", "je", "ee", "ie", "total")
 
 
@@ -177,6 +230,7 @@ class Oracle:
             if k in cfg:
                 p[k] = cfg[k]
         p.update(over)
+        table = p.pop("psp_table", cfg.get("psp_table")); dk = p.pop("psp_dk", cfg.get("psp_dk", 0.0))
         self.cell = _f64(cfg["cell"]); self.grid = np.ascontiguousarray(cfg["grid"], dtype=np.int32)
         self._Z = _f64(cfg["Z"]); self._m = _f64(cfg["mass"])
         self.n_ions = len(self._Z)
@@ -185,6 +239,9 @@ class Oracle:
         P.n_ions = self.n_ions; P.Z = _dp(self._Z); P.mass = _dp(self._m); P.kT = float(cfg["kT"])
         for k, v in p.items():
             setattr(P, k, v)
+        if table is not None:                     # f2: tabulated form factor (non-Coulomb part per unit charge)
+            self._tab = _f64(table)
+            P.psp = 1; P.psp_nk = len(self._tab); P.psp_dk = float(dk); P.psp_table = _dp(self._tab)
         self.params = P
         self._h = C.c_void_p()
         rc = lib().oracle_init(C.byref(P), C.byref(self._h))

@@ -224,6 +224,40 @@ double oracle_vps_unit(double k, double rc) {
   return -cos(2.0 * PI * k * rc) / (PI * k * k);
 }
 
+/* f2: tabulated form factor per unit charge, u(k) = -1/(pi k^2) + Du(k), with the smooth non-Coulomb
+ * part Du on the uniform grid k_m = m dk (m = 0..nk-1) interpolated by the cubic Lagrange polynomial through the four
+ * nodes m0..m0+3, m0 = clamp(floor(k/dk) - 1, 0, nk - 4) (reading A22).  *du_dk = dDu/dk of that cubic. */
+double oracle_table_interp(int nk, double dk, const double *tab, double k, double *du_dk) {
+  double s = k / dk;
+  int m0 = (int)floor(s) - 1;
+  if (m0 < 0) m0 = 0;
+  if (m0 > nk - 4) m0 = nk - 4;
+  double t = s - m0, y0 = tab[m0], y1 = tab[m0 + 1], y2 = tab[m0 + 2], y3 = tab[m0 + 3];
+  double l0 = -(t - 1.0) * (t - 2.0) * (t - 3.0) / 6.0, l1 = t * (t - 2.0) * (t - 3.0) / 2.0;
+  double l2 = -t * (t - 1.0) * (t - 3.0) / 2.0, l3 = t * (t - 1.0) * (t - 2.0) / 6.0;
+  if (du_dk) {
+    double d0 = -((t - 2.0) * (t - 3.0) + (t - 1.0) * (t - 3.0) + (t - 1.0) * (t - 2.0)) / 6.0;
+    double d1 = ((t - 2.0) * (t - 3.0) + t * (t - 3.0) + t * (t - 2.0)) / 2.0;
+    double d2 = -((t - 1.0) * (t - 3.0) + t * (t - 3.0) + t * (t - 1.0)) / 2.0;
+    double d3 = ((t - 1.0) * (t - 2.0) + t * (t - 2.0) + t * (t - 1.0)) / 6.0;
+    *du_dk = (y0 * d0 + y1 * d1 + y2 * d2 + y3 * d3) / dk;
+  }
+  return y0 * l0 + y1 * l1 + y2 * l2 + y3 * l3;
+}
+
+/* form factor per unit charge of the context's pseudopotential and its derivative dv/dk (k > 0) */
+static double vps_ctx(const oracle_params *p, double k, double *dv) {
+  if (k == 0.0) { if (dv) *dv = 0.0; return 0.0; }
+  if (p->psp == 1) {
+    double du = 0.0, u = oracle_table_interp(p->psp_nk, p->psp_dk, p->psp_table, k, dv ? &du : NULL);
+    if (dv) *dv = 2.0 / (PI * k * k * k) + du;
+    return -1.0 / (PI * k * k) + u;
+  }
+  double rc = p->psp_rc;
+  if (dv) *dv = 2.0 * rc * sin(2.0 * PI * k * rc) / (k * k) + 2.0 * cos(2.0 * PI * k * rc) / (PI * k * k * k);
+  return oracle_vps_unit(k, rc);
+}
+
 void oracle_structure_factor(const double cell[3], const int grid[3], int n_ions, const double *pos,
                              const double *Z, double *S_out) {
   cplx *S = (cplx *)S_out;
@@ -314,8 +348,17 @@ void oracle_ewald(const double cell[3], const int grid[3], int n, const double *
 
 /* F^ie, Eq. 56 with the normalisation/sign of DESIGN.md reading A17:                         */
 /* F_j = -(2 pi/|Omega|) Z_j sum_k k v(k) Im( conj(nhat(k)) exp(-2 pi i k.r_j) )               */
+static void force_ie_p(const oracle_params *pp, const double cell[3], const int grid[3], int n, const double *pos,
+                       const double *Z, const double *nhat_in, double *F);
 void oracle_force_ie(const double cell[3], const int grid[3], int n, const double *pos, const double *Z,
                      double rc, const double *nhat_in, double *F) {
+  oracle_params pp;
+  memset(&pp, 0, sizeof(pp));
+  pp.psp = 0; pp.psp_rc = rc;
+  force_ie_p(&pp, cell, grid, n, pos, Z, nhat_in, F);
+}
+static void force_ie_p(const oracle_params *pp, const double cell[3], const int grid[3], int n, const double *pos,
+                       const double *Z, const double *nhat_in, double *F) {
   const cplx *nh = (const cplx *)nhat_in;
   double vol = cell[0] * cell[1] * cell[2];
   int nx = grid[0], ny = grid[1], nz = grid[2];
@@ -328,7 +371,7 @@ void oracle_force_ie(const double cell[3], const int grid[3], int n, const doubl
       double kx = kindex(ix, nx) / cell[0], ky = kindex(iy, ny) / cell[1], kz = kindex(iz, nz) / cell[2];
       double k = sqrt(kx * kx + ky * ky + kz * kz);
       if (k == 0.0) continue;
-      double v = oracle_vps_unit(k, rc);
+      double v = vps_ctx(pp, k, NULL);
       double ph = -2.0 * PI * (kx * pos[3 * j] + ky * pos[3 * j + 1] + kz * pos[3 * j + 2]);
       double im = cimag(conj(nh[g]) * (cos(ph) + I * sin(ph)));
       f[0] += v * im * kx; f[1] += v * im * ky; f[2] += v * im * kz;
@@ -342,7 +385,7 @@ void oracle_force_ie(const double cell[3], const int grid[3], int n, const doubl
 /* ======================================================================================== */
 struct oracle_ctx {
   oracle_params p;
-  double *Z, *mass, *pos, *F;
+  double *Z, *mass, *pos, *F, *psp_table;
   size_t ng;
   double vol, dV, cTF, Ne, Q, alpha, E_ie0, U_ii;
   double *n_i, *n_a, *V_i, *tmp1, *tmp2, *tmp3;
@@ -379,6 +422,15 @@ int oracle_init(const oracle_params *p, oracle_ctx **out) {
   c->F_ii = (double *)calloc(3 * n + 1, sizeof(double));
   if (n > 0) { memcpy(c->Z, p->Z, sizeof(double) * n); memcpy(c->mass, p->mass, sizeof(double) * n); }
   c->p.Z = c->Z; c->p.mass = c->mass;
+  if (p->psp == 1) {
+    if (p->psp_nk < 4 || !(p->psp_dk > 0.0) || !p->psp_table) return -1;
+    double kmax = 0.0;
+    for (int a = 0; a < 3; ++a) { double ka = (p->grid[a] / 2) / p->cell[a]; kmax += ka * ka; }
+    if (sqrt(kmax) > (p->psp_nk - 1) * p->psp_dk) return -1; /* the table must cover every |k| of the grid */
+    c->psp_table = (double *)malloc(sizeof(double) * p->psp_nk);
+    memcpy(c->psp_table, p->psp_table, sizeof(double) * p->psp_nk);
+    c->p.psp_table = c->psp_table;
+  }
   c->ng = (size_t)p->grid[0] * p->grid[1] * p->grid[2];
   c->vol = p->cell[0] * p->cell[1] * p->cell[2];
   c->dV = c->vol / (double)c->ng;
@@ -389,7 +441,8 @@ int oracle_init(const oracle_params *p, oracle_ctx **out) {
   c->alpha = p->ewald_alpha > 0.0 ? p->ewald_alpha : oracle_ewald_alpha(p->cell, p->grid);
   /* non-Coulomb k=0 term (reading A16): alpha_s = 2 pi Z rc^2 per ion */
   double asum = 0.0;
-  for (int j = 0; j < n; ++j) asum += 2.0 * PI * c->Z[j] * p->psp_rc * p->psp_rc;
+  /* table pseudopotential (f2): alpha_s = Z_s Du(0), the k -> 0 value of the non-Coulomb part */
+  for (int j = 0; j < n; ++j) asum += p->psp == 1 ? c->Z[j] * p->psp_table[0] : 2.0 * PI * c->Z[j] * p->psp_rc * p->psp_rc;
   c->E_ie0 = c->Ne / c->vol * asum;
   {
     /* uniform-gas response chi0 = dn/dmu at n0 = Ne/|Omega| (d/dmu of Eq. 9, I_j' = j I_{j-1}); the largest single-mode
@@ -419,6 +472,7 @@ int oracle_init(const oracle_params *p, oracle_ctx **out) {
 
 void oracle_destroy(oracle_ctx *c) {
   if (!c) return;
+  free(c->psp_table);
   free(c->Z); free(c->mass); free(c->pos); free(c->F); free(c->F_ii);
   free(c->n_i); free(c->n_a); free(c->V_i); free(c->tmp1); free(c->tmp2); free(c->tmp3);
   free(c->nh_i); free(c->nh_a); free(c->Vh_ie); free(c->S); free(c->gh); free(c->work);
@@ -468,7 +522,7 @@ int oracle_scf_begin(oracle_ctx *c, const double *pos) {
     double k[3];
     kvec(c, g, k);
     double ka = sqrt(k[0] * k[0] + k[1] * k[1] + k[2] * k[2]);
-    c->Vh_ie[g] = oracle_vps_unit(ka, c->p.psp_rc) * c->S[g];
+    c->Vh_ie[g] = vps_ctx(&c->p, ka, NULL) * c->S[g];
   }
   /* P3: Ewald */
   double U[3];
@@ -678,7 +732,7 @@ int oracle_scf_solve(oracle_ctx *c, const double *pos, oracle_result *out) {
 int oracle_forces(oracle_ctx *c, double *F) {
   if (!c->have_solution) return -1;
   int n = c->p.n_ions;
-  oracle_force_ie(c->p.cell, c->p.grid, n, c->pos, c->Z, c->p.psp_rc, (const double *)c->nh_a, c->F);
+  force_ie_p(&c->p, c->p.cell, c->p.grid, n, c->pos, c->Z, (const double *)c->nh_a, c->F);
   for (int i = 0; i < 3 * n; ++i) c->F[i] += c->F_ii[i];
   c->have_forces = 1;
   if (F) memcpy(F, c->F, sizeof(double) * 3 * n);
@@ -721,7 +775,7 @@ int oracle_stress(oracle_ctx *c, const double *vel, double *out) {
   if (!c->have_solution) return -1;
   static const int MU[6] = {0, 1, 2, 1, 0, 0}, NU[6] = {0, 1, 2, 2, 2, 1};
   const int n = c->p.n_ions;
-  const double vol = c->vol, a = c->alpha, rc = c->p.psp_rc;
+  const double vol = c->vol, a = c->alpha;
   long double s[9][6];
   for (int r = 0; r < 9; ++r)
     for (int q = 0; q < 6; ++q) s[r][q] = 0.0L;
@@ -765,8 +819,9 @@ int oracle_stress(oracle_ctx *c, const double *vel, double *out) {
     double S2 = creal(c->S[g]) * creal(c->S[g]) + cimag(c->S[g]) * cimag(c->S[g]);
     double va = exp(-PI * PI * k2 / (a * a)) / (PI * k2);
     double n2 = creal(c->nh_a[g]) * creal(c->nh_a[g]) + cimag(c->nh_a[g]) * cimag(c->nh_a[g]);
-    /* d/dk of the Ashcroft form factor -cos(2 pi k rc)/(pi k^2) */
-    double dv = 2.0 * rc * sin(2.0 * PI * ka * rc) / k2 + 2.0 * cos(2.0 * PI * ka * rc) / (PI * k2 * ka);
+    /* d/dk of the form factor: Ashcroft -cos(2 pi k rc)/(pi k^2), or the tabulated one (f2) */
+    double dv;
+    vps_ctx(&c->p, ka, &dv);
     /* nhat(k) sum_j Z_j dv e^{+2 pi i k.r_j} = nhat conj(S_Z) dv; its real part (the sum is real, reading A6) */
     double nS = creal(c->nh_a[g] * conj(c->S[g]));
     for (int q = 0; q < 6; ++q) {

@@ -46,6 +46,10 @@ typedef struct {
   double n_electrons;  /* <=0: sum_j Z_j (neutral cell); >0: that many electrons on a
                           uniform neutralising background (uniform-gas and linear-response pins) */
   double mix_mu_tol;   /* >0: More's w only once |mu_k - mu_{k-1}| <= mix_mu_tol kT (reading A11b) */
+  int psp;             /* 0 Ashcroft empty core (psp_rc); 1 tabulated form factor (f2) */
+  int psp_nk;          /* table length */
+  double psp_dk;       /* table spacing in k (1/bohr, ordinary frequency) */
+  const double *psp_table; /* [psp_nk] Du(k_m): non-Coulomb part of the form factor per unit charge, u = -1/(pi k^2) + Du */
 } oracle_params;
 
 typedef struct {
@@ -67,6 +71,8 @@ void oracle_xc(int xc, double n, double *eps_xc, double *v_xc);
 /* S_Z(k) = sum_j Z_j exp(-2 pi i k.r_j) on the grid */
 void oracle_structure_factor(const double cell[3], const int grid[3], int n_ions,
                              const double *pos, const double *Z, double *S_complex);
+/* cubic Lagrange interpolation of a uniform table (f2; reading A22); du_dk may be NULL */
+double oracle_table_interp(int nk, double dk, const double *tab, double k, double *du_dk);
 /* Ashcroft empty-core form factor per unit charge: -cos(2 pi k rc)/(pi k^2), 0 at k=0 */
 double oracle_vps_unit(double kabs, double rc);
 double oracle_ewald_alpha(const double cell[3], const int grid[3]);
@@ -105,6 +111,24 @@ void oracle_force_ie(const double cell[3], const int grid[3], int n_ions, const 
 #define ORACLE_STRESS_DOUBLES 55
 int oracle_stress(oracle_ctx *c, const double *vel, double *out);
 int oracle_num_threads(void);
+
+/* --- f2: average-atom norm-conserving pseudopotential (aa_pseudopotential.c; Eq. 16-18) ---------- */
+/* I_j(eta) for any eta (Sommerfeld expansion beyond eta = 500, 0 below -600) and the inverse of I_{1/2} built on it */
+double oracle_fd_wide(int twice_j, double eta);
+double oracle_fd_half_inverse_wide(double y);
+/* Radial grid r_i = (i h)^2, i = 0..n-1 (n odd), h = sqrt(r_ws)/(n-1); all arrays [n], caller-owned. */
+/* finite-T Thomas-Fermi average atom: nucleus Z in a neutral sphere of radius r_ws; fills r, n_aa (n_aa[0] = 0 stands for
+ * the integrable r^(-3/2) singularity), *mu; returns 0 when converged */
+int oracle_aa_solve(double Z, double r_ws, double kT, int xc, int n, double *r, double *n_aa, double *mu, int *iters);
+/* Eq. 16-17 with r_cut = r[ic]: n_ps[n], abc = {a, b, c} */
+int oracle_aa_pseudize(int n, const double *r, const double *n_aa, int ic, double *n_ps, double abc[3]);
+/* Eq. 18 for any density of the sphere: V_ext[n]; n0lim = lim r^(3/2) dens (0 for a regular density) */
+int oracle_aa_invert(double kT, int xc, int n, const double *r, const double *dens, double n0lim, double mu, double *V_ext);
+/* out[m] = int_0^{r[ic]} f(r) 4 pi r^2 sin(2 pi k_m r)/(2 pi k_m r) dr */
+void oracle_radial_ft(int n, const double *r, const double *f, int ic, int nk, const double *k, double *out);
+/* out = {K_e, E_ext, E_H, E_xc} of a density in the sphere; V_ext == NULL: the Coulomb potential -Zc/r */
+int oracle_aa_energy(double kT, int xc, int n, const double *r, const double *dens, double n0lim, const double *V_ext,
+                     double Zc, double out[4]);
 
 #ifdef __cplusplus
 }

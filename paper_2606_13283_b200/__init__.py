@@ -36,7 +36,8 @@ class Params(C.Structure):
                 ("psp_rc", C.c_double), ("init_mode", C.c_int), ("mix_mode", C.c_int),
                 ("mix_w_fixed", C.c_double), ("mix_warmup", C.c_int), ("scf_tol_F", C.c_double),
                 ("scf_tol_dn", C.c_double), ("scf_max_iter", C.c_int), ("scf_fixed_iter", C.c_int),
-                ("ewald_alpha", C.c_double), ("n_electrons", C.c_double), ("mix_mu_tol", C.c_double),
+                ("ewald_alpha", C.c_double), ("n_electrons", C.c_double), ("psp", C.c_int), ("psp_nk", C.c_int),
+                ("psp_dk", C.c_double), ("h_psp_table", C.c_void_p), ("mix_mu_tol", C.c_double),
                 ("d_workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p)]
 
@@ -115,6 +116,7 @@ class Arche:
             if k in cfg:
                 p[k] = cfg[k]
         p.update(over)
+        table = p.pop("psp_table", cfg.get("psp_table")); dk = p.pop("psp_dk", cfg.get("psp_dk", 0.0))
         self._Z = np.ascontiguousarray(cfg["Z"], dtype=np.float64)
         self._m = np.ascontiguousarray(cfg["mass"], dtype=np.float64)
         self.n_ions = len(self._Z)
@@ -130,6 +132,9 @@ class Arche:
         P.kT = float(cfg["kT"])
         for k, v in p.items():
             setattr(P, k, v)
+        if table is not None:                     # f2: tabulated form factor (non-Coulomb part per unit charge)
+            self._tab = np.ascontiguousarray(table, dtype=np.float64)
+            P.psp = 1; P.psp_nk = len(self._tab); P.psp_dk = float(dk); P.h_psp_table = self._tab.ctypes.data
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         P.stream = self.stream.cuda_stream
         nbytes = self.lib.arche_workspace_bytes(C.byref(P))

@@ -90,7 +90,8 @@ struct arche_ctx {
   int r_blocks;    // resident blocks per SM of the streamed real-space Fermi-Dirac kernels
   int force_slabs, force_rows_per_slab, force_ipt;   // ions per thread of the force kernel's register tile
   // device arrays (all inside the caller's workspace)
-  double *n_i, *n_a, *V_i, *vps, *va;
+  double *n_i, *n_a, *V_i, *vps, *va, *psp_tab;
+  PspTable T;      // f2: tabulated pseudopotential (device table inside the workspace)
   double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
   long long nh;      // P*ny*nz
   int nxh, P;
@@ -182,6 +183,7 @@ size_t layout(arche_ctx *c, char *base) {
   const size_t nh = (size_t)c->nh;
   c->n_i = w.take<double>(ng); c->n_a = w.take<double>(ng); c->V_i = w.take<double>(ng);
   c->vps = w.take<double>(nh); c->va = w.take<double>(nh);
+  c->psp_tab = w.take<double>(c->p.psp == 1 && c->p.psp_nk > 0 ? (size_t)c->p.psp_nk : 1);
   c->nh_i = w.take<double2>(nh); c->nh_a = w.take<double2>(nh); c->vh_ie = w.take<double2>(nh);
   c->S = w.take<double2>(nh); c->S2 = w.take<double2>(nh); c->gh = w.take<double2>(nh); c->gh2 = w.take<double2>(nh);
   c->work = w.take<double2>(nh);
@@ -233,6 +235,13 @@ bool params_ok(const arche_params *p) {
     if (!grid_ok(p->grid[a]) || !(p->cell[a] > 0.0)) return false;
   if (p->n_ions > 0 && (!p->h_Z || !p->h_mass)) return false;
   if (p->xc < 0 || p->xc > 2) return false;
+  if (p->psp != 0 && p->psp != 1) return false;
+  if (p->psp == 1) {   // the table must cover every |k| of the grid
+    if (p->psp_nk < 4 || !(p->psp_dk > 0.0) || !p->h_psp_table) return false;
+    double k2 = 0.0;
+    for (int a = 0; a < 3; ++a) { const double ka = (p->grid[a] / 2) / p->cell[a]; k2 += ka * ka; }
+    if (sqrt(k2) > (p->psp_nk - 1) * p->psp_dk) return false;
+  }
   return true;
 }
 
@@ -313,7 +322,8 @@ static int init_body(arche_ctx *c, const arche_params *p) {
   if (!(C.Ne > 0.0)) return fail(c, ARCHE_EINVAL, "no electrons");
   C.eta0 = fd_half_inverse_host(C.Ne / (G.vol * C.cTF));
   double asum = 0.0;
-  for (int j = 0; j < c->nions; ++j) asum += 2.0 * ARCHE_PI * hZ[j] * p->psp_rc * p->psp_rc;  // alpha_s = 2 pi Z rc^2
+  for (int j = 0; j < c->nions; ++j)   // alpha_s = 2 pi Z rc^2 (Ashcroft) or Z Du(0) (table, f2)
+    asum += p->psp == 1 ? hZ[j] * p->h_psp_table[0] : 2.0 * ARCHE_PI * hZ[j] * p->psp_rc * p->psp_rc;
   C.E_ie0 = C.Ne / G.vol * asum;
   C.xc = p->xc; C.mix_mode = p->mix_mode; C.mix_warmup = p->mix_warmup;
   {  // uniform-gas response chi0 = dn/dmu at Ne/|Omega|; largest single-mode value of More's w (reading A11d)
@@ -397,10 +407,12 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     CK(cudaMemsetAsync(a, 0, (size_t)c->nh * sizeof(double2), c->stream));
   CK(cudaMemsetAsync(c->sc, 0, sizeof(DevScalars), c->stream));
   CK(cudaMemsetAsync(c->F, 0, 3 * (c->nions > 0 ? c->nions : 1) * sizeof(double), c->stream));
-  form_factor_kernel<<<c->ew_grid, 256, 0, c->stream>>>(G, p->psp_rc, c->alpha, c->vps, c->va);
+  c->T.on = p->psp == 1 ? 1 : 0; c->T.nk = p->psp_nk; c->T.dk = p->psp_dk; c->T.tab = c->psp_tab;
+  if (c->T.on) CK(cudaMemcpyAsync(c->psp_tab, p->h_psp_table, (size_t)p->psp_nk * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  form_factor_kernel<<<c->ew_grid, 256, 0, c->stream>>>(G, p->psp_rc, c->T, c->alpha, c->vps, c->va);
   LAUNCHED(c);
   CK(cudaStreamSynchronize(c->stream));
-  c->p.h_Z = nullptr; c->p.h_mass = nullptr;  // copied; do not keep the caller's pointers
+  c->p.h_Z = nullptr; c->p.h_mass = nullptr; c->p.h_psp_table = nullptr;  // copied; do not keep the caller's pointers
   return ARCHE_OK;
 }
 
@@ -724,7 +736,7 @@ int compute_stress(arche_ctx *c, const double *d_vel) {
   if (nb > cap) nb = cap;
   { ProfScope ps(c, PC_STRESS);
   stress_fields_kernel<<<(unsigned)nb, kStressThreads, 0, c->stream>>>(G, c->nh_a, c->S, c->S2, c->n_a, c->p.xc, c->alpha,
-                                                                     c->p.psp_rc, c->partials);
+                                                                     c->p.psp_rc, c->T, c->partials);
   LAUNCHED(c); }
   if (ni > 0) {
     stress_pp_kernel<<<ni, 128, 0, c->stream>>>(c->pos, c->Z, ni, G.Lx, G.Ly, G.Lz, c->alpha, c->pp_part);

@@ -26,10 +26,28 @@ __global__ void phase_table_kernel(const double *__restrict__ pos, int comp, dou
   }
 }
 
-// reciprocal-space form factors that depend only on the cell, on the half spectrum [nz][ny][P]: Ashcroft
-// v(k) = -cos(2 pi k rc)/(pi k^2) (per unit charge, 0 at k=0) and the Ewald kernel
-// V_alpha(k) = exp(-(pi k/alpha)^2)/(pi k^2) (Eq. 43).  Zero in the padding columns.
-__global__ void form_factor_kernel(GridGeom G, double rc, double alpha, double *__restrict__ vps, double *__restrict__ va) {
+// f2: tabulated local pseudopotential.  u(k) = -1/(pi k^2) + Du(k) per unit charge; Du on the uniform grid
+// k_m = m dk, cubic Lagrange polynomial through the nodes m0..m0+3, m0 = clamp(floor(k/dk) - 1, 0, nk - 4)
+// (reading A22).  Returns Du(k); *du_dk (optional) the derivative of that cubic.
+struct PspTable { int on, nk; double dk; const double *tab; };
+__device__ __forceinline__ double psp_table_interp(const PspTable &T, double k, double *du_dk) {
+  const double s = k / T.dk;
+  int m0 = (int)floor(s) - 1;
+  m0 = max(0, min(m0, T.nk - 4));
+  const double t = s - (double)m0, y0 = T.tab[m0], y1 = T.tab[m0 + 1], y2 = T.tab[m0 + 2], y3 = T.tab[m0 + 3];
+  const double t1 = t - 1.0, t2 = t - 2.0, t3 = t - 3.0;
+  if (du_dk) {
+    const double d0 = -(t2 * t3 + t1 * t3 + t1 * t2) * (1.0 / 6.0), d1 = (t2 * t3 + t * t3 + t * t2) * 0.5;
+    const double d2 = -(t1 * t3 + t * t3 + t * t1) * 0.5, d3 = (t1 * t2 + t * t2 + t * t1) * (1.0 / 6.0);
+    *du_dk = (y0 * d0 + y1 * d1 + y2 * d2 + y3 * d3) / T.dk;
+  }
+  return y0 * (-t1 * t2 * t3 * (1.0 / 6.0)) + y1 * (t * t2 * t3 * 0.5) + y2 * (-t * t1 * t3 * 0.5) + y3 * (t * t1 * t2 * (1.0 / 6.0));
+}
+
+// reciprocal-space form factors that depend only on the cell, on the half spectrum [nz][ny][P]: the pseudopotential per
+// unit charge -- Ashcroft v(k) = -cos(2 pi k rc)/(pi k^2) or the tabulated one (f2) --, 0 at k = 0, and the
+// Ewald kernel V_alpha(k) = exp(-(pi k/alpha)^2)/(pi k^2) (Eq. 43).  Zero in the padding columns.
+__global__ void form_factor_kernel(GridGeom G, double rc, PspTable T, double alpha, double *__restrict__ vps, double *__restrict__ va) {
   const long long nh = (long long)G.P * G.ny * G.nz;
   for (long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x; g < nh; g += (long long)gridDim.x * blockDim.x) {
     const int ix = (int)(g % G.P), iy = (int)((g / G.P) % G.ny), iz = (int)(g / ((long long)G.P * G.ny));
@@ -37,7 +55,7 @@ __global__ void form_factor_kernel(GridGeom G, double rc, double alpha, double *
     const double k2 = G.kx2[ix] + G.ky2[iy] + G.kz2[iz];
     if (k2 == 0.0) { vps[g] = 0.0; va[g] = 0.0; continue; }
     const double k = sqrt(k2);
-    vps[g] = -cospi(2.0 * k * rc) / (ARCHE_PI * k2);
+    vps[g] = T.on ? -1.0 / (ARCHE_PI * k2) + psp_table_interp(T, k, nullptr) : -cospi(2.0 * k * rc) / (ARCHE_PI * k2);
     va[g] = exp(-ARCHE_PI * ARCHE_PI * k2 / (alpha * alpha)) / (ARCHE_PI * k2);
   }
 }

@@ -24,7 +24,7 @@ constexpr int kStressOut = 55;    // 9 rows x 6 columns + P
 
 __global__ void __launch_bounds__(kStressThreads) stress_fields_kernel(
     GridGeom G, const double2 *__restrict__ nh_a, const double2 *__restrict__ S, const double2 *__restrict__ S2,
-    const double *__restrict__ n_a, int xc, double alpha, double rc, double *__restrict__ partials /*[grid][21]*/) {
+    const double *__restrict__ n_a, int xc, double alpha, double rc, PspTable T, double *__restrict__ partials /*[grid][21]*/) {
   __shared__ double s_red[kStressSums * 32];
   double acc[kStressSums];
 #pragma unroll
@@ -51,9 +51,16 @@ __global__ void __launch_bounds__(kStressThreads) stress_fields_kernel(
     // Eq. 54: |nhat|^2/(pi k^2) [2 k_m k_n/k^2 - delta]
     const double e = (n.x * n.x + n.y * n.y) * inv_pi * ik2;
     // Re(nhat conj(S_Z)) v'(k) k_m k_n/|k|, v(k) = -cos(2 pi k rc)/(pi k^2)
-    double sn, cs;
-    sincospi(two_rc * ka, &sn, &cs);
-    const double dv_k = (2.0 * rc * sn * ik2 + 2.0 * cs * inv_pi * ik2 * ik) * ik;
+    double dv_k;   // v'(k)/k
+    if (T.on) {    // f2: derivative of the tabulated form factor, -1/(pi k^2) + Du(k)
+      double du;
+      psp_table_interp(T, ka, &du);
+      dv_k = (2.0 * inv_pi * ik2 * ik + du) * ik;
+    } else {
+      double sn, cs;
+      sincospi(two_rc * ka, &sn, &cs);
+      dv_k = (2.0 * rc * sn * ik2 + 2.0 * cs * inv_pi * ik2 * ik) * ik;
+    }
     const double b1 = dv_k * (n.x * s1.x + n.y * s1.y), b2 = dv_k * (n.x * s2.x + n.y * s2.y);
     acc[0] += hw * (a1 + a2);
     acc[7] += 2.0 * hw * e;

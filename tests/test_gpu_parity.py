@@ -353,3 +353,45 @@ def test_determinism(orc, torch_cuda):
         r.append((res["F_total"], res["mu"], g.get_real("n_a").cpu().numpy(), g.forces().cpu().numpy()))
     assert r[0][0] == r[1][0] and r[0][1] == r[1][1]
     assert np.array_equal(r[0][2], r[1][2]) and np.array_equal(r[0][3], r[1][3])
+
+
+def test_tabulated_pseudopotential(orc, torch_cuda):
+    """f2: the average-atom norm-conserving pseudopotential as a form-factor table (arche_params.psp = 1).
+    Dense hydrogen (4 protons, r_ws = 1.5 bohr, kT = 2 Ha, 16^3), table from the oracle-side generator (test data, like
+    the positions): V_ie, three iterations field by field, forces, the stress table; and the Ashcroft potential fed as
+    a table must reproduce psp = 0 on the device as well."""
+    torch = torch_cuda
+    Z, rws, kT, n = 1.0, 1.5, 2.0, 401
+    r, dens, mu, _ = orc.aa_solve(Z, rws, kT, 0, n)
+    ic = int(round((n - 1) * np.sqrt(0.5)))
+    ps, _ = orc.aa_pseudize(r, dens, ic)
+    V = orc.aa_invert(kT, 0, r, ps, 0.0, mu)
+    dVr = np.zeros(n); dVr[1:] = V[1:] + Z / r[1:]
+    dk = 0.02
+    table = orc.radial_ft(r, dVr, ic, dk * np.arange(int(4.0 / dk) + 3)) / Z
+    L = (4 * 4.0 / 3.0 * np.pi * rws ** 3) ** (1.0 / 3.0)
+    cfg = ai.make_small(n_ions=4, cell=[L, L * 1.1, L / 1.1], grid=(16, 12, 18), seed=17, dmin=1.2)
+    cfg["Z"] = np.full(4, Z); cfg["kT"] = kT; cfg["xc"] = 0
+    kw = dict(psp_table=table, psp_dk=dk)
+    g = _gpu(cfg, **kw); o = orc.Oracle(cfg, **kw)
+    g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
+    assert _rel(g.get_complex("Vhat_ie").cpu().numpy(), o.get_complex("Vhat_ie")) < 1e-12
+    for it in range(3):
+        rg = g.scf_iter(); ro = o.scf_iter()
+        assert _rel(g.get_real("n_a").cpu().numpy(), o.get_real("n_a")) < TOL_N
+        for k in ("mu", "F_total", "E_ie", "E_ie0", "E_H", "U_ii", "w_last"):
+            assert abs(rg[k] - ro[k]) <= TOL_F * max(1.0, abs(ro[k])), (it, k, rg[k], ro[k])
+    Fg = g.forces().cpu().numpy(); Fo = o.forces()
+    assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max()
+    _check_stress(g.stress(torch.as_tensor(cfg["vel"], device="cuda")), o.stress(cfg["vel"]))
+    # Ashcroft as a table against the built-in Ashcroft path, both on the device
+    c2 = ai.make_small(n_ions=3, cell=[7.0, 7.6, 8.3], grid=(12, 12, 12), T_eV=10.0, seed=5, dmin=2.5)
+    kk = 0.002 * np.arange(int(1.6 / 0.002) + 4)
+    du = np.empty_like(kk); du[1:] = (1 - np.cos(2 * np.pi * kk[1:] * 1.12)) / (np.pi * kk[1:] ** 2); du[0] = 2 * np.pi * 1.12 ** 2
+    ga = _gpu(c2, scf_fixed_iter=12); gt = _gpu(c2, scf_fixed_iter=12, psp_table=du, psp_dk=0.002)
+    ra = ga.scf_solve(c2["pos"]); rt = gt.scf_solve(c2["pos"])
+    assert abs(rt["F_total"] - ra["F_total"]) < 1e-8 * abs(ra["F_total"]) and abs(rt["E_ie0"] / ra["E_ie0"] - 1) < 1e-14
+    assert np.abs((gt.forces() - ga.forces()).cpu().numpy()).max() < 1e-7 * float(ga.forces().abs().max())
+    from paper_2606_13283_b200 import ArcheError
+    with pytest.raises(ArcheError):
+        _gpu(c2, psp_table=du[:100], psp_dk=0.002)                  # the table does not cover the grid's largest |k|
