@@ -32,7 +32,7 @@ import arche_inputs as ai  # noqa: E402
 TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000, mix_warmup=3, mix_w_fixed=0.95, xc=2)
 # c4 (T = 1 eV, 61-bohr cell): the longest wave has lambda = chi0/(pi k_min^2) ~ 110, so the fixed w of the warm-up must
 # exceed (lambda-1)/(lambda+1): automatic w = lambda/(1+lambda), More's w once |mu_k - mu_{k-1}| < 1e-3 kT (reading A11b)
-TOL_BY_WORKLOAD = {"c4": dict(scf_max_iter=12000, mix_w_fixed=0.0, mix_mu_tol=1e-3)}
+TOL_BY_WORKLOAD = {"c4": dict(scf_max_iter=12000, mix_w_fixed=0.0, mix_mu_tol=1e-3, mix_chi_floor=1e-3)}
 NCU_TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_c5_384_ncu_full.csv")
 
 

@@ -63,6 +63,10 @@ typedef struct {
                             k = 0 constant alpha_s/Z_s of Eq. 55 */
   double mix_mu_tol;     /* > 0: More's w is used only once two successive mu_a differ by <= mix_mu_tol kT ("once the
                             chemical potential fluctuations are small"; latched; reading A11b); <= 0: off */
+  double mix_chi_floor;  /* > 0: in K of Eq. 31 dn_a/dmu is bounded below by mix_chi_floor x its uniform-gas value chi_0: where
+                            n_a underflows (chi -> 0) next to a finite n_i the quadratic model overstates the stiffness by
+                            hundreds of orders of magnitude and w collapses to 0 (reading A11c); <= 0: Eq. 31 as
+                            printed */
   void *d_workspace;     /* device memory, >= arche_workspace_bytes(), 256-byte aligned */
   size_t workspace_bytes;
   void *stream;          /* cudaStream_t (0 = default stream) */

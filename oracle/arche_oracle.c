@@ -398,6 +398,7 @@ struct oracle_ctx {
   int more_on;    /* More's w has been switched on in this solve (reading A11b) */
   double mu_iter_prev;
   double w_fixed; /* mix_w_fixed, or lambda/(1+lambda) when that is <= 0 (reading A11d) */
+  double chi_floor; /* absolute lower bound of dn_a/dmu in K (reading A11c); 0: Eq. 31 as printed */
   double dF_prev; /* F_{k-1} - F_{k-2} (signed) */
   oracle_result last;
 };
@@ -452,6 +453,7 @@ int oracle_init(const oracle_params *p, oracle_ctx **out) {
     double Lmax = fmax(p->cell[0], fmax(p->cell[1], p->cell[2]));
     double lam = chi0 * Lmax * Lmax / PI;
     c->w_fixed = p->mix_w_fixed > 0.0 ? p->mix_w_fixed : lam / (1.0 + lam);
+    c->chi_floor = p->mix_chi_floor > 0.0 ? p->mix_chi_floor * chi0 : 0.0;
   }
   size_t ng = c->ng;
   c->n_i = (double *)calloc(ng, sizeof(double));
@@ -632,7 +634,7 @@ int oracle_scf_iter(oracle_ctx *c, oracle_result *out) {
   long double sK = 0, sdn2 = 0, sna2 = 0, sF0 = 0, sKe = 0, sExc = 0;
   for (size_t g = 0; g < ng; ++g) {
     double dn = c->n_i[g] - c->n_a[g];
-    sK += dn * dn / t_chi[g];                    /* Eq. 31 */
+    sK += dn * dn / fmax(t_chi[g], c->chi_floor); /* Eq. 31; reading A11c: optional lower bound of dn_a/dmu (default off) */
     sdn2 += dn * dn;
     sna2 += c->n_a[g] * c->n_a[g];
     sF0 += t_f0[g];

@@ -49,6 +49,7 @@ typedef struct {
   int psp;             /* 0 Ashcroft empty core (psp_rc); 1 tabulated form factor (f2) */
   int psp_nk;          /* table length */
   double psp_dk;       /* table spacing in k (1/bohr, ordinary frequency) */
+  double mix_chi_floor; /* >0: lower bound of dn_a/dmu in K (Eq. 31) in units of the uniform-gas value (reading A11c) */
   const double *psp_table; /* [psp_nk] Du(k_m): non-Coulomb part of the form factor per unit charge, u = -1/(pi k^2) + Du */
 } oracle_params;
 

@@ -331,6 +331,7 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     const double Lmax = fmax(G.Lx, fmax(G.Ly, G.Lz)), lam = chi0 * Lmax * Lmax / ARCHE_PI;
     C.mix_w_fixed = p->mix_w_fixed > 0.0 ? p->mix_w_fixed : lam / (1.0 + lam);
     C.mix_mu_tol = p->mix_mu_tol;
+    C.chi_floor = p->mix_chi_floor > 0.0 ? p->mix_chi_floor * chi0 : 0.0;
   }
   C.tol_F = p->scf_tol_F; C.tol_dn = p->scf_tol_dn;
   C.q_F = 0.0; C.q_dn = 0.0; C.inv_qF = 0.0; C.inv_vol = 1.0 / G.vol;

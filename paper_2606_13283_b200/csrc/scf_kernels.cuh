@@ -38,6 +38,7 @@ struct ScfConst {
   double inv_vol, inv_qF;   // reciprocals for the single-thread scalar updates (fp64 divisions cost ~300 cycles each there)
   double q_F, q_dn;   // reading A13: free-energy quantum of one PZ81 branch flip; chi(n*) x V_c jump x sqrt(dV)
   double mix_mu_tol;  // reading A11b: More's w only once |mu_k - mu_{k-1}| <= mix_mu_tol kT (latched); <= 0: off
+  double chi_floor;   // reading A11c: lower bound of dn_a/dmu in K (Eq. 31), absolute; 0: Eq. 31 as printed
 };
 
 // Perdew-Zunger 1981 LDA (unpolarised), Hartree units; restated from the publication (reading D5).
@@ -62,24 +63,27 @@ __device__ __forceinline__ double rcp_fast(double x) {
   e = fma(-x, r, 1.0);
   return fma(r, e, r);
 }
-// u = n^(-1/6) for n > 0: every power PZ81 needs is a product of u (r_s = c u^2, sqrt r_s = sqrt(c) u, n^(1/3) = n u^4),
-// so one Newton iteration chain replaces a cube root and a square root.  fp32 seed exp2(-log2(n)/6) (two MUFU), two
-// steps of u <- u + u (1 - n u^6)/6 (quadratic: 1e-6 -> 4e-12 -> round-off).  Densities below the fp32 range (the
-// empty cores at T = 1 eV) are scaled by 2^96 first: u(n) = 2^16 u(2^96 n).
+// u = n^(-1/6) for n >= 1e-250: every power PZ81 needs is a product of u (r_s = c u^2, sqrt r_s = sqrt(c) u,
+// n^(1/3) = n u^4), so one Newton iteration chain replaces a cube root and a square root.  The argument is first
+// brought into [1, 64) by an exact power of two taken from its exponent field (n = ns 2^(6k), u = u(ns) 2^(-k)): the
+// densities of a degenerate plasma span 1e-100 ... 10 (empty cores at T = 1 eV) and an fp32 seed of n itself would
+// underflow.  fp32 seed exp2(-log2(ns)/6) (two MUFU), two steps of u <- u + u (1 - ns u^6)/6 (quadratic:
+// 1e-6 -> 4e-12 -> round-off).
 __device__ __forceinline__ double inv_sixth_root(double n) {
-  const bool tiny = n < 1.0e-30;
-  const double ns = tiny ? n * 79228162514264337593543950336.0 : n;   // 2^96
-  float seed = exp2f(__log2f((float)ns) * (-1.0f / 6.0f));
-  double u = (double)seed;
+  const int e = (__double2hiint(n) >> 20) - 1023;      // n > 0, normal: sign bit clear
+  const int k = (e >= 0 ? e : e - 5) / 6;              // floor(e / 6)
+  const double ns = n * __hiloint2double((1023 - 6 * k) << 20, 0);
+  double u = (double)exp2f(__log2f((float)ns) * (-1.0f / 6.0f));
 #pragma unroll
-  for (int k = 0; k < 2; ++k) {
+  for (int it = 0; it < 2; ++it) {
     const double u2 = u * u, u6 = u2 * u2 * u2;
     u = fma(u * (1.0 / 6.0), fma(-ns, u6, 1.0), u);
   }
-  return tiny ? u * 65536.0 : u;
+  return u * __hiloint2double((1023 - k) << 20, 0);
 }
 __device__ __forceinline__ void xc_pz81(double n, double &eps, double &v, int xc = 1) {
-  if (!(n > 0.0)) { eps = 0.0; v = 0.0; return; }
+  // below 1e-250 the potential -(3n/pi)^(1/3) is < 1e-83 Ha and the energy density n eps_xc < 1e-333: taken as zero
+  if (!(n > 1.0e-250)) { eps = 0.0; v = 0.0; return; }
   const double cx = 0.73855876638202240588;   // (3/4) (3/pi)^(1/3)
   const double c0 = 0.62035049089940001667;   // (3/(4 pi))^(1/3): r_s = c0 n^(-1/3)
   const double sc0 = 0.78762331789974325053;  // sqrt(c0)
@@ -439,7 +443,7 @@ struct LoadDensity {
     const double chi = C.cTF * 0.5 * im12 * inv_kT;   // dn_a/dmu
     const double dn = n_i[g] - na;
     n_a[g] = na;
-    if (chi > 1.0e-290) sK += dn * dn * rcp_fast(chi);   // Eq. 31
+    if (chi > 1.0e-290) sK += dn * dn * rcp_fast(fmax(chi, C.chi_floor));   // Eq. 31 (reading A11c: optional lower bound)
     sdn2 += dn * dn; sna2 += na * na; sChi += chi;
     sF0 += eta * i12 - (2.0 / 3.0) * i32;             // f_0/(kT cTF), from Eq. 38-39
     sKe += i32;                                       // Eq. 38
@@ -462,7 +466,7 @@ struct LoadDensity {
       const double chi = C.cTF * 0.5 * im12[m] * inv_kT;
       const double dn = ni[m] - na[m];
       n_a[g[m]] = na[m];
-      if (chi > 1.0e-290) sK += dn * dn * rcp_fast(chi);   // Eq. 31 (chi underflows only where n_a does: no weight)
+      if (chi > 1.0e-290) sK += dn * dn * rcp_fast(fmax(chi, C.chi_floor));   // Eq. 31 (reading A11c: optional lower bound)
       sdn2 += dn * dn; sna2 += na[m] * na[m]; sChi += chi;
       sF0 += eta[m] * i12[m] - (2.0 / 3.0) * i32[m];
       sKe += i32[m];
