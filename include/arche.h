@@ -61,7 +61,7 @@ typedef struct {
                             form factor per unit charge, V_s(k) = Z_s (-1/(pi k^2) + Du(k)), interpolated by the cubic
                             Lagrange polynomial through the four nearest nodes (reading A22); Du(0) is the
                             k = 0 constant alpha_s/Z_s of Eq. 55 */
-  double mix_mu_tol;     /* > 0: More's w is used only once two successive mu_a differ by <= mix_mu_tol kT ("once the
+  double mix_mu_tol;     /* > 0: More's w is used only once two successive mu_a differ by <= mix_mu_tol kT (1 - w_prev) ("once the
                             chemical potential fluctuations are small"; latched; reading A11b); <= 0: off */
   double mix_chi_floor;  /* > 0: in K of Eq. 31 dn_a/dmu is bounded below by mix_chi_floor x its uniform-gas value chi_0: where
                             n_a underflows (chi -> 0) next to a finite n_i the quadratic model overstates the stiffness by

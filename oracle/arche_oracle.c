@@ -663,8 +663,10 @@ int oracle_scf_iter(oracle_ctx *c, oracle_result *out) {
   int it = c->last.scf_iters + 1;
   /* "w is computed and updated only after a few SCF iterations, once the chemical potential
    * fluctuations are small" -- reading A11b: after the warm-up count and, when mix_mu_tol > 0, once two successive
-   * mu_a differ by at most mix_mu_tol kT (latched for the rest of the solve) */
-  if (c->p.mix_mu_tol > 0.0 && !c->more_on && it >= 2 && fabs(mu - c->mu_iter_prev) <= c->p.mix_mu_tol * kT) c->more_on = 1;
+   * mu_a differ by at most mix_mu_tol kT (1 - w_prev) (latched for the rest of the solve) */
+  /* per unit of undamped step: the input moved by (1 - w_prev)(n_a - n_i) since the last iteration */
+  if (c->p.mix_mu_tol > 0.0 && !c->more_on && it >= 2 &&
+      fabs(mu - c->mu_iter_prev) <= c->p.mix_mu_tol * kT * (1.0 - c->last.w_last)) c->more_on = 1;
   c->mu_iter_prev = mu;
   double w;
   if (c->p.mix_mode == 1 && it > c->warmup_eff && (c->p.mix_mu_tol <= 0.0 || c->more_on)) w = (K + U > 0.0) ? U / (K + U) : 0.0;

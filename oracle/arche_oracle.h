@@ -45,7 +45,7 @@ typedef struct {
   double ewald_alpha;  /* <=0: auto */
   double n_electrons;  /* <=0: sum_j Z_j (neutral cell); >0: that many electrons on a
                           uniform neutralising background (uniform-gas and linear-response pins) */
-  double mix_mu_tol;   /* >0: More's w only once |mu_k - mu_{k-1}| <= mix_mu_tol kT (reading A11b) */
+  double mix_mu_tol;   /* >0: More's w only once |mu_k - mu_{k-1}| <= mix_mu_tol kT (1 - w_prev) (reading A11b) */
   int psp;             /* 0 Ashcroft empty core (psp_rc); 1 tabulated form factor (f2) */
   int psp_nk;          /* table length */
   double psp_dk;       /* table spacing in k (1/bohr, ordinary frequency) */

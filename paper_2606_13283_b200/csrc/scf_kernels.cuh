@@ -575,7 +575,11 @@ struct StoreNhatA {
       // reading A11b ("w is computed and updated only after a few SCF iterations, once the chemical potential
       // fluctuations are small"): after the warm-up count, and -- when mix_mu_tol > 0 -- once two successive mu_a differ
       // by at most mix_mu_tol kT; the switch is latched for the rest of the solve
-      if (C.mix_mu_tol > 0.0 && !sc->more_on && it >= 2 && fabs(sc->mu - sc->mu_iter_prev) <= C.mix_mu_tol * C.kT) sc->more_on = 1;
+      // the fluctuation is measured per unit of undamped step: the input moved by (1 - w_prev)(n_a - n_i) since the last
+      // iteration, so |mu_k - mu_{k-1}|/(1 - w_prev) estimates what a full step would do to mu (with w_prev = 0.99 two
+      // successive mu agree to 1e-3 kT by construction, however far the density is from the fixed point)
+      if (C.mix_mu_tol > 0.0 && !sc->more_on && it >= 2 &&
+          fabs(sc->mu - sc->mu_iter_prev) <= C.mix_mu_tol * C.kT * (1.0 - sc->w)) sc->more_on = 1;
       sc->mu_iter_prev = sc->mu;
       double w;
       if (C.mix_mode == 1 && it > C.mix_warmup && (C.mix_mu_tol <= 0.0 || sc->more_on)) w = (K + U > 0.0) ? U / (K + U) : 0.0;   // w = U/(K+U)

@@ -71,7 +71,7 @@ def test_c4_full_size(orc, torch_cuda):
     with every scalar, forces and the stress table against the oracle (~2 min of oracle time on 16 cores)."""
     torch = torch_cuda
     cfg = ai.make_config("c4")
-    kw = dict(mix_warmup=3, mix_w_fixed=0.0, mix_mu_tol=1e-3, mix_chi_floor=1e-3, xc=2)   # the settings bench.py runs c4 with
+    kw = dict(mix_warmup=3, mix_w_fixed=0.0, mix_mu_tol=1e-3, xc=2)   # the settings bench.py runs c4 with
     g = _gpu(cfg, **kw); o = orc.Oracle(cfg, **kw)
     assert not g.is_fused()
     g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])

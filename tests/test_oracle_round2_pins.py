@@ -258,7 +258,7 @@ def test_total_force_sum_is_the_egg_box_derivative(orc):
 # ---------------------------------------------------------------- mixing: readings A11b, A11c, A11d
 def test_mixing_switch_guard_and_automatic_w(orc):
     """A11d: mix_w_fixed <= 0 is lambda/(1+lambda), lambda = chi_0 L_max^2/pi (chi_0 by a central difference of Eq. 9 here).
-    A11b: with mix_mu_tol the fixed w is kept until two successive mu_a agree to mix_mu_tol kT, then More's w, latched.
+    A11b: with mix_mu_tol the fixed w is kept until two successive mu_a agree to mix_mu_tol kT (1 - w), then More's w, latched.
     A11c: where n_a underflows next to a finite n_i, Eq. 31 as printed makes K astronomically large and w = 0; the
     lower bound chi >= mix_chi_floor chi_0 keeps K finite, and it changes nothing where chi never gets that small."""
     cfg = ai.make_small(n_ions=2, cell=[9.0, 6.0, 6.0], grid=(12, 8, 8), T_eV=10.0, seed=5)
@@ -271,14 +271,14 @@ def test_mixing_switch_guard_and_automatic_w(orc):
     o.scf_begin(cfg["pos"]); r = o.scf_iter()
     assert abs(r["w_last"] - lam / (1 + lam)) < 1e-7
     # A11b: the switch
-    o = orc.Oracle(cfg, mix_mode=1, mix_warmup=0, mix_w_fixed=0.9, mix_mu_tol=1e-2, init_mode=0)
+    o = orc.Oracle(cfg, mix_mode=1, mix_warmup=0, mix_w_fixed=0.9, mix_mu_tol=1e-1, init_mode=0)
     o.scf_begin(cfg["pos"])
     hist = [o.scf_iter() for _ in range(25)]
     w = np.array([x["w_last"] for x in hist]); mu = np.array([x["mu"] for x in hist])
     fixed = np.isclose(w, 0.9)
     k = int(np.argmin(fixed))                               # first iteration with More's w
     assert k >= 2 and fixed[:k].all() and not fixed[k:].any()
-    assert abs(mu[k] - mu[k - 1]) <= 1e-2 * kT and np.all(np.abs(np.diff(mu[:k])) > 1e-2 * kT)
+    assert abs(mu[k] - mu[k - 1]) <= 1e-1 * kT * 0.1 and np.all(np.abs(np.diff(mu[:k])) > 1e-1 * kT * 0.1)   # (1 - w) = 0.1
     assert np.all(np.abs(w[k:] - np.array([x["U_mix"] / (x["K_mix"] + x["U_mix"]) for x in hist[k:]])) < 1e-12)
     # A11c: a cold cell, input density at the clip floor where the active density vanishes
     cold = ai.make_small(n_ions=2, cell=[9.0, 6.0, 6.0], grid=(12, 8, 8), T_eV=0.3, seed=5)
