@@ -145,6 +145,17 @@ int arche_get_density(arche_ctx *c, double *d_n); /* = arche_get_real(c, 0, d_n)
 /* 3D complex FFT, unnormalised, out-of-place or in-place (d_in == d_out allowed); sign = -1 forward, +1 inverse.
  * d_scratch: 16*Nx*Ny*Nz bytes. */
 int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, double *d_scratch, int sign);
+/* The same transform for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): no d_scratch argument, no cudaMalloc / cudaFree / allocating library call inside.  The scratch is a
+ * file-scope `static __device__` array of ARCHE_FFT3D_STATIC_MAX_POINTS complex doubles (4 MiB) in the library image:
+ * every GPU that loads the library holds it until exit.  Grids with Nx*Ny*Nz > ARCHE_FFT3D_STATIC_MAX_POINTS are rejected
+ * with ARCHE_EINVAL and a message in arche_last_error.  d_in / d_out: device pointers, 16*Nx*Ny*Nz bytes each, caller
+ * owned, d_in == d_out allowed.  Results are bit-identical to arche_fft3d.  ALL calls on one GPU (any context, any
+ * stream) share the one array and it keeps the last call's contents: nothing in it needs clearing (the first pass
+ * overwrites every element before it is read), but two calls that overlap on the GPU -- different streams, different
+ * contexts or processes' threads on the same device without ordering -- race on it.  Serialise them. */
+#define ARCHE_FFT3D_STATIC_MAX_POINTS (64 * 64 * 64)
+int arche_fft3d_static(arche_ctx *c, const double *d_in, double *d_out, int sign);
 /* The transform pair the SCF itself uses: real field [Nz][Ny][Nx] <-> half spectrum, through the r2c / c2r x passes and
  * the y/z passes (register two-stage kernels for N in {32,64,128,192,256,384}, generic radix kernels otherwise).
  * forward: d_full_out receives the full unnormalised spectrum [Nz][Ny][Nx] complex (the stored half expanded by

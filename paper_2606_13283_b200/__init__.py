@@ -21,7 +21,7 @@ SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_la
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
            "arche_rfft3d_forward", "arche_rfft3d_inverse",
            "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused", "arche_is_persistent",
-           "arche_peak_fp64", "arche_peak_l2", "arche_set_scf_iterations"]
+           "arche_peak_fp64", "arche_peak_l2", "arche_set_scf_iterations", "arche_fft3d_static"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
 
@@ -81,6 +81,7 @@ def load(rebuild_if_stale: bool = True):
     L.arche_get_complex.argtypes = [vp, C.c_int, dp]
     L.arche_get_density.argtypes = [vp, dp]
     L.arche_fft3d.argtypes = [vp, dp, dp, dp, C.c_int]
+    L.arche_fft3d_static.argtypes = [vp, dp, dp, C.c_int]
     L.arche_rfft3d_forward.argtypes = [vp, dp, dp]
     L.arche_rfft3d_inverse.argtypes = [vp, dp, dp]
     L.arche_fermi_dirac.argtypes = [vp, C.c_int, dp, dp, C.c_size_t]
@@ -252,6 +253,15 @@ class Arche:
         a = a.to(device=self.device, dtype=t.complex128).contiguous()
         out = t.empty_like(a); scratch = t.empty_like(a)
         self._check(self.lib.arche_fft3d(self._h, a.data_ptr(), out.data_ptr(), scratch.data_ptr(), int(sign)))
+        return out
+
+    def fft3d_static(self, a, sign: int, out=None):
+        """arche_fft3d_static: no scratch argument, nothing allocated inside the call (grids up to 64^3 points)"""
+        t = self.torch
+        a = a.to(device=self.device, dtype=t.complex128).contiguous()
+        if out is None:
+            out = t.empty_like(a)
+        self._check(self.lib.arche_fft3d_static(self._h, a.data_ptr(), out.data_ptr(), int(sign)))
         return out
 
     def rfft3d_forward(self, a):

@@ -93,6 +93,7 @@ struct arche_ctx {
   double *n_i, *n_a, *V_i, *vps, *va, *psp_tab;
   PspTable T;      // f2: tabulated pseudopotential (device table inside the workspace)
   double2 *nh_i, *nh_a, *vh_ie, *S, *S2, *gh, *gh2, *work;  // half spectrum [nz][ny][P]
+  double2 *fft_static = nullptr;   // device address of g_fft3d_static_scratch on this context's device
   long long nh;      // P*ny*nz
   int nxh, P;
   bool persist;      // whole solve in one cooperative launch (scf_persistent.cuh): fused form, 32^3 / 64^3 grids
@@ -269,6 +270,25 @@ extern "C" void arche_destroy(arche_ctx *c) {
   delete c;
 }
 
+// Scratch of arche_fft3d_static: lives in the library image, one copy on every GPU that loads the library, until exit.
+// In host code `g_fft3d_static_scratch` is a host-side stand-in, NOT a device address: the address the kernels get is
+// the one cudaGetSymbolAddress returns, taken once per device at set-up with that device current.
+static __device__ __align__(256) double2 g_fft3d_static_scratch[ARCHE_FFT3D_STATIC_MAX_POINTS];
+static double2 *g_fft3d_static_ptr[64];   // per device ordinal; written at set-up (arche_scf_init)
+static int fft3d_static_setup(arche_ctx *c) {
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(c, ARCHE_EINVAL, "device ordinal beyond the static-scratch table");
+  if (!g_fft3d_static_ptr[dev]) {
+    double2 *ptr = nullptr;
+    CK(cudaGetSymbolAddress((void **)&ptr, g_fft3d_static_scratch));
+    if (!ptr) return fail(c, ARCHE_ECUDA, "cudaGetSymbolAddress returned a null address for the static FFT scratch");
+    g_fft3d_static_ptr[dev] = ptr;
+  }
+  c->fft_static = g_fft3d_static_ptr[dev];
+  return ARCHE_OK;
+}
+
 static int init_body(arche_ctx *c, const arche_params *p);
 
 extern "C" int arche_scf_init(const arche_params *p, arche_ctx **out) {
@@ -414,7 +434,7 @@ static int init_body(arche_ctx *c, const arche_params *p) {
   LAUNCHED(c);
   CK(cudaStreamSynchronize(c->stream));
   c->p.h_Z = nullptr; c->p.h_mass = nullptr; c->p.h_psp_table = nullptr;  // copied; do not keep the caller's pointers
-  return ARCHE_OK;
+  return fft3d_static_setup(c);
 }
 
 // =============================================================================================
@@ -885,6 +905,20 @@ extern "C" int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, doub
     CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz, LoadComplex{w}, StoreComplex{o}, c->stream))); ++c->launches;
   }
   return ARCHE_OK;
+}
+
+// arche_fft3d without caller scratch and without any allocation: the intermediate passes go through the file-scope
+// device array (see its declaration above).  Nothing in it has to start at zero: the first pass writes all Nx*Ny*Nz
+// elements before any later pass reads them.  All calls on a device share the array.
+extern "C" int arche_fft3d_static(arche_ctx *c, const double *d_in, double *d_out, int sign) {
+  if (!c || !d_in || !d_out || (sign != 1 && sign != -1)) return ARCHE_EINVAL;
+  if (c->ng > (long long)ARCHE_FFT3D_STATIC_MAX_POINTS) {
+    snprintf(c->err, sizeof(c->err), "arche_fft3d_static: grid of %lld points exceeds ARCHE_FFT3D_STATIC_MAX_POINTS = %d "
+             "(use arche_fft3d with caller scratch)", c->ng, (int)ARCHE_FFT3D_STATIC_MAX_POINTS);
+    return ARCHE_EINVAL;
+  }
+  if (!c->fft_static) return fail(c, ARCHE_ECUDA, "static FFT scratch address was not taken at set-up");
+  return arche_fft3d(c, d_in, d_out, reinterpret_cast<double *>(c->fft_static), sign);
 }
 
 extern "C" int arche_rfft3d_forward(arche_ctx *c, const double *d_real_in, double *d_full_out) {
