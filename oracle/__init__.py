@@ -37,7 +37,8 @@ class Params(C.Structure):
                 ("scf_tol_F", C.c_double), ("scf_tol_dn", C.c_double), ("scf_max_iter", C.c_int),
                 ("scf_fixed_iter", C.c_int), ("ewald_alpha", C.c_double),
                 ("n_electrons", C.c_double), ("mix_mu_tol", C.c_double), ("psp", C.c_int), ("psp_nk", C.c_int),
-                ("psp_dk", C.c_double), ("mix_chi_floor", C.c_double), ("psp_table", C.POINTER(C.c_double))]
+                ("psp_dk", C.c_double), ("mix_chi_floor", C.c_double), ("psp_table", C.POINTER(C.c_double)),
+                ("ensemble", C.c_int)]
 
 
 class Result(C.Structure):
@@ -85,6 +86,7 @@ def lib():
         L.oracle_forces.argtypes = [C.c_void_p, dp]
         L.oracle_md_step.argtypes = [C.c_void_p, C.c_double, dp, dp, C.POINTER(Result)]
         L.oracle_stress.argtypes = [C.c_void_p, dp, dp]
+        L.oracle_isokinetic_kick.argtypes = [C.c_int, dp, dp, C.c_double, dp]
         L.oracle_get_real.argtypes = [C.c_void_p, C.c_int, dp]
         L.oracle_get_complex.argtypes = [C.c_void_p, C.c_int, dp]
         L.oracle_num_threads.restype = C.c_int
@@ -177,6 +179,13 @@ def force_ie(cell, grid, pos, Z, rc, nhat) -> np.ndarray:
 
 
 # ---- f2: average-atom pseudopotential (aa_pseudopotential.c)
+def isokinetic_kick(mass, F, t, vel) -> np.ndarray:
+    """Exact constant-force flow of the Gaussian isokinetic equations over a time t (reading A23); returns the new velocities."""
+    m = _f64(mass); f = _f64(F); v = _f64(vel).copy()
+    lib().oracle_isokinetic_kick(len(m), _dp(m), _dp(f), float(t), _dp(v))
+    return v
+
+
 def fd_wide(twice_j, eta):
     return lib().oracle_fd_wide(int(twice_j), float(eta))
 
@@ -225,7 +234,7 @@ class Oracle:
     def __init__(self, cfg: dict, **over):
         p = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=3,
                  scf_tol_F=1e-10, scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0,
-                 ewald_alpha=0.0, n_electrons=0.0, mix_mu_tol=0.0, mix_chi_floor=0.0)
+                 ewald_alpha=0.0, n_electrons=0.0, mix_mu_tol=0.0, mix_chi_floor=0.0, ensemble=0)
         for k in p:
             if k in cfg:
                 p[k] = cfg[k]

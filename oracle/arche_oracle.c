@@ -743,23 +743,49 @@ int oracle_forces(oracle_ctx *c, double *F) {
   return 0;
 }
 
+/* Isokinetic ensemble ("the isokinetic ensemble algorithm, also implemented in Arche, follows similar
+ * lines [48]"; reading A23).  Gauss's principle of least constraint for K = sum m v^2/2 = const gives
+ *   m_j dv_j/dt = F_j - alpha m_j v_j,   alpha = sum_j F_j.v_j / (2K).
+ * With the forces frozen, u(t) = exp(int_0^t alpha) turns this into d(u v_j)/dt = u F_j/m_j, so that with s = int_0^t u
+ * (s(0) = 0, s'(0) = 1) v_j(t) = (v_j(0) + (F_j/m_j) s)/s'; inserting that into alpha = s''/s' gives
+ *   s'' = a + b s,   a = sum F.v(0)/(2K),  b = sum F^2/m /(2K),
+ * so s(t) = (a/b)(cosh(t sqrt b) - 1) + sinh(t sqrt b)/sqrt b, s'(t) = (a/sqrt b) sinh(t sqrt b) + cosh(t sqrt b)
+ * and v_j(t) = (v_j(0) + (F_j/m_j) s(t)) / s'(t).  K is conserved exactly by this map. */
+void oracle_isokinetic_kick(int n, const double *mass, const double *F, double t, double *vel) {
+  long double twoK = 0.0L, fv = 0.0L, ff = 0.0L;
+  for (int j = 0; j < n; ++j)
+    for (int d = 0; d < 3; ++d) {
+      twoK += (long double)mass[j] * vel[3 * j + d] * vel[3 * j + d];
+      fv += (long double)F[3 * j + d] * vel[3 * j + d];
+      ff += (long double)F[3 * j + d] * F[3 * j + d] / mass[j];
+    }
+  if (twoK <= 0.0L || ff <= 0.0L) return; /* no motion to constrain, or no force: v stays */
+  long double a = fv / twoK, b = ff / twoK, rb = sqrtl(b);
+  long double sh = sinhl(t * rb), ch = coshl(t * rb);
+  long double s = (a / b) * (ch - 1.0L) + sh / rb, sd = (a / rb) * sh + ch;
+  for (int j = 0; j < n; ++j)
+    for (int d = 0; d < 3; ++d) vel[3 * j + d] = (double)((vel[3 * j + d] + (long double)F[3 * j + d] / mass[j] * s) / sd);
+}
+
 int oracle_md_step(oracle_ctx *c, double dt, double *pos, double *vel, oracle_result *out) {
   int n = c->p.n_ions, rc = 0;
   if (!c->have_forces) { /* forces at the starting positions */
     rc = oracle_scf_solve(c, pos, NULL);
     oracle_forces(c, NULL);
   }
+  if (c->p.ensemble == 1) oracle_isokinetic_kick(n, c->mass, c->F, 0.5 * dt, vel);
   for (int j = 0; j < n; ++j)
     for (int d = 0; d < 3; ++d) {
-      vel[3 * j + d] += 0.5 * dt * c->F[3 * j + d] / c->mass[j];
+      if (c->p.ensemble != 1) vel[3 * j + d] += 0.5 * dt * c->F[3 * j + d] / c->mass[j];
       pos[3 * j + d] += dt * vel[3 * j + d];
     }
   rc = oracle_scf_solve(c, pos, NULL);
   oracle_forces(c, NULL);
+  if (c->p.ensemble == 1) oracle_isokinetic_kick(n, c->mass, c->F, 0.5 * dt, vel);
   long double ki = 0.0L;
   for (int j = 0; j < n; ++j)
     for (int d = 0; d < 3; ++d) {
-      vel[3 * j + d] += 0.5 * dt * c->F[3 * j + d] / c->mass[j];
+      if (c->p.ensemble != 1) vel[3 * j + d] += 0.5 * dt * c->F[3 * j + d] / c->mass[j];
       ki += 0.5 * c->mass[j] * vel[3 * j + d] * vel[3 * j + d]; /* Eq. 36 */
     }
   c->last.K_i = (double)ki;

@@ -51,6 +51,9 @@ typedef struct {
   double psp_dk;       /* table spacing in k (1/bohr, ordinary frequency) */
   double mix_chi_floor; /* >0: lower bound of dn_a/dmu in K (Eq. 31) in units of the uniform-gas value (reading A11c) */
   const double *psp_table; /* [psp_nk] Du(k_m): non-Coulomb part of the form factor per unit charge, u = -1/(pi k^2) + Du */
+  int ensemble;        /* 0 microcanonical: velocity Verlet; 1 isokinetic: the ion kinetic energy is a
+                          constant of the motion ("the isokinetic ensemble algorithm ... follows similar
+                          lines [48]"; reading A23) */
 } oracle_params;
 
 typedef struct {
@@ -96,7 +99,11 @@ int oracle_scf_iter(oracle_ctx *c, oracle_result *out);
 int oracle_scf_solve(oracle_ctx *c, const double *pos, oracle_result *out);
 /* total force F^ie + F^ii on every ion from the last active density */
 int oracle_forces(oracle_ctx *c, double *F);
-/* one velocity-Verlet step (reading D2) */
+/* Gaussian isokinetic half step (ref. [48]; reading A23): the exact flow over a time t of
+ * m_j dv_j/dt = F_j - alpha m_j v_j, alpha = sum F.v / sum m v^2, for forces held constant; vel updated in place. */
+void oracle_isokinetic_kick(int n_ions, const double *mass, const double *F, double t, double *vel);
+/* one velocity-Verlet step (reading D2); ensemble = 1: the same splitting with the isokinetic
+ * kick in place of the free one */
 int oracle_md_step(oracle_ctx *c, double dt, double *pos, double *vel, oracle_result *out);
 /* field access: which = 0 n_a, 1 n_i (next input), 2 V_i ; complex: 0 nhat_a, 1 Vhat_ie, 2 S_Z, 3 ghat, 4 nhat_i */
 int oracle_get_real(oracle_ctx *c, int which, double *dst);
