@@ -67,6 +67,10 @@ typedef struct {
                             n_a underflows (chi -> 0) next to a finite n_i the quadratic model overstates the stiffness by
                             hundreds of orders of magnitude and w collapses to 0 (reading A11c); <= 0: Eq. 31 as
                             printed */
+  int ensemble;          /* arche_md_step: 0 microcanonical, velocity Verlet; 1 isokinetic (ref. [48]; SURVEY.md 8
+                            f4; reading A23): the half kicks are the exact constant-force flow of the Gaussian
+                            isokinetic equations m dv/dt = F - alpha m v, alpha = sum F.v / sum m v^2, so the ion kinetic
+                            energy of the initial velocities is conserved to round-off */
   void *d_workspace;     /* device memory, >= arche_workspace_bytes(), 256-byte aligned */
   size_t workspace_bytes;
   void *stream;          /* cudaStream_t (0 = default stream) */
@@ -125,7 +129,7 @@ int arche_stress(arche_ctx *c, const double *d_vel, double *h_out);
 int arche_set_scf_iterations(arche_ctx *c, int scf_max_iter, int scf_fixed_iter);
 
 /* One velocity-Verlet step of length dt (a.u.) (reading D2): half kick, drift, SCF solve at the
- * new positions, forces, half kick.  d_pos/d_vel [n_ions*3] are updated in place.  The first call also solves
+ * new positions, forces, half kick (params.ensemble = 1: isokinetic half kicks, same splitting).  d_pos/d_vel [n_ions*3] are updated in place.  The first call also solves
  * at the starting positions to obtain the initial forces.  Later calls reuse the forces of the previous step: a caller
  * that edits the positions between two steps must call arche_scf_solve + arche_forces on them first.
  * Returns ARCHE_ENOCONV when either solve of the step hit scf_max_iter (the step is still taken). */

@@ -38,7 +38,7 @@ class Params(C.Structure):
                 ("scf_tol_dn", C.c_double), ("scf_max_iter", C.c_int), ("scf_fixed_iter", C.c_int),
                 ("ewald_alpha", C.c_double), ("n_electrons", C.c_double), ("psp", C.c_int), ("psp_nk", C.c_int),
                 ("psp_dk", C.c_double), ("h_psp_table", C.c_void_p), ("mix_mu_tol", C.c_double), ("mix_chi_floor", C.c_double),
-                ("d_workspace", C.c_void_p),
+                ("ensemble", C.c_int), ("d_workspace", C.c_void_p),
                 ("workspace_bytes", C.c_size_t), ("stream", C.c_void_p)]
 
 
@@ -98,7 +98,8 @@ def load(rebuild_if_stale: bool = True):
 
 
 _DEFAULTS = dict(xc=1, psp_rc=1.12, init_mode=1, mix_mode=1, mix_w_fixed=0.95, mix_warmup=3, scf_tol_F=1e-10,
-                 scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0, ewald_alpha=0.0, n_electrons=0.0, mix_mu_tol=0.0, mix_chi_floor=0.0)
+                 scf_tol_dn=1e-12, scf_max_iter=500, scf_fixed_iter=0, ewald_alpha=0.0, n_electrons=0.0, mix_mu_tol=0.0, mix_chi_floor=0.0,
+                 ensemble=0)
 
 
 class Arche:

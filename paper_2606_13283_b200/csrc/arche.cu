@@ -237,6 +237,7 @@ bool params_ok(const arche_params *p) {
   if (p->n_ions > 0 && (!p->h_Z || !p->h_mass)) return false;
   if (p->xc < 0 || p->xc > 2) return false;
   if (p->psp != 0 && p->psp != 1) return false;
+  if (p->ensemble != 0 && p->ensemble != 1) return false;
   if (p->psp == 1) {   // the table must cover every |k| of the grid
     if (p->psp_nk < 4 || !(p->psp_dk > 0.0) || !p->h_psp_table) return false;
     double k2 = 0.0;
@@ -835,12 +836,14 @@ extern "C" int arche_md_step(arche_ctx *c, double dt, double *d_pos, double *d_v
     rc = compute_forces(c);
     if (rc) return rc;
   }
-  kick_drift_kernel<<<nb, 128, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, dt, ni, 1); LAUNCHED(c);
+  if (c->p.ensemble == 1) { isokinetic_kick_kernel<<<1, 1024, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, 0.5 * dt, dt, ni, 1); LAUNCHED(c); }
+  else { kick_drift_kernel<<<nb, 128, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, dt, ni, 1); LAUNCHED(c); }
   int rc_solve = scf_solve(c, d_pos);
   if (rc_solve != ARCHE_OK && rc_solve != ARCHE_ENOCONV) return rc_solve;
   rc = compute_forces(c);
   if (rc) return rc;
-  kick_drift_kernel<<<nb, 128, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, dt, ni, 0); LAUNCHED(c);
+  if (c->p.ensemble == 1) { isokinetic_kick_kernel<<<1, 1024, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, 0.5 * dt, dt, ni, 0); LAUNCHED(c); }
+  else { kick_drift_kernel<<<nb, 128, 0, c->stream>>>(d_pos, d_vel, c->F, c->mass, dt, ni, 0); LAUNCHED(c); }
   kinetic_kernel<<<1, 256, 0, c->stream>>>(d_vel, c->mass, ni, c->sc); LAUNCHED(c);
   rc = read_scalars(c);
   if (rc) return rc;

@@ -468,6 +468,41 @@ __global__ void kick_drift_kernel(double *__restrict__ pos, double *__restrict__
   if (drift) pos[e] += dt * v;
 }
 
+// Isokinetic ensemble (ref. [48]; reading A23): the exact flow over a time t of the Gaussian isokinetic
+// equations m dv/dt = F - alpha m v, alpha = sum F.v / sum m v^2, with the forces held constant, followed (drift = 1) by
+// the position update.  v(t) = (v(0) + (F/m) s)/s', s'' = a + b s with a = sum F.v/(2K), b = sum F^2/m /(2K); expm1 keeps
+// cosh - 1 exact for the small arguments of an MD step.  One block: the three sums are O(N_i).
+__global__ void __launch_bounds__(1024) isokinetic_kick_kernel(double *__restrict__ pos, double *__restrict__ vel,
+                                                               const double *__restrict__ F, const double *__restrict__ mass,
+                                                               double t, double dt, int nions, int drift) {
+  __shared__ double s_red[3 * 32];
+  __shared__ double s_s, s_sd;
+  double v[3] = {0.0, 0.0, 0.0};
+  for (int e = threadIdx.x; e < 3 * nions; e += blockDim.x) {
+    const double m = mass[e / 3], u = vel[e], f = F[e];
+    v[0] = fma(m * u, u, v[0]); v[1] = fma(f, u, v[1]); v[2] = fma(f / m, f, v[2]);
+  }
+  const int op[3] = {0, 0, 0};
+  block_reduce<3>(v, op, s_red);
+  if (threadIdx.x == 0) {
+    double s = 0.0, sd = 1.0;   // no motion to constrain, or no force: v stays
+    if (v[0] > 0.0 && v[2] > 0.0) {
+      const double a = v[1] / v[0], b = v[2] / v[0], rb = sqrt(b), x = t * rb;
+      const double ep = expm1(x), em = expm1(-x), sh = 0.5 * (ep - em), chm1 = 0.5 * (ep + em);
+      s = (a / b) * chm1 + sh / rb;
+      sd = (a / rb) * sh + chm1 + 1.0;
+    }
+    s_s = s; s_sd = sd;
+  }
+  __syncthreads();
+  const double s = s_s, rsd = 1.0 / s_sd;
+  for (int e = threadIdx.x; e < 3 * nions; e += blockDim.x) {
+    const double u = (vel[e] + F[e] / mass[e / 3] * s) * rsd;
+    vel[e] = u;
+    if (drift) pos[e] += dt * u;
+  }
+}
+
 __global__ void __launch_bounds__(256) kinetic_kernel(const double *__restrict__ vel, const double *__restrict__ mass,
                                                       int nions, DevScalars *sc) {
   __shared__ double s_red[32];

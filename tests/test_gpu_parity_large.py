@@ -174,6 +174,44 @@ def test_c1_md_trajectory_replayed(orc, torch_cuda):
         assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max(), step
 
 
+@pytest.mark.parametrize("n_ions,grid", [(5, (16, 12, 24)), (1100, (16, 12, 8))])
+def test_isokinetic_md_trajectory_replayed(orc, torch_cuda, n_ions, grid):
+    """f4, isokinetic ensemble (ref. [48]; reading A23): three steps with the oracle's iteration counts replayed.
+    Positions, velocities, forces and F against the oracle, and the ion kinetic energy constant to round-off on the
+    device's own trajectory.  Case 2 has more velocity components (3300) than the kick kernel has threads."""
+    torch = torch_cuda
+    if n_ions < 100:
+        cfg = ai.make_small(n_ions=n_ions, L=8.0, grid=grid, T_eV=10.0, seed=41)
+    else:
+        cfg = ai.make_small(n_ions=n_ions, grid=grid, cell=[40.0, 33.0, 27.0], T_eV=30.0, seed=42, dmin=1.2)
+        cfg["Z"] = np.full(n_ions, 0.1)
+    kw = dict(scf_tol_F=1e-10, scf_tol_dn=1e-9, scf_max_iter=300, ensemble=1)
+    o = orc.Oracle(cfg, **kw); g = _gpu(cfg, **kw)
+    po = cfg["pos"].copy(); vo = cfg["vel"].copy()
+    pg = torch.as_tensor(cfg["pos"].copy(), device="cuda"); vg = torch.as_tensor(cfg["vel"].copy(), device="cuda")
+    K0 = 0.5 * float(np.sum(cfg["mass"][:, None] * cfg["vel"] ** 2))
+    ro = o.scf_solve(po); o.forces()
+    g.set_scf_iterations(fixed_iter=ro["scf_iters"])
+    g.scf_solve(pg); g.forces()
+    for step in range(3):
+        ro = o.md_step(cfg["dt"], po, vo)
+        g.set_scf_iterations(fixed_iter=ro["scf_iters"])
+        rg = g.md_step(cfg["dt"], pg, vg)
+        assert abs(rg["K_i"] - K0) < 1e-13 * K0, step                   # the constant of the motion
+        assert abs(rg["K_i"] - ro["K_i"]) < 1e-13 * K0, step
+        assert abs(rg["F_total"] - ro["F_total"]) < TOL_F * abs(ro["F_total"]), step
+        assert np.abs(pg.cpu().numpy() - po).max() < 1e-10, step
+        assert np.abs(vg.cpu().numpy() - vo).max() < 1e-10 * np.abs(vo).max(), step
+        Fo = o.forces(); Fg = g.forces().cpu().numpy()
+        assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max(), step
+    assert np.abs(po - cfg["pos"]).max() > 1e-4                        # the ions moved
+    # the microcanonical step from the same state is a different map (the flag is honoured)
+    g0 = _gpu(cfg, **dict(kw, ensemble=0))
+    p0 = torch.as_tensor(cfg["pos"].copy(), device="cuda"); v0 = torch.as_tensor(cfg["vel"].copy(), device="cuda")
+    r0 = g0.md_step(cfg["dt"], p0, v0)
+    assert abs(r0["K_i"] - K0) > 1e-9 * K0
+
+
 @pytest.mark.parametrize("name,grid", [("c1", None), ("streamed-128", (128, 32, 16))])
 def test_one_center_start_field_by_field(orc, torch_cuda, monkeypatch, name, grid):
     """P4 (Eq. 20, reading A10): after a first solve, ions are displaced and scf_begin builds n_i = clip/renormalise of the
