@@ -89,6 +89,9 @@ struct arche_ctx {
   bool pdl;        // programmatic dependent launch between the kernels of an SCF iteration (ARCHE_PDL=0 disables)
   int r_blocks;    // resident blocks per SM of the streamed real-space Fermi-Dirac kernels
   int force_slabs, force_rows_per_slab, force_ipt;   // ions per thread of the force kernel's register tile
+  int force_ch, force_chunks, force_zslabs;          // > 0: column-resident force kernel with force_ch columns per thread
+  double2 *force_wb, *force_rk;                      // W of the flipped Nyquist rows; signed ky, kz per virtual row
+  int4 *force_ri;                                    // iy, iz, sign masks per virtual row
   // device arrays (all inside the caller's workspace)
   double *n_i, *n_a, *V_i, *vps, *va, *psp_tab;
   PspTable T;      // f2: tabulated pseudopotential (device table inside the workspace)
@@ -198,6 +201,11 @@ size_t layout(arche_ctx *c, char *base) {
   c->vel_tmp = w.take<double>(3 * ni);
   c->pp_part = w.take<double>(6 * ni); c->stress = w.take<double>(64);
   c->F_part = w.take<double>((size_t)c->force_slabs * ni * 3);
+  {  // column-resident force kernel: W of the virtual rows beyond ny nz, row tables (1 element when unused)
+    const size_t nvp = c->force_ch > 0 ? (size_t)force_vrows_padded(ny, nz) : 1, nrw = (size_t)ny * nz;
+    c->force_wb = w.take<double2>(c->force_ch > 0 ? (nvp - nrw) * (size_t)c->P : 1);
+    c->force_ri = w.take<int4>(nvp); c->force_rk = w.take<double2>(nvp);
+  }
   c->fdtab = w.take<double>(kFdTabDoubles);
   c->partials = w.take<double>((size_t)c->red_blocks * kMaxRed);
   c->counter = w.take<unsigned int>(64);
@@ -228,6 +236,30 @@ void derive_sizes(arche_ctx *c) {
   if (slabs < 1) slabs = 1;
   c->force_rows_per_slab = (int)((rows + slabs - 1) / slabs);
   c->force_slabs = (int)((rows + c->force_rows_per_slab - 1) / c->force_rows_per_slab);
+  c->force_ch = 0;
+  if (c->nions >= 256 && !getenv("ARCHE_FORCE_ROWS")) {   // column-resident force kernel (force_cols_kernel)
+    static const int kCh[4] = {13, 17, 20, 25};
+    int best = 0, bestpad = 1 << 30;
+    for (int q = 0; q < 4; ++q) {   // fewest padded columns; ties go to the wider chunk (less per-row overhead)
+      const int pad = (c->nxh + kCh[q] - 1) / kCh[q] * kCh[q];
+      if (pad <= bestpad) { bestpad = pad; best = kCh[q]; }
+    }
+    if (const char *e = getenv("ARCHE_FORCE_CH")) {   // tuning override
+      const int v = atoi(e);
+      if (v == 13 || v == 17 || v == 20 || v == 25) best = v;
+    }
+    c->force_ch = best;
+    c->force_chunks = (c->nxh + best - 1) / best;
+    const long long vrows = force_vrows_padded(ny, nz);
+    const int t128 = (c->nions + FCC_THREADS - 1) / FCC_THREADS, per = t128 * c->force_chunks;
+    int z = (148 * 3 * 8 + per - 1) / per;        // about 8 waves of 3 resident blocks per SM
+    if (z > vrows / (4 * FCC_GR)) z = (int)(vrows / (4 * FCC_GR));
+    if (z < 1) z = 1;
+    c->force_rows_per_slab = (int)((vrows + z - 1) / z);
+    c->force_rows_per_slab = (c->force_rows_per_slab + FCC_GR - 1) / FCC_GR * FCC_GR;
+    c->force_zslabs = (int)((vrows + c->force_rows_per_slab - 1) / c->force_rows_per_slab);
+    c->force_slabs = c->force_zslabs * c->force_chunks;
+  }
 }
 
 bool params_ok(const arche_params *p) {
@@ -432,6 +464,7 @@ static int init_body(arche_ctx *c, const arche_params *p) {
   c->T.on = p->psp == 1 ? 1 : 0; c->T.nk = p->psp_nk; c->T.dk = p->psp_dk; c->T.tab = c->psp_tab;
   if (c->T.on) CK(cudaMemcpyAsync(c->psp_tab, p->h_psp_table, (size_t)p->psp_nk * sizeof(double), cudaMemcpyHostToDevice, c->stream));
   form_factor_kernel<<<c->ew_grid, 256, 0, c->stream>>>(G, p->psp_rc, c->T, c->alpha, c->vps, c->va);
+  if (c->force_ch > 0) force_rowinfo_kernel<<<64, 256, 0, c->stream>>>(G, c->force_ri, c->force_rk);
   LAUNCHED(c);
   CK(cudaStreamSynchronize(c->stream));
   c->p.h_Z = nullptr; c->p.h_mass = nullptr; c->p.h_psp_table = nullptr;  // copied; do not keep the caller's pointers
@@ -729,7 +762,14 @@ int compute_forces(arche_ctx *c) {
   dim3 fg((unsigned)((ni + per_block - 1) / per_block), (unsigned)c->force_slabs);
   const size_t fsm = FC_RPT * c->nxh * sizeof(double2) + c->nxh * sizeof(double);
   { ProfScope ps(c, PC_FORCE);
-  if (ipt == 4)
+  if (c->force_ch > 0) {
+    dim3 cg((unsigned)((ni + FCC_THREADS - 1) / FCC_THREADS), (unsigned)c->force_chunks, (unsigned)c->force_zslabs);
+    force_w_kernel<<<c->ew_grid, 256, 0, c->stream>>>(G, c->vps, c->va, c->nh_a, c->S, c->S2, c->work, c->force_wb); LAUNCHED(c);
+#define ARCHE_FCC(CH) force_cols_kernel<CH><<<cg, FCC_THREADS, 0, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, \
+                                                                       c->cz_ij, c->work, c->force_wb, c->force_ri, c->force_rk, c->F_part)
+    if (c->force_ch == 13) ARCHE_FCC(13); else if (c->force_ch == 17) ARCHE_FCC(17); else if (c->force_ch == 20) ARCHE_FCC(20); else ARCHE_FCC(25);
+#undef ARCHE_FCC
+  } else if (ipt == 4)
     force_kernel<4><<<fg, FC_THREADS, fsm, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,
                                                         c->nh_a, c->S, c->S2, c->F_part);
   else if (ipt == 2)

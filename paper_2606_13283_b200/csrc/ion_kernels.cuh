@@ -447,6 +447,166 @@ __global__ void __launch_bounds__(FC_THREADS) force_kernel(
   }
 }
 
+// Column-resident form of the force sum (round 2; n_ions >= 256).  ncu of force_kernel<4> at 384^3 / 2000 ions: 236
+// registers, two blocks per SM, fp64 pipe 58% busy, the top stalls are the L2 loads of a_j(kx) (re-read for every group
+// of four rows: 229 GB per call) and fixed-latency waits that two warps per scheduler cannot cover.  Here a thread
+// owns one ion and CH kx columns and keeps a_j(kx) of those columns IN REGISTERS for its whole life; it walks over the
+// (virtual) rows of its slab, and the only operand of the inner loop is W(row, kx), which the copy engine brings into
+// shared memory (cp.async.bulk completing on an mbarrier, FCC_NST stages of FCC_GR rows in flight: no staging
+// instructions in the compute warps) and every warp reads as a broadcast.  Per (ion, row, kx): t = W a_j, P += t,
+// Q' += c t with the column number c an immediate (kx = (c0 + c)/Lx is linear in c: the kx-weighted sum is
+// (c0 P + Q')/Lx), 8 fp64 instructions and one LDS.128; per (ion, row) 11 more to fold P, Q' with b_j(ky) c_j(kz) into
+// the four running sums.
+// Virtual rows: v < ny nz is row v in its literal form; v >= ny nz runs over the rows with a Nyquist ky or kz once more
+// in the flipped variant (see force_kernel); the list is padded to a multiple of FCC_GR with rows of W = 0.
+// force_rowinfo_kernel (once per context) tabulates iy, iz, the sign masks and the signed ky, kz of every virtual row;
+// force_w_kernel (once per call) forms the weighted W of every virtual row: rows v < ny nz in Wa [ny nz][P] (the FFT
+// scratch array), the others in Wb [.][P].  Grid of force_cols_kernel: x = tiles of 128 ions, y = column chunks, z =
+// slabs of virtual rows; F_part[(z gridDim.y + y)][j][3].
+constexpr int FCC_THREADS = 128;
+constexpr int FCC_GR = 4;    // rows per shared-memory stage
+constexpr int FCC_R = 2;     // rows in flight per thread
+constexpr int FCC_NST = 3;   // stages in flight
+struct ForceVRow { int iy, iz, var; bool nyq; };
+__device__ __forceinline__ ForceVRow force_vrow(const GridGeom &G, int v, int nrows, int nyq_y, int nyq_z) {
+  ForceVRow r;
+  if (v < nrows) { r.iy = v % G.ny; r.iz = v / G.ny; r.var = 0; }
+  else {
+    const int ra = v - nrows;
+    r.var = 1;
+    if (nyq_z >= 0 && ra < G.ny) { r.iy = ra; r.iz = nyq_z; }
+    else { const int q = ra - (nyq_z >= 0 ? G.ny : 0); r.iy = nyq_y; r.iz = (nyq_z >= 0 && q >= nyq_z) ? q + 1 : q; }
+  }
+  r.nyq = r.iy == nyq_y || r.iz == nyq_z;
+  return r;
+}
+__host__ __device__ inline long long force_vrows(int ny, int nz) {   // virtual rows, not padded
+  const bool ey = ny % 2 == 0, ez = nz % 2 == 0;
+  return (long long)ny * nz + (ez ? ny : 0) + (ey ? (ez ? nz - 1 : nz) : 0);
+}
+__host__ __device__ inline long long force_vrows_padded(int ny, int nz) {
+  return (force_vrows(ny, nz) + FCC_GR - 1) / FCC_GR * FCC_GR;
+}
+__device__ __forceinline__ double flip_sign(double x, unsigned int mask) {   // mask = 0 or 0x80000000
+  return __hiloint2double(__double2hiint(x) ^ (int)mask, __double2loint(x));
+}
+__global__ void force_rowinfo_kernel(GridGeom G, int4 *__restrict__ ri, double2 *__restrict__ rk) {
+  const int nrows = G.ny * G.nz, nv = (int)force_vrows(G.ny, G.nz), nvp = (int)force_vrows_padded(G.ny, G.nz);
+  const int nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
+  for (int v = blockIdx.x * blockDim.x + threadIdx.x; v < nvp; v += gridDim.x * blockDim.x) {
+    if (v >= nv) { ri[v] = make_int4(0, 0, 0, 0); rk[v] = make_double2(0.0, 0.0); continue; }
+    const ForceVRow r = force_vrow(G, v, nrows, nyq_y, nyq_z);
+    const bool fy = r.var == 1 && r.iy == nyq_y, fz = r.var == 1 && r.iz == nyq_z;
+    ri[v] = make_int4(r.iy, r.iz, fy ? (int)0x80000000u : 0, fz ? (int)0x80000000u : 0);
+    rk[v] = make_double2(fy ? -G.ky[r.iy] : G.ky[r.iy], fz ? -G.kz[r.iz] : G.kz[r.iz]);
+  }
+}
+__global__ void __launch_bounds__(256) force_w_kernel(GridGeom G, const double *__restrict__ vps, const double *__restrict__ va,
+                                                      const double2 *__restrict__ nh_a, const double2 *__restrict__ S,
+                                                      const double2 *__restrict__ S2, double2 *__restrict__ Wa,
+                                                      double2 *__restrict__ Wb) {
+  const int nrows = G.ny * G.nz, nv = (int)force_vrows(G.ny, G.nz), nvp = (int)force_vrows_padded(G.ny, G.nz);
+  const int nyq_y = (G.ny % 2 == 0) ? G.ny / 2 : -1, nyq_z = (G.nz % 2 == 0) ? G.nz / 2 : -1;
+  const long long tot = (long long)nvp * G.P;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < tot; e += (long long)gridDim.x * blockDim.x) {
+    const int v = (int)(e / G.P), ix = (int)(e - (long long)v * G.P);
+    double2 w = make_double2(0.0, 0.0);
+    if (v < nv && ix < G.nxh) {
+      const ForceVRow r = force_vrow(G, v, nrows, nyq_y, nyq_z);
+      const long long g = ((long long)r.iz * G.ny + r.iy) * G.P + ix;
+      const bool edge = ix == 0 || 2 * ix == G.nx;
+      const double wt = edge ? (r.var == 0 ? 1.0 : 0.0) : (r.nyq ? 1.0 : 2.0);
+      const double2 n = nh_a[g], sf = r.var == 0 ? S[g] : S2[g];
+      const double pv = vps[g], pa = va[g];
+      w = make_double2(wt * (pv * n.x + pa * sf.x), -wt * (pv * n.y + pa * sf.y));
+    }
+    if (v < nrows) Wa[e] = w; else Wb[e - (long long)nrows * G.P] = w;
+  }
+}
+template <int CH>
+__global__ void __launch_bounds__(FCC_THREADS, 3) force_cols_kernel(
+    GridGeom G, int nions, int vrows_per_slab /* multiple of FCC_GR */, const double2 *__restrict__ ax_ij /*[ix][j]*/,
+    const double2 *__restrict__ by_ij, const double2 *__restrict__ cz_ij, const double2 *__restrict__ Wa,
+    const double2 *__restrict__ Wb, const int4 *__restrict__ ri_tab, const double2 *__restrict__ rk_tab,
+    double *__restrict__ F_part) {
+  static_assert(FCC_GR % FCC_R == 0, "rows in flight");
+  __shared__ __align__(16) double2 s_w[FCC_NST][FCC_GR][CH];
+  __shared__ __align__(16) int4 s_ri[FCC_NST][FCC_GR];      // iy, iz, sign masks of the flipped variant for b_j(ky).y, c_j(kz).y
+  __shared__ __align__(16) double2 s_rk[FCC_NST][FCC_GR];   // ky, kz (signed for the flipped variant)
+  __shared__ unsigned long long s_bar[FCC_NST];
+  const int tid = threadIdx.x, j = blockIdx.x * FCC_THREADS + tid, c0 = blockIdx.y * CH;
+  const bool jok = j < nions;
+  const int jc = jok ? j : nions - 1;
+  const int nrows = G.ny * G.nz, nvp = (int)force_vrows_padded(G.ny, G.nz);
+  const int v0 = blockIdx.z * vrows_per_slab, v1 = min(nvp, v0 + vrows_per_slab);
+  const int nstages = v1 > v0 ? (v1 - v0) / FCC_GR : 0;
+  const int ncol = min(CH, G.P - c0);                        // columns of this chunk that exist in the arrays
+  const unsigned stage_bytes = (unsigned)(FCC_GR * ncol * sizeof(double2) + FCC_GR * (sizeof(int4) + sizeof(double2)));
+  for (int e = tid; e < FCC_NST * FCC_GR * CH; e += FCC_THREADS) (&s_w[0][0][0])[e] = make_double2(0.0, 0.0);
+  if (tid == 0)
+    for (int q = 0; q < FCC_NST; ++q) mbar_init(&s_bar[q], 1);
+  __syncthreads();
+  auto issue = [&](int st) {   // thread 0: bring stage st into buffer st % FCC_NST
+    const int q = st % FCC_NST, vb = v0 + st * FCC_GR;
+    mbar_arrive_expect_tx(&s_bar[q], stage_bytes);
+#pragma unroll
+    for (int r = 0; r < FCC_GR; ++r) {
+      const int v = vb + r;
+      const double2 *src = v < nrows ? Wa + (long long)v * G.P + c0 : Wb + (long long)(v - nrows) * G.P + c0;
+      bulk_copy_g2s(&s_w[q][r][0], src, (unsigned)(ncol * sizeof(double2)), &s_bar[q]);
+    }
+    bulk_copy_g2s(&s_ri[q][0], ri_tab + vb, FCC_GR * sizeof(int4), &s_bar[q]);
+    bulk_copy_g2s(&s_rk[q][0], rk_tab + vb, FCC_GR * sizeof(double2), &s_bar[q]);
+  };
+  if (tid == 0)
+    for (int st = 0; st < FCC_NST && st < nstages; ++st) issue(st);
+  double2 a[CH];
+#pragma unroll
+  for (int c = 0; c < CH; ++c)
+    a[c] = (jok && c0 + c < G.nxh) ? ax_ij[(long long)(c0 + c) * nions + j] : make_double2(0.0, 0.0);
+  double sP = 0.0, sQ = 0.0, fy = 0.0, fz = 0.0;
+  for (int st = 0; st < nstages; ++st) {
+    const int buf = st % FCC_NST;
+    mbar_wait(&s_bar[buf], (unsigned)((st / FCC_NST) & 1));
+#pragma unroll
+    for (int rr = 0; rr < FCC_GR; rr += FCC_R) {
+      double2 b[FCC_R], cc[FCC_R];
+#pragma unroll
+      for (int q = 0; q < FCC_R; ++q) {
+        const int4 ri = s_ri[buf][rr + q];
+        b[q] = by_ij[(long long)ri.x * nions + jc]; cc[q] = cz_ij[(long long)ri.y * nions + jc];
+        b[q].y = flip_sign(b[q].y, (unsigned int)ri.z); cc[q].y = flip_sign(cc[q].y, (unsigned int)ri.w);
+      }
+      double2 P[FCC_R], Q[FCC_R];
+#pragma unroll
+      for (int q = 0; q < FCC_R; ++q) { P[q] = make_double2(0.0, 0.0); Q[q] = make_double2(0.0, 0.0); }
+#pragma unroll
+      for (int c = 0; c < CH; ++c) {
+#pragma unroll
+        for (int q = 0; q < FCC_R; ++q) {
+          const double2 w = s_w[buf][rr + q][c];
+          const double2 t = make_double2(fma(w.x, a[c].x, -w.y * a[c].y), fma(w.x, a[c].y, w.y * a[c].x));
+          P[q].x += t.x; P[q].y += t.y;
+          if (c > 0) { Q[q].x = fma((double)c, t.x, Q[q].x); Q[q].y = fma((double)c, t.y, Q[q].y); }
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < FCC_R; ++q) {
+        const double2 k = s_rk[buf][rr + q];
+        const double2 bc = make_double2(b[q].x * cc[q].x - b[q].y * cc[q].y, b[q].x * cc[q].y + b[q].y * cc[q].x);
+        const double imP = P[q].x * bc.y + P[q].y * bc.x, imQ = Q[q].x * bc.y + Q[q].y * bc.x;
+        sP += imP; sQ += imQ; fy = fma(k.x, imP, fy); fz = fma(k.y, imP, fz);
+      }
+    }
+    __syncthreads();                                   // every warp is done with this buffer
+    if (tid == 0 && st + FCC_NST < nstages) issue(st + FCC_NST);
+  }
+  if (jok) {
+    double *o = F_part + ((size_t)(blockIdx.z * gridDim.y + blockIdx.y) * nions + j) * 3;
+    o[0] = ((double)c0 * sP + sQ) / G.Lx; o[1] = fy; o[2] = fz;
+  }
+}
+
 // one warp per force component: the lanes stride over the slabs, fixed-order shuffle tree (deterministic)
 __global__ void force_finish_kernel(int nions, int nslabs, const double *__restrict__ F_part, const double *__restrict__ F_pp,
                                     const double *__restrict__ Z, double pref /* -2 pi/|Omega| */, double *__restrict__ F) {
