@@ -238,21 +238,24 @@ void derive_sizes(arche_ctx *c) {
   c->force_slabs = (int)((rows + c->force_rows_per_slab - 1) / c->force_rows_per_slab);
   c->force_ch = 0;
   if (c->nions >= 256 && !getenv("ARCHE_FORCE_ROWS")) {   // column-resident force kernel (force_cols_kernel)
-    static const int kCh[4] = {13, 17, 20, 25};
-    int best = 0, bestpad = 1 << 30;
-    for (int q = 0; q < 4; ++q) {   // fewest padded columns; ties go to the wider chunk (less per-row overhead)
-      const int pad = (c->nxh + kCh[q] - 1) / kCh[q] * kCh[q];
-      if (pad <= bestpad) { bestpad = pad; best = kCh[q]; }
+    // columns per thread: the cost of a (row, ion) is 8 fp64 instructions per column, padded columns included, plus about
+    // 30 instruction slots per chunk (fold with b_j c_j, row tables, barrier); measured at 384^3 / 2000 ions: 37.7, 36.8,
+    // 34.6, 33.4, 32.0 ms for 13, 17, 20, 25, 33 columns (33 columns: 216 registers, two blocks per SM)
+    static const int kCh[5] = {13, 17, 20, 25, 33};
+    int best = 0; long long bestcost = 1LL << 60;
+    for (int q = 0; q < 5; ++q) {
+      const long long cost = (long long)((c->nxh + kCh[q] - 1) / kCh[q]) * (8 * kCh[q] + 30);
+      if (cost <= bestcost) { bestcost = cost; best = kCh[q]; }
     }
     if (const char *e = getenv("ARCHE_FORCE_CH")) {   // tuning override
       const int v = atoi(e);
-      if (v == 13 || v == 17 || v == 20 || v == 25) best = v;
+      for (int q = 0; q < 5; ++q) if (v == kCh[q]) best = v;
     }
     c->force_ch = best;
     c->force_chunks = (c->nxh + best - 1) / best;
     const long long vrows = force_vrows_padded(ny, nz);
     const int t128 = (c->nions + FCC_THREADS - 1) / FCC_THREADS, per = t128 * c->force_chunks;
-    int z = (148 * 3 * 8 + per - 1) / per;        // about 8 waves of 3 resident blocks per SM
+    int z = (148 * (best > 25 ? 2 : 3) * 8 + per - 1) / per;        // about 8 waves of the resident blocks
     if (z > vrows / (4 * FCC_GR)) z = (int)(vrows / (4 * FCC_GR));
     if (z < 1) z = 1;
     c->force_rows_per_slab = (int)((vrows + z - 1) / z);
@@ -767,7 +770,7 @@ int compute_forces(arche_ctx *c) {
     force_w_kernel<<<c->ew_grid, 256, 0, c->stream>>>(G, c->vps, c->va, c->nh_a, c->S, c->S2, c->work, c->force_wb); LAUNCHED(c);
 #define ARCHE_FCC(CH) force_cols_kernel<CH><<<cg, FCC_THREADS, 0, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, \
                                                                        c->cz_ij, c->work, c->force_wb, c->force_ri, c->force_rk, c->F_part)
-    if (c->force_ch == 13) ARCHE_FCC(13); else if (c->force_ch == 17) ARCHE_FCC(17); else if (c->force_ch == 20) ARCHE_FCC(20); else ARCHE_FCC(25);
+    if (c->force_ch == 13) ARCHE_FCC(13); else if (c->force_ch == 17) ARCHE_FCC(17); else if (c->force_ch == 20) ARCHE_FCC(20); else if (c->force_ch == 33) ARCHE_FCC(33); else ARCHE_FCC(25);
 #undef ARCHE_FCC
   } else if (ipt == 4)
     force_kernel<4><<<fg, FC_THREADS, fsm, c->stream>>>(G, ni, c->force_rows_per_slab, c->ax_ij, c->by_ij, c->cz_ij, c->vps, c->va,

@@ -524,7 +524,7 @@ __global__ void __launch_bounds__(256) force_w_kernel(GridGeom G, const double *
   }
 }
 template <int CH>
-__global__ void __launch_bounds__(FCC_THREADS, 3) force_cols_kernel(
+__global__ void __launch_bounds__(FCC_THREADS, CH > 25 ? 2 : 3) force_cols_kernel(
     GridGeom G, int nions, int vrows_per_slab /* multiple of FCC_GR */, const double2 *__restrict__ ax_ij /*[ix][j]*/,
     const double2 *__restrict__ by_ij, const double2 *__restrict__ cz_ij, const double2 *__restrict__ Wa,
     const double2 *__restrict__ Wb, const int4 *__restrict__ ri_tab, const double2 *__restrict__ rk_tab,

@@ -46,12 +46,20 @@ def _check_iteration_fields(g, o):
     assert _rel(g.get_complex("nhat_a").cpu().numpy(), o.get_complex("nhat_a")) < TOL_N
 
 
-def test_force_kernel_four_ions_per_thread(orc, torch_cuda):
-    """force_kernel<4> (n_ions >= 1024; the register tile of 4 ions x 4 rows per thread, the j >= n_ions tail of the last
-    block and the slab split) on a grid the oracle does in seconds: 1100 weak ions (Z = 0.1) in an anisotropic cell on
-    32 x 24 x 16, two SCF iterations, then the total forces."""
-    n = 1100
-    cfg = ai.make_small(n_ions=n, grid=(32, 24, 16), cell=[16.0, 12.0, 9.0], T_eV=10.0, seed=41, dmin=0.5)
+@pytest.mark.parametrize("variant,n,grid", [("cols", 1100, (32, 24, 16)), ("cols", 300, (18, 9, 12)), ("cols-odd", 300, (16, 9, 27)),
+                                            ("cols-13", 300, (48, 8, 12)), ("cols-17", 300, (64, 8, 9)), ("cols-20", 300, (36, 8, 12)),
+                                            ("cols-25", 300, (96, 8, 8)), ("rows-4", 1100, (32, 24, 16)), ("rows-2", 300, (18, 9, 12))])
+def test_force_kernels_many_ions(orc, torch_cuda, monkeypatch, variant, n, grid):
+    """The force kernels of n_ions >= 256 on grids the oracle does in seconds: weak ions (Z = 0.1) in an anisotropic cell,
+    two SCF iterations, then the total forces.  "cols": force_cols_kernel (a_j(kx) of a chunk of columns in registers, W
+    staged by the copy engine; every chunk width, the j >= n_ions tail of the last ion tile, chunks that end beyond the
+    last stored column, slabs whose last stage is padding, odd ny / nz without Nyquist rows); "rows-4" / "rows-2":
+    force_kernel<4> / <2>, the row-tiled form (ARCHE_FORCE_ROWS=1)."""
+    if variant.startswith("rows"):
+        monkeypatch.setenv("ARCHE_FORCE_ROWS", "1")
+    elif "-" in variant and variant.split("-")[1].isdigit():
+        monkeypatch.setenv("ARCHE_FORCE_CH", variant.split("-")[1])
+    cfg = ai.make_small(n_ions=n, grid=grid, cell=[16.0, 12.0, 9.0], T_eV=10.0, seed=41, dmin=0.5)
     cfg["Z"] = np.full(n, 0.1)
     g = _gpu(cfg); o = orc.Oracle(cfg)
     g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
@@ -62,6 +70,9 @@ def test_force_kernel_four_ions_per_thread(orc, torch_cuda):
         _check_scalars(rg, ro, it)
     Fg = g.forces().cpu().numpy(); Fo = o.forces()
     assert np.abs(Fg - Fo).max() < TOL_FORCE * np.abs(Fo).max()
+    # the scratch array the force pass borrows for W is the FFT scratch: the next iteration must be unaffected
+    rg = g.scf_iter(); ro = o.scf_iter()
+    _check_scalars(rg, ro, "after forces")
 
 
 def test_c4_full_size(orc, torch_cuda):
