@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  bool lazy_F;     // free energy only where the stop rule needs it (ARCHE_LAZY_F=0 disables); see ScfConst::lazy_F
   bool pdl;        // programmatic dependent launch between the kernels of an SCF iteration (ARCHE_PDL=0 disables)
   int r_blocks;    // resident blocks per SM of the streamed real-space Fermi-Dirac kernels
   int force_slabs, force_rows_per_slab, force_ipt;   // ions per thread of the force kernel's register tile
@@ -422,6 +423,7 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     // 155 -> 177 MD steps/s, 192^3 +1.4%) and costs ~2% at 384^3, where early-resident blocks of the next kernel take
     // shared memory from the tail of the running one: on by default up to 8 M grid points
     { const char *e = getenv("ARCHE_PDL"); c->pdl = e ? e[0] != '0' : c->ng <= 8000000LL; }
+    { const char *e = getenv("ARCHE_LAZY_F"); c->lazy_F = e ? e[0] != '0' : true; }
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, kFdTabBytes));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
@@ -682,6 +684,8 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
   CK(cudaMemsetAsync(&c->sc->iter, 0, sizeof(int) * 6, c->stream));   // iter, converged, mu_evals_total, flip_seen, more_on, pad
   CK(cudaMemsetAsync(&c->sc->F_total, 0, sizeof(double), c->stream));
   CK(cudaMemsetAsync(&c->sc->mu_evals_total, 0, sizeof(int), c->stream));
+  CK(cudaMemsetAsync(&c->sc->skip_F, 0, 2 * sizeof(int), c->stream));   // skip_F, F_valid
+  c->C.lazy_F = 0;   // the split form (arche_scf_iter) evaluates the free energy in every iteration
   c->have_solution = false;
   c->have_forces = false;
   c->mix_pending = false;  // a new input density replaces any unapplied mixing step
@@ -730,6 +734,9 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   // kernels of the remaining iterations of the batch return at once, so the state stays that of the converged
   // iteration.  Parity replays (scf_fixed_iter) run every iteration.
   {
+  // lazy free energy (ScfConst::lazy_F): under the stop rule F is evaluated only where the rule can use it.  Not with the
+  // printed PZ81 constants (the branch-flip detection of reading A13 watches F in every iteration), not in parity replays.
+  c->C.lazy_F = (fixed <= 0 && c->p.xc != 1 && c->lazy_F) ? maxit : 0;
   const int batch = fixed > 0 ? maxit : kScfBatch;
   for (int it = 0; it < maxit && !conv;) {
     c->stop = fixed > 0 ? nullptr : &c->sc->converged;
@@ -747,6 +754,7 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   }
   }
 solved:
+  c->C.lazy_F = 0;
   // P6: one-center profile of this step's converged density (reading A10)
   if (c->nions > 0) {
     g_store_kernel<<<c->ew_grid, 256, 0, c->stream>>>(c->gh, c->gh2, c->nh_a, c->S, c->S2, c->nh, 1e-8 * c->Q * c->Q);

@@ -29,11 +29,18 @@ struct DevScalars {
   double mu_iter_prev, tolF_eff, toldn_eff;         // mu_a of the previous iteration; the tolerances the stop rule applied
   // per-MD-step
   double U_pp, U_pm_sum, U_pm_fix, U_ii, init_sum, init_scale, K_i;
+  // lazy free energy (ScfConst::lazy_F): skip_F = the running iteration leaves out the terms only F needs (I_{3/2}, eps_xc,
+  // E_ie); F_valid = F_total is the free energy of the previous iteration
+  int skip_F, F_valid;
 };
 
 struct ScfConst {
   double kT, cTF, Ne, vol, dV, eta0, E_ie0;
-  int xc, mix_mode, mix_warmup, pad;
+  int xc, mix_mode, mix_warmup;
+  int lazy_F;   // > 0: solves under the stop rule evaluate the free energy only from the iteration at which the density
+                // criterion is predicted to be met within two iterations, and in iteration lazy_F (= scf_max_iter), so that
+                // a solve never ends without it.  The paper's own stop rule needs no F; BASELINE's |dF| criterion
+                // needs F_k and F_{k-1} of the last two iterations only.  0: every iteration (parity replays, xc = 1)
   double mix_w_fixed, tol_F, tol_dn;
   double inv_vol, inv_qF;   // reciprocals for the single-thread scalar updates (fp64 divisions cost ~300 cycles each there)
   double q_F, q_dn;   // reading A13: free-energy quantum of one PZ81 branch flip; chi(n*) x V_c jump x sqrt(dV)
@@ -429,25 +436,29 @@ struct LoadDensity {
   const double *fdtab;
   ScfConst C;
   double mu, inv_kT, sK, sdn2, sna2, sF0, sKe, sExc, sChi;
+  bool wantF;   // uniform: this iteration evaluates the free-energy terms (F_0, K_e, E_xc)
   __device__ __forceinline__ void set_table(const double *t) { fdtab = t; }
   __device__ __forceinline__ void begin() {
     mu = sc->mu; inv_kT = 1.0 / C.kT;
     sK = sdn2 = sna2 = sF0 = sKe = sExc = sChi = 0.0;
+    wantF = sc->skip_F == 0;
   }
   __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(V_i + idx); prefetch_l2(n_i + idx); }
   __device__ __forceinline__ double load_real(long long g, int, int, int) {
     const double eta = (mu - V_i[g]) * inv_kT;
-    double im12, i12, i32;
-    fd_eval<7>(fdtab, eta, im12, i12, i32);
+    double im12, i12, i32 = 0.0;
+    if (wantF) fd_eval<7>(fdtab, eta, im12, i12, i32); else fd_eval<3>(fdtab, eta, im12, i12, i32);
     const double na = C.cTF * i12;                    // Eq. 9
     const double chi = C.cTF * 0.5 * im12 * inv_kT;   // dn_a/dmu
     const double dn = n_i[g] - na;
     n_a[g] = na;
     if (chi > 1.0e-290) sK += dn * dn * rcp_fast(fmax(chi, C.chi_floor));   // Eq. 31 (reading A11c: optional lower bound)
     sdn2 += dn * dn; sna2 += na * na; sChi += chi;
-    sF0 += eta * i12 - (2.0 / 3.0) * i32;             // f_0/(kT cTF), from Eq. 38-39
-    sKe += i32;                                       // Eq. 38
-    if (C.xc) { double e, vx; xc_pz81(na, e, vx, C.xc); sExc += na * e; }
+    if (wantF) {
+      sF0 += eta * i12 - (2.0 / 3.0) * i32;           // f_0/(kT cTF), from Eq. 38-39
+      sKe += i32;                                     // Eq. 38
+      if (C.xc) { double e, vx; xc_pz81(na, e, vx, C.xc); sExc += na * e; }
+    }
     return na;
   }
   struct Pre { double v0, v1, n0, n1; };
@@ -456,9 +467,9 @@ struct LoadDensity {
   }
   __device__ __forceinline__ void compute(long long ia, long long ib, const Pre &p, double &ra, double &rb) {
     const long long g[2] = {ia, ib};
-    double eta[2] = {(mu - p.v0) * inv_kT, (mu - p.v1) * inv_kT}, im12[2], i12[2], i32[2];
+    double eta[2] = {(mu - p.v0) * inv_kT, (mu - p.v1) * inv_kT}, im12[2], i12[2], i32[2] = {0.0, 0.0};
     const double ni[2] = {p.n0, p.n1};
-    fd_eval_multi<7, 2>(fdtab, eta, im12, i12, i32);
+    if (wantF) fd_eval_multi<7, 2>(fdtab, eta, im12, i12, i32); else fd_eval_multi<3, 2>(fdtab, eta, im12, i12, i32);
     double na[2];
 #pragma unroll
     for (int m = 0; m < 2; ++m) {
@@ -468,9 +479,14 @@ struct LoadDensity {
       n_a[g[m]] = na[m];
       if (chi > 1.0e-290) sK += dn * dn * rcp_fast(fmax(chi, C.chi_floor));   // Eq. 31 (reading A11c: optional lower bound)
       sdn2 += dn * dn; sna2 += na[m] * na[m]; sChi += chi;
-      sF0 += eta[m] * i12[m] - (2.0 / 3.0) * i32[m];
-      sKe += i32[m];
-      if (C.xc) { double e, vx; xc_pz81(na[m], e, vx, C.xc); sExc += na[m] * e; }
+    }
+    if (wantF) {
+#pragma unroll
+      for (int m = 0; m < 2; ++m) {
+        sF0 += eta[m] * i12[m] - (2.0 / 3.0) * i32[m];
+        sKe += i32[m];
+        if (C.xc) { double e, vx; xc_pz81(na[m], e, vx, C.xc); sExc += na[m] * e; }
+      }
     }
     ra = na[0]; rb = na[1];
   }
@@ -521,14 +537,14 @@ struct StoreNhatA {
   HalfGeom H;
   int prestored;   // 1: the value is already scaled and stored in nh_a (streaming reduction after a plain z pass)
   double aU, aEH, aEie;
-  __device__ __forceinline__ void begin() { aU = aEH = aEie = 0.0; }
-  __device__ __forceinline__ void prefetch(long long idx) const { prefetch_l2(vh_ie + idx); prefetch_l2(nh_i + idx); }
+  bool wantF;   // uniform: this iteration evaluates E_ie (the only use of Vhat_ie in S5)
+  __device__ __forceinline__ void begin() { aU = aEH = aEie = 0.0; wantF = sc->skip_F == 0; }
+  __device__ __forceinline__ void prefetch(long long idx) const { if (wantF) prefetch_l2(vh_ie + idx); prefetch_l2(nh_i + idx); }
   __device__ __forceinline__ void store(long long idx, int ix, int iy, int iz, double re, double im) {
     if (ix >= H.nxh) { if (!prestored) nh_a[idx] = make_double2(0.0, 0.0); return; }
     if (!prestored) { re *= C.dV; im *= C.dV; nh_a[idx] = make_double2(re, im); }
     const double wt = H.wt(ix);
-    const double2 b = vh_ie[idx];
-    aEie += wt * (re * b.x + im * b.y);                  // Re conj(nhat_a) Vhat_ie
+    if (wantF) { const double2 b = vh_ie[idx]; aEie += wt * (re * b.x + im * b.y); }   // Re conj(nhat_a) Vhat_ie
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 != 0.0) {
       const double inv = wt * __drcp_rn(ARCHE_PI * k2);
@@ -543,8 +559,7 @@ struct StoreNhatA {
     if (ix >= H.nxh) { v = make_double2(0.0, 0.0); return; }
     v.x *= C.dV; v.y *= C.dV;
     const double wt = H.wt(ix);
-    const double2 b = vh_ie[idx];
-    aEie += wt * (v.x * b.x + v.y * b.y);
+    if (wantF) { const double2 b = vh_ie[idx]; aEie += wt * (v.x * b.x + v.y * b.y); }
     const double k2 = kx2[ix] + ky2[iy] + kz2[iz];
     if (k2 != 0.0) {
       const double inv = wt * __drcp_rn(ARCHE_PI * k2);
@@ -584,7 +599,8 @@ struct StoreNhatA {
       double w;
       if (C.mix_mode == 1 && it > C.mix_warmup && (C.mix_mu_tol <= 0.0 || sc->more_on)) w = (K + U > 0.0) ? U / (K + U) : 0.0;   // w = U/(K+U)
       else w = C.mix_w_fixed;
-      const double F = sc->F0 + sc->Exc + EH + Eie + C.E_ie0 + sc->U_ii;
+      const bool haveF = sc->skip_F == 0;   // this iteration evaluated F0, E_xc, E_ie (always, unless C.lazy_F)
+      const double F = haveF ? sc->F0 + sc->Exc + EH + Eie + C.E_ie0 + sc->U_ii : sc->F_total;
       const double dn_rel = sqrt(sc->dn2 / sc->na2);
       // reading A13: PZ81's two branches differ by 3.2e-5 Ha (eps_c) / 2.7e-5 Ha (V_c) at r_s = 1, n* = 3/(4 pi).  A grid
       // point whose converged density sits on n* flips branch between iterations: F then moves by whole quanta
@@ -592,7 +608,7 @@ struct StoreNhatA {
       // q_dn/||n_a|| -- neither criterion can be met below that.  A jump of F by an integer number (1..8) of quanta
       // marks the solve; from then on two quanta are tolerated in both criteria.  flip_seen and the tolerances applied
       // are reported in arche_result.
-      const double dFs = F - sc->F_total, dF = fabs(dFs);
+      const double dFs = F - sc->F_total, dF = (haveF && (sc->F_valid || !C.lazy_F)) ? fabs(dFs) : 1.0e300;
       if (C.xc == 1 && it >= 3 && C.q_F > 0.0) {
         const double dFp = sc->F_total - sc->F_prev;
         const double m = dF * C.inv_qF, r = rint(m), mp = fabs(dFp) * C.inv_qF, rp = rint(mp);
@@ -607,7 +623,15 @@ struct StoreNhatA {
       const double toldn = C.tol_dn + (sc->flip_seen ? 2.0 * C.q_dn / sqrt(sc->na2) : 0.0);
       sc->converged = (it >= 2 && dF < tolF && dn_rel < toldn) ? 1 : 0;
       sc->tolF_eff = tolF; sc->toldn_eff = toldn;
-      sc->F_prev = sc->F_total; sc->F_total = F; sc->w = w; sc->dn_rel = dn_rel; sc->iter = it;
+      if (C.lazy_F > 0) {
+        // F is needed in the iteration that meets the density criterion and in the one before it: predict the residual
+        // two iterations ahead from the last contraction factor (a wrong guess costs iterations, never the result)
+        const double rho = (it >= 2 && sc->dn_rel > 0.0) ? fmin(fmax(dn_rel / sc->dn_rel, 0.05), 1.0) : 1.0;
+        sc->skip_F = (dn_rel * rho * rho > 4.0 * toldn && it + 1 < C.lazy_F) ? 1 : 0;
+      }
+      sc->F_valid = haveF ? 1 : 0;
+      if (haveF) sc->F_prev = sc->F_total;
+      sc->F_total = F; sc->w = w; sc->dn_rel = dn_rel; sc->iter = it;
       sc->mu_have_prev = 1;
     }
   }
