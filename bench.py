@@ -104,7 +104,7 @@ def ncu_traffic():
 
 
 def roofline_entry(name, ms_per_launch, ng, bpp, peak_gbs, peak_src, fp64_peak, fp64_src, evals_per_launch=1.0,
-                   pairs=None):
+                   pairs=None, flops_per_point=None):
     """roofline object of one kernel class: HBM bytes for the streaming/FFT classes, fp64 flops for the
     arithmetic-bound ones (whichever bound is the higher fraction is the binding one and is reported)"""
     t = ms_per_launch * 1e-3
@@ -115,8 +115,9 @@ def roofline_entry(name, ms_per_launch, ng, bpp, peak_gbs, peak_src, fp64_peak, 
     hbm = bpp.get(name, 0.0) * evals_per_launch * ng / t / 1e9 if t > 0 else 0.0
     out = {"bound": "hbm", "kernel": name, "achieved": hbm, "peak": peak_gbs, "unit": "GB/s",
            "frac": hbm / peak_gbs, "traffic": None, "peak_source": peak_src}
-    if name in FLOPS_PER_POINT and t > 0 and not (name == "fft_inv_x_vi" and "vi_r" in bpp):
-        tf = FLOPS_PER_POINT[name] * evals_per_launch * ng / t / 1e12
+    fpp = flops_per_point or FLOPS_PER_POINT
+    if name in fpp and t > 0 and not (name == "fft_inv_x_vi" and "vi_r" in bpp):
+        tf = fpp[name] * evals_per_launch * ng / t / 1e12
         if tf / fp64_peak > out["frac"]:
             out = {"bound": "alu", "kernel": name, "achieved": tf, "peak": fp64_peak, "unit": "TFLOP/s",
                    "frac": tf / fp64_peak, "traffic": None, "peak_source": fp64_src, "hbm_gbs": hbm}
@@ -235,6 +236,9 @@ def workload_config(cfg, name):
                          (" (widened by two PZ81 branch-flip quanta when a flip is detected: DESIGN.md reading A13; "
                           "flagged per run as flip_steps)" if tol["xc"] == 1 else " (strict: the XC potential is continuous)"),
             "mixing": mix,
+            "free_energy": ("evaluated in every SCF iteration" if tol["xc"] == 1 or os.environ.get("ARCHE_LAZY_F", "1")[0] == "0" else
+                            "evaluated only in the iterations where the stop rule can use it (the last ones of a solve; "
+                            "free_energy_evals_per_step in the line; DESIGN.md section 5)"),
             "l2": ("L2 flushed between timed steps (256 MiB write); fields of %.1f GB per step exceed the 126 MB L2"
                    % (99.0 * ng / 1e9) if ng >= 192 ** 3 else
                    "L2 flushed between timed steps (256 MiB write); the working set is L2-resident within a step")}
@@ -275,13 +279,13 @@ class MdRun:
     def timed(self, K, step_fn):
         torch = self.torch
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
-        out = dict(iters=0, mu_evals=0, not_converged=0, flips=0)
+        out = dict(iters=0, mu_evals=0, not_converged=0, flips=0, F_evals=0)
         for a, b in ev:
             self.flush.fill_(1)                      # evict L2 between timed steps
             a.record(self.g.stream)
             r = step_fn()
             b.record(self.g.stream)
-            out["iters"] += r["scf_iters"]; out["mu_evals"] += r["mu_evals"]
+            out["iters"] += r["scf_iters"]; out["mu_evals"] += r["mu_evals"]; out["F_evals"] += r.get("F_evals", r["scf_iters"])
             out["not_converged"] += int(r["converged"] != 1 or r["rc"] != 0); out["flips"] += int(r["flip_seen"])
         torch.cuda.synchronize()
         out["seconds"] = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
@@ -330,6 +334,19 @@ def class_table(run, prof_out, K, dev_out, peak, peak_src, fp64_peak, fp64_src, 
     bpp = bytes_per_point(g.grid[0], g.is_fused())
     tot = sum(v[0] for v in prof.values()) or 1.0
     evals_per_iter = dev_out["mu_evals"] / max(dev_out["iters"], 1)
+    # lazy free energy: only the fraction f_F of the iterations evaluates I_{3/2}, eps_xc (density classes) and E_ie
+    # (the Vhat_ie read of the S5 reduction); the launches of a class are timed together, so the work per launch is
+    # the mix of the two forms
+    f_F = prof_out["F_evals"] / max(prof_out["iters"], 1)
+    bpp = dict(bpp)
+    h = 16.0 * ((g.grid[0] // 2 + 1 + 7) // 8 * 8) / g.grid[0]
+    if "reduce_g" in bpp:
+        bpp["reduce_g"] = (2.0 + f_F) * h
+    elif "fft_fwd_z_reduce" in bpp:
+        bpp["fft_fwd_z_reduce"] = (3.0 + f_F) * h
+    flops = dict(FLOPS_PER_POINT)
+    for k in ("density", "density_r"):
+        flops[k] = (2 * 30 + 14) + f_F * (30 + 90 + 6)
     P = (g.grid[0] // 2 + 1 + 7) // 8 * 8
     pairs = float(g.n_ions) * P * g.grid[1] * g.grid[2]
     rl, kernels = {}, {}
@@ -340,7 +357,7 @@ def class_table(run, prof_out, K, dev_out, peak, peak_src, fp64_peak, fp64_src, 
         if k in bpp or k in FLOPS_PER_POINT or k in FLOPS_PER_PAIR:
             # the mu kernel's launches carry (evals_per_iter - 1) evaluations each: the first rides in the S2 pass
             per = max(evals_per_iter - 1.0, 1e-9) if k == "mu_pass" else 1.0
-            e = roofline_entry(k, ms / n, ng, bpp, peak, peak_src, fp64_peak, fp64_src, per, pairs)
+            e = roofline_entry(k, ms / n, ng, bpp, peak, peak_src, fp64_peak, fp64_src, per, pairs, flops)
             e["traffic"] = traffic.get(k)
             rl[k] = e
             ent.update({"bound": e["bound"], "achieved": round(e["achieved"], 2), "unit": e["unit"], "frac": round(e["frac"], 4)})
@@ -348,6 +365,9 @@ def class_table(run, prof_out, K, dev_out, peak, peak_src, fp64_peak, fp64_src, 
                 ent["ncu_dram_bytes_per_launch"] = e["traffic"]
                 ent["algorithmic_bytes_per_launch"] = bpp.get(k, 0.0) * per * ng
         kernels[k] = ent
+    for k in ("density", "density_r", "reduce_g", "fft_fwd_z_reduce"):
+        if k in kernels:
+            kernels[k]["free_energy_fraction_of_launches"] = round(f_F, 4)
     return rl, kernels, tot, evals_per_iter, bpp
 
 
@@ -380,7 +400,7 @@ def bench_config_block(name, dev, flush, K, W, peak, peak_src, fp64_peak, fp64_s
     blk = {"workload": workload_config(cfg, name)["workload"], "steps": K, "warmup": W,
            "md_steps_per_s": K / d["seconds"], "ms_per_step": 1e3 * d["seconds"] / K,
            "scf_iterations_per_s": d["iters"] / d["seconds"], "scf_iters_per_step": d["iters"] / K,
-           "e2e_md_steps_per_s": K / h["seconds"], "not_converged_steps": d["not_converged"], "flip_steps": d["flips"],
+           "free_energy_evals_per_step": d["F_evals"] / K, "e2e_md_steps_per_s": K / h["seconds"], "not_converged_steps": d["not_converged"], "flip_steps": d["flips"],
            "gpu_launches": int(d["launches"]), "mixing": workload_config(cfg, name)["mixing"],
            "form": "persistent" if run.g.is_persistent() else ("fused" if run.g.is_fused() else "streamed"),
            "kernels": {k: {kk: v[kk] for kk in ("share", "us_per_launch", "bound", "frac") if kk in v} for k, v in kernels.items()}}
@@ -522,6 +542,7 @@ def main():
             "ms_per_scf_iteration_incl_ion_work": 1e3 * t_dev_max / max(d["iters"], 1),
             "grid_points_per_s": world * d["iters"] * g.ng / t_dev_max,
             "not_converged_steps": d["not_converged"], "flip_steps": d["flips"],
+            "free_energy_evals_per_step": d["F_evals"] / K,
             "clocks": cs.summary(),
             "e2e": {"value": world * K / t_e2e_max, "unit": "md_steps/s",
                     "h2d_bytes_per_step": h["h2d_bytes_per_step"], "d2h_bytes_per_step": h["d2h_bytes_per_step"],

@@ -86,6 +86,10 @@ typedef struct {
   double tol_F_eff, tol_dn_eff;                /* the tolerances the stop rule applied in the last iteration (reading A13) */
   int scf_iters, mu_evals, converged;
   int flip_seen;                               /* 1: a PZ81 branch flip was detected and the tolerances were widened (A13) */
+  int F_evals;                                 /* iterations of the solve that evaluated the free energy: all of them in the
+                                                  split form, in parity replays and with xc = 1; under the stop rule with
+                                                  xc = 0 / 2 only those where the rule can use it (the last two or so:
+                                                  the paper's own criterion P:231 needs no F; ARCHE_LAZY_F=0 disables) */
 } arche_result;
 
 /* Bytes of device workspace arche_scf_init will carve up for these parameters (0 on bad parameters). */

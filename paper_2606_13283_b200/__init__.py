@@ -45,7 +45,7 @@ class Params(C.Structure):
 class Result(C.Structure):
     _fields_ = [(k, C.c_double) for k in ("mu", "F_total", "F0", "E_H", "E_xc", "E_ie", "E_ie0", "U_ii", "K_e",
                                           "K_i", "dn_l2", "w_last", "U_mix", "K_mix", "tol_F_eff", "tol_dn_eff")] + \
-               [(k, C.c_int) for k in ("scf_iters", "mu_evals", "converged", "flip_seen")]
+               [(k, C.c_int) for k in ("scf_iters", "mu_evals", "converged", "flip_seen", "F_evals")]
 
     def asdict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -541,6 +541,7 @@ void fill_result(const arche_ctx *c, arche_result *r) {
   r->E_ie0 = c->C.E_ie0; r->U_ii = s.U_ii; r->K_e = s.Ke; r->K_i = s.K_i; r->dn_l2 = s.dn_rel;
   r->w_last = s.w; r->U_mix = s.U; r->K_mix = s.K; r->tol_F_eff = s.tolF_eff; r->tol_dn_eff = s.toldn_eff;
   r->scf_iters = s.iter; r->mu_evals = s.mu_evals_total; r->converged = s.converged; r->flip_seen = s.flip_seen;
+  r->F_evals = s.F_evals;
 }
 
 // forward transform of the real input density into nhat_i (scaled by dV)
@@ -684,7 +685,7 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
   CK(cudaMemsetAsync(&c->sc->iter, 0, sizeof(int) * 6, c->stream));   // iter, converged, mu_evals_total, flip_seen, more_on, pad
   CK(cudaMemsetAsync(&c->sc->F_total, 0, sizeof(double), c->stream));
   CK(cudaMemsetAsync(&c->sc->mu_evals_total, 0, sizeof(int), c->stream));
-  CK(cudaMemsetAsync(&c->sc->skip_F, 0, 2 * sizeof(int), c->stream));   // skip_F, F_valid
+  CK(cudaMemsetAsync(&c->sc->skip_F, 0, 4 * sizeof(int), c->stream));   // skip_F, F_valid, F_evals, pad
   c->C.lazy_F = 0;   // the split form (arche_scf_iter) evaluates the free energy in every iteration
   c->have_solution = false;
   c->have_forces = false;

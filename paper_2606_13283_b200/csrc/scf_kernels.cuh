@@ -31,7 +31,7 @@ struct DevScalars {
   double U_pp, U_pm_sum, U_pm_fix, U_ii, init_sum, init_scale, K_i;
   // lazy free energy (ScfConst::lazy_F): skip_F = the running iteration leaves out the terms only F needs (I_{3/2}, eps_xc,
   // E_ie); F_valid = F_total is the free energy of the previous iteration
-  int skip_F, F_valid;
+  int skip_F, F_valid, F_evals, pad2;   // F_evals: iterations of this solve that evaluated the free energy
 };
 
 struct ScfConst {
@@ -630,6 +630,7 @@ struct StoreNhatA {
         sc->skip_F = (dn_rel * rho * rho > 4.0 * toldn && it + 1 < C.lazy_F) ? 1 : 0;
       }
       sc->F_valid = haveF ? 1 : 0;
+      if (haveF) sc->F_evals += 1;
       if (haveF) sc->F_prev = sc->F_total;
       sc->F_total = F; sc->w = w; sc->dn_rel = dn_rel; sc->iter = it;
       sc->mu_have_prev = 1;

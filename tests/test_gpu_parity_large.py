@@ -223,6 +223,41 @@ def test_isokinetic_md_trajectory_replayed(orc, torch_cuda, n_ions, grid):
     assert abs(r0["K_i"] - K0) > 1e-9 * K0
 
 
+@pytest.mark.parametrize("mode", ["fused", "streamed"])
+def test_lazy_free_energy_is_the_same_solve(orc, torch_cuda, monkeypatch, mode):
+    """Under the stop rule the device evaluates the free-energy terms (I_3/2, eps_xc, E_ie) only where the rule can use
+    them (ScfConst::lazy_F).  The iterates do not depend on F, so against the same solve with ARCHE_LAZY_F=0: the same
+    iteration count, bit-identical density and forces, the same final F and energy terms -- with fewer evaluations; and
+    against the oracle's own free stop: within one iteration, F to 1e-9.  A solve that hits scf_max_iter still ends
+    with the free energy of its last iterate."""
+    monkeypatch.setenv("ARCHE_FUSE", "1" if mode == "fused" else "0")
+    monkeypatch.setenv("ARCHE_PERSIST", "0")
+    cfg = ai.make_small(n_ions=5, L=9.0, grid=(24, 16, 18), T_eV=15.0, seed=52)
+    kw = dict(xc=2, scf_tol_F=1e-10, scf_tol_dn=1e-9, scf_max_iter=400)
+    res = {}
+    for lazy in ("1", "0"):
+        monkeypatch.setenv("ARCHE_LAZY_F", lazy)
+        g = _gpu(cfg, **kw)
+        r = g.scf_solve(cfg["pos"])
+        res[lazy] = (r, g.get_real("n_a").cpu().numpy(), g.forces().cpu().numpy())
+    (r1, n1, F1), (r0, n0, F0) = res["1"], res["0"]
+    assert r1["converged"] == 1 and r0["converged"] == 1 and r1["scf_iters"] == r0["scf_iters"]
+    assert r0["F_evals"] == r0["scf_iters"] and 2 <= r1["F_evals"] <= 12 < r1["scf_iters"]
+    assert np.array_equal(n1, n0) and np.array_equal(F1, F0)
+    for k in ("F_total", "F0", "E_H", "E_xc", "E_ie", "K_e", "mu", "w_last", "dn_l2"):
+        assert r1[k] == r0[k], k
+    o = orc.Oracle(cfg, **kw); ro = o.scf_solve(cfg["pos"])
+    assert abs(r1["scf_iters"] - ro["scf_iters"]) <= 1
+    assert abs(r1["F_total"] - ro["F_total"]) < 1e-9 * abs(ro["F_total"])
+    # no convergence within scf_max_iter: the last iteration evaluates F all the same
+    monkeypatch.setenv("ARCHE_LAZY_F", "1")
+    g = _gpu(cfg, **dict(kw, scf_max_iter=9))
+    r9 = g.scf_solve(cfg["pos"])
+    assert r9["rc"] == -3 and r9["converged"] == 0 and r9["scf_iters"] == 9 and r9["F_evals"] < 9
+    g2 = _gpu(cfg, **dict(kw, scf_fixed_iter=9)); rf = g2.scf_solve(cfg["pos"])
+    assert rf["F_evals"] == 9 and r9["F_total"] == rf["F_total"] and r9["E_ie"] == rf["E_ie"]
+
+
 @pytest.mark.parametrize("name,grid", [("c1", None), ("streamed-128", (128, 32, 16))])
 def test_one_center_start_field_by_field(orc, torch_cuda, monkeypatch, name, grid):
     """P4 (Eq. 20, reading A10): after a first solve, ions are displaced and scf_begin builds n_i = clip/renormalise of the
