@@ -699,6 +699,9 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   const int fixed = c->p.scf_fixed_iter;
   const int maxit = fixed > 0 ? fixed : (c->p.scf_max_iter > 0 ? c->p.scf_max_iter : 200);
   bool conv = false;
+  // lazy free energy (ScfConst::lazy_F): under the stop rule F is evaluated only where the rule can use it.  Not with the
+  // printed PZ81 constants (the branch-flip detection of reading A13 watches F in every iteration), not in parity replays.
+  c->C.lazy_F = (fixed <= 0 && c->p.xc != 1 && c->lazy_F) ? maxit : 0;
   // L2-resident production grids: the whole solve in one cooperative launch (with per-class profiling on, block 0
   // times the phases with %globaltimer and the classes receive those times)
   if (c->persist) {
@@ -735,9 +738,6 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
   // kernels of the remaining iterations of the batch return at once, so the state stays that of the converged
   // iteration.  Parity replays (scf_fixed_iter) run every iteration.
   {
-  // lazy free energy (ScfConst::lazy_F): under the stop rule F is evaluated only where the rule can use it.  Not with the
-  // printed PZ81 constants (the branch-flip detection of reading A13 watches F in every iteration), not in parity replays.
-  c->C.lazy_F = (fixed <= 0 && c->p.xc != 1 && c->lazy_F) ? maxit : 0;
   const int batch = fixed > 0 ? maxit : kScfBatch;
   for (int it = 0; it < maxit && !conv;) {
     c->stop = fixed > 0 ? nullptr : &c->sc->converged;

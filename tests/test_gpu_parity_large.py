@@ -223,21 +223,25 @@ def test_isokinetic_md_trajectory_replayed(orc, torch_cuda, n_ions, grid):
     assert abs(r0["K_i"] - K0) > 1e-9 * K0
 
 
-@pytest.mark.parametrize("mode", ["fused", "streamed"])
+@pytest.mark.parametrize("mode", ["fused", "streamed", "persistent"])
 def test_lazy_free_energy_is_the_same_solve(orc, torch_cuda, monkeypatch, mode):
     """Under the stop rule the device evaluates the free-energy terms (I_3/2, eps_xc, E_ie) only where the rule can use
     them (ScfConst::lazy_F).  The iterates do not depend on F, so against the same solve with ARCHE_LAZY_F=0: the same
     iteration count, bit-identical density and forces, the same final F and energy terms -- with fewer evaluations; and
     against the oracle's own free stop: within one iteration, F to 1e-9.  A solve that hits scf_max_iter still ends
     with the free energy of its last iterate."""
-    monkeypatch.setenv("ARCHE_FUSE", "1" if mode == "fused" else "0")
-    monkeypatch.setenv("ARCHE_PERSIST", "0")
-    cfg = ai.make_small(n_ions=5, L=9.0, grid=(24, 16, 18), T_eV=15.0, seed=52)
+    if mode == "persistent":      # the whole solve in one cooperative launch (32^3: the c1 grid)
+        cfg = ai.make_small(n_ions=6, L=10.0, grid=(32, 32, 32), T_eV=15.0, seed=53)
+    else:
+        monkeypatch.setenv("ARCHE_FUSE", "1" if mode == "fused" else "0")
+        monkeypatch.setenv("ARCHE_PERSIST", "0")
+        cfg = ai.make_small(n_ions=5, L=9.0, grid=(24, 16, 18), T_eV=15.0, seed=52)
     kw = dict(xc=2, scf_tol_F=1e-10, scf_tol_dn=1e-9, scf_max_iter=400)
     res = {}
     for lazy in ("1", "0"):
         monkeypatch.setenv("ARCHE_LAZY_F", lazy)
         g = _gpu(cfg, **kw)
+        assert g.is_persistent() == (mode == "persistent")
         r = g.scf_solve(cfg["pos"])
         res[lazy] = (r, g.get_real("n_a").cpu().numpy(), g.forces().cpu().numpy())
     (r1, n1, F1), (r0, n0, F0) = res["1"], res["0"]
