@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  bool s5_rows;    // S5 reduction of the streamed form as a row walk (ARCHE_S5_ROWS=0: the generic grid-stride kernel)
   bool lazy_F;     // free energy only where the stop rule needs it (ARCHE_LAZY_F=0 disables); see ScfConst::lazy_F
   bool pdl;        // programmatic dependent launch between the kernels of an SCF iteration (ARCHE_PDL=0 disables)
   int r_blocks;    // resident blocks per SM of the streamed real-space Fermi-Dirac kernels
@@ -424,6 +425,7 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     // shared memory from the tail of the running one: on by default up to 8 M grid points
     { const char *e = getenv("ARCHE_PDL"); c->pdl = e ? e[0] != '0' : c->ng <= 8000000LL; }
     { const char *e = getenv("ARCHE_LAZY_F"); c->lazy_F = e ? e[0] != '0' : true; }
+    { const char *e = getenv("ARCHE_S5_ROWS"); c->s5_rows = e ? e[0] != '0' : true; }
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, kFdTabBytes));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
@@ -619,7 +621,17 @@ int scf_iteration(arche_ctx *c) {
     rc = fft3d_forward(c, LoadReal{c->n_a}, StoreScaled{c->nh_a, G.dV, c->nxh}, PC_FFT_FWD_X, PC_FFT_FWD_Z);
     if (rc) return rc;
     { ProfScope ps(c, PC_RED_G);
-      CK(launch_k(c, pointwise_g_kernel<LoadComplex, StoreNhatA>, pg, 256, 0, LoadComplex{c->nh_a}, sn, c->P, G.ny, c->nh, c->stop)); ++c->launches; }
+      const int nrows = G.ny * G.nz;
+      if (c->s5_rows && c->nxh <= 1024) {   // row walk: a thread keeps its kx column, four rows in flight
+        const int th = (c->nxh + 31) / 32 * 32 < 256 ? (c->nxh + 31) / 32 * 32 : 256;
+        int blocks = c->sm_count * (2048 / th > 8 ? 8 : 2048 / th);
+        if (blocks > nrows / 4) blocks = nrows / 4 > 0 ? nrows / 4 : 1;
+        const int rpb = (nrows + blocks - 1) / blocks;
+        blocks = (nrows + rpb - 1) / rpb;
+        CK(launch_k(c, s5_rows_kernel<4>, blocks, th, 0, sn, c->P, G.ny, nrows, rpb, c->stop)); ++c->launches;
+      } else {
+        CK(launch_k(c, pointwise_g_kernel<LoadComplex, StoreNhatA>, pg, 256, 0, LoadComplex{c->nh_a}, sn, c->P, G.ny, c->nh, c->stop)); ++c->launches;
+      } }
   }
   c->mix_pending = true;   // S6 is applied by the next iteration's S1/S2 passes, or by flush_mix()
   c->have_solution = true;

@@ -795,6 +795,52 @@ __global__ void __launch_bounds__(256) pointwise_g_kernel(LoadOp ld_in, StoreOp 
   st.finish(s_red);
 }
 
+// S5 reduction of the streamed form as a row walk (round 2).  ncu of pointwise_g_kernel<LoadComplex, StoreNhatA> at
+// 384^3: 3.4 TB/s where a plain reduction of the same bytes reaches 6.9 TB/s on this GPU -- one element per thread and
+// step, four 64-bit divisions per element to recover (ix, iy, iz), long_scoreboard 13 warps per issue.  Here a thread
+// keeps its column: kx^2 and the half-spectrum weight are registers, a block walks over a contiguous range of (ky, kz)
+// rows and carries (iy, iz) along, four rows -- eight or twelve 16-byte loads per thread -- are in flight at a time, and
+// the only per-element arithmetic left is the reciprocal of pi k^2.  Same sums, same closing step (StoreNhatA::finish).
+template <int ROWS>
+__global__ void __launch_bounds__(256) s5_rows_kernel(StoreNhatA st_in, int P, int ny, int nrows, int rows_per_block, const int *stop) {
+  __shared__ double s_red[kMaxRed * 33];
+  pdl_launch_dependents();
+  pdl_wait();
+  if (stop && *stop) return;
+  StoreNhatA st = st_in;
+  st.begin();
+  const int r0 = blockIdx.x * rows_per_block, r1 = min(nrows, r0 + rows_per_block);
+  for (int ix = threadIdx.x; ix < st.H.nxh; ix += blockDim.x) {
+    const double kx2 = st.kx2[ix], wt = st.H.wt(ix);
+    int iy = r0 % ny, iz = r0 / ny;
+    for (int r = r0; r < r1; r += ROWS) {
+      double2 v[ROWS], a[ROWS], b[ROWS];
+      double k2[ROWS];
+#pragma unroll
+      for (int q = 0; q < ROWS; ++q) {
+        const bool ok = r + q < r1;
+        const long long h = (long long)(ok ? r + q : r) * P + ix;
+        v[q] = st.nh_a[h]; a[q] = st.nh_i[h];
+        if (st.wantF) b[q] = st.vh_ie[h];
+        k2[q] = ok ? kx2 + st.ky2[iy] + st.kz2[iz] : 0.0;   // a row past the end counts like k = 0: nothing
+        if (!ok) { v[q] = make_double2(0.0, 0.0); b[q] = v[q]; }
+        if (++iy == ny) { iy = 0; ++iz; }
+      }
+#pragma unroll
+      for (int q = 0; q < ROWS; ++q) {
+        if (st.wantF) st.aEie += wt * (v[q].x * b[q].x + v[q].y * b[q].y);   // Re conj(nhat_a) Vhat_ie
+        if (k2[q] != 0.0) {
+          const double inv = wt * __drcp_rn(ARCHE_PI * k2[q]);
+          const double dr = a[q].x - v[q].x, di = a[q].y - v[q].y;
+          st.aU += (dr * dr + di * di) * inv;                              // Eq. 30
+          st.aEH += (v[q].x * v[q].x + v[q].y * v[q].y) * inv;             // Eq. 53
+        }
+      }
+    }
+  }
+  st.finish(s_red);
+}
+
 // real fields, two elements per thread and step (the functors interleave their two Fermi-Dirac evaluations); ng even.
 // SMEM_TAB: the block first copies the Fermi-Dirac table (g_tab) to shared memory and the functors read it there --
 // for the streamed form, launched with as many blocks as are co-resident (the table copy is paid once per block).
