@@ -33,7 +33,7 @@ TOL = dict(scf_tol_F=1e-10, scf_tol_dn=1e-8, scf_max_iter=2000, mix_warmup=3, mi
 # c4 (T = 1 eV, 61-bohr cell): the longest wave has lambda = chi0/(pi k_min^2) ~ 110, so the fixed w of the warm-up must
 # exceed (lambda-1)/(lambda+1): automatic w = lambda/(1+lambda), More's w once |mu_k - mu_{k-1}| < 1e-3 kT (1 - w) (reading A11b)
 TOL_BY_WORKLOAD = {"c4": dict(scf_max_iter=12000, mix_w_fixed=0.0, mix_mu_tol=1e-3)}
-NCU_TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_c5_384_ncu_full.csv")
+NCU_TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02b_c5_384_ncu_full.csv")
 
 
 XC_NAME = {1: "PZ81 LDA (constants as printed; eps_c, V_c jump 3e-5 Ha at r_s=1)",
@@ -91,7 +91,7 @@ def peaks():
 
 def ncu_traffic():
     """DRAM bytes per launch of each kernel class from the committed `ncu --set full` capture of this workload
-    (profiles/r02_c5_384_ncu_full.csv, written by paper_2606_13283_b200/ncu_summary.py): class -> bytes"""
+    (profiles/r02b_c5_384_ncu_full.csv, written by paper_2606_13283_b200/ncu_summary.py): class -> bytes"""
     out = {}
     try:
         with open(NCU_TRAFFIC_CSV) as fh:
@@ -531,7 +531,7 @@ def main():
         roof["hbm_classes_share_of_step"] = round(tot_t * 1e3 / tot_prof, 4)
         if roof.get("traffic") is not None:
             roof["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum per launch, parsed at run time from " \
-                                     "profiles/r02_c5_384_ncu_full.csv (ncu --set full capture of this command)"
+                                     "profiles/r02b_c5_384_ncu_full.csv (ncu --set full capture of this command)"
     roof["measured"] = ("second pass over the following steps with per-class timing: CUDA events on the library's stream "
                         "around every launch of the class")
     line = {"metric": "md_steps_per_s", "value": world * K / t_dev_max, "unit": "md_steps/s",

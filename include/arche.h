@@ -164,6 +164,35 @@ int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, double *d_scrat
  * contexts or processes' threads on the same device without ordering -- race on it.  Serialise them. */
 #define ARCHE_FFT3D_STATIC_MAX_POINTS (64 * 64 * 64)
 int arche_fft3d_static(arche_ctx *c, const double *d_in, double *d_out, int sign);
+/* f4 (grids beyond one GPU): the complex transform of arche_fft3d decomposed into slabs
+ * over n_ranks GPUs (one process per GPU, or several slabs on one GPU), unnormalised, same sign convention.
+ * Layouts: "z slab" of rank r = planes r Nz/R ... (r+1) Nz/R - 1 of the field, [Nz/R][Ny][Nx]; "y slab" of rank r = rows
+ * r Ny/R ... of every plane, [Nz][Ny/R][Nx].  sign = -1 maps z slabs (real space) to y slabs (reciprocal space,
+ * transposed output); sign = +1 maps y slabs back to z slabs.  Ny and Nz must be multiples of n_ranks <= 16.
+ * The transpose is not a separate exchange: the pass before it stores every element straight into the slab of the
+ * rank that owns it afterwards -- h_peer[q] is the DEVICE address, valid on the calling GPU, of rank q's destination
+ * slab (its y slab for sign = -1, its z slab for sign = +1): peer memory mapped over NVLink (arche_ipc_open, or
+ * cudaDeviceEnablePeerAccess within a process) or a local buffer.  h_peer itself is a HOST array of n_ranks pointers.
+ *   arche_fft3d_slab_scatter: sign = -1: x and y passes on the z slab d_in (d_scratch: 16 Nx Ny Nz/R bytes, device), the
+ *     y pass scattering into the peers' y slabs; sign = +1: z pass on the y slab d_in scattering into the peers' z slabs
+ *     (d_scratch unused, may be NULL).  d_in is not modified.
+ *   -- every rank's scatter must have completed (stream synchronise + a barrier across the ranks) --
+ *   arche_fft3d_slab_finish: sign = -1: z pass in place on this rank's y slab; sign = +1: y and x passes in place on this
+ *     rank's z slab.
+ * Both are stream-ordered on the context's stream and allocate nothing.  The context supplies the axis plans of the
+ * GLOBAL grid (its SCF arrays are not touched). */
+int arche_fft3d_slab_scatter(arche_ctx *c, const double *d_in, double *d_scratch, double *const *h_peer, int n_ranks,
+                             int rank, int sign);
+int arche_fft3d_slab_finish(arche_ctx *c, double *d_slab, int n_ranks, int sign);
+/* Slab buffers that another process can map: arche_slab_alloc is a plain cudaMalloc on the current device (an IPC
+ * handle names a whole allocation, so such buffers must not come from a caching allocator's pool); arche_ipc_export
+ * writes the 64-byte handle of such a buffer to HOST memory, arche_ipc_open maps a peer's buffer into this process
+ * (peer access enabled lazily) and returns its device address here, arche_ipc_close unmaps it. */
+int arche_slab_alloc(size_t bytes, void **d_out);
+int arche_slab_free(void *d_ptr);
+int arche_ipc_export(const void *d_ptr, unsigned char *h_handle64);
+int arche_ipc_open(const unsigned char *h_handle64, void **d_out);
+int arche_ipc_close(void *d_ptr);
 /* The transform pair the SCF itself uses: real field [Nz][Ny][Nx] <-> half spectrum, through the r2c / c2r x passes and
  * the y/z passes (register two-stage kernels for N in {32,64,128,192,256,384}, generic radix kernels otherwise).
  * forward: d_full_out receives the full unnormalised spectrum [Nz][Ny][Nx] complex (the stored half expanded by

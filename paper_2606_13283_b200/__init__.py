@@ -21,7 +21,9 @@ SYMBOLS = ["arche_workspace_bytes", "arche_scf_init", "arche_destroy", "arche_la
            "arche_md_step_host", "arche_get_real", "arche_get_complex", "arche_get_density", "arche_fft3d",
            "arche_rfft3d_forward", "arche_rfft3d_inverse",
            "arche_fermi_dirac", "arche_launch_count", "arche_profile_enable", "arche_profile_get", "arche_is_fused", "arche_is_persistent",
-           "arche_peak_fp64", "arche_peak_l2", "arche_set_scf_iterations", "arche_fft3d_static"]
+           "arche_peak_fp64", "arche_peak_l2", "arche_set_scf_iterations", "arche_fft3d_static",
+           "arche_fft3d_slab_scatter", "arche_fft3d_slab_finish", "arche_slab_alloc", "arche_slab_free",
+           "arche_ipc_export", "arche_ipc_open", "arche_ipc_close"]
 
 ERRORS = {-1: "ARCHE_EINVAL", -2: "ARCHE_ENOMEM", -3: "ARCHE_ENOCONV", -4: "ARCHE_ENAN", -5: "ARCHE_ECUDA"}
 
@@ -93,6 +95,13 @@ def load(rebuild_if_stale: bool = True):
     L.arche_peak_fp64.argtypes = [vp, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.arche_peak_l2.argtypes = [vp, C.POINTER(C.c_double)]
     L.arche_set_scf_iterations.argtypes = [vp, C.c_int, C.c_int]
+    L.arche_fft3d_slab_scatter.argtypes = [vp, vp, vp, C.POINTER(vp), C.c_int, C.c_int, C.c_int]
+    L.arche_fft3d_slab_finish.argtypes = [vp, vp, C.c_int, C.c_int]
+    L.arche_slab_alloc.argtypes = [C.c_size_t, C.POINTER(vp)]
+    L.arche_slab_free.argtypes = [vp]
+    L.arche_ipc_export.argtypes = [vp, C.c_char_p]
+    L.arche_ipc_open.argtypes = [C.c_char_p, C.POINTER(vp)]
+    L.arche_ipc_close.argtypes = [vp]
     _lib = L
     return L
 
@@ -264,6 +273,15 @@ class Arche:
             out = t.empty_like(a)
         self._check(self.lib.arche_fft3d_static(self._h, a.data_ptr(), out.data_ptr(), int(sign)))
         return out
+
+    def fft3d_slab_scatter(self, d_in, d_scratch, peers, rank: int, sign: int):
+        """arche_fft3d_slab_scatter: d_in / d_scratch / peers[q] are device addresses (int); see include/arche.h"""
+        arr = (C.c_void_p * len(peers))(*[int(p) for p in peers])
+        self._check(self.lib.arche_fft3d_slab_scatter(self._h, int(d_in), int(d_scratch) if d_scratch else None, arr,
+                                                      len(peers), int(rank), int(sign)))
+
+    def fft3d_slab_finish(self, d_slab, n_ranks: int, sign: int):
+        self._check(self.lib.arche_fft3d_slab_finish(self._h, int(d_slab), int(n_ranks), int(sign)))
 
     def rfft3d_forward(self, a):
         """real [nz,ny,nx] -> full unnormalised complex spectrum, through the SCF's own r2c passes"""

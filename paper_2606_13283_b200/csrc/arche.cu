@@ -974,6 +974,76 @@ extern "C" int arche_fft3d(arche_ctx *c, const double *d_in, double *d_out, doub
   return ARCHE_OK;
 }
 
+// f4: slab-decomposed complex transform (fft.cuh StoreSlabScatter).  Phase 1 runs the passes before the transpose, the
+// last of them storing into the peers' slabs; phase 2, after every rank's phase 1 has completed, the passes after it.
+extern "C" int arche_fft3d_slab_scatter(arche_ctx *c, const double *d_in, double *d_scratch, double *const *h_peer,
+                                        int n_ranks, int rank, int sign) {
+  if (!c || !d_in || !h_peer || (sign != 1 && sign != -1)) return ARCHE_EINVAL;
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  if (n_ranks < 1 || n_ranks > kSlabMaxRanks || rank < 0 || rank >= n_ranks || ny % n_ranks || nz % n_ranks)
+    return fail(c, ARCHE_EINVAL, "arche_fft3d_slab: Ny and Nz must be multiples of n_ranks <= 16");
+  const int nyl = ny / n_ranks, nzl = nz / n_ranks;
+  for (int a = 0; a < 3; ++a) c->plan[a].stop = nullptr;
+  StoreSlabScatter st;
+  for (int q = 0; q < kSlabMaxRanks; ++q) st.peer[q] = q < n_ranks ? (double2 *)h_peer[q] : nullptr;
+  for (int q = 0; q < n_ranks; ++q) if (!h_peer[q]) return ARCHE_EINVAL;
+  st.nx = nx;
+  const double2 *in = (const double2 *)d_in;
+  if (sign < 0) {   // z slab [nzl][ny][nx]: x pass, then the y pass that scatters into the y slabs [nz][nyl][nx]
+    if (!d_scratch) return ARCHE_EINVAL;
+    double2 *w = (double2 *)d_scratch;
+    st.nloc_dst = nyl; st.pitch_dst = nyl; st.off_src = rank * nzl; st.forward = 1;
+    CK((fft_launch_pass<0, false>(c->plan[0], nx, ny, nzl, LoadComplex{in}, StoreComplex{w}, c->stream))); ++c->launches;
+    CK((fft_launch_pass<1, false>(c->plan[1], nx, ny, nzl, LoadComplex{w}, st, c->stream))); ++c->launches;
+  } else {          // y slab [nz][nyl][nx]: the z pass scatters into the z slabs [nzl][ny][nx]
+    st.nloc_dst = nzl; st.pitch_dst = ny; st.off_src = rank * nyl; st.forward = 0;
+    CK((fft_launch_pass<2, true>(c->plan[2], nx, nyl, nz, LoadComplex{in}, st, c->stream))); ++c->launches;
+  }
+  return ARCHE_OK;
+}
+
+extern "C" int arche_fft3d_slab_finish(arche_ctx *c, double *d_slab, int n_ranks, int sign) {
+  if (!c || !d_slab || (sign != 1 && sign != -1)) return ARCHE_EINVAL;
+  const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz;
+  if (n_ranks < 1 || n_ranks > kSlabMaxRanks || ny % n_ranks || nz % n_ranks)
+    return fail(c, ARCHE_EINVAL, "arche_fft3d_slab: Ny and Nz must be multiples of n_ranks <= 16");
+  for (int a = 0; a < 3; ++a) c->plan[a].stop = nullptr;
+  double2 *s = (double2 *)d_slab;
+  if (sign < 0) {   // y slab: z pass in place
+    CK((fft_launch_pass<2, false>(c->plan[2], nx, ny / n_ranks, nz, LoadComplex{s}, StoreComplex{s}, c->stream))); ++c->launches;
+  } else {          // z slab: y and x passes in place
+    CK((fft_launch_pass<1, true>(c->plan[1], nx, ny, nz / n_ranks, LoadComplex{s}, StoreComplex{s}, c->stream))); ++c->launches;
+    CK((fft_launch_pass<0, true>(c->plan[0], nx, ny, nz / n_ranks, LoadComplex{s}, StoreComplex{s}, c->stream))); ++c->launches;
+  }
+  return ARCHE_OK;
+}
+
+// slab buffers that other processes can map: plain cudaMalloc allocations (an IPC handle names a whole allocation,
+// so these do not come out of a caching allocator's pool)
+extern "C" int arche_slab_alloc(size_t bytes, void **d_out) {
+  if (!d_out || bytes == 0) return ARCHE_EINVAL;
+  *d_out = nullptr;
+  return cudaMalloc(d_out, bytes) == cudaSuccess ? ARCHE_OK : ARCHE_ENOMEM;
+}
+extern "C" int arche_slab_free(void *d_ptr) { return cudaFree(d_ptr) == cudaSuccess ? ARCHE_OK : ARCHE_ECUDA; }
+extern "C" int arche_ipc_export(const void *d_ptr, unsigned char *h_handle64) {
+  if (!d_ptr || !h_handle64) return ARCHE_EINVAL;
+  cudaIpcMemHandle_t h;
+  static_assert(sizeof(h) == 64, "cudaIpcMemHandle_t is 64 bytes");
+  if (cudaIpcGetMemHandle(&h, const_cast<void *>(d_ptr)) != cudaSuccess) { (void)cudaGetLastError(); return ARCHE_ECUDA; }
+  memcpy(h_handle64, &h, 64);
+  return ARCHE_OK;
+}
+extern "C" int arche_ipc_open(const unsigned char *h_handle64, void **d_out) {
+  if (!h_handle64 || !d_out) return ARCHE_EINVAL;
+  cudaIpcMemHandle_t h;
+  memcpy(&h, h_handle64, 64);
+  *d_out = nullptr;
+  if (cudaIpcOpenMemHandle(d_out, h, cudaIpcMemLazyEnablePeerAccess) != cudaSuccess) { (void)cudaGetLastError(); return ARCHE_ECUDA; }
+  return ARCHE_OK;
+}
+extern "C" int arche_ipc_close(void *d_ptr) { return cudaIpcCloseMemHandle(d_ptr) == cudaSuccess ? ARCHE_OK : ARCHE_ECUDA; }
+
 // arche_fft3d without caller scratch and without any allocation: the intermediate passes go through the file-scope
 // device array (see its declaration above).  Nothing in it has to start at zero: the first pass writes all Nx*Ny*Nz
 // elements before any later pass reads them.  All calls on a device share the array.

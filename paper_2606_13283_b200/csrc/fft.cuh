@@ -138,6 +138,34 @@ struct StoreComplex {
   __device__ __forceinline__ void finish(double *) {}
 };
 
+// f4: slab-decomposed transform over several GPUs.  The pass that precedes the transpose stores every
+// element straight into the slab of the rank that owns it after the transpose -- peer memory mapped over NVLink (or,
+// with one rank, the local buffer): the all-to-all is the store phase of the pass, there is no pack/exchange/unpack.
+// Forward: the y pass of rank r, working on its z slab [nzl][ny][nx], writes (ix, iy, izl) to rank q = iy / nyl at
+// [(r nzl + izl)][iy - q nyl][ix] of that rank's y slab [nz][nyl][nx].  Inverse: the z pass of rank r, working on its y
+// slab, writes (ix, iyl, iz) to rank q = iz / nzl at [iz - q nzl][r nyl + iyl][ix] of that rank's z slab.
+constexpr int kSlabMaxRanks = 16;
+struct StoreSlabScatter {
+  static constexpr bool kSplitStore = false;
+  double2 *peer[kSlabMaxRanks];
+  int nx, nloc_dst;     // row length; slab thickness of the destination layout (nyl forward, nzl inverse)
+  int pitch_dst;        // middle extent of the destination layout (nyl forward, ny inverse)
+  int off_src;          // this rank's offset along the axis it owned before the transpose (r nzl forward, r nyl inverse)
+  int forward;
+  __device__ __forceinline__ void begin() {}
+  __device__ __forceinline__ void prefetch(long long) const {}
+  __device__ __forceinline__ void store(long long, int ix, int iy, int iz, double re, double im) {
+    if (forward) {
+      const int q = iy / nloc_dst;
+      peer[q][((long long)(off_src + iz) * pitch_dst + (iy - q * nloc_dst)) * nx + ix] = make_double2(re, im);
+    } else {
+      const int q = iz / nloc_dst;
+      peer[q][((long long)(iz - q * nloc_dst) * pitch_dst + (off_src + iy)) * nx + ix] = make_double2(re, im);
+    }
+  }
+  __device__ __forceinline__ void finish(double *) {}
+};
+
 template <int AXIS, bool INVERSE, class LoadOp, class StoreOp>
 __global__ void __launch_bounds__(kFftThreads) fft_pass_kernel(FftPass P, LoadOp ld_in, StoreOp st_in) {
   extern __shared__ double smem[];

@@ -17,6 +17,7 @@ import sys
 CLASSES = [
     (r"pointwise_g_kernel<.*LoadPotentialG", "potential_g"),
     (r"pointwise_g_kernel<.*StoreNhatA", "reduce_g"),
+    (r"s5_rows_kernel", "reduce_g"),
     (r"pointwise_r_kernel<.*StoreVi", "vi_r"),
     (r"pointwise_r_kernel<.*LoadDensity", "density_r"),
     (r"mu_solve_kernel", "mu_pass"),
@@ -27,6 +28,7 @@ CLASSES = [
     (r"fft_r2c\w*kernel", "fft_fwd_x_real"),
     (r"structure_factor", "structure_factor"),
     (r"force_kernel", "force"),
+    (r"force_cols_kernel|force_w_kernel", "force"),
     (r"stress_fields_kernel", "stress_fields"),
     (r"scf_persistent_kernel", "scf_persistent"),
 ]
