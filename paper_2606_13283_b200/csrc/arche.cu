@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  bool sf_tma;     // structure factor: register tile fed by the copy engine (ARCHE_SF_TMA=0: global loads of a_j)
   bool s5_rows;    // S5 reduction of the streamed form as a row walk (ARCHE_S5_ROWS=0: the generic grid-stride kernel)
   bool lazy_F;     // free energy only where the stop rule needs it (ARCHE_LAZY_F=0 disables); see ScfConst::lazy_F
   bool pdl;        // programmatic dependent launch between the kernels of an SCF iteration (ARCHE_PDL=0 disables)
@@ -426,6 +427,7 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     { const char *e = getenv("ARCHE_PDL"); c->pdl = e ? e[0] != '0' : c->ng <= 8000000LL; }
     { const char *e = getenv("ARCHE_LAZY_F"); c->lazy_F = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_S5_ROWS"); c->s5_rows = e ? e[0] != '0' : true; }
+    { const char *e = getenv("ARCHE_SF_TMA"); c->sf_tma = e ? e[0] != '0' : true; }
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, kFdTabBytes));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
@@ -655,7 +657,19 @@ int scf_begin(arche_ctx *c, const double *d_pos) {
     const int nxm = G.nx / 2;
     const int ixt = (G.nx % 2 == 0 && ni >= 256) ? (nxm % 128 == 0 ? 4 : (nxm % 96 == 0 ? 3 : (nxm % 64 == 0 ? 2 : 0))) : 0;
     int own_nyq_x = 0;
-    if (ixt) {
+    const int txb_t = ixt ? nxm / ixt : 0, rg_t = txb_t ? 128 / txb_t : 0;
+    const bool tma_ok = c->sf_tma && ixt && txb_t * rg_t == 128 &&
+                        ((ixt == 3 && rg_t == 2) || (ixt == 4 && rg_t == 4) || (ixt == 3 && rg_t == 4) || (ixt == 2 && rg_t == 4));
+    if (tma_ok) {   // register tile fed by the copy engine (structure_factor_tma_kernel)
+      const unsigned blocks = (unsigned)(((long long)G.ny * G.nz + SF2_ROWS * rg_t - 1) / (SF2_ROWS * rg_t));
+      const size_t smem = ((size_t)SF3_NST * SF3_JT * nxm + 2 * (size_t)SF2_ROWS * rg_t * SF3_JT) * sizeof(double2);
+#define ARCHE_SFT(I, R) { auto kern = structure_factor_tma_kernel<I, R>; \
+        CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        kern<<<blocks, 128, smem, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc); }
+      if (ixt == 3 && rg_t == 2) ARCHE_SFT(3, 2) else if (ixt == 4) ARCHE_SFT(4, 4) else if (ixt == 3) ARCHE_SFT(3, 4) else ARCHE_SFT(2, 4)
+#undef ARCHE_SFT
+      own_nyq_x = 1;
+    } else if (ixt) {
       const unsigned blocks = (unsigned)(((long long)G.ny * G.nz + SF2_ROWS - 1) / SF2_ROWS);
       const int txb = nxm / ixt;
       if (ixt == 4) structure_factor_tiled_kernel<4><<<blocks, txb, 0, c->stream>>>(G, ni, c->Z, c->ax_ji, c->by_ij, c->cz_ij, c->vps, c->va, c->S, c->S2, c->vh_ie, c->partials, c->counter, c->sc);

@@ -42,6 +42,9 @@ __device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned arri
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(arrivals) : "memory");
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // make the initialised barrier visible to the copy engine
 }
+// orders this thread's earlier generic-proxy writes to shared memory before later writes of the copy engine (async
+// proxy) to the same addresses: call it after clearing a buffer that bulk copies will fill, before the block barrier
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long *bar, unsigned bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr_u32(bar)), "r"(bytes) : "memory");
 }

@@ -225,6 +225,129 @@ __global__ void __launch_bounds__(256) structure_factor_tiled_kernel(
   if (grid_reduce<1>(v, op, partials, counter, s_red) && threadIdx.x == 0) sc->U_pm_sum = s_red[32];
 }
 
+// The same register tile fed by the copy engine (round 2).  ncu of the kernel above at 384^3 / 2000 ions: fp64 pipe 51%
+// busy, long_scoreboard 4.3 warps per issue at the first DFMA that uses a_j(kx) -- the global loads of a_j are exposed,
+// and a register prefetch only moves the stall (ptxas sinks the loads).  Here the a_j(kx) rows of
+// SF3_JT ions at a time (one contiguous run of nx/2 complex numbers per ion) come into shared memory by cp.async.bulk
+// completing on an mbarrier, two stages in flight, issued by one thread; d_j = Z_j b_j c_j of the next stage is fetched
+// into registers before the current stage is consumed and written to the other half of a double buffer after it.  A
+// block owns 8 RG rows (RG row groups share every a_j word).  Same outputs and the same closing reduction.
+constexpr int SF3_JT = 8;
+constexpr int SF3_NST = 2;
+template <int IXT, int RG>
+__global__ void __launch_bounds__(128, IXT * RG >= 12 ? 2 : 3) structure_factor_tma_kernel(
+    GridGeom G, int nions, const double *__restrict__ Z, const double2 *__restrict__ ax_ji /*[j][ix]*/,
+    const double2 *__restrict__ by_ij /*[iy][j]*/, const double2 *__restrict__ cz_ij /*[iz][j]*/,
+    const double *__restrict__ vps, const double *__restrict__ va, double2 *__restrict__ S, double2 *__restrict__ S2,
+    double2 *__restrict__ vh_ie, double *partials, unsigned int *counter, DevScalars *sc) {
+  constexpr int ROWS = SF2_ROWS * RG, DE = ROWS * SF3_JT;   // rows per block; d_j elements per stage
+  extern __shared__ __align__(16) double2 s_dyn[];
+  __shared__ double s_red[32 + 1 + 1];
+  __shared__ unsigned long long s_bar[SF3_NST];
+  const int txb = blockDim.x / RG, nxm = IXT * txb;          // nxm = nx/2 columns
+  double2 *s_a = s_dyn;                                      // [SF3_NST][SF3_JT][nxm]
+  double2 *s_d = s_dyn + (size_t)SF3_NST * SF3_JT * nxm;     // [2][ROWS][SF3_JT]
+  const int tid = threadIdx.x, tx = tid % txb, ty = tid / txb;
+  const long long nrows = (long long)G.ny * G.nz, row0 = (long long)blockIdx.x * ROWS;
+  const int nstages = (nions + SF3_JT - 1) / SF3_JT;
+  for (int e = tid; e < SF3_NST * SF3_JT * nxm; e += blockDim.x) s_a[e] = make_double2(0.0, 0.0);
+  fence_proxy_async();
+  if (tid == 0)
+    for (int q = 0; q < SF3_NST; ++q) mbar_init(&s_bar[q], 1);
+  __syncthreads();
+  auto issue = [&](int st) {   // thread 0: rows a_j(0 .. nx/2 - 1) of the ions of stage st
+    const int q = st % SF3_NST, j0 = st * SF3_JT, nj = min(SF3_JT, nions - j0);
+    mbar_arrive_expect_tx(&s_bar[q], (unsigned)(nj * nxm * sizeof(double2)));
+    for (int jj = 0; jj < nj; ++jj)
+      bulk_copy_g2s(s_a + ((size_t)q * SF3_JT + jj) * nxm, ax_ji + (long long)(j0 + jj) * G.nx, (unsigned)(nxm * sizeof(double2)), &s_bar[q]);
+  };
+  if (tid == 0)
+    for (int st = 0; st < SF3_NST && st < nstages; ++st) issue(st);
+  // the d_j elements this thread stages: element e = (row r, ion slot jj); its (iy, iz) never change
+  constexpr int DPT = (DE + 127) / 128;
+  int d_iy[DPT], d_iz[DPT];
+  bool d_ok[DPT];
+#pragma unroll
+  for (int k = 0; k < DPT; ++k) {
+    const int e = tid + k * 128, r = e / SF3_JT;
+    const long long row = row0 + r;
+    d_ok[k] = e < DE && row < nrows;
+    d_iy[k] = d_ok[k] ? (int)(row % G.ny) : 0; d_iz[k] = d_ok[k] ? (int)(row / G.ny) : 0;
+  }
+  double2 fb[DPT], fc[DPT]; double fz[DPT];
+  auto fetch = [&](int st) {
+#pragma unroll
+    for (int k = 0; k < DPT; ++k) {
+      const int j = st * SF3_JT + (tid + k * 128) % SF3_JT;
+      fz[k] = 0.0;
+      if (d_ok[k] && j < nions) { fb[k] = by_ij[(long long)d_iy[k] * nions + j]; fc[k] = cz_ij[(long long)d_iz[k] * nions + j]; fz[k] = Z[j]; }
+    }
+  };
+  auto stash = [&](int dbuf) {
+#pragma unroll
+    for (int k = 0; k < DPT; ++k) {
+      const int e = tid + k * 128;
+      if (e < DE) {
+        double2 d = make_double2(0.0, 0.0);
+        if (fz[k] != 0.0) d = make_double2(fz[k] * (fb[k].x * fc[k].x - fb[k].y * fc[k].y), fz[k] * (fb[k].x * fc[k].y + fb[k].y * fc[k].x));
+        s_d[(size_t)dbuf * DE + e] = d;
+      }
+    }
+  };
+  double2 acc[IXT][SF2_ROWS];
+#pragma unroll
+  for (int q = 0; q < IXT; ++q)
+#pragma unroll
+    for (int r = 0; r < SF2_ROWS; ++r) acc[q][r] = make_double2(0.0, 0.0);
+  fetch(0); stash(0);
+  __syncthreads();
+  for (int st = 0; st < nstages; ++st) {
+    const int buf = st % SF3_NST, dbuf = st & 1;
+    if (st + 1 < nstages) fetch(st + 1);
+    mbar_wait(&s_bar[buf], (unsigned)((st / SF3_NST) & 1));
+    const double2 *pa = s_a + (size_t)buf * SF3_JT * nxm + tx;
+    const double2 *pd = s_d + (size_t)dbuf * DE + (size_t)ty * SF2_ROWS * SF3_JT;
+#pragma unroll 2
+    for (int jj = 0; jj < SF3_JT; ++jj) {
+      double2 a[IXT];
+#pragma unroll
+      for (int q = 0; q < IXT; ++q) a[q] = pa[jj * nxm + q * txb];
+#pragma unroll
+      for (int r = 0; r < SF2_ROWS; ++r) {
+        const double2 d = pd[r * SF3_JT + jj];
+#pragma unroll
+        for (int q = 0; q < IXT; ++q) {
+          acc[q][r].x = fma(a[q].x, d.x, fma(-a[q].y, d.y, acc[q][r].x));
+          acc[q][r].y = fma(a[q].x, d.y, fma(a[q].y, d.x, acc[q][r].y));
+        }
+      }
+    }
+    if (st + 1 < nstages) stash(dbuf ^ 1);
+    __syncthreads();                                   // every warp is done with this stage's a_j rows and d_j
+    if (tid == 0 && st + SF3_NST < nstages) issue(st + SF3_NST);
+  }
+  double epm = 0.0;
+#pragma unroll
+  for (int q = 0; q < IXT; ++q) {
+    const int ix = tx + q * txb;
+    const double wt = ix == 0 ? 1.0 : 2.0;
+#pragma unroll
+    for (int r = 0; r < SF2_ROWS; ++r) {
+      const long long row = row0 + ty * SF2_ROWS + r;
+      if (row < nrows) {
+        const long long g = row * G.P + ix;
+        S[g] = acc[q][r]; S2[g] = acc[q][r];
+        const double v = vps[g];
+        vh_ie[g] = make_double2(v * acc[q][r].x, v * acc[q][r].y);
+        epm += wt * va[g] * (acc[q][r].x * acc[q][r].x + acc[q][r].y * acc[q][r].y);
+      }
+    }
+  }
+  double v[1] = {epm};
+  const int op[1] = {0};
+  if (grid_reduce<1>(v, op, partials, counter, s_red) && threadIdx.x == 0) sc->U_pm_sum = s_red[32];
+}
+
 // Nyquist planes (reading A6).  With the literal index set of P:142 a Nyquist component is +N/2, whose mirror -N/2 is
 // not on the grid, so S_Z is not Hermitian there.  For every stored point with a Nyquist component this kernel forms
 // S2 = S_Z(k''), k'' = k with every Nyquist component flipped to -N/2 (phase-table entries conjugated), and
@@ -543,6 +666,7 @@ __global__ void __launch_bounds__(FCC_THREADS, CH > 25 ? 2 : 3) force_cols_kerne
   const int ncol = min(CH, G.P - c0);                        // columns of this chunk that exist in the arrays
   const unsigned stage_bytes = (unsigned)(FCC_GR * ncol * sizeof(double2) + FCC_GR * (sizeof(int4) + sizeof(double2)));
   for (int e = tid; e < FCC_NST * FCC_GR * CH; e += FCC_THREADS) (&s_w[0][0][0])[e] = make_double2(0.0, 0.0);
+  fence_proxy_async();
   if (tid == 0)
     for (int q = 0; q < FCC_NST; ++q) mbar_init(&s_bar[q], 1);
   __syncthreads();

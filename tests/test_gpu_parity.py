@@ -101,12 +101,19 @@ def test_structure_factor_and_ionic_potential(orc, torch_cuda):
         assert _rel(g.get_complex(name).cpu().numpy(), o.get_complex(name)) < 1e-12
 
 
-@pytest.mark.parametrize("grid", [(128, 16, 8), (192, 8, 8), (256, 8, 12), (384, 12, 8)])
-def test_structure_factor_register_tiled(orc, torch_cuda, grid):
-    """the register-tiled structure-factor kernel (2, 3 or 4 kx columns x 8 rows per thread, column kx = nx/2 left to
-    the Nyquist-plane kernel) on long-x cells with 256 ions: S_Z, V_ie and the Ewald energy against the oracle"""
-    cfg = ai.make_small(n_ions=256, grid=grid, cell=[40.0, 8.0, 8.0], seed=31, dmin=0.8)
-    cfg["Z"] = np.full(256, 0.25)                      # weak ions: a dense cell the oracle's quadrature handles quickly
+@pytest.mark.parametrize("feed", ["copy-engine", "global-loads"])
+@pytest.mark.parametrize("grid,n_ions", [((128, 16, 8), 256), ((192, 8, 8), 256), ((256, 8, 12), 256), ((384, 12, 8), 256),
+                                         ((384, 9, 6), 261)])
+def test_structure_factor_register_tiled(orc, torch_cuda, monkeypatch, grid, n_ions, feed):
+    """the register-tiled structure-factor kernels (2, 3 or 4 kx columns x 8 rows per thread, column kx = nx/2 left to
+    the Nyquist-plane kernel) on long-x cells with 256 ions: S_Z, V_ie and the Ewald energy against the oracle.
+    "copy-engine": structure_factor_tma_kernel (a_j rows by cp.async.bulk, every (columns, row groups) instantiation; the
+    last case has an ion count that is no multiple of the stage and a row count that is no multiple of the block's rows);
+    "global-loads": structure_factor_tiled_kernel (ARCHE_SF_TMA=0)."""
+    if feed == "global-loads":
+        monkeypatch.setenv("ARCHE_SF_TMA", "0")
+    cfg = ai.make_small(n_ions=n_ions, grid=grid, cell=[40.0, 8.0, 8.0], seed=31, dmin=0.8)
+    cfg["Z"] = np.full(n_ions, 0.25)                   # weak ions: a dense cell the oracle's quadrature handles quickly
     g = _gpu(cfg); o = orc.Oracle(cfg)
     g.scf_begin(cfg["pos"]); o.scf_begin(cfg["pos"])
     for name in ("S_Z", "Vhat_ie"):
