@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  bool r2c_tma;    // plain r2c x pass fed by the copy engine (ARCHE_R2C_TMA)
   bool sf_tma;     // structure factor: register tile fed by the copy engine (ARCHE_SF_TMA=0: global loads of a_j)
   bool s5_rows;    // S5 reduction of the streamed form as a row walk (ARCHE_S5_ROWS=0: the generic grid-stride kernel)
   bool lazy_F;     // free energy only where the stop rule needs it (ARCHE_LAZY_F=0 disables); see ScfConst::lazy_F
@@ -428,6 +429,7 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     { const char *e = getenv("ARCHE_LAZY_F"); c->lazy_F = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_S5_ROWS"); c->s5_rows = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_SF_TMA"); c->sf_tma = e ? e[0] != '0' : true; }
+    { const char *e = getenv("ARCHE_R2C_TMA"); c->r2c_tma = e ? e[0] != '0' : false; }
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, kFdTabBytes));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
@@ -497,7 +499,7 @@ cudaError_t pass_yz(arche_ctx *c, LoadOp ld, StoreOp st) {
 template <bool INVERSE, class LoadOp, class StoreOp>
 cudaError_t pass_x(arche_ctx *c, LoadOp ld, StoreOp st) {
   const int nx = c->G.nx, ny = c->G.ny, nz = c->G.nz, P = c->P;
-  FastGeom fg{nx, ny, nz, P, c->tw[0], c->stop, c->pdl ? 1 : 0};
+  FastGeom fg{nx, ny, nz, P, c->tw[0], c->stop, c->pdl ? 1 : 0, c->r2c_tma ? 1 : 0};
   // plain passes of the streamed form run the light configuration (LoadReal / StoreRealPlain / LoadComplex / StoreComplex)
   constexpr bool plain = (std::is_same<LoadOp, LoadReal>::value || std::is_same<LoadOp, LoadComplex>::value) &&
                          (std::is_same<StoreOp, StoreComplex>::value || std::is_same<StoreOp, StoreRealPlain>::value);

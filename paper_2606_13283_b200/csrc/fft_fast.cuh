@@ -117,11 +117,13 @@ template <> struct FastPlan<192> { static constexpr bool ok = true; static const
 template <> struct FastPlan<256> { static constexpr bool ok = true; static constexpr int R1 = 16, R2 = 16; };
 template <> struct FastPlan<384> { static constexpr bool ok = true; static constexpr int R1 = 16, R2 = 24; };
 
+struct LoadReal;   // scf_kernels.cuh: plain real input (the one load functor the copy-engine r2c pass replaces)
 struct FastGeom {
   int nx, ny, nz, P;        // real grid and half-spectrum pitch
   const double2 *tw;        // exp(-2 pi i a/N) of the transformed axis
   const int *stop;          // optional device flag: non-zero skips the pass
   int pdl;                  // host side: launch with programmatic stream serialization (common.cuh)
+  int tma;                  // host side: plain r2c x pass with its input through the copy engine (fft_r2c_tma_kernel)
 };
 
 // kernel launch with optional programmatic dependent launch
@@ -454,6 +456,75 @@ __global__ void __launch_bounds__(reg_threads_x<N>(), reg_blocks_r2c<N>()) fft_r
   st.finish(smem_raw);
 }
 
+// The same pass with its input brought in by the copy engine (plain real input only).  ncu of fft_r2c_reg_kernel<384>:
+// long_scoreboard 8.3 warps per issue, 17% warps, 0.67 of the HBM peak -- 3072 eight-byte loads per block have to be issued
+// by 96 threads before the first butterfly can start.  The 2 LP real lines of a block are ONE contiguous run
+// (2 LP N doubles): a single cp.async.bulk completing on an mbarrier brings it into shared memory, stage 1 reads its
+// operands from there (LDS.64, conflict-free), the rest is the kernel above.
+template <int N, class StoreOp>
+__global__ void __launch_bounds__(reg_threads_x<N>(), reg_blocks_r2c<N>()) fft_r2c_tma_kernel(FastGeom G, const double *__restrict__ src, StoreOp st_in) {
+  constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, ROW = fast_row_x<N>(), LP = kFastLPLight;
+  static_assert(R2 % 2 == 0, "the Hermitian exchange splits stage-2 outputs at q = R2/2");
+  extern __shared__ double smem_raw[];
+  double2 *buf = reinterpret_cast<double2 *>(smem_raw);   // [LP][ROW]
+  double *s_in = smem_raw + 2 * LP * ROW;                  // [2 LP][N]
+  __shared__ unsigned long long s_bar;
+  StoreOp st = st_in;
+  pdl_launch_dependents();
+  const int t = threadIdx.x;
+  const long long line0 = (long long)blockIdx.x * (2 * LP);
+  if (t == 0) mbar_init(&s_bar, 1);
+  pdl_wait();
+  if (G.stop && *G.stop) return;
+  if (t == 0) {
+    mbar_arrive_expect_tx(&s_bar, (unsigned)(2 * LP * N * sizeof(double)));
+    bulk_copy_g2s(s_in, src + line0 * N, (unsigned)(2 * LP * N * sizeof(double)), &s_bar);
+  }
+  st.begin();
+  __syncthreads();   // the barrier is initialised
+  mbar_wait(&s_bar, 0);
+  if (t < LP * R2) {   // stage 1: shared -> registers -> shared
+    const int p = t / R2, j1 = t % R2;
+    const double *la = s_in + (2 * p) * N, *lb = la + N;
+    double2 v[R1];
+#pragma unroll
+    for (int q = 0; q < R1; ++q) v[q] = make_double2(la[j1 + q * R2], lb[j1 + q * R2]);
+    Dft<R1>::run(v);
+#pragma unroll
+    for (int q = 0; q < R1; ++q) buf[p * ROW + j1 * (R1 + 1) + q] = v[q];
+  }
+  __syncthreads();
+  const bool act = t < LP * R1;
+  const int p = t / R1, j2 = t % R1;
+  double2 v[R2];
+  if (act) {           // stage 2: shared -> registers; v[q] = z[j2 + q R1]
+#pragma unroll
+    for (int q = 0; q < R2; ++q) v[q] = buf[p * ROW + j2 + q * (R1 + 1)];
+#pragma unroll
+    for (int q = 1; q < R2; ++q) v[q] = cmul(v[q], G.tw[q * j2]);
+    Dft<R2>::run(v);
+  }
+  __syncthreads();
+  if (act) {           // upper half of the spectrum (k >= N/2) to shared memory, natural order
+#pragma unroll
+    for (int q = R2 / 2; q < R2; ++q) buf[p * ROW + j2 + q * R1] = v[q];
+  }
+  __syncthreads();
+  if (act) {           // k <= N/2 takes its partner z[N-k] and stores A[k], B[k] straight from registers
+    const long long la = line0 + 2 * p, lb = la + 1;
+    const int iya = (int)(la % G.ny), iza = (int)(la / G.ny), iyb = (int)(lb % G.ny), izb = (int)(lb / G.ny);
+#pragma unroll
+    for (int q = 0; q <= R2 / 2; ++q) {
+      if (q == R2 / 2 && j2 != 0) break;          // k = N/2 belongs to j2 = 0 only
+      const int k = j2 + q * R1;
+      const double2 z = v[q], m = k == 0 ? v[0] : buf[p * ROW + (N - k)];
+      st.store(la * G.P + k, k, iya, iza, 0.5 * (z.x + m.x), 0.5 * (z.y - m.y));
+      st.store(lb * G.P + k, k, iyb, izb, 0.5 * (z.y + m.y), -0.5 * (z.x - m.x));
+    }
+  }
+  st.finish(smem_raw);
+}
+
 template <int N, class LoadOp, class StoreOp>
 __global__ void __launch_bounds__(reg_threads_x<N>(), reg_blocks_x<N>()) fft_c2r_reg_kernel(FastGeom G, LoadOp ld_in, StoreOp st_in) {
   constexpr int R1 = FastPlan<N>::R1, R2 = FastPlan<N>::R2, ROW = fast_row_x<N>(), LP = kFastLPLight;
@@ -560,6 +631,21 @@ static inline cudaError_t fft_launch_x_fast_n(const FastGeom &G, LoadOp ld, Stor
   cudaGetDevice(&dev);
   const bool attr_set = attr_dev == dev;
   const void *kern;
+  if constexpr (!INVERSE && LIGHT && std::is_same<LoadOp, LoadReal>::value) {
+    if (G.tma) {   // input through the copy engine
+      auto tk = fft_r2c_tma_kernel<N, StoreOp>;
+      const size_t tsmem = sizeof(double2) * LP * fast_row_x<N>() + sizeof(double) * 2 * LP * N;
+      static int tattr_dev = -1;
+      if (tattr_dev != dev) {
+        cudaError_t e = cudaFuncSetAttribute(tk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tsmem);
+        if (e != cudaSuccess) return e;
+        tattr_dev = dev;
+      }
+      const double *srcp = ld.src;
+      void *targs[] = {(void *)&G, (void *)&srcp, (void *)&st};
+      return launch_maybe_pdl((const void *)tk, dim3(blocks), dim3(TH), targs, tsmem, stream, G.pdl != 0);
+    }
+  }
   if constexpr (INVERSE) {
     if constexpr (LIGHT) kern = (const void *)fft_c2r_reg_kernel<N, LoadOp, StoreOp>;
     else kern = (const void *)fft_c2r_fast_kernel<N, false, LoadOp, StoreOp>;
