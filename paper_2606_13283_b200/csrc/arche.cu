@@ -429,7 +429,9 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     { const char *e = getenv("ARCHE_LAZY_F"); c->lazy_F = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_S5_ROWS"); c->s5_rows = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_SF_TMA"); c->sf_tma = e ? e[0] != '0' : true; }
-    { const char *e = getenv("ARCHE_R2C_TMA"); c->r2c_tma = e ? e[0] != '0' : false; }
+    // measured: 384^3 210 -> 172 us (0.67 -> 0.82 of the HBM peak); 256^3 49.5 -> 52.9 us, 192^3 27.5 -> 29.0 us (the register
+    // kernel is already at 0.87 there and the extra 2 LP N doubles of shared memory cost a resident block)
+    { const char *e = getenv("ARCHE_R2C_TMA"); c->r2c_tma = e ? e[0] != '0' : p->grid[0] >= 384; }
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mu_solve_kernel, 256, kFdTabBytes));
     // one block per SM while the grid fits the per-thread register cache (cheapest grid barrier), else all co-resident blocks
     if (per_sm < 1) return fail(c, ARCHE_ECUDA, "cooperative kernel cannot be resident");
