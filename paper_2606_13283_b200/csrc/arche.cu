@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  bool mu_split;   // first evaluation of the mu iteration as an ordinary launch (mu_first_eval_kernel; ARCHE_MU_SPLIT=0: off)
   bool r2c_tma;    // plain r2c x pass fed by the copy engine (ARCHE_R2C_TMA)
   bool sf_tma;     // structure factor: register tile fed by the copy engine (ARCHE_SF_TMA=0: global loads of a_j)
   bool s5_rows;    // S5 reduction of the streamed form as a row walk (ARCHE_S5_ROWS=0: the generic grid-stride kernel)
@@ -429,6 +430,8 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     { const char *e = getenv("ARCHE_LAZY_F"); c->lazy_F = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_S5_ROWS"); c->s5_rows = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_SF_TMA"); c->sf_tma = e ? e[0] != '0' : true; }
+    { const char *e = getenv("ARCHE_MU_SPLIT"); c->mu_split = e ? e[0] != '0' : true; }
+    CK(cudaFuncSetAttribute(mu_first_eval_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
     // measured: 384^3 210 -> 172 us (0.67 -> 0.82 of the HBM peak); 256^3 49.5 -> 52.9 us, 192^3 27.5 -> 29.0 us (the register
     // kernel is already at 0.87 there and the extra 2 LP N doubles of shared memory cost a resident block)
     { const char *e = getenv("ARCHE_R2C_TMA"); c->r2c_tma = e ? e[0] != '0' : p->grid[0] >= 384; }
@@ -605,6 +608,12 @@ int scf_iteration(arche_ctx *c) {
     const double *aV = c->V_i; long long ang = c->ng; ScfConst aC = C;
     DevScalars *asc = c->sc; const double *atab = c->fdtab; double *apart = c->partials;
     int amax = kMuMaxPasses; const int *astop = c->stop;
+    // streamed grids: the one evaluation a steady-state iteration needs as an ordinary dependent launch; the cooperative
+    // kernel then returns at once (mu_done) or takes over a hard case
+    if (c->mu_split && !(c->ng & 1) && c->ng > (long long)c->mu_grid * 256 * kMuCache) {
+      CK(launch_k(c, mu_first_eval_kernel, c->mu_grid, 256, kFdTabBytes, aV, ang, aC, asc, atab, apart, c->counter, astop));
+      ++c->launches;
+    }
     void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax, &astop};
     CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, kFdTabBytes, c->stream));
     ++c->launches; }

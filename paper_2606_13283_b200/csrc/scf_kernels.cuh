@@ -241,6 +241,7 @@ struct StoreVi {
   // grid totals {min, max, sum of V_i, sum I_{1/2}} -> scalars and the mu bracket
   static __device__ __forceinline__ void apply(const double *t, double kT_eta0, DevScalars *sc) {
     sc->vmin = t[0]; sc->vmax = t[1]; sc->vsum = t[2]; sc->n0sum = t[3];
+    sc->mu_done = 0;   // a new potential: the mu iteration of this SCF iteration has not run yet
     // bracket of the root of Eq. 19: N(mu) is increasing and eta0 solves the flat-potential problem
     const double lo = t[0] + kT_eta0, hi = t[1] + kT_eta0;
     const double pad = 1e-12 * (fabs(lo) + fabs(hi) + fabs(kT_eta0));
@@ -411,11 +412,103 @@ __device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &g
   return mu;   // identical in every thread of the grid
 }
 
+// First evaluation of the mu iteration as an ordinary (non-cooperative, programmatic-dependent) launch.  On mid-size
+// grids the cooperative kernel below costs more in launch serialisation, table copies and grid barriers than in work
+// (192^3: 52 us per evaluation against ~15 us of work; it also breaks the dependent-launch chain of the iteration), and
+// in steady state the iteration needs exactly one evaluation: the verification of the Newton step taken from the fused
+// evaluation of the S2 pass.  This kernel takes that step (same rules as mu_solve_dev: bracket, bisection when Newton
+// leaves it), evaluates N(mu_1), and its last block decides: done (neutral to 1e-14 N_e, or the secant step passes the
+// second-order bound) -> mu, bracket, counters are written and mu_done = 1, the cooperative kernel returns at once;
+// not done -> (mu_1, sum I_1/2, slope) are handed over in the fields the cooperative kernel reads as "previous mu with a
+// fused evaluation" and it carries on from there.  Streaming form of the evaluation only (even point count).
+__global__ void __launch_bounds__(256, 3) mu_first_eval_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
+                                                            DevScalars *sc, const double *__restrict__ fdtab,
+                                                            double *partials, unsigned int *counter, const int *stop) {
+  extern __shared__ __align__(16) double s_tab[];
+  __shared__ double s_red[64 + 2];
+  __shared__ unsigned long long s_bar;
+  pdl_launch_dependents();
+  fd_load_tables_async(s_tab, fdtab, &s_bar);
+  pdl_wait();
+  if (stop && *stop) { fd_tables_wait(&s_bar); return; }
+  // the state every block derives for itself (sc is only written by the last block, after the grid reduction)
+  const double inv_kT = 1.0 / C.kT, scaleN = C.cTF * C.dV;
+  double lo = sc->mu_lo, hi = sc->mu_hi;
+  const double mu0 = sc->mu, f0 = scaleN * sc->n0sum - C.Ne, slope0 = sc->dNdmu;
+  const bool usable = sc->mu_have_prev && slope0 > 0.0 && !(hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi)));
+  if (!usable) { fd_tables_wait(&s_bar); return; }          // first iteration / flat potential: the cooperative kernel
+  bool at_once = fabs(f0) <= 1e-14 * C.Ne;                   // the fused evaluation is already neutral
+  double mu1 = mu0;
+  if (!at_once) {
+    if (f0 > 0.0) hi = fmin(hi, mu0); else lo = fmax(lo, mu0);
+    mu1 = mu0 - f0 / slope0;
+    if (!(mu1 > lo && mu1 < hi)) mu1 = 0.5 * (lo + hi);
+    if (fabs(mu1 - mu0) <= 2e-16 * fmax(fabs(mu0), C.kT)) at_once = true;
+  }
+  if (at_once) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+      sc->mu_evals = 1; sc->mu_evals_total += 1; sc->N_last = f0 + C.Ne; sc->mu_done = 1;
+    }
+    fd_tables_wait(&s_bar);
+    return;
+  }
+  fd_tables_wait(&s_bar);
+  double s1 = 0.0;
+  {
+    const double sA = inv_kT * FD_INV_W, sB = (mu1 * inv_kT - FD_ETA_A) * FD_INV_W;   // s = sB - v sA
+    const double2 *V2 = reinterpret_cast<const double2 *>(V_i);
+    const int n2 = (int)(ng >> 1), nth = (int)(gridDim.x * blockDim.x);
+    int i = (int)(blockIdx.x * blockDim.x + threadIdx.x);
+    const double2 zero2 = make_double2(0.0, 0.0);
+    double2 a = i < n2 ? V2[i] : zero2, b = i + nth < n2 ? V2[i + nth] : zero2;
+    for (; i < n2; i += 2 * nth) {
+      const int in = i + 2 * nth;
+      const double2 an = in < n2 ? V2[in] : zero2, bn = in + nth < n2 ? V2[in + nth] : zero2;
+      if (i + nth < n2) {
+        const double sg[4] = {fma(-a.x, sA, sB), fma(-a.y, sA, sB), fma(-b.x, sA, sB), fma(-b.y, sA, sB)};
+        double im12[4], i12[4], d[4];
+        fd_eval_multi_s<2, 4>(s_tab, sg, im12, i12, d);
+        s1 += (i12[0] + i12[1]) + (i12[2] + i12[3]);
+      } else {
+        const double sg[2] = {fma(-a.x, sA, sB), fma(-a.y, sA, sB)};
+        double im12[2], i12[2], d[2];
+        fd_eval_multi_s<2, 2>(s_tab, sg, im12, i12, d);
+        s1 += i12[0] + i12[1];
+      }
+      a = an; b = bn;
+    }
+  }
+  double v[1] = {s1};
+  const int op[1] = {0};
+  if (grid_reduce<1>(v, op, partials, counter, s_red) && threadIdx.x == 0) {
+    const double S1 = s_red[32], f1 = scaleN * S1 - C.Ne;
+    bool done = false;
+    double mu = mu1, fres = f1, slope = slope0;
+    if (fabs(f1) <= 1e-14 * C.Ne) done = true;
+    else {
+      if (f1 > 0.0) hi = fmin(hi, mu1); else lo = fmax(lo, mu1);
+      bool fresh = false;
+      if (mu1 != mu0) { const double sct = (f1 - f0) / (mu1 - mu0); if (sct > 0.0) { slope = sct; fresh = true; } }
+      double mu2 = mu1 - f1 / slope;
+      if (!(mu2 > lo && mu2 < hi)) mu2 = 0.5 * (lo + hi);
+      if (fabs(mu2 - mu1) <= 2e-16 * fmax(fabs(mu1), C.kT)) done = true;
+      else if (fresh) {
+        const double st = fmax(fabs(mu2 - mu1), fabs(mu1 - mu0));
+        if (fabs(f1) * st * inv_kT <= 2e-15 * C.Ne) { mu = mu2; fres = 0.0; done = true; }
+      }
+    }
+    sc->mu_lo = lo; sc->mu_hi = hi; sc->mu = mu;
+    if (done) { sc->mu_evals = 2; sc->mu_evals_total += 2; sc->N_last = fres + C.Ne; sc->mu_done = 1; }
+    else { sc->n0sum = S1; sc->dNdmu = slope; sc->mu_evals_total += 1; }   // hand-over: (mu_1, f_1) as the "fused" evaluation
+  }
+}
+
 __global__ void __launch_bounds__(256, 3) mu_solve_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
                                                        DevScalars *sc, const double *__restrict__ fdtab,
                                                        double *partials, int max_pass, const int *stop) {
   namespace cg = cooperative_groups;
   if (stop && *stop) return;   // uniform over the grid: no block reaches a barrier
+  if (sc->mu_done) return;     // mu_first_eval_kernel finished the iteration (uniform: written before this launch)
   cg::grid_group grid = cg::this_grid();
   extern __shared__ __align__(16) double s_tab[];   // kFdTabDoubles (49.5 KB: dynamic, beyond the 48 KB static limit)
   __shared__ double s_red[2 * 32 + 2];
