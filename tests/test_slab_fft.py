@@ -104,3 +104,36 @@ def test_ipc_export_round_trip_within_a_process(orc):
     h = C.create_string_buffer(64)
     assert g.lib.arche_ipc_export(p.value, h) == 0 and any(h.raw)
     assert g.lib.arche_slab_free(p.value) == 0
+
+
+@pytest.mark.gpu
+def test_slabfft_object_in_a_world_of_one(orc):
+    """paper_2606_13283_b200.slab.SlabFFT, the one-process-per-GPU object, in a process group of size 1 (gloo): buffer
+    allocation and IPC export, the handle exchange, the views over library-owned memory, barriers, both directions.
+    (Opening a peer's handle needs a second GPU process; the decomposition itself is covered by VirtualSlabs above.)"""
+    import torch
+    import torch.distributed as dist
+    import arche_inputs as ai
+    from paper_2606_13283_b200 import Arche
+    from paper_2606_13283_b200.slab import SlabFFT
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]
+    dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
+    try:
+        grid = (24, 16, 36)
+        cfg = ai.make_small(n_ions=2, grid=grid, cell=[6.0, 5.0, 7.0], seed=61)
+        g = Arche(cfg)
+        fft = SlabFFT(g)
+        assert fft.plan.z_slab_shape == (36, 16, 24) and fft.peer_y == [fft.buf.y] and fft.peer_z == [fft.buf.z]
+        rng = np.random.default_rng(9)
+        f = rng.normal(size=(36, 16, 24)) + 1j * rng.normal(size=(36, 16, 24))
+        fft.z_slab().copy_(torch.as_tensor(f))
+        fft.forward()
+        ref = orc.fft3d(f, -1)
+        assert np.abs(fft.y_slab().cpu().numpy() - ref).max() < 1e-12 * np.abs(ref).max()
+        fft.z_slab().zero_()
+        fft.inverse()
+        assert np.abs(fft.z_slab().cpu().numpy() - f * f.size).max() < 1e-12 * np.abs(f).max() * f.size
+        fft.close()
+    finally:
+        dist.destroy_process_group()
