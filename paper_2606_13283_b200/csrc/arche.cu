@@ -86,6 +86,7 @@ struct arche_ctx {
   int red_blocks;  // capacity of the partials buffer (blocks)
   int mu_grid;     // co-resident blocks of the cooperative mu/density kernel
   int ew_grid;     // blocks of grid-stride elementwise kernels
+  bool mu_regular; int mu_coop_iters;   // mu as ordinary launches only from iteration mu_coop_iters of a solve (ARCHE_MU_REGULAR, ARCHE_MU_COOP_ITERS)
   bool mu_split;   // first evaluation of the mu iteration as an ordinary launch (mu_first_eval_kernel; ARCHE_MU_SPLIT=0: off)
   bool r2c_tma;    // plain r2c x pass fed by the copy engine (ARCHE_R2C_TMA)
   bool sf_tma;     // structure factor: register tile fed by the copy engine (ARCHE_SF_TMA=0: global loads of a_j)
@@ -431,6 +432,8 @@ static int init_body(arche_ctx *c, const arche_params *p) {
     { const char *e = getenv("ARCHE_S5_ROWS"); c->s5_rows = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_SF_TMA"); c->sf_tma = e ? e[0] != '0' : true; }
     { const char *e = getenv("ARCHE_MU_SPLIT"); c->mu_split = e ? e[0] != '0' : true; }
+    { const char *e = getenv("ARCHE_MU_REGULAR"); c->mu_regular = e ? e[0] != '0' : true; }
+    { const char *e = getenv("ARCHE_MU_COOP_ITERS"); c->mu_coop_iters = e ? atoi(e) : 3; }
     CK(cudaFuncSetAttribute(mu_first_eval_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFdTabBytes));
     // measured: 384^3 210 -> 172 us (0.67 -> 0.82 of the HBM peak); 256^3 49.5 -> 52.9 us, 192^3 27.5 -> 29.0 us (the register
     // kernel is already at 0.87 there and the extra 2 LP N doubles of shared memory cost a resident block)
@@ -570,7 +573,13 @@ int flush_mix(arche_ctx *c) {
   return ARCHE_OK;
 }
 
-int scf_iteration(arche_ctx *c) {
+static inline bool mu_split_applies(const arche_ctx *c) {
+  return c->mu_split && !(c->ng & 1) && c->ng > (long long)c->mu_grid * 256 * kMuCache;
+}
+// parts: 1 = S1 + S2, 2 = S3 (mu), 4 = S4 + S5.  mu_mode: 0 = first evaluation as an ordinary launch (where it applies),
+// then the cooperative kernel; 1 = two ordinary launches and no cooperative one (an iteration they cannot close halts the
+// batch: stop flag = 2, scf_solve finishes it); 2 = the cooperative kernel alone
+int scf_iteration(arche_ctx *c, int parts = 7, int mu_mode = 0) {
   const GridGeom &G = c->G;
   const ScfConst &C = c->C;
   const int mix = c->mix_pending ? 1 : 0;
@@ -589,7 +598,8 @@ int scf_iteration(arche_ctx *c) {
   sv.V_i = c->V_i; sv.n_i = c->n_i; sv.n_a = c->n_a; sv.sc = c->sc; sv.partials = c->partials; sv.counter = c->counter;
   sv.fdtab = c->fdtab; sv.inv_vol = 1.0 / G.vol; sv.kT_eta0 = C.kT * C.eta0; sv.inv_kT = 1.0 / C.kT; sv.xc = C.xc; sv.mix = mix;
   int rc;
-  if (c->fuse) {
+  if (!(parts & 1)) {
+  } else if (c->fuse) {
     rc = fft3d_inverse(c, lp, sv, PC_FFT_INV_Z, PC_FFT_INV_X);
     if (rc) return rc;
   } else {
@@ -602,21 +612,28 @@ int scf_iteration(arche_ctx *c) {
       else CK(launch_k(c, pointwise_r_kernel<LoadReal, StoreVi, true, 3>, prt(3), 256, kFdTabBytes, LoadReal{c->V_i}, sv, c->ng, c->stop, (const double *)c->fdtab));
       ++c->launches; }
   }
-  c->mix_pending = false;
+  if (parts & 1) c->mix_pending = false;
   // S3: persistent cooperative kernel (Newton/secant passes separated by grid barriers)
-  { ProfScope ps(c, PC_MU);
+  if (parts & 2) { ProfScope ps(c, PC_MU);
     const double *aV = c->V_i; long long ang = c->ng; ScfConst aC = C;
     DevScalars *asc = c->sc; const double *atab = c->fdtab; double *apart = c->partials;
     int amax = kMuMaxPasses; const int *astop = c->stop;
     // streamed grids: the one evaluation a steady-state iteration needs as an ordinary dependent launch; the cooperative
     // kernel then returns at once (mu_done) or takes over a hard case
-    if (c->mu_split && !(c->ng & 1) && c->ng > (long long)c->mu_grid * 256 * kMuCache) {
-      CK(launch_k(c, mu_first_eval_kernel, c->mu_grid, 256, kFdTabBytes, aV, ang, aC, asc, atab, apart, c->counter, astop));
+    if (mu_mode != 2 && mu_split_applies(c)) {
+      CK(launch_k(c, mu_first_eval_kernel, c->mu_grid, 256, kFdTabBytes, aV, ang, aC, asc, atab, apart, c->counter, astop, 0));
       ++c->launches;
+      if (mu_mode == 1) {
+        CK(launch_k(c, mu_first_eval_kernel, c->mu_grid, 256, kFdTabBytes, aV, ang, aC, asc, atab, apart, c->counter, astop, 1));
+        ++c->launches;
+      }
     }
-    void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax, &astop};
-    CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, kFdTabBytes, c->stream));
-    ++c->launches; }
+    if (mu_mode != 1 || !mu_split_applies(c)) {
+      void *args[] = {&aV, &ang, &aC, &asc, &atab, &apart, &amax, &astop};
+      CK(cudaLaunchCooperativeKernel((const void *)mu_solve_kernel, dim3(c->mu_grid), dim3(256), args, kFdTabBytes, c->stream));
+      ++c->launches;
+    } }
+  if (!(parts & 4)) return ARCHE_OK;
   // S4 + S5 (+ w, F, stop flags in the last block of the G-space reduction)
   LoadDensity ldn;
   ldn.V_i = c->V_i; ldn.n_i = c->n_i; ldn.n_a = c->n_a; ldn.sc = c->sc; ldn.partials = c->partials; ldn.counter = c->counter;
@@ -787,13 +804,26 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
     c->stop = fixed > 0 ? nullptr : &c->sc->converged;
     const int n = it + batch <= maxit ? batch : maxit - it;
     for (int b = 0; b < n; ++b) {
-      rc = scf_iteration(c);
+      // after the first iterations of a solve (no previous mu, large steps) the mu iteration runs as ordinary launches only
+      const int mode = (fixed <= 0 && c->mu_regular && mu_split_applies(c) && it + b >= c->mu_coop_iters) ? 1 : 0;
+      rc = scf_iteration(c, 7, mode);
+      if (rc) { c->stop = nullptr; return rc; }
+    }
+    rc = read_scalars(c);
+    if (rc) { c->stop = nullptr; return rc; }
+    if (fixed <= 0 && c->h_sc->converged == 2) {
+      // an iteration whose mu the ordinary launches could not close halted the batch (every later kernel returned at
+      // once): the cooperative kernel takes over from the handed-over state, then the rest of that iteration runs
+      CK(cudaMemsetAsync(&c->sc->converged, 0, sizeof(int), c->stream));
+      rc = scf_iteration(c, 2 | 4, 2);
+      if (rc) { c->stop = nullptr; return rc; }
+      rc = read_scalars(c);
       if (rc) { c->stop = nullptr; return rc; }
     }
     c->stop = nullptr;
-    it += n;
-    rc = read_scalars(c);
-    if (rc) return rc;
+    const int it_before = it;
+    it = fixed > 0 ? it + n : c->h_sc->iter;   // the device's count: a halted batch completed fewer iterations than launched
+    const int n_done = it > it_before ? it - it_before : 1;
     if (!isfinite(c->h_sc->F_total) || !isfinite(c->h_sc->mu)) return fail(c, ARCHE_ENAN, "non-finite free energy or mu");
     if (fixed <= 0 && c->h_sc->converged) conv = true;
     if (fixed <= 0 && !conv) {
@@ -802,7 +832,7 @@ int scf_solve(arche_ctx *c, const double *d_pos) {
       if (dn > 0.0 && tol > 0.0) {
         if (dn <= tol) batch = 1;                                  // waiting for the free-energy criterion only
         else if (dn_prev > dn) {
-          const double rem = log(tol / dn) * (double)n / log(dn / dn_prev);   // iterations until ||dn|| meets the tolerance
+          const double rem = log(tol / dn) * (double)n_done / log(dn / dn_prev);   // iterations until ||dn|| meets the tolerance
           batch = rem < 1.0 ? 1 : (rem > 2.0 * kScfBatch ? 2 * kScfBatch : (int)ceil(rem));
         }
       }

@@ -423,20 +423,28 @@ __device__ __forceinline__ double mu_solve_dev(cooperative_groups::grid_group &g
 // fused evaluation" and it carries on from there.  Streaming form of the evaluation only (even point count).
 __global__ void __launch_bounds__(256, 3) mu_first_eval_kernel(const double *__restrict__ V_i, long long ng, ScfConst C,
                                                             DevScalars *sc, const double *__restrict__ fdtab,
-                                                            double *partials, unsigned int *counter, const int *stop) {
+                                                            double *partials, unsigned int *counter, const int *stop,
+                                                            int final_try) {
+  // final_try (the last of a chain of these launches that is NOT followed by the cooperative kernel): when the iteration
+  // is still open at the end, the stop flag is set to 2 -- every later kernel of the batch returns at once and the host
+  // finishes this SCF iteration with the cooperative kernel (arche.cu: scf_solve)
   extern __shared__ __align__(16) double s_tab[];
   __shared__ double s_red[64 + 2];
   __shared__ unsigned long long s_bar;
   pdl_launch_dependents();
   fd_load_tables_async(s_tab, fdtab, &s_bar);
   pdl_wait();
-  if (stop && *stop) { fd_tables_wait(&s_bar); return; }
+  if ((stop && *stop) || sc->mu_done) { fd_tables_wait(&s_bar); return; }   // uniform: written by earlier kernels only
   // the state every block derives for itself (sc is only written by the last block, after the grid reduction)
   const double inv_kT = 1.0 / C.kT, scaleN = C.cTF * C.dV;
   double lo = sc->mu_lo, hi = sc->mu_hi;
   const double mu0 = sc->mu, f0 = scaleN * sc->n0sum - C.Ne, slope0 = sc->dNdmu;
   const bool usable = sc->mu_have_prev && slope0 > 0.0 && !(hi - lo <= 4e-16 * fmax(fabs(lo), fabs(hi)));
-  if (!usable) { fd_tables_wait(&s_bar); return; }          // first iteration / flat potential: the cooperative kernel
+  if (!usable) {                                             // first iteration / flat potential: the cooperative kernel
+    if (final_try && stop && blockIdx.x == 0 && threadIdx.x == 0) sc->converged = 2;
+    fd_tables_wait(&s_bar);
+    return;
+  }
   bool at_once = fabs(f0) <= 1e-14 * C.Ne;                   // the fused evaluation is already neutral
   double mu1 = mu0;
   if (!at_once) {
@@ -499,7 +507,10 @@ __global__ void __launch_bounds__(256, 3) mu_first_eval_kernel(const double *__r
     }
     sc->mu_lo = lo; sc->mu_hi = hi; sc->mu = mu;
     if (done) { sc->mu_evals = 2; sc->mu_evals_total += 2; sc->N_last = fres + C.Ne; sc->mu_done = 1; }
-    else { sc->n0sum = S1; sc->dNdmu = slope; sc->mu_evals_total += 1; }   // hand-over: (mu_1, f_1) as the "fused" evaluation
+    else {   // hand-over: (mu_1, f_1) as the "fused" evaluation of whoever continues
+      sc->n0sum = S1; sc->dNdmu = slope; sc->mu_evals_total += 1;
+      if (final_try && stop) sc->converged = 2;
+    }
   }
 }
 

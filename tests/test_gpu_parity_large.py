@@ -262,6 +262,40 @@ def test_lazy_free_energy_is_the_same_solve(orc, torch_cuda, monkeypatch, mode):
     assert rf["F_evals"] == 9 and r9["F_total"] == rf["F_total"] and r9["E_ie"] == rf["E_ie"]
 
 
+def test_mu_iteration_as_ordinary_launches_and_its_recovery(orc, torch_cuda, monkeypatch):
+    """On streamed grids the mu iteration of a stop-rule solve runs, after the first iterations, as two ordinary launches
+    without the cooperative kernel; an iteration they cannot close sets the stop flag to 2, every later kernel of the batch
+    returns at once and the host finishes that iteration with the cooperative kernel.  ARCHE_MU_COOP_ITERS=0 forces that
+    recovery from the first iteration on (no previous mu there).  Against the cooperative-only solve (ARCHE_MU_REGULAR=0,
+    ARCHE_MU_SPLIT=0): the same iteration count, mu and F to 1e-12, density to 1e-11, forces to 1e-9; and the default
+    configuration likewise.  Grid of 1.05 M points (beyond the register-cached form of the mu kernel)."""
+    monkeypatch.setenv("ARCHE_FUSE", "0")
+    cfg = ai.make_small(n_ions=12, grid=(128, 128, 64), cell=[16.0, 16.0, 8.0], T_eV=20.0, seed=77, dmin=2.0)
+    kw = dict(xc=2, scf_tol_F=1e-10, scf_tol_dn=1e-9, scf_max_iter=300)
+    out = {}
+    for tag, env in (("coop", {"ARCHE_MU_REGULAR": "0", "ARCHE_MU_SPLIT": "0"}),
+                     ("default", {}),
+                     ("recovery", {"ARCHE_MU_REGULAR": "1", "ARCHE_MU_COOP_ITERS": "0"})):
+        for k in ("ARCHE_MU_REGULAR", "ARCHE_MU_SPLIT", "ARCHE_MU_COOP_ITERS"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        g = _gpu(cfg, **kw)
+        assert not g.is_fused() and not g.is_persistent()
+        r1 = g.scf_solve(cfg["pos"])
+        pos2 = cfg["pos"] + 0.05                       # a second solve: one-center start, previous mu available
+        r2 = g.scf_solve(pos2)
+        out[tag] = (r1, r2, g.get_real("n_a").cpu().numpy(), g.forces().cpu().numpy())
+    ref = out["coop"]
+    assert ref[0]["converged"] == 1 and ref[1]["converged"] == 1
+    for tag in ("default", "recovery"):
+        r1, r2, n, F = out[tag]
+        for a, b in ((r1, ref[0]), (r2, ref[1])):
+            assert a["converged"] == 1 and a["scf_iters"] == b["scf_iters"] and a["mu_evals"] == b["mu_evals"], tag
+            assert abs(a["mu"] - b["mu"]) < 1e-12 * max(1.0, abs(b["mu"])) and abs(a["F_total"] - b["F_total"]) < 1e-12 * abs(b["F_total"]), tag
+        assert _rel(n, ref[2]) < 1e-11 and np.abs(F - ref[3]).max() < 1e-9 * np.abs(ref[3]).max(), tag
+
+
 @pytest.mark.parametrize("name,grid", [("c1", None), ("streamed-128", (128, 32, 16))])
 def test_one_center_start_field_by_field(orc, torch_cuda, monkeypatch, name, grid):
     """P4 (Eq. 20, reading A10): after a first solve, ions are displaced and scf_begin builds n_i = clip/renormalise of the
